@@ -1,0 +1,14 @@
+"""Seeded synthetic workloads for the chi0(q, i*omega) build.
+
+This package holds ONLY input generation (shapes, random draws, occupations that
+are *inputs* at the C-ABI boundary).  It contains none of the method's arithmetic
+(no z, no pair weights, no chi0) and is the only module shared by the oracle
+tests, the CUDA parity tests and bench.py.  Recipe: DESIGN.md section "Inputs".
+"""
+from .configs import CONFIGS, WorkloadConfig, get_config, scaled_config
+from .generate import Problem, SpinChannel, generate, haar_unitary
+
+__all__ = [
+    "CONFIGS", "WorkloadConfig", "get_config", "scaled_config",
+    "Problem", "SpinChannel", "generate", "haar_unitary",
+]

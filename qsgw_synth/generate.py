@@ -1,0 +1,109 @@
+"""Seeded input generator (NumPy only; no method arithmetic).
+
+Draw order: P, then per (spin, k): unitary for k, unitary for
+k+q, eps_k, eps_{k+q}.  Seed = 250603477 + config index (+ optional offset).
+
+Layouts returned are the boundary layouts of include/qsgw.h:
+  P      complex128 [sum_s m_s*b_s*b_s], site-major, each site [I][alpha][beta]
+  Ck     complex128 [n_k][n_o][N_b]   (row = band, i.e. column-major N_b x n_o)
+  Ckq    complex128 [n_k][n_u][N_b]
+  eps_k, f_k   float64 [n_k][n_o];  eps_kq, f_kq  float64 [n_k][n_u]
+  omega  float64 [n_freq]
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import List
+
+import numpy as np
+
+from .configs import BASE_SEED, WorkloadConfig
+
+
+def haar_unitary(rng: np.random.Generator, n: int) -> np.ndarray:
+    """Haar-distributed n x n unitary: QR of a complex Ginibre matrix with the
+    diag(R)/|diag(R)| phase fix."""
+    g = (rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))) / np.sqrt(2.0)
+    q, r = np.linalg.qr(g)
+    d = np.diagonal(r)
+    return q * (d / np.abs(d))[None, :]
+
+
+def omega_grid(cfg: WorkloadConfig) -> np.ndarray:
+    """omega_0 = 0, then geometric from omega_1 to omega_max (n_freq points in all)."""
+    om = np.zeros(cfg.n_freq)
+    if cfg.n_freq > 1:
+        if cfg.n_freq == 2:
+            om[1] = cfg.omega_max
+        else:
+            om[1:] = np.geomspace(cfg.omega_1, cfg.omega_max, cfg.n_freq - 1)
+    return om
+
+
+@dataclass
+class SpinChannel:
+    Ck: np.ndarray
+    Ckq: np.ndarray
+    eps_k: np.ndarray
+    f_k: np.ndarray
+    eps_kq: np.ndarray
+    f_kq: np.ndarray
+
+
+@dataclass
+class Problem:
+    cfg: WorkloadConfig
+    P: np.ndarray            # flat, site-major
+    omega: np.ndarray
+    spins: List[SpinChannel]
+
+    def P_site(self, s: int) -> np.ndarray:
+        b, m = self.cfg.orb_per_site, self.cfg.pb_per_site
+        off = sum(mm * bb * bb for bb, mm in zip(b[:s], m[:s]))
+        return self.P[off: off + m[s] * b[s] * b[s]].reshape(m[s], b[s], b[s])
+
+
+def _fermi(eps: np.ndarray, kT: float) -> np.ndarray:
+    x = np.clip(eps / kT, -700.0, 700.0)
+    return 1.0 / (1.0 + np.exp(x))
+
+
+def generate(cfg: WorkloadConfig, seed_offset: int = 0, n_k: int | None = None) -> Problem:
+    """Generate the seeded problem.  `n_k` truncates the k loop (same stream prefix,
+    so the first n_k k-points equal those of the full problem)."""
+    rng = np.random.default_rng(BASE_SEED + cfg.index + seed_offset)
+    nk = cfg.n_k if n_k is None else n_k
+    nb = cfg.n_b
+    parts = []
+    for b, m in zip(cfg.orb_per_site, cfg.pb_per_site):
+        sd = np.sqrt(0.5 / b)   # E|P|^2 = 1/b_s
+        parts.append((sd * (rng.standard_normal((m, b, b)) +
+                            1j * rng.standard_normal((m, b, b)))).reshape(-1))
+    P = np.concatenate(parts)
+    spins = []
+    for _ in range(cfg.n_spin):
+        Ck = np.empty((nk, cfg.n_o, nb), dtype=np.complex128)
+        Ckq = np.empty((nk, cfg.n_u, nb), dtype=np.complex128)
+        eps_k = np.empty((nk, cfg.n_o)); f_k = np.empty((nk, cfg.n_o))
+        eps_kq = np.empty((nk, cfg.n_u)); f_kq = np.empty((nk, cfg.n_u))
+        for k in range(nk):
+            Uk = haar_unitary(rng, nb)
+            Ukq = haar_unitary(rng, nb)
+            if cfg.kind == "insulator":
+                o0, u0 = 0, cfg.n_o
+                e_o = np.sort(rng.uniform(*cfg.eps_occ, cfg.n_o))
+                e_u = np.sort(rng.uniform(*cfg.eps_unocc, cfg.n_u))
+                fo, fu = np.ones(cfg.n_o), np.zeros(cfg.n_u)
+            else:
+                o0, u0 = cfg.o_first, cfg.u_first
+                ek_all = np.sort(rng.uniform(*cfg.eps_all, nb))
+                ekq_all = np.sort(rng.uniform(*cfg.eps_all, nb))
+                e_o = ek_all[o0:o0 + cfg.n_o]
+                e_u = ekq_all[u0:u0 + cfg.n_u]
+                fo, fu = _fermi(e_o, cfg.kT), _fermi(e_u, cfg.kT)
+            # column n of the unitary = band n; stored band-major (row = band)
+            Ck[k] = Uk[:, o0:o0 + cfg.n_o].T
+            Ckq[k] = Ukq[:, u0:u0 + cfg.n_u].T
+            eps_k[k], f_k[k], eps_kq[k], f_kq[k] = e_o, fo, e_u, fu
+        spins.append(SpinChannel(Ck, Ckq, eps_k, f_k, eps_kq, f_kq))
+    return Problem(cfg=cfg, P=P, omega=omega_grid(cfg), spins=spins)
