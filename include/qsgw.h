@@ -1,0 +1,151 @@
+/*
+ * qsgw.h -- C ABI of the B200-native polarization build chi0(q, i*omega) for QSGW.
+ *
+ * Method: arxiv 2506.03477.  One context = one (q, spin) problem:
+ *
+ *   stage (a)  z[n,n',I] = sum_{alpha,beta in site(I)} conj(C_{k+q}[alpha,n']) P_s[I,alpha,beta] C_k[beta,n]
+ *              muffin-tin part of the matrix elements of Eq. (8) with the
+ *              eigenfunction expansion of Eq. (4); "prepared on the fly"
+ *               per band batch (Alg. 1 lines 10-12).
+ *   stage (b)  acc_j[I,J] += sum_{pairs kept} w_j(n,n') conj(z[n,n',I]) z[n,n',J],  I <= J
+ *              w_j = -2 f_n (1-f_n') D / (D^2 + omega_j^2),  D = eps_{k+q,n'} - eps_{k,n}
+ *              Eq. (14) on the imaginary axis = Alg. 1 lines 16-21
+ *               with a dense Lorentzian weight per frequency.
+ *   finalize   chi0_j = acc_j / N_k, lower triangle = conj(upper), Im(diag) = 0
+ *              (the matrix part is Hermitian).
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE pointers owned by the caller; h_* are HOST pointers that
+ *     are read (or written, for outputs) during the call and never retained.
+ *   - complex128 = interleaved (re, im) pairs of IEEE doubles.  Boundary data are always
+ *     complex128 / float64; QSGW_PREC_MIXED converts internally.
+ *   - Every call returns an int32 status (QSGW_OK = 0); nothing throws or aborts.  Calls are
+ *     stream-ordered on the stream given to qsgw_create and never synchronise the device,
+ *     except qsgw_sync, qsgw_destroy and the *_host entry point.  Asynchronous CUDA faults
+ *     surface as QSGW_ERR_CUDA on a later call.
+ *   - The library owns only its context (accumulators, z workspace, weight table, TMA
+ *     descriptors).  There is no CPU fallback: without a CUDA device every compute call fails.
+ *   - Orbitals are grouped by site: site s owns the contiguous orbital range
+ *     [sum_{t<s} b_t, +b_s); product functions likewise with m_s.  N_b = sum b_s, N_M = sum m_s.
+ *   - State machine: create -> set_product_tensor -> { zmel_build -> chi0_accumulate }* ->
+ *     chi0_finalize -> ( reset -> ... ).  Out-of-order calls return QSGW_ERR_STATE.
+ */
+#ifndef QSGW_H_
+#define QSGW_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qsgw_ctx qsgw_ctx;
+
+enum {
+  QSGW_OK = 0,
+  QSGW_ERR_INVALID_ARG = 1, /* null pointer, bad enum, bad leading dimension            */
+  QSGW_ERR_SHAPE = 2,       /* non-positive extent, batch larger than declared, bad omega */
+  QSGW_ERR_STATE = 3,       /* call out of order                                        */
+  QSGW_ERR_ALLOC = 4,       /* device allocation failed or workspace cap too small      */
+  QSGW_ERR_CUDA = 5,        /* CUDA runtime / driver error (see qsgw_last_error)        */
+  QSGW_ERR_UNSUPPORTED = 6  /* no sm_100 device, or feature not built                   */
+};
+
+enum { QSGW_PREC_FP64 = 0, QSGW_PREC_MIXED = 1 };
+
+/* Problem descriptor (host memory; copied by qsgw_create). */
+typedef struct {
+  int32_t n_sites;               /* S >= 1                                                     */
+  const int32_t* h_orb_per_site; /* b_s > 0, S entries                                         */
+  const int32_t* h_pb_per_site;  /* m_s > 0, S entries                                         */
+  int32_t n_freq;                /* N_omega >= 1                                               */
+  const double* h_omega;         /* imaginary frequencies omega_j >= 0, strictly increasing    */
+  int32_t n_k;                   /* N_k >= 1: the 1/N_k normalisation applied by finalize      */
+  int32_t max_n_o, max_n_u;      /* largest band batch (n_o, n_u) any zmel_build call passes   */
+  int32_t precision;             /* QSGW_PREC_FP64 | QSGW_PREC_MIXED                           */
+  double occ_tol;                /* pair kept iff f_n*(1-f_n') > occ_tol; <0 selects 1e-12     */
+  size_t workspace_bytes;        /* cap on the z workspace; 0 = no cap.  If max_n_o*max_n_u    */
+                                 /* pairs do not fit, create fails with QSGW_ERR_ALLOC         */
+} qsgw_desc;
+
+/* Create a context on the current CUDA device.  `cuda_stream` is a cudaStream_t (NULL =
+ * legacy default stream) on which every later call is ordered.  Allocates the FP64
+ * accumulator (N_omega * N_M * ld * 16 B), the z workspace and the weight table, and zeroes
+ * the accumulator. */
+int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out);
+
+/* Set P_s[I, alpha, beta] = <phi_alpha | M_I phi_beta> (Eq. 8 restricted to one muffin tin,
+ * PAPER.md:130).  d_P: complex128, packed, site-major: for each site s a block
+ * [m_s][b_s][b_s] (I slowest, beta fastest).  Copied/converted into the context. */
+int32_t qsgw_set_product_tensor(qsgw_ctx* ctx, const void* d_P);
+
+/* Stage (a) for one k-point and one band batch (Alg. 1 line 12).
+ *   d_Ck  : complex128, column-major N_b x (>= n_begin+n_o), column = band n of C_k; element
+ *           (beta, n) at d_Ck[n*ld_k + beta]; ld_k >= N_b.  Same memory as a row-major
+ *           [band][orbital] array.
+ *   d_Ckq : likewise for C_{k+q}, bands n'.
+ *   Band batch: n in [n_begin, n_begin+n_o), n' in [np_begin, np_begin+n_u);
+ *           n_o <= max_n_o, n_u <= max_n_u.
+ *   d_z_out: optional complex128 [n_o][n_u][N_M] (I fastest) copy of the batch for tests;
+ *           NULL keeps z internal only.  In mixed mode the exported values are the FP32 z
+ *           widened to FP64.
+ * The batch stays in the context until the next zmel_build. */
+int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const void* d_Ckq,
+                        int64_t ld_kq, int32_t n_begin, int32_t n_o, int32_t np_begin,
+                        int32_t n_u, void* d_z_out);
+
+/* Stage (b) for one band batch (Eq. 14; Alg. 1 lines 16-21).
+ *   d_z   : NULL = use the batch built by the last zmel_build (the normal path; z never leaves
+ *           the context).  Non-NULL = complex128 [n_o][n_u][N_M] (I fastest, the d_z_out layout),
+ *           imported into the context first; lets stage (b) be driven with a caller-made z.
+ *   d_eps_k, d_f_k   : float64[n_o]  energies (Ha) and occupations of the batch's bands n
+ *   d_eps_kq, d_f_kq : float64[n_u]  same for n'
+ *   With d_z == NULL, n_o and n_u must equal the last zmel_build's.
+ * Adds into the accumulator (upper-triangle tiles only). */
+int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps_k,
+                             const double* d_f_k, const double* d_eps_kq, const double* d_f_kq,
+                             int32_t n_o, int32_t n_u);
+
+/* Convenience driver of the band-batch loop (Alg. 1 lines 9-23) for one k-point: splits
+ * n in [0,n_o_total) x n' in [0,n_u_total) into batches of at most (max_n_o, max_n_u) and
+ * calls zmel_build + chi0_accumulate for each.  Energies/occupations cover all bands. */
+int32_t qsgw_chi0_add_kpoint(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const void* d_Ckq,
+                             int64_t ld_kq, const double* d_eps_k, const double* d_f_k,
+                             const double* d_eps_kq, const double* d_f_kq, int32_t n_o_total,
+                             int32_t n_u_total);
+
+/* chi0[j][I][J] = acc/N_k as a full Hermitian matrix: d_chi0_out complex128
+ * [n_freq][N_M][N_M], row-major.  May be called again after more accumulation. */
+int32_t qsgw_chi0_finalize(qsgw_ctx* ctx, void* d_chi0_out);
+
+/* Zero the accumulator and return to the state after set_product_tensor. */
+int32_t qsgw_reset(qsgw_ctx* ctx);
+/* Block until the context's stream is idle; reports deferred CUDA errors. */
+int32_t qsgw_sync(qsgw_ctx* ctx);
+void qsgw_destroy(qsgw_ctx* ctx);
+
+/* Whole job from HOST buffers (H2D copies, all k-points, D2H of the result), for end-to-end
+ * timing.  Host arrays: h_P as set_product_tensor; h_Ck complex128 [n_k][n_o][N_b] (row =
+ * band), h_Ckq [n_k][n_u][N_b]; h_eps_k,h_f_k float64 [n_k][n_o]; h_eps_kq,h_f_kq
+ * [n_k][n_u]; h_chi0_out complex128 [n_freq][N_M][N_M].  desc->max_n_o/max_n_u give the band
+ * batch.  Creates and destroys its own context and stream; synchronous. */
+int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h_Ck,
+                           const void* h_Ckq, const double* h_eps_k, const double* h_f_k,
+                           const double* h_eps_kq, const double* h_f_kq, int32_t n_o,
+                           int32_t n_u, void* h_chi0_out, int64_t* out_kernel_launches);
+
+/* Introspection (host side, no device work). */
+const char* qsgw_last_error(const qsgw_ctx* ctx);       /* "" if none; valid until next call   */
+const char* qsgw_last_create_error(void);               /* error text of a failed qsgw_create  */
+int64_t qsgw_kernel_launches(const qsgw_ctx* ctx);      /* kernels launched by this context    */
+int64_t qsgw_pairs_accumulated(const qsgw_ctx* ctx);    /* band pairs passed to stage (b)      */
+size_t qsgw_device_bytes(const qsgw_ctx* ctx);          /* device memory owned by the context  */
+int32_t qsgw_n_m(const qsgw_ctx* ctx);                  /* N_M                                 */
+int32_t qsgw_n_b(const qsgw_ctx* ctx);                  /* N_b                                 */
+const char* qsgw_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QSGW_H_ */

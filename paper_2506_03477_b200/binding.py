@@ -1,0 +1,223 @@
+"""ctypes binding of include/qsgw.h.  Function names mirror the C ABI (qsgw_* -> methods of
+Chi0Context); tensors are torch CUDA tensors (device memory + streams only) whose data_ptr()
+is passed straight through.  No arithmetic of the method happens here, and there is no CPU
+fallback: if libqsgw.so is missing or no sm_100 GPU is present the calls raise QsgwError.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+from .build import LIB_PATH
+
+PREC_FP64, PREC_MIXED = 0, 1
+_STATUS = {0: "QSGW_OK", 1: "QSGW_ERR_INVALID_ARG", 2: "QSGW_ERR_SHAPE", 3: "QSGW_ERR_STATE",
+           4: "QSGW_ERR_ALLOC", 5: "QSGW_ERR_CUDA", 6: "QSGW_ERR_UNSUPPORTED"}
+
+
+class QsgwError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{_STATUS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class _Desc(C.Structure):
+    _fields_ = [("n_sites", C.c_int32), ("h_orb_per_site", C.POINTER(C.c_int32)),
+                ("h_pb_per_site", C.POINTER(C.c_int32)), ("n_freq", C.c_int32),
+                ("h_omega", C.POINTER(C.c_double)), ("n_k", C.c_int32), ("max_n_o", C.c_int32),
+                ("max_n_u", C.c_int32), ("precision", C.c_int32), ("occ_tol", C.c_double),
+                ("workspace_bytes", C.c_size_t)]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return LIB_PATH
+
+
+def lib() -> C.CDLL:
+    """Load libqsgw.so (built in-tree by paper_2506_03477_b200.build).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise QsgwError(6, f"{LIB_PATH} not found: run `python -m paper_2506_03477_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64, dp = C.c_void_p, C.c_int32, C.c_int64, C.c_void_p
+    L.qsgw_create.argtypes = [C.POINTER(_Desc), vp, C.POINTER(vp)]
+    L.qsgw_set_product_tensor.argtypes = [vp, vp]
+    L.qsgw_zmel_build.argtypes = [vp, vp, i64, vp, i64, i32, i32, i32, i32, vp]
+    L.qsgw_chi0_accumulate.argtypes = [vp, vp, dp, dp, dp, dp, i32, i32]
+    L.qsgw_chi0_add_kpoint.argtypes = [vp, vp, i64, vp, i64, dp, dp, dp, dp, i32, i32]
+    L.qsgw_chi0_finalize.argtypes = [vp, vp]
+    L.qsgw_reset.argtypes = [vp]
+    L.qsgw_sync.argtypes = [vp]
+    L.qsgw_destroy.argtypes = [vp]
+    L.qsgw_destroy.restype = None
+    L.qsgw_chi0_run_host.argtypes = [C.POINTER(_Desc), vp, vp, vp, vp, vp, vp, vp, i32, i32, vp,
+                                     C.POINTER(i64)]
+    for name in ("qsgw_create", "qsgw_set_product_tensor", "qsgw_zmel_build", "qsgw_chi0_accumulate",
+                 "qsgw_chi0_add_kpoint", "qsgw_chi0_finalize", "qsgw_reset", "qsgw_sync",
+                 "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b"):
+        getattr(L, name).restype = i32
+    for name in ("qsgw_last_error", "qsgw_last_create_error", "qsgw_version"):
+        getattr(L, name).restype = C.c_char_p
+    L.qsgw_last_error.argtypes = [vp]
+    for name in ("qsgw_kernel_launches", "qsgw_pairs_accumulated"):
+        getattr(L, name).restype = i64
+        getattr(L, name).argtypes = [vp]
+    L.qsgw_device_bytes.restype = C.c_size_t
+    L.qsgw_device_bytes.argtypes = [vp]
+    L.qsgw_n_m.argtypes = [vp]
+    L.qsgw_n_b.argtypes = [vp]
+    _lib = L
+    return L
+
+
+def version() -> str:
+    return lib().qsgw_version().decode()
+
+
+def _make_desc(orb_per_site, pb_per_site, omega, n_k, max_n_o, max_n_u, precision, occ_tol,
+               workspace_bytes):
+    s = len(orb_per_site)
+    orb = (C.c_int32 * s)(*[int(x) for x in orb_per_site])
+    pb = (C.c_int32 * len(pb_per_site))(*[int(x) for x in pb_per_site])
+    om = (C.c_double * len(omega))(*[float(x) for x in omega])
+    d = _Desc(s, orb, pb, len(omega), om, int(n_k), int(max_n_o), int(max_n_u), int(precision),
+              float(occ_tol), int(workspace_bytes))
+    d._keep = (orb, pb, om)
+    return d
+
+
+def _ptr(t, dtype=None):
+    """data_ptr of a contiguous CUDA tensor (None -> NULL)."""
+    if t is None:
+        return None
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("expected a torch CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    return C.c_void_p(t.data_ptr())
+
+
+class Chi0Context:
+    """One (q, spin) polarization build.  Methods map 1:1 to the qsgw_* entry points."""
+
+    def __init__(self, orb_per_site: Sequence[int], pb_per_site: Sequence[int], omega, n_k: int,
+                 max_n_o: int, max_n_u: int, precision: int = PREC_FP64, occ_tol: float = 1e-12,
+                 workspace_bytes: int = 0, stream=None):
+        import torch
+        self._L = lib()
+        self._h = C.c_void_p()
+        self.n_freq = len(omega)
+        if stream is None and torch.cuda.is_available():
+            stream = torch.cuda.current_stream()
+        self._stream = stream
+        sp = C.c_void_p(stream.cuda_stream) if stream is not None else None
+        d = _make_desc(orb_per_site, pb_per_site, omega, n_k, max_n_o, max_n_u, precision, occ_tol,
+                       workspace_bytes)
+        rc = self._L.qsgw_create(C.byref(d), sp, C.byref(self._h))
+        if rc != 0:
+            self._h = C.c_void_p()
+            raise QsgwError(rc, self._L.qsgw_last_create_error().decode())
+        self.n_m = self._L.qsgw_n_m(self._h)
+        self.n_b = self._L.qsgw_n_b(self._h)
+
+    def _check(self, rc: int):
+        if rc != 0:
+            raise QsgwError(rc, self._L.qsgw_last_error(self._h).decode())
+
+    def set_product_tensor(self, d_P):
+        import torch
+        self._check(self._L.qsgw_set_product_tensor(self._h, _ptr(d_P, torch.complex128)))
+
+    def zmel_build(self, d_Ck, d_Ckq, n_begin: int, n_o: int, np_begin: int, n_u: int, d_z_out=None,
+                   ld_k: Optional[int] = None, ld_kq: Optional[int] = None):
+        import torch
+        ld_k = d_Ck.shape[-1] if ld_k is None else ld_k
+        ld_kq = d_Ckq.shape[-1] if ld_kq is None else ld_kq
+        self._check(self._L.qsgw_zmel_build(self._h, _ptr(d_Ck, torch.complex128), ld_k,
+                                            _ptr(d_Ckq, torch.complex128), ld_kq, n_begin, n_o,
+                                            np_begin, n_u, _ptr(d_z_out, torch.complex128)))
+
+    def chi0_accumulate(self, d_eps_k, d_f_k, d_eps_kq, d_f_kq, n_o: int, n_u: int, d_z=None):
+        import torch
+        f64 = torch.float64
+        self._check(self._L.qsgw_chi0_accumulate(self._h, _ptr(d_z, torch.complex128),
+                                                 _ptr(d_eps_k, f64), _ptr(d_f_k, f64),
+                                                 _ptr(d_eps_kq, f64), _ptr(d_f_kq, f64), n_o, n_u))
+
+    def chi0_add_kpoint(self, d_Ck, d_Ckq, d_eps_k, d_f_k, d_eps_kq, d_f_kq):
+        import torch
+        f64 = torch.float64
+        self._check(self._L.qsgw_chi0_add_kpoint(
+            self._h, _ptr(d_Ck, torch.complex128), d_Ck.shape[-1], _ptr(d_Ckq, torch.complex128),
+            d_Ckq.shape[-1], _ptr(d_eps_k, f64), _ptr(d_f_k, f64), _ptr(d_eps_kq, f64),
+            _ptr(d_f_kq, f64), d_Ck.shape[0], d_Ckq.shape[0]))
+
+    def chi0_finalize(self, d_chi0_out=None):
+        import torch
+        if d_chi0_out is None:
+            d_chi0_out = torch.empty((self.n_freq, self.n_m, self.n_m), dtype=torch.complex128,
+                                     device="cuda")
+        self._check(self._L.qsgw_chi0_finalize(self._h, _ptr(d_chi0_out, torch.complex128)))
+        return d_chi0_out
+
+    def reset(self):
+        self._check(self._L.qsgw_reset(self._h))
+
+    def sync(self):
+        self._check(self._L.qsgw_sync(self._h))
+
+    @property
+    def kernel_launches(self) -> int:
+        return int(self._L.qsgw_kernel_launches(self._h))
+
+    @property
+    def pairs_accumulated(self) -> int:
+        return int(self._L.qsgw_pairs_accumulated(self._h))
+
+    @property
+    def device_bytes(self) -> int:
+        return int(self._L.qsgw_device_bytes(self._h))
+
+    def destroy(self):
+        if self._h:
+            self._L.qsgw_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def chi0_run_host(orb_per_site, pb_per_site, omega, P, Ck, Ckq, eps_k, f_k, eps_kq, f_kq,
+                  max_n_o: int, max_n_u: int, precision: int = PREC_FP64, occ_tol: float = 1e-12,
+                  out=None):
+    """qsgw_chi0_run_host: whole job from HOST (NumPy) buffers; returns (chi0, kernel_launches)."""
+    import numpy as np
+    L = lib()
+    n_k, n_o, _ = Ck.shape
+    n_u = Ckq.shape[1]
+    n_m = int(sum(pb_per_site))
+    arrs = [np.ascontiguousarray(a, dtype=dt) for a, dt in
+            ((P, np.complex128), (Ck, np.complex128), (Ckq, np.complex128), (eps_k, np.float64),
+             (f_k, np.float64), (eps_kq, np.float64), (f_kq, np.float64))]
+    if out is None:
+        out = np.empty((len(omega), n_m, n_m), dtype=np.complex128)
+    d = _make_desc(orb_per_site, pb_per_site, omega, n_k, max_n_o, max_n_u, precision, occ_tol, 0)
+    launches = C.c_int64(0)
+    rc = L.qsgw_chi0_run_host(C.byref(d), *[a.ctypes.data_as(C.c_void_p) for a in arrs], n_o, n_u,
+                              out.ctypes.data_as(C.c_void_p), C.byref(launches))
+    if rc != 0:
+        raise QsgwError(rc, L.qsgw_last_create_error().decode())
+    return out, int(launches.value)

@@ -1,0 +1,230 @@
+// Stage (b), FP64 mode: acc_j[I,J] += sum_p conj(z[p,I]) w_j(p) z[p,J] for one 64x64 tile and one
+// frequency per CTA (Eq. 14; Alg. 1 lines 16-21), on the FP64 tensor
+// pipe (DMMA.8x8x4), and the finalize kernel (1/N_k, Hermitian mirror).
+//
+// z = x + i y:  Re += x_I (w x_J) + y_I (w y_J),  Im += x_I (w y_J) - y_I (w x_J)   ("4M").
+// The 64-column x KP-pair tiles of both planes arrive by one 4-D TMA box per operand with the
+// 128-byte swizzle; w_j(p) for the stage arrives by a 1-D bulk copy; the frequency-scaled operand
+// w*z is formed in registers.  4 warps, each a 32x32 complex sub-tile = 64 DMMA per 4 pairs.
+#include "kernels.h"
+#include "ptx.cuh"
+
+namespace qsgw {
+
+namespace {
+
+constexpr int KP = kChi0F64KP;         // pairs per stage
+constexpr int STAGES = 3;
+constexpr int kThreads = 128;
+constexpr int OPER_BYTES = 2 * 4 * KP * 128;   // planes x column groups x rows x 128 B
+constexpr int PLANE_BYTES = 4 * KP * 128;
+constexpr int CGRP_BYTES = KP * 128;
+constexpr int W_BYTES = KP * 8;
+constexpr int SMEM_OPERANDS = STAGES * 2 * OPER_BYTES;
+constexpr int SMEM_BYTES = SMEM_OPERANDS + STAGES * W_BYTES + 2 * STAGES * 8 + 1024 /*align slack*/;
+
+static_assert(KP % 8 == 0, "swizzle atom is 8 rows");
+static_assert(CGRP_BYTES % 1024 == 0, "column-group blocks must keep the 1024 B swizzle alignment");
+
+__global__ void __launch_bounds__(kThreads, 2) chi0_f64_kernel(const __grid_constant__ Chi0F64Args a) {
+  extern __shared__ unsigned char smem_dyn[];
+  const uint32_t raw = smem_u32(smem_dyn);
+  const uint32_t base = (raw + 1023u) & ~1023u;
+  unsigned char* sm = smem_dyn + (base - raw);
+  double* wsm = reinterpret_cast<double*>(sm + SMEM_OPERANDS);
+  uint64_t* full = reinterpret_cast<uint64_t*>(sm + SMEM_OPERANDS + STAGES * W_BYTES);
+  uint64_t* empty = full + STAGES;
+
+  const int tid = threadIdx.x;
+  const int lane = tid & 31, warp = tid >> 5;
+  const int g = lane >> 2, t = lane & 3;
+  const int wm = warp >> 1, wn = warp & 1;
+
+  const int j = blockIdx.x % a.n_freq;
+  const int tile = blockIdx.x / a.n_freq;
+  const int2 tt = a.d_tiles[tile];
+  const bool diag = (tt.x == tt.y);
+  const int n_iter = (int)(a.n_pairs_padded / KP);
+  const double* wrow = a.wtab + (long long)j * a.kpad;
+
+  if (tid == 0) {
+    tma_prefetch_desc(&a.tmap_z);
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], kThreads / 32);
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  const uint32_t stage_bytes = (diag ? OPER_BYTES : 2 * OPER_BYTES) + W_BYTES;
+  auto issue = [&](int slot, int it) {
+    unsigned char* dstA = sm + slot * (2 * OPER_BYTES);
+    mbar_arrive_expect_tx(&full[slot], stage_bytes);
+    tma_load_4d(dstA, &a.tmap_z, &full[slot], 0, it * KP, tt.x * 4, 0);
+    if (!diag) tma_load_4d(dstA + OPER_BYTES, &a.tmap_z, &full[slot], 0, it * KP, tt.y * 4, 0);
+    bulk_load_1d(wsm + slot * KP, wrow + (long long)it * KP, W_BYTES, &full[slot]);
+  };
+
+  if (tid == 0) {
+    for (int it = 0; it < STAGES - 1 && it < n_iter; ++it) issue(it, it);
+  }
+
+  // per-thread swizzled offsets: row r = 8*(q>>1) + 2t + (q&1); 16-byte chunk ^= r&7
+  uint32_t thr_off[2][2];
+#pragma unroll
+  for (int s = 0; s < 2; ++s)
+#pragma unroll
+    for (int par = 0; par < 2; ++par)
+      thr_off[s][par] = (uint32_t)((2 * t + s) * 128 + ((((4 * par + (g >> 1)) ^ (2 * t + s)) << 4) | ((g & 1) << 3)));
+
+  double cre[4][4][2], cim[4][4][2];
+#pragma unroll
+  for (int mi = 0; mi < 4; ++mi)
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni) {
+      cre[mi][ni][0] = cre[mi][ni][1] = 0.0;
+      cim[mi][ni][0] = cim[mi][ni][1] = 0.0;
+    }
+
+  for (int it = 0; it < n_iter; ++it) {
+    const int slot = it % STAGES;
+    if (tid == 0) {
+      const int nxt = it + STAGES - 1;
+      if (nxt < n_iter) {
+        const int s2 = nxt % STAGES;
+        if (nxt >= STAGES) mbar_wait(&empty[s2], ((nxt / STAGES) - 1) & 1);
+        issue(s2, nxt);
+      }
+    }
+    __syncwarp();
+    mbar_wait(&full[slot], (it / STAGES) & 1);
+
+    const uint32_t aBase = base + slot * (2 * OPER_BYTES) + (2 * wm) * CGRP_BYTES;
+    const uint32_t bBase = base + slot * (2 * OPER_BYTES) + (diag ? 0 : OPER_BYTES) + (2 * wn) * CGRP_BYTES;
+    const uint32_t wBase = base + SMEM_OPERANDS + slot * W_BYTES;
+
+#pragma unroll
+    for (int q = 0; q < KP / 4; ++q) {
+      const uint32_t rq = (uint32_t)((q >> 1) * 1024);
+      const double w = ld_shared_f64(wBase + (uint32_t)((8 * (q >> 1) + 2 * t + (q & 1)) * 8));
+      double ax[4], ay[4], bx[4], by[4];
+#pragma unroll
+      for (int mi = 0; mi < 4; ++mi) {
+        const uint32_t ad = aBase + (mi >> 1) * CGRP_BYTES + rq + thr_off[q & 1][mi & 1];
+        ax[mi] = ld_shared_f64(ad);
+        ay[mi] = ld_shared_f64(ad + PLANE_BYTES);
+      }
+#pragma unroll
+      for (int ni = 0; ni < 4; ++ni) {
+        const uint32_t ad = bBase + (ni >> 1) * CGRP_BYTES + rq + thr_off[q & 1][ni & 1];
+        bx[ni] = w * ld_shared_f64(ad);
+        by[ni] = w * ld_shared_f64(ad + PLANE_BYTES);
+      }
+#pragma unroll
+      for (int mi = 0; mi < 4; ++mi)
+#pragma unroll
+        for (int ni = 0; ni < 4; ++ni) {
+          dmma884(cre[mi][ni][0], cre[mi][ni][1], ax[mi], bx[ni]);
+          dmma884(cim[mi][ni][0], cim[mi][ni][1], ax[mi], by[ni]);
+        }
+#pragma unroll
+      for (int ni = 0; ni < 4; ++ni) bx[ni] = -bx[ni];
+#pragma unroll
+      for (int mi = 0; mi < 4; ++mi)
+#pragma unroll
+        for (int ni = 0; ni < 4; ++ni) {
+          dmma884(cre[mi][ni][0], cre[mi][ni][1], ay[mi], by[ni]);
+          dmma884(cim[mi][ni][0], cim[mi][ni][1], ay[mi], bx[ni]);
+        }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[slot]);
+  }
+
+  // epilogue: exclusive owner of (tile, j) -> plain read-modify-write
+  const long long plane = (long long)a.n_m_pad * a.n_m_pad;
+  double* are = a.acc_re + (long long)j * plane;
+  double* aim = a.acc_im + (long long)j * plane;
+#pragma unroll
+  for (int mi = 0; mi < 4; ++mi) {
+    const int row = tt.x * kTile + (4 * wm + mi) * 8 + g;
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni) {
+      const int col = tt.y * kTile + (4 * wn + ni) * 8 + 2 * t;
+      const long long off = (long long)row * a.n_m_pad + col;
+      double2 r = *reinterpret_cast<double2*>(are + off);
+      r.x += cre[mi][ni][0];
+      r.y += cre[mi][ni][1];
+      *reinterpret_cast<double2*>(are + off) = r;
+      double2 m = *reinterpret_cast<double2*>(aim + off);
+      m.x += cim[mi][ni][0];
+      m.y += cim[mi][ni][1];
+      *reinterpret_cast<double2*>(aim + off) = m;
+    }
+  }
+}
+
+// chi0[j][I][J] = acc/N_k, lower = conj(upper), Im(diag) = 0  (Hermiticity)
+__global__ void __launch_bounds__(256) finalize_kernel(const double* __restrict__ acc_re,
+                                                       const double* __restrict__ acc_im, int n_m, int n_m_pad,
+                                                       double inv_nk, double2* __restrict__ out) {
+  __shared__ double tre[32][33], tim[32][33];
+  const int bi = blockIdx.y, bj = blockIdx.x;
+  if (bi > bj) return;
+  const int j = blockIdx.z;
+  const long long plane = (long long)n_m_pad * n_m_pad;
+  const double* are = acc_re + (long long)j * plane;
+  const double* aim = acc_im + (long long)j * plane;
+  double2* o = out + (long long)j * n_m * n_m;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  for (int r = ty; r < 32; r += 8) {
+    const int I = bi * 32 + r, J = bj * 32 + tx;
+    const long long off = (long long)I * n_m_pad + J;
+    const double vr = are[off] * inv_nk, vi = aim[off] * inv_nk;
+    tre[r][tx] = vr;
+    tim[r][tx] = vi;
+    if (bi != bj && I < n_m && J < n_m) o[(long long)I * n_m + J] = make_double2(vr, vi);
+  }
+  __syncthreads();
+  if (bi != bj) {
+    for (int r = ty; r < 32; r += 8) {
+      const int I = bj * 32 + r, J = bi * 32 + tx;   // mirrored block: out[I][J] = conj(acc[J][I])
+      if (I < n_m && J < n_m) o[(long long)I * n_m + J] = make_double2(tre[tx][r], -tim[tx][r]);
+    }
+  } else {
+    for (int r = ty; r < 32; r += 8) {
+      const int I = bi * 32 + r, J = bj * 32 + tx;
+      if (I < n_m && J < n_m) {
+        double2 v;
+        if (r < tx) v = make_double2(tre[r][tx], tim[r][tx]);
+        else if (r == tx) v = make_double2(tre[r][tx], 0.0);
+        else v = make_double2(tre[tx][r], -tim[tx][r]);
+        o[(long long)I * n_m + J] = v;
+      }
+    }
+  }
+}
+
+}  // namespace
+
+cudaError_t chi0_f64_configure() {
+  return cudaFuncSetAttribute(chi0_f64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+}
+
+cudaError_t launch_chi0_f64(const Chi0F64Args& a, cudaStream_t s) {
+  if (a.n_pairs_padded <= 0 || a.n_tiles <= 0) return cudaSuccess;
+  dim3 grid((unsigned)(a.n_tiles * a.n_freq));
+  chi0_f64_kernel<<<grid, kThreads, SMEM_BYTES, s>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_finalize(const double* acc_re, const double* acc_im, int n_m, int n_m_pad, int n_freq,
+                            double inv_nk, double2* out, cudaStream_t s) {
+  const int nb = (n_m + 31) / 32;
+  dim3 grid(nb, nb, n_freq);
+  finalize_kernel<<<grid, 256, 0, s>>>(acc_re, acc_im, n_m, n_m_pad, inv_nk, out);
+  return cudaGetLastError();
+}
+
+}  // namespace qsgw

@@ -1,0 +1,520 @@
+// C-ABI layer of include/qsgw.h: context, argument validation, state machine, band-batch loop,
+// host-buffer driver.  All arithmetic of the path runs in the kernels of zmel_kernels.cu and
+// chi0_*_kernels.cu; there is no CPU fallback.
+#include "../../include/qsgw.h"
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "kernels.h"
+
+namespace {
+
+enum State { ST_CREATED = 0, ST_READY = 1, ST_Z_BUILT = 2 };
+
+thread_local std::string g_create_error;
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_tiled() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+inline long long round_up(long long x, long long m) { return (x + m - 1) / m * m; }
+
+}  // namespace
+
+struct qsgw_ctx {
+  // problem
+  int n_sites = 0, n_b = 0, n_m = 0, b_max = 0, n_freq = 0, n_k = 0;
+  int max_n_o = 0, max_n_u = 0, precision = 0;
+  double occ_tol = 1e-12;
+  std::vector<int> orb, pb;
+  std::vector<double> omega;
+  cudaStream_t stream = nullptr;
+  // derived
+  int ncg = 0, n_m_pad = 0, n_tiles = 0;
+  long long kpad = 0;
+  // device
+  int* d_pb_site = nullptr;
+  int* d_pb_off = nullptr;
+  int* d_orb_off = nullptr;
+  long long* d_p_off = nullptr;
+  int2* d_tiles = nullptr;
+  double* d_omega = nullptr;
+  double2* d_P = nullptr;
+  long long p_elems = 0;
+  double* d_zws = nullptr;
+  double* d_wtab = nullptr;
+  double* d_acc_re = nullptr;
+  double* d_acc_im = nullptr;
+  size_t device_bytes = 0;
+  CUtensorMap tmap_z;
+  // state
+  int state = ST_CREATED;
+  int last_n_o = 0, last_n_u = 0;
+  long long launches = 0, pairs = 0;
+  std::string err;
+
+  int fail(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof(buf), fmt, ap);
+    va_end(ap);
+    err = buf;
+    return code;
+  }
+  int cuda_fail(cudaError_t e, const char* what) {
+    return fail(QSGW_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+  }
+};
+
+namespace {
+
+template <typename T>
+cudaError_t dev_alloc(qsgw_ctx* c, T** p, size_t n) {
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T));
+  if (e == cudaSuccess) c->device_bytes += n * sizeof(T);
+  return e;
+}
+
+void free_all(qsgw_ctx* c) {
+  cudaFree(c->d_pb_site);
+  cudaFree(c->d_pb_off);
+  cudaFree(c->d_orb_off);
+  cudaFree(c->d_p_off);
+  cudaFree(c->d_tiles);
+  cudaFree(c->d_omega);
+  cudaFree(c->d_P);
+  cudaFree(c->d_zws);
+  cudaFree(c->d_wtab);
+  cudaFree(c->d_acc_re);
+  cudaFree(c->d_acc_im);
+}
+
+int create_fail(qsgw_ctx* c, int code, const std::string& msg) {
+  g_create_error = msg;
+  if (c) {
+    free_all(c);
+    delete c;
+  }
+  return code;
+}
+
+int validate_desc(const qsgw_desc* d, std::string& why) {
+  if (!d) { why = "desc is NULL"; return QSGW_ERR_INVALID_ARG; }
+  if (!d->h_orb_per_site || !d->h_pb_per_site || !d->h_omega) { why = "NULL array in desc"; return QSGW_ERR_INVALID_ARG; }
+  if (d->precision != QSGW_PREC_FP64 && d->precision != QSGW_PREC_MIXED) { why = "bad precision enum"; return QSGW_ERR_INVALID_ARG; }
+  if (d->n_sites < 1 || d->n_freq < 1 || d->n_k < 1 || d->max_n_o < 1 || d->max_n_u < 1) {
+    why = "non-positive extent in desc"; return QSGW_ERR_SHAPE;
+  }
+  for (int s = 0; s < d->n_sites; ++s)
+    if (d->h_orb_per_site[s] < 1 || d->h_pb_per_site[s] < 1) { why = "non-positive b_s or m_s"; return QSGW_ERR_SHAPE; }
+  for (int j = 0; j < d->n_freq; ++j) {
+    const double w = d->h_omega[j];
+    if (!(w >= 0.0) || (j > 0 && !(w > d->h_omega[j - 1]))) {
+      why = "omega must be >= 0 and strictly increasing"; return QSGW_ERR_SHAPE;
+    }
+  }
+  return QSGW_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* qsgw_version(void) { return "qsgw-chi0 0.1 (sm_100a)"; }
+const char* qsgw_last_create_error(void) { return g_create_error.c_str(); }
+const char* qsgw_last_error(const qsgw_ctx* ctx) { return ctx ? ctx->err.c_str() : "ctx is NULL"; }
+int64_t qsgw_kernel_launches(const qsgw_ctx* ctx) { return ctx ? ctx->launches : 0; }
+int64_t qsgw_pairs_accumulated(const qsgw_ctx* ctx) { return ctx ? ctx->pairs : 0; }
+size_t qsgw_device_bytes(const qsgw_ctx* ctx) { return ctx ? ctx->device_bytes : 0; }
+int32_t qsgw_n_m(const qsgw_ctx* ctx) { return ctx ? ctx->n_m : 0; }
+int32_t qsgw_n_b(const qsgw_ctx* ctx) { return ctx ? ctx->n_b : 0; }
+
+int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
+  g_create_error.clear();
+  if (!out) return create_fail(nullptr, QSGW_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  std::string why;
+  int rc = validate_desc(desc, why);
+  if (rc != QSGW_OK) return create_fail(nullptr, rc, why);
+  if (desc->precision == QSGW_PREC_MIXED)
+    return create_fail(nullptr, QSGW_ERR_UNSUPPORTED, "mixed precision is not built yet");
+
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return create_fail(nullptr, QSGW_ERR_UNSUPPORTED, std::string("no CUDA device: ") + cudaGetErrorString(e));
+  cudaDeviceProp prop;
+  e = cudaGetDeviceProperties(&prop, dev);
+  if (e != cudaSuccess) return create_fail(nullptr, QSGW_ERR_CUDA, cudaGetErrorString(e));
+  if (prop.major != 10) return create_fail(nullptr, QSGW_ERR_UNSUPPORTED, "kernels are built for sm_100a only");
+
+  qsgw_ctx* c = new (std::nothrow) qsgw_ctx();
+  if (!c) return create_fail(nullptr, QSGW_ERR_ALLOC, "host allocation failed");
+  c->stream = static_cast<cudaStream_t>(cuda_stream);
+  c->n_sites = desc->n_sites;
+  c->n_freq = desc->n_freq;
+  c->n_k = desc->n_k;
+  c->max_n_o = desc->max_n_o;
+  c->max_n_u = desc->max_n_u;
+  c->precision = desc->precision;
+  c->occ_tol = desc->occ_tol < 0 ? 1e-12 : desc->occ_tol;
+  c->orb.assign(desc->h_orb_per_site, desc->h_orb_per_site + desc->n_sites);
+  c->pb.assign(desc->h_pb_per_site, desc->h_pb_per_site + desc->n_sites);
+  c->omega.assign(desc->h_omega, desc->h_omega + desc->n_freq);
+
+  std::vector<int> orb_off(c->n_sites + 1, 0), pb_off(c->n_sites + 1, 0);
+  std::vector<long long> p_off(c->n_sites, 0);
+  long long pe = 0;
+  for (int s = 0; s < c->n_sites; ++s) {
+    orb_off[s + 1] = orb_off[s] + c->orb[s];
+    pb_off[s + 1] = pb_off[s] + c->pb[s];
+    p_off[s] = pe;
+    pe += (long long)c->pb[s] * c->orb[s] * c->orb[s];
+    if (c->orb[s] > c->b_max) c->b_max = c->orb[s];
+  }
+  c->n_b = orb_off[c->n_sites];
+  c->n_m = pb_off[c->n_sites];
+  c->p_elems = pe;
+  std::vector<int> pb_site(c->n_m);
+  for (int s = 0; s < c->n_sites; ++s)
+    for (int I = pb_off[s]; I < pb_off[s + 1]; ++I) pb_site[I] = s;
+
+  c->ncg = (c->n_m + qsgw::kCG - 1) / qsgw::kCG;
+  c->n_m_pad = (int)round_up(c->n_m, qsgw::kTile);
+  const long long max_pairs = (long long)c->max_n_o * c->max_n_u;
+  c->kpad = round_up(max_pairs, qsgw::kPairAlign);
+  const size_t z_bytes = (size_t)2 * c->ncg * c->kpad * qsgw::kCG * sizeof(double);
+  if (desc->workspace_bytes != 0 && z_bytes > desc->workspace_bytes) {
+    char buf[256];
+    snprintf(buf, sizeof(buf), "z workspace for %d x %d band pairs needs %zu bytes > workspace_bytes cap %zu; "
+             "pass smaller max_n_o/max_n_u", c->max_n_o, c->max_n_u, z_bytes, desc->workspace_bytes);
+    return create_fail(c, QSGW_ERR_ALLOC, buf);
+  }
+  const int nt = c->n_m_pad / qsgw::kTile;
+  std::vector<int2> tiles;
+  for (int tj = 0; tj < nt; ++tj)
+    for (int ti = 0; ti <= tj; ++ti) tiles.push_back(make_int2(ti, tj));
+  c->n_tiles = (int)tiles.size();
+
+#define QSGW_TRY_ALLOC(expr)                                                                     \
+  do {                                                                                           \
+    cudaError_t _e = (expr);                                                                     \
+    if (_e != cudaSuccess) {                                                                     \
+      cudaGetLastError();                                                                        \
+      return create_fail(c, QSGW_ERR_ALLOC, std::string("device allocation failed: ") + cudaGetErrorString(_e)); \
+    }                                                                                            \
+  } while (0)
+  const size_t acc_elems = (size_t)c->n_freq * c->n_m_pad * c->n_m_pad;
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_pb_site, (size_t)c->n_m));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_pb_off, (size_t)c->n_sites + 1));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_orb_off, (size_t)c->n_sites + 1));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_p_off, (size_t)c->n_sites));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_tiles, tiles.size()));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_omega, (size_t)c->n_freq));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_P, (size_t)c->p_elems));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zws, z_bytes / sizeof(double)));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab, (size_t)c->n_freq * c->kpad));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_acc_re, acc_elems));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_acc_im, acc_elems));
+#undef QSGW_TRY_ALLOC
+
+#define QSGW_TRY_CUDA(expr)                                                                      \
+  do {                                                                                           \
+    cudaError_t _e = (expr);                                                                     \
+    if (_e != cudaSuccess) return create_fail(c, QSGW_ERR_CUDA, std::string(#expr ": ") + cudaGetErrorString(_e)); \
+  } while (0)
+  cudaStream_t st = c->stream;
+  // small tables: synchronous copies from pageable host memory are fine at create time
+  QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_pb_site, pb_site.data(), sizeof(int) * c->n_m, cudaMemcpyHostToDevice, st));
+  QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_pb_off, pb_off.data(), sizeof(int) * (c->n_sites + 1), cudaMemcpyHostToDevice, st));
+  QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_orb_off, orb_off.data(), sizeof(int) * (c->n_sites + 1), cudaMemcpyHostToDevice, st));
+  QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_p_off, p_off.data(), sizeof(long long) * c->n_sites, cudaMemcpyHostToDevice, st));
+  QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_tiles, tiles.data(), sizeof(int2) * tiles.size(), cudaMemcpyHostToDevice, st));
+  QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_omega, c->omega.data(), sizeof(double) * c->n_freq, cudaMemcpyHostToDevice, st));
+  QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zws, 0, z_bytes, st));
+  QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wtab, 0, sizeof(double) * c->n_freq * c->kpad, st));
+  QSGW_TRY_CUDA(cudaMemsetAsync(c->d_acc_re, 0, sizeof(double) * acc_elems, st));
+  QSGW_TRY_CUDA(cudaMemsetAsync(c->d_acc_im, 0, sizeof(double) * acc_elems, st));
+  QSGW_TRY_CUDA(cudaStreamSynchronize(st));   // host vectors above go out of scope
+  QSGW_TRY_CUDA(qsgw::chi0_f64_configure());
+#undef QSGW_TRY_CUDA
+
+  EncodeTiledFn enc = get_encode_tiled();
+  if (!enc) return create_fail(c, QSGW_ERR_UNSUPPORTED, "cuTensorMapEncodeTiled not available from the driver");
+  {
+    const cuuint64_t gdim[4] = {(cuuint64_t)qsgw::kCG, (cuuint64_t)c->kpad, (cuuint64_t)c->ncg, 2};
+    const cuuint64_t gstr[3] = {(cuuint64_t)qsgw::kCG * 8, (cuuint64_t)c->kpad * qsgw::kCG * 8,
+                                (cuuint64_t)c->ncg * c->kpad * qsgw::kCG * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)qsgw::kCG, (cuuint32_t)qsgw::kChi0F64KP, 4, 2};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = enc(&c->tmap_z, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->d_zws, gdim, gstr, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+      char buf[128];
+      snprintf(buf, sizeof(buf), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+      return create_fail(c, QSGW_ERR_CUDA, buf);
+    }
+  }
+  c->state = ST_CREATED;
+  *out = c;
+  return QSGW_OK;
+}
+
+void qsgw_destroy(qsgw_ctx* ctx) {
+  if (!ctx) return;
+  cudaStreamSynchronize(ctx->stream);
+  free_all(ctx);
+  delete ctx;
+}
+
+int32_t qsgw_sync(qsgw_ctx* ctx) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  cudaError_t e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "cudaStreamSynchronize");
+  return QSGW_OK;
+}
+
+int32_t qsgw_set_product_tensor(qsgw_ctx* ctx, const void* d_P) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  if (!d_P) return ctx->fail(QSGW_ERR_INVALID_ARG, "d_P is NULL");
+  cudaError_t e = cudaMemcpyAsync(ctx->d_P, d_P, sizeof(double2) * ctx->p_elems, cudaMemcpyDeviceToDevice, ctx->stream);
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "copy of P");
+  if (ctx->state == ST_CREATED) ctx->state = ST_READY;
+  ctx->err.clear();
+  return QSGW_OK;
+}
+
+int32_t qsgw_reset(qsgw_ctx* ctx) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  const size_t acc_elems = (size_t)ctx->n_freq * ctx->n_m_pad * ctx->n_m_pad;
+  cudaError_t e = cudaMemsetAsync(ctx->d_acc_re, 0, sizeof(double) * acc_elems, ctx->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_acc_im, 0, sizeof(double) * acc_elems, ctx->stream);
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "reset");
+  if (ctx->state != ST_CREATED) ctx->state = ST_READY;
+  ctx->pairs = 0;
+  ctx->err.clear();
+  return QSGW_OK;
+}
+
+static int check_batch(qsgw_ctx* ctx, int n_o, int n_u) {
+  if (n_o < 1 || n_u < 1) return ctx->fail(QSGW_ERR_SHAPE, "band batch must be non-empty (n_o=%d, n_u=%d)", n_o, n_u);
+  if (n_o > ctx->max_n_o || n_u > ctx->max_n_u)
+    return ctx->fail(QSGW_ERR_SHAPE, "band batch %d x %d exceeds the declared maximum %d x %d", n_o, n_u,
+                     ctx->max_n_o, ctx->max_n_u);
+  return QSGW_OK;
+}
+
+int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const void* d_Ckq, int64_t ld_kq,
+                        int32_t n_begin, int32_t n_o, int32_t np_begin, int32_t n_u, void* d_z_out) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  if (ctx->state == ST_CREATED) return ctx->fail(QSGW_ERR_STATE, "set_product_tensor must precede zmel_build");
+  if (!d_Ck || !d_Ckq) return ctx->fail(QSGW_ERR_INVALID_ARG, "d_Ck / d_Ckq is NULL");
+  if (ld_k < ctx->n_b || ld_kq < ctx->n_b)
+    return ctx->fail(QSGW_ERR_INVALID_ARG, "leading dimension smaller than N_b=%d", ctx->n_b);
+  if (n_begin < 0 || np_begin < 0) return ctx->fail(QSGW_ERR_SHAPE, "negative band offset");
+  int rc = check_batch(ctx, n_o, n_u);
+  if (rc != QSGW_OK) return rc;
+
+  qsgw::ZmelArgs a;
+  a.st.n_sites = ctx->n_sites;
+  a.st.n_b = ctx->n_b;
+  a.st.n_m = ctx->n_m;
+  a.st.b_max = ctx->b_max;
+  a.st.d_pb_site = ctx->d_pb_site;
+  a.st.d_pb_off = ctx->d_pb_off;
+  a.st.d_orb_off = ctx->d_orb_off;
+  a.st.d_p_off = ctx->d_p_off;
+  a.P = ctx->d_P;
+  a.Ck = static_cast<const double2*>(d_Ck);
+  a.ld_k = ld_k;
+  a.Ckq = static_cast<const double2*>(d_Ckq);
+  a.ld_kq = ld_kq;
+  a.n_begin = n_begin;
+  a.n_o = n_o;
+  a.np_begin = np_begin;
+  a.n_u = n_u;
+  a.zws = ctx->d_zws;
+  a.kpad = ctx->kpad;
+  a.ncg = ctx->ncg;
+  cudaError_t e = qsgw::launch_zmel_f64(a, ctx->stream);
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "zmel kernel launch");
+  ctx->launches += 1;
+  if (d_z_out) {
+    e = qsgw::launch_z_export(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u,
+                              static_cast<double2*>(d_z_out), ctx->stream);
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "z export kernel launch");
+    ctx->launches += 1;
+  }
+  ctx->last_n_o = n_o;
+  ctx->last_n_u = n_u;
+  ctx->state = ST_Z_BUILT;
+  ctx->err.clear();
+  return QSGW_OK;
+}
+
+int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps_k, const double* d_f_k,
+                             const double* d_eps_kq, const double* d_f_kq, int32_t n_o, int32_t n_u) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  if (ctx->state == ST_CREATED) return ctx->fail(QSGW_ERR_STATE, "set_product_tensor must precede chi0_accumulate");
+  if (!d_eps_k || !d_f_k || !d_eps_kq || !d_f_kq) return ctx->fail(QSGW_ERR_INVALID_ARG, "NULL energy/occupation array");
+  int rc = check_batch(ctx, n_o, n_u);
+  if (rc != QSGW_OK) return rc;
+  const long long n_pairs = (long long)n_o * n_u;
+  cudaError_t e;
+  if (d_z) {
+    e = qsgw::launch_z_import(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, static_cast<const double2*>(d_z),
+                              ctx->stream);
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "z import kernel launch");
+    ctx->launches += 1;
+    ctx->last_n_o = n_o;
+    ctx->last_n_u = n_u;
+  } else {
+    if (ctx->state != ST_Z_BUILT) return ctx->fail(QSGW_ERR_STATE, "no z batch: call zmel_build first or pass d_z");
+    if (n_o != ctx->last_n_o || n_u != ctx->last_n_u)
+      return ctx->fail(QSGW_ERR_SHAPE, "batch %d x %d differs from the last zmel_build (%d x %d)", n_o, n_u,
+                       ctx->last_n_o, ctx->last_n_u);
+  }
+  const long long n_pad = round_up(n_pairs, qsgw::kPairAlign);
+  e = qsgw::launch_pair_weights(d_eps_k, d_f_k, d_eps_kq, d_f_kq, n_o, n_u, ctx->d_omega, ctx->n_freq, ctx->occ_tol,
+                                ctx->d_wtab, ctx->kpad, n_pad, ctx->stream);
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "pair weights kernel launch");
+  ctx->launches += 1;
+
+  qsgw::Chi0F64Args a;
+  a.tmap_z = ctx->tmap_z;
+  a.wtab = ctx->d_wtab;
+  a.kpad = ctx->kpad;
+  a.acc_re = ctx->d_acc_re;
+  a.acc_im = ctx->d_acc_im;
+  a.n_m_pad = ctx->n_m_pad;
+  a.n_freq = ctx->n_freq;
+  a.n_pairs_padded = n_pad;
+  a.d_tiles = ctx->d_tiles;
+  a.n_tiles = ctx->n_tiles;
+  e = qsgw::launch_chi0_f64(a, ctx->stream);
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 kernel launch");
+  ctx->launches += 1;
+  ctx->pairs += n_pairs;
+  ctx->state = ST_READY;   // the batch has been consumed
+  ctx->err.clear();
+  return QSGW_OK;
+}
+
+int32_t qsgw_chi0_add_kpoint(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const void* d_Ckq, int64_t ld_kq,
+                             const double* d_eps_k, const double* d_f_k, const double* d_eps_kq,
+                             const double* d_f_kq, int32_t n_o_total, int32_t n_u_total) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  if (n_o_total < 1 || n_u_total < 1) return ctx->fail(QSGW_ERR_SHAPE, "n_o_total and n_u_total must be positive");
+  if (!d_eps_k || !d_f_k || !d_eps_kq || !d_f_kq) return ctx->fail(QSGW_ERR_INVALID_ARG, "NULL energy/occupation array");
+  for (int n0 = 0; n0 < n_o_total; n0 += ctx->max_n_o) {
+    const int no = (n_o_total - n0 < ctx->max_n_o) ? n_o_total - n0 : ctx->max_n_o;
+    for (int u0 = 0; u0 < n_u_total; u0 += ctx->max_n_u) {
+      const int nu = (n_u_total - u0 < ctx->max_n_u) ? n_u_total - u0 : ctx->max_n_u;
+      int rc = qsgw_zmel_build(ctx, d_Ck, ld_k, d_Ckq, ld_kq, n0, no, u0, nu, nullptr);
+      if (rc != QSGW_OK) return rc;
+      rc = qsgw_chi0_accumulate(ctx, nullptr, d_eps_k + n0, d_f_k + n0, d_eps_kq + u0, d_f_kq + u0, no, nu);
+      if (rc != QSGW_OK) return rc;
+    }
+  }
+  return QSGW_OK;
+}
+
+int32_t qsgw_chi0_finalize(qsgw_ctx* ctx, void* d_chi0_out) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  if (ctx->state == ST_CREATED) return ctx->fail(QSGW_ERR_STATE, "nothing accumulated: set_product_tensor not called");
+  if (!d_chi0_out) return ctx->fail(QSGW_ERR_INVALID_ARG, "d_chi0_out is NULL");
+  cudaError_t e = qsgw::launch_finalize(ctx->d_acc_re, ctx->d_acc_im, ctx->n_m, ctx->n_m_pad, ctx->n_freq,
+                                        1.0 / (double)ctx->n_k, static_cast<double2*>(d_chi0_out), ctx->stream);
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "finalize kernel launch");
+  ctx->launches += 1;
+  ctx->err.clear();
+  return QSGW_OK;
+}
+
+int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h_Ck, const void* h_Ckq,
+                           const double* h_eps_k, const double* h_f_k, const double* h_eps_kq, const double* h_f_kq,
+                           int32_t n_o, int32_t n_u, void* h_chi0_out, int64_t* out_kernel_launches) {
+  g_create_error.clear();
+  if (!desc || !h_P || !h_Ck || !h_Ckq || !h_eps_k || !h_f_k || !h_eps_kq || !h_f_kq || !h_chi0_out) {
+    g_create_error = "NULL argument";
+    return QSGW_ERR_INVALID_ARG;
+  }
+  if (n_o < 1 || n_u < 1) { g_create_error = "n_o and n_u must be positive"; return QSGW_ERR_SHAPE; }
+  cudaStream_t st = nullptr;
+  cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+  if (e != cudaSuccess) { g_create_error = cudaGetErrorString(e); return QSGW_ERR_CUDA; }
+  qsgw_ctx* c = nullptr;
+  int rc = qsgw_create(desc, st, &c);
+  if (rc != QSGW_OK) { cudaStreamDestroy(st); return rc; }
+
+  const int nb = c->n_b, nm = c->n_m, nk = c->n_k;
+  const size_t ck_e = (size_t)n_o * nb, ckq_e = (size_t)n_u * nb;
+  double2 *dP = nullptr, *dCk[2] = {nullptr, nullptr}, *dCkq[2] = {nullptr, nullptr}, *dOut = nullptr;
+  double* dE[2] = {nullptr, nullptr};   // eps_k | f_k | eps_kq | f_kq
+  cudaEvent_t done[2] = {nullptr, nullptr};
+  const size_t e_len = 2 * (size_t)n_o + 2 * (size_t)n_u;
+  const size_t out_e = (size_t)c->n_freq * nm * nm;
+  auto cleanup = [&]() {
+    cudaFree(dP); cudaFree(dOut);
+    for (int i = 0; i < 2; ++i) { cudaFree(dCk[i]); cudaFree(dCkq[i]); cudaFree(dE[i]); if (done[i]) cudaEventDestroy(done[i]); }
+    qsgw_destroy(c);
+    cudaStreamDestroy(st);
+  };
+#define QSGW_H(expr)                                                                   \
+  do {                                                                                 \
+    cudaError_t _e = (expr);                                                           \
+    if (_e != cudaSuccess) { g_create_error = std::string(#expr ": ") + cudaGetErrorString(_e); cleanup(); return QSGW_ERR_CUDA; } \
+  } while (0)
+  QSGW_H(cudaMalloc(&dP, sizeof(double2) * c->p_elems));
+  QSGW_H(cudaMalloc(&dOut, sizeof(double2) * out_e));
+  for (int i = 0; i < 2; ++i) {
+    QSGW_H(cudaMalloc(&dCk[i], sizeof(double2) * ck_e));
+    QSGW_H(cudaMalloc(&dCkq[i], sizeof(double2) * ckq_e));
+    QSGW_H(cudaMalloc(&dE[i], sizeof(double) * e_len));
+    QSGW_H(cudaEventCreateWithFlags(&done[i], cudaEventDisableTiming));
+  }
+  QSGW_H(cudaMemcpyAsync(dP, h_P, sizeof(double2) * c->p_elems, cudaMemcpyHostToDevice, st));
+  rc = qsgw_set_product_tensor(c, dP);
+  if (rc != QSGW_OK) { g_create_error = c->err; cleanup(); return rc; }
+  for (int k = 0; k < nk; ++k) {
+    const int b = k & 1;
+    if (k >= 2) QSGW_H(cudaEventSynchronize(done[b]));   // buffer b free again (copies are stream-ordered anyway)
+    QSGW_H(cudaMemcpyAsync(dCk[b], static_cast<const double2*>(h_Ck) + (size_t)k * ck_e, sizeof(double2) * ck_e, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(dCkq[b], static_cast<const double2*>(h_Ckq) + (size_t)k * ckq_e, sizeof(double2) * ckq_e, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(dE[b], h_eps_k + (size_t)k * n_o, sizeof(double) * n_o, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(dE[b] + n_o, h_f_k + (size_t)k * n_o, sizeof(double) * n_o, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(dE[b] + 2 * n_o, h_eps_kq + (size_t)k * n_u, sizeof(double) * n_u, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(dE[b] + 2 * n_o + n_u, h_f_kq + (size_t)k * n_u, sizeof(double) * n_u, cudaMemcpyHostToDevice, st));
+    rc = qsgw_chi0_add_kpoint(c, dCk[b], nb, dCkq[b], nb, dE[b], dE[b] + n_o, dE[b] + 2 * n_o, dE[b] + 2 * n_o + n_u, n_o, n_u);
+    if (rc != QSGW_OK) { g_create_error = c->err; cleanup(); return rc; }
+    QSGW_H(cudaEventRecord(done[b], st));
+  }
+  rc = qsgw_chi0_finalize(c, dOut);
+  if (rc != QSGW_OK) { g_create_error = c->err; cleanup(); return rc; }
+  QSGW_H(cudaMemcpyAsync(h_chi0_out, dOut, sizeof(double2) * out_e, cudaMemcpyDeviceToHost, st));
+  QSGW_H(cudaStreamSynchronize(st));
+#undef QSGW_H
+  if (out_kernel_launches) *out_kernel_launches = c->launches;
+  cleanup();
+  return QSGW_OK;
+}
+
+}  // extern "C"
