@@ -1,0 +1,45 @@
+"""Full-size parity (the launch configuration bench.py times): sampled entries and the exact
+sketch chi0 @ V computed by the oracle without forming chi0."""
+import numpy as np
+import pytest
+
+import oracle
+from qsgw_synth import generate, get_config
+from gpu_helpers import run_cuda, sites_of
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+
+def _sampled_and_sketch(prob, spin, got, tol):
+    cfg = prob.cfg
+    sp = prob.spins[spin]
+    rng = np.random.default_rng(1234 + cfg.index)
+    n_m = cfg.n_m
+    V = (rng.standard_normal((n_m, 4)) + 1j * rng.standard_normal((n_m, 4))) / np.sqrt(2)
+    S = oracle.chi0_sketch_ref(sites_of(prob), sp.Ck, sp.Ckq, sp.eps_k, sp.f_k, sp.eps_kq, sp.f_kq,
+                               prob.omega, V, occ_tol=cfg.occ_tol)
+    num = np.linalg.norm((got @ V - S).reshape(len(prob.omega), -1), axis=1)
+    den = np.linalg.norm(S.reshape(len(prob.omega), -1), axis=1)
+    assert (num / den).max() <= tol, num / den
+    # sampled entries incl. diagonal, tile edges and the ragged tail; upper and lower triangle
+    rows = np.concatenate([rng.integers(0, n_m, 40), [0, n_m - 1, 63, 64, n_m - 1, 5]])
+    cols = np.concatenate([rng.integers(0, n_m, 40), [0, n_m - 1, 64, 63, 0, 5]])
+    E = oracle.chi0_entries_ref(sites_of(prob), sp.Ck, sp.Ckq, sp.eps_k, sp.f_k, sp.eps_kq, sp.f_kq,
+                                prob.omega, rows, cols, occ_tol=cfg.occ_tol)
+    scale = np.abs(E).max(axis=1, keepdims=True)
+    assert (np.abs(got[:, rows, cols] - E) / scale).max() <= tol
+
+
+def test_cfg2_full_size_fp64():
+    cfg = get_config(2)
+    prob = generate(cfg)
+    for spin in range(cfg.n_spin):
+        got = run_cuda(prob, spin=spin)
+        _sampled_and_sketch(prob, spin, got, 1e-11)
+
+
+def test_cfg4_full_size_fp64():
+    cfg = get_config(4)
+    prob = generate(cfg)
+    got = run_cuda(prob)
+    _sampled_and_sketch(prob, 0, got, 1e-11)
