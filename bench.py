@@ -1,0 +1,409 @@
+#!/usr/bin/env python
+"""bench.py -- chi0(q, i*omega) build throughput on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path over one synthetic workload: for every spin channel
+and k-point {qsgw_zmel_build, qsgw_chi0_accumulate} over all band batches, then
+qsgw_chi0_finalize.  Default workload: cfg 4 (superlattice-scale cell),
+the configuration the BASELINE.json targets are quoted on.
+
+  value      credited complex-arithmetic TFLOP/s (8 real flop per complex multiply-add; stage (a)
+             two-step count + stage (b) upper triangle over kept pairs only), inputs resident in
+             HBM, CUDA events on the launching stream, max over ranks.
+  e2e        same metric through qsgw_chi0_run_host: pinned HOST buffers in, HOST chi0 out.
+  roofline   stage (b) kernel: credited flop per launch / mean launch time (CUDA events recorded
+             by the library around each launch, inside the timed region) vs the tensor-pipe peak.
+  cpu_baseline  the oracle (NumPy/BLAS, FP64) on a bounded sample of the same workload.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--mode fp64|mixed|both]
+  python bench.py --impl reference ...      # times the oracle on the host cores
+Multi-GPU: the path does not shard in this build ("replicas only"): each rank runs
+the same workload; value = units of all ranks / max-over-ranks time; no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "chi0_build_complex_tflops"
+UNIT = "TFLOP/s"
+
+# Nominal dense B200 tensor peaks (guide: B200_PROFILING.md / blackwell_cuda_programming.md) used
+# only as RATIOS to the measured bf16 peak of MEASURED_PEAKS.json.
+NOMINAL_TF = {"bf16": 2250.0, "tf32": 1100.0, "f64": 40.0}
+
+
+# ----------------------------------------------------------------------------- bookkeeping
+def kept_pairs(cfg, prob, n_k):
+    """Band pairs that pass the occupation filter f_n (1-f_n') > occ_tol (an input property)."""
+    import numpy as np
+    tot = 0
+    for sp in prob.spins:
+        occ = sp.f_k[:n_k, :, None] * (1.0 - sp.f_kq[:n_k, None, :])
+        tot += int(np.count_nonzero(occ > cfg.occ_tol))
+    return tot
+
+
+def credited_flops(cfg, n_spin, n_k, n_freq, pairs_kept):
+    """(stage a, stage b) credited real flops of the job."""
+    a = 8.0 * cfg.stage_a_cmac() * n_k * n_spin
+    b = 8.0 * n_freq * pairs_kept * (cfg.n_m * (cfg.n_m + 1) // 2)
+    return a, b
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return {"bf16_burst": float(p["bf16_tflops"]), "bf16_sustained": float(p["bf16_tflops_sustained"]),
+                "source": "measured"}
+    return {"bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback"}
+
+
+def tensor_peak(dtype_key, sustained=True):
+    pk = load_peaks()
+    base = pk["bf16_sustained"] if sustained else pk["bf16_burst"]
+    return base * NOMINAL_TF[dtype_key] / NOMINAL_TF["bf16"], pk["source"]
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "200",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), \
+        int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def max_over_ranks(value, world, device=None):
+    """MAX of a python float over all ranks (identity at world == 1)."""
+    if world == 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+# ----------------------------------------------------------------------------- oracle legs
+def oracle_sample(cfg, prob, seconds_hint=20.0):
+    """Bounded sample of the workload for the CPU legs: (n_k_sample, freq indices)."""
+    # cost model: one k-point and one frequency is one (pairs x N_M)^H (pairs x N_M) ZGEMM
+    flop_kf = 8.0 * cfg.n_o * cfg.n_u * cfg.n_m * cfg.n_m
+    budget = seconds_hint * 150e9            # ~150 GF/s ZGEMM on 8 cores
+    n_units = max(1, int(budget / flop_kf))
+    n_f = min(cfg.n_freq, n_units)
+    n_k = max(1, min(cfg.n_k, n_units // n_f))
+    step = max(1, cfg.n_freq // n_f)
+    return n_k, list(range(0, cfg.n_freq, step))[:n_f]
+
+
+def run_oracle_sample(cfg, prob, n_k_s, fsel):
+    """One pass of the oracle, as it stands, over the sample.  Returns (seconds, credited flops)."""
+    import numpy as np
+    import oracle
+    sites = [prob.P_site(s) for s in range(cfg.n_sites)]
+    t0 = time.perf_counter()
+    for sp in prob.spins[:1]:
+        oracle.chi0_ref(sites, sp.Ck[:n_k_s], sp.Ckq[:n_k_s], sp.eps_k[:n_k_s], sp.f_k[:n_k_s],
+                        sp.eps_kq[:n_k_s], sp.f_kq[:n_k_s], prob.omega[fsel], occ_tol=cfg.occ_tol,
+                        n_k_norm=cfg.n_k)
+    dt = time.perf_counter() - t0
+    sp = prob.spins[0]
+    occ = sp.f_k[:n_k_s, :, None] * (1.0 - sp.f_kq[:n_k_s, None, :])
+    kept = int(np.count_nonzero(occ > cfg.occ_tol))
+    fa, fb = credited_flops(cfg, 1, n_k_s, len(fsel), kept)
+    return dt, fa + fb
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p.get("num_threads", 0) for p in threadpool_info() if p.get("user_api") == "blas"]
+        return max(n) if n else len(os.sched_getaffinity(0))
+    except Exception:
+        return len(os.sched_getaffinity(0))
+
+
+def sample_text(cfg, n_k_s, fsel):
+    return (f"{cfg.name}: spin 0, {n_k_s} of {cfg.n_k} k-points x {len(fsel)} of {cfg.n_freq} frequencies, "
+            f"full N_M={cfg.n_m} matrix, all {cfg.n_o}x{cfg.n_u} band pairs; credited flops as for the GPU")
+
+
+# ----------------------------------------------------------------------------- reference arm
+def main_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    from qsgw_synth import generate, get_config
+    cfg = get_config(args.config)
+    n_k_s, fsel = oracle_sample(cfg, None, seconds_hint=args.cpu_seconds)
+    prob = generate(cfg, n_k=n_k_s)
+    for _ in range(args.warmup):
+        run_oracle_sample(cfg, prob, n_k_s, fsel)
+    tot, flops = 0.0, 0.0
+    for _ in range(args.steps):
+        dt, fl = run_oracle_sample(cfg, prob, n_k_s, fsel)
+        tot += dt
+        flops += fl
+    value = flops / tot / 1e12
+    cores = blas_threads()
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": cfg.name, "mode": "oracle (NumPy/BLAS FP64) on host cores",
+                                            "step": "bounded sample of the workload"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": sample_text(cfg, n_k_s, fsel)},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------- CUDA arm
+def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
+    import numpy as np
+    import torch
+    import paper_2506_03477_b200 as q
+
+    dev = torch.device("cuda", local_rank)
+    n_spin, n_k, n_f = cfg.n_spin, cfg.n_k, cfg.n_freq
+    pairs = kept_pairs(cfg, prob, n_k)
+    fa, fb = credited_flops(cfg, n_spin, n_k, n_f, pairs)
+    flops_step = fa + fb
+
+    ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, n_k, args.max_n_o or cfg.n_o,
+                        args.max_n_u or cfg.n_u, precision=precision, occ_tol=cfg.occ_tol)
+    ctx.set_product_tensor(torch.from_numpy(prob.P).to(dev))
+    d_in = [[torch.from_numpy(a).to(dev) for a in (sp.Ck, sp.Ckq, sp.eps_k, sp.f_k, sp.eps_kq, sp.f_kq)]
+            for sp in prob.spins]
+    out = torch.empty((n_f, cfg.n_m, cfg.n_m), dtype=torch.complex128, device=dev)
+
+    def step():
+        for s in range(n_spin):
+            ctx.reset()
+            Ck, Ckq, ek, fk, ekq, fkq = d_in[s]
+            for k in range(n_k):
+                ctx.chi0_add_kpoint(Ck[k], Ckq[k], ek[k], fk[k], ekq[k], fkq[k])
+            ctx.chi0_finalize(out)
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize(dev)
+    ctx.set_stage_timing(True)
+    l0 = ctx.kernel_launches
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    torch.cuda.synchronize(dev)
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+    ev1.record()
+    torch.cuda.synchronize(dev)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = max_over_ranks(ev0.elapsed_time(ev1), world, dev)
+    launches = ctx.kernel_launches - l0
+    stage = {nm: ctx.stage_time_ms(i) for i, nm in enumerate(("zmel", "weights", "chi0", "finalize"))}
+    ctx.set_stage_timing(False)
+    ctx.destroy()
+    del d_in, out
+    torch.cuda.empty_cache()
+
+    value = world * args.steps * flops_step / (ms_total * 1e-3) / 1e12
+    chi_ms, chi_n = stage["chi0"]
+    # stage (b) kernel: credited flop per launch (one k-point and band batch, all frequencies)
+    ach = (fb * args.steps / max(chi_n, 1)) / (chi_ms / max(chi_n, 1) * 1e-3) / 1e12 if chi_n else None
+    dkey = "f64" if precision == q.PREC_FP64 else "tf32"
+    peak, src = tensor_peak(dkey, sustained=True)
+    roofline = {"bound": "tensor", "kernel": "chi0_f64_kernel" if dkey == "f64" else "chi0_tf32_kernel",
+                "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": (ach / peak) if ach else None,
+                "traffic": None,
+                "peak_source": f"{src} bf16 sustained x nominal {dkey}/bf16 ratio "
+                               f"({NOMINAL_TF[dkey]:g}/{NOMINAL_TF['bf16']:g})",
+                "avg_launch_ms": chi_ms / max(chi_n, 1), "launches_timed": chi_n,
+                "stage_ms_per_step": {nm: v[0] / args.steps for nm, v in stage.items()}}
+
+    # end to end through the host-buffer entry point (pinned host memory in and out)
+    e2e = None
+    if not args.no_e2e:
+        hp = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+        h_P = hp(prob.P)
+        h_in = [[hp(a) for a in (sp.Ck, sp.Ckq, sp.eps_k, sp.f_k, sp.eps_kq, sp.f_kq)] for sp in prob.spins]
+        h_out = torch.empty((n_f, cfg.n_m, cfg.n_m), dtype=torch.complex128).pin_memory().numpy()
+        h2d = n_spin * h_P.nbytes + sum(a.nbytes for sp in h_in for a in sp)
+        d2h = n_spin * h_out.nbytes
+
+        def e2e_step():
+            n = 0
+            for s in range(n_spin):
+                _, ln = q.chi0_run_host(cfg.orb_per_site, cfg.pb_per_site, prob.omega, h_P, *h_in[s],
+                                        args.max_n_o or cfg.n_o, args.max_n_u or cfg.n_u, precision=precision,
+                                        occ_tol=cfg.occ_tol, out=h_out)
+                n += ln
+            return n
+        e2e_step()
+        barrier()
+        n_e = max(1, min(args.steps, args.e2e_steps))
+        t0 = time.perf_counter()
+        for _ in range(n_e):
+            e2e_step()
+        dt = max_over_ranks(time.perf_counter() - t0, world, dev)
+        barrier()
+        e2e = {"value": world * n_e * flops_step / dt / 1e12, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * dt / n_e, "steps": n_e,
+               "api": "qsgw_chi0_run_host (pinned host buffers, H2D + all kernels + D2H inside the timed region)"}
+
+    return {"mode": mode_name, "value": value, "ms_per_step": ms_total / args.steps, "launches": launches,
+            "roofline": roofline, "e2e": e2e, "clocks": clocks, "flops_step": flops_step,
+            "flops_stage_a": fa, "flops_stage_b": fb, "pairs_kept": pairs}
+
+
+def main_cuda(args):
+    rank, local_rank, world = dist_env()
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    import paper_2506_03477_b200 as q
+    from paper_2506_03477_b200 import build as qbuild
+    if rank == 0:
+        qbuild.build()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    q.lib()
+    from qsgw_synth import generate, get_config
+    cfg = get_config(args.config)
+    prob = generate(cfg)
+
+    modes = {"fp64": [("fp64", q.PREC_FP64)], "mixed": [("mixed", q.PREC_MIXED)],
+             "both": [("fp64", q.PREC_FP64), ("mixed", q.PREC_MIXED)]}[args.mode]
+    if args.mode == "both" and cfg.precision == "mixed":
+        modes = modes[::-1]
+    res = []
+    for name, prec in modes:
+        try:
+            res.append(run_mode(args, cfg, prob, prec, name, rank, local_rank, world))
+        except q.QsgwError as e:
+            if e.code == 6 and len(modes) > 1:       # QSGW_ERR_UNSUPPORTED: mode not built
+                res.append({"mode": name, "unavailable": str(e)})
+            else:
+                raise
+    if rank != 0:
+        return 0
+    main = next(r for r in res if "value" in r)
+    line = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if main["mode"] == "fp64" else "tf32+f64acc",
+            "data": "synthetic",
+            "config": {"workload": cfg.name, "mode": main["mode"], "n_m": cfg.n_m, "n_b": cfg.n_b, "n_k": cfg.n_k,
+                       "n_spin": cfg.n_spin, "n_o": cfg.n_o, "n_u": cfg.n_u, "n_freq": cfg.n_freq,
+                       "pairs_kept": main["pairs_kept"], "credited_flop_per_step": main["flops_step"],
+                       "parallelism": "replicas only" if world > 1 else "1 gpu",
+                       "l2": "no flush needed: accumulator + z workspace per step far exceed the 126 MB L2"
+                             if cfg.n_m >= 600 else "working set fits L2 (latency-bound config)"},
+            "roofline": main["roofline"], "e2e": main["e2e"], "gpu_launches": main["launches"],
+            "clocks": main["clocks"]}
+    for r in res:
+        if r is not main:
+            line[r["mode"]] = r
+    if world == 1 and not args.no_cpu:
+        n_k_s, fsel = oracle_sample(cfg, prob, seconds_hint=args.cpu_seconds)
+        dt, fl = run_oracle_sample(cfg, prob, n_k_s, fsel)
+        line["cpu_baseline"] = {"value": fl / dt / 1e12, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+                                "sample": sample_text(cfg, n_k_s, fsel), "seconds": dt}
+    print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
+def parse_args(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--mode", default="both", choices=["fp64", "mixed", "both"])
+    ap.add_argument("--max-n-o", type=int, default=0, help="band batch (default: whole O side)")
+    ap.add_argument("--max-n-u", type=int, default=0, help="band batch (default: whole U side)")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    return ap.parse_args(argv)
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    sys.exit(main_reference(a) if a.impl == "reference" else main_cuda(a))

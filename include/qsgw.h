@@ -135,6 +135,16 @@ int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h
                            const double* h_eps_kq, const double* h_f_kq, int32_t n_o,
                            int32_t n_u, void* h_chi0_out, int64_t* out_kernel_launches);
 
+/* Per-stage device timing, for roofline measurement.  While enabled, every kernel launch of
+ * the path is bracketed by CUDA events on the context's stream (Eq. 8 / Eq. 14 stages:
+ * QSGW_STAGE_ZMEL, _WEIGHTS, _CHI0, _FINALIZE).  qsgw_stage_time_ms synchronises the stream,
+ * returns the summed event time (ms) and launch count of `stage` since the last
+ * qsgw_set_stage_timing call, and keeps accumulating.  Off by default (no events recorded). */
+enum { QSGW_STAGE_ZMEL = 0, QSGW_STAGE_WEIGHTS = 1, QSGW_STAGE_CHI0 = 2, QSGW_STAGE_FINALIZE = 3,
+       QSGW_N_STAGES = 4 };
+int32_t qsgw_set_stage_timing(qsgw_ctx* ctx, int32_t enable);
+int32_t qsgw_stage_time_ms(qsgw_ctx* ctx, int32_t stage, double* out_ms, int64_t* out_launches);
+
 /* Introspection (host side, no device work). */
 const char* qsgw_last_error(const qsgw_ctx* ctx);       /* "" if none; valid until next call   */
 const char* qsgw_last_create_error(void);               /* error text of a failed qsgw_create  */

@@ -12,6 +12,7 @@ from typing import Optional, Sequence
 from .build import LIB_PATH
 
 PREC_FP64, PREC_MIXED = 0, 1
+STAGE_ZMEL, STAGE_WEIGHTS, STAGE_CHI0, STAGE_FINALIZE = 0, 1, 2, 3
 _STATUS = {0: "QSGW_OK", 1: "QSGW_ERR_INVALID_ARG", 2: "QSGW_ERR_SHAPE", 3: "QSGW_ERR_STATE",
            4: "QSGW_ERR_ALLOC", 5: "QSGW_ERR_CUDA", 6: "QSGW_ERR_UNSUPPORTED"}
 
@@ -69,6 +70,10 @@ def lib() -> C.CDLL:
     for name in ("qsgw_kernel_launches", "qsgw_pairs_accumulated"):
         getattr(L, name).restype = i64
         getattr(L, name).argtypes = [vp]
+    L.qsgw_set_stage_timing.argtypes = [vp, i32]
+    L.qsgw_set_stage_timing.restype = i32
+    L.qsgw_stage_time_ms.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64)]
+    L.qsgw_stage_time_ms.restype = i32
     L.qsgw_device_bytes.restype = C.c_size_t
     L.qsgw_device_bytes.argtypes = [vp]
     L.qsgw_n_m.argtypes = [vp]
@@ -175,6 +180,15 @@ class Chi0Context:
 
     def sync(self):
         self._check(self._L.qsgw_sync(self._h))
+
+    def set_stage_timing(self, enable: bool):
+        self._check(self._L.qsgw_set_stage_timing(self._h, int(bool(enable))))
+
+    def stage_time_ms(self, stage: int):
+        """(summed event time in ms, launches) of `stage` since set_stage_timing; synchronises."""
+        ms, n = C.c_double(0.0), C.c_int64(0)
+        self._check(self._L.qsgw_stage_time_ms(self._h, int(stage), C.byref(ms), C.byref(n)))
+        return float(ms.value), int(n.value)
 
     @property
     def kernel_launches(self) -> int:

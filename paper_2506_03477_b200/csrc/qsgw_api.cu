@@ -69,6 +69,13 @@ struct qsgw_ctx {
   int last_n_o = 0, last_n_u = 0;
   long long launches = 0, pairs = 0;
   std::string err;
+  // per-stage event timing (qsgw_set_stage_timing)
+  bool timing = false;
+  struct EvPair { cudaEvent_t a, b; int stage; };
+  std::vector<EvPair> ev_pending;
+  std::vector<cudaEvent_t> ev_free;
+  double stage_ms[QSGW_N_STAGES] = {0, 0, 0, 0};
+  long long stage_n[QSGW_N_STAGES] = {0, 0, 0, 0};
 
   int fail(int code, const char* fmt, ...) {
     char buf[512];
@@ -94,6 +101,10 @@ cudaError_t dev_alloc(qsgw_ctx* c, T** p, size_t n) {
 }
 
 void free_all(qsgw_ctx* c) {
+  for (auto& p : c->ev_pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
+  for (auto e : c->ev_free) cudaEventDestroy(e);
+  c->ev_pending.clear();
+  c->ev_free.clear();
   cudaFree(c->d_pb_site);
   cudaFree(c->d_pb_off);
   cudaFree(c->d_orb_off);
@@ -106,6 +117,60 @@ void free_all(qsgw_ctx* c) {
   cudaFree(c->d_acc_re);
   cudaFree(c->d_acc_im);
 }
+
+cudaEvent_t ev_get(qsgw_ctx* c) {
+  if (!c->ev_free.empty()) {
+    cudaEvent_t e = c->ev_free.back();
+    c->ev_free.pop_back();
+    return e;
+  }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+
+// move finished event pairs into the per-stage sums; `block` waits for all of them
+void ev_harvest(qsgw_ctx* c, bool block) {
+  size_t keep = 0;
+  for (size_t i = 0; i < c->ev_pending.size(); ++i) {
+    qsgw_ctx::EvPair& p = c->ev_pending[i];
+    cudaError_t q = block ? cudaEventSynchronize(p.b) : cudaEventQuery(p.b);
+    if (q == cudaSuccess) {
+      float ms = 0.f;
+      if (cudaEventElapsedTime(&ms, p.a, p.b) == cudaSuccess) {
+        c->stage_ms[p.stage] += ms;
+        c->stage_n[p.stage] += 1;
+      }
+      c->ev_free.push_back(p.a);
+      c->ev_free.push_back(p.b);
+    } else {
+      if (q == cudaErrorNotReady) cudaGetLastError();
+      c->ev_pending[keep++] = p;
+    }
+  }
+  c->ev_pending.resize(keep);
+}
+
+// Brackets one kernel launch with events when stage timing is on.
+struct StageScope {
+  qsgw_ctx* c;
+  cudaEvent_t a = nullptr;
+  int stage;
+  StageScope(qsgw_ctx* ctx, int st) : c(ctx), stage(st) {
+    if (c->timing) {
+      if (c->ev_pending.size() > 4096) ev_harvest(c, false);
+      a = ev_get(c);
+      cudaEventRecord(a, c->stream);
+    }
+  }
+  ~StageScope() {
+    if (a) {
+      cudaEvent_t b = ev_get(c);
+      cudaEventRecord(b, c->stream);
+      c->ev_pending.push_back({a, b, stage});
+    }
+  }
+};
 
 int create_fail(qsgw_ctx* c, int code, const std::string& msg) {
   g_create_error = msg;
@@ -146,6 +211,26 @@ int64_t qsgw_pairs_accumulated(const qsgw_ctx* ctx) { return ctx ? ctx->pairs : 
 size_t qsgw_device_bytes(const qsgw_ctx* ctx) { return ctx ? ctx->device_bytes : 0; }
 int32_t qsgw_n_m(const qsgw_ctx* ctx) { return ctx ? ctx->n_m : 0; }
 int32_t qsgw_n_b(const qsgw_ctx* ctx) { return ctx ? ctx->n_b : 0; }
+
+int32_t qsgw_set_stage_timing(qsgw_ctx* ctx, int32_t enable) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  ev_harvest(ctx, true);
+  for (int s = 0; s < QSGW_N_STAGES; ++s) {
+    ctx->stage_ms[s] = 0.0;
+    ctx->stage_n[s] = 0;
+  }
+  ctx->timing = enable != 0;
+  return QSGW_OK;
+}
+
+int32_t qsgw_stage_time_ms(qsgw_ctx* ctx, int32_t stage, double* out_ms, int64_t* out_launches) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  if (stage < 0 || stage >= QSGW_N_STAGES) return ctx->fail(QSGW_ERR_INVALID_ARG, "bad stage %d", stage);
+  ev_harvest(ctx, true);
+  if (out_ms) *out_ms = ctx->stage_ms[stage];
+  if (out_launches) *out_launches = ctx->stage_n[stage];
+  return QSGW_OK;
+}
 
 int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   g_create_error.clear();
@@ -354,7 +439,11 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   a.zws = ctx->d_zws;
   a.kpad = ctx->kpad;
   a.ncg = ctx->ncg;
-  cudaError_t e = qsgw::launch_zmel_f64(a, ctx->stream);
+  cudaError_t e;
+  {
+    StageScope ts(ctx, QSGW_STAGE_ZMEL);
+    e = qsgw::launch_zmel_f64(a, ctx->stream);
+  }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "zmel kernel launch");
   ctx->launches += 1;
   if (d_z_out) {
@@ -393,8 +482,11 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
                        ctx->last_n_o, ctx->last_n_u);
   }
   const long long n_pad = round_up(n_pairs, qsgw::kPairAlign);
-  e = qsgw::launch_pair_weights(d_eps_k, d_f_k, d_eps_kq, d_f_kq, n_o, n_u, ctx->d_omega, ctx->n_freq, ctx->occ_tol,
-                                ctx->d_wtab, ctx->kpad, n_pad, ctx->stream);
+  {
+    StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
+    e = qsgw::launch_pair_weights(d_eps_k, d_f_k, d_eps_kq, d_f_kq, n_o, n_u, ctx->d_omega, ctx->n_freq,
+                                  ctx->occ_tol, ctx->d_wtab, ctx->kpad, n_pad, ctx->stream);
+  }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "pair weights kernel launch");
   ctx->launches += 1;
 
@@ -409,7 +501,10 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
   a.n_pairs_padded = n_pad;
   a.d_tiles = ctx->d_tiles;
   a.n_tiles = ctx->n_tiles;
-  e = qsgw::launch_chi0_f64(a, ctx->stream);
+  {
+    StageScope ts(ctx, QSGW_STAGE_CHI0);
+    e = qsgw::launch_chi0_f64(a, ctx->stream);
+  }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 kernel launch");
   ctx->launches += 1;
   ctx->pairs += n_pairs;
@@ -441,8 +536,12 @@ int32_t qsgw_chi0_finalize(qsgw_ctx* ctx, void* d_chi0_out) {
   if (!ctx) return QSGW_ERR_INVALID_ARG;
   if (ctx->state == ST_CREATED) return ctx->fail(QSGW_ERR_STATE, "nothing accumulated: set_product_tensor not called");
   if (!d_chi0_out) return ctx->fail(QSGW_ERR_INVALID_ARG, "d_chi0_out is NULL");
-  cudaError_t e = qsgw::launch_finalize(ctx->d_acc_re, ctx->d_acc_im, ctx->n_m, ctx->n_m_pad, ctx->n_freq,
-                                        1.0 / (double)ctx->n_k, static_cast<double2*>(d_chi0_out), ctx->stream);
+  cudaError_t e;
+  {
+    StageScope ts(ctx, QSGW_STAGE_FINALIZE);
+    e = qsgw::launch_finalize(ctx->d_acc_re, ctx->d_acc_im, ctx->n_m, ctx->n_m_pad, ctx->n_freq,
+                              1.0 / (double)ctx->n_k, static_cast<double2*>(d_chi0_out), ctx->stream);
+  }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "finalize kernel launch");
   ctx->launches += 1;
   ctx->err.clear();
