@@ -145,6 +145,14 @@ enum { QSGW_STAGE_ZMEL = 0, QSGW_STAGE_WEIGHTS = 1, QSGW_STAGE_CHI0 = 2, QSGW_ST
 int32_t qsgw_set_stage_timing(qsgw_ctx* ctx, int32_t enable);
 int32_t qsgw_stage_time_ms(qsgw_ctx* ctx, int32_t stage, double* out_ms, int64_t* out_launches);
 
+/* Roofline denominators measured on this device (MEASURED_PEAKS.json has no FP64 / TF32 tensor
+ * figure): an issue-rate loop of register-resident MMAs with no memory traffic, timed with CUDA
+ * events on a private stream (synchronous; a few tens of ms).  kind = QSGW_PEAK_FP64_MMA: FP64
+ * tensor pipe (DMMA.8x8x4).  *out_tflops = real TFLOP/s (2 flop per FMA).  Does no work of the
+ * method. */
+enum { QSGW_PEAK_FP64_MMA = 0, QSGW_PEAK_TF32_MMA = 1 };
+int32_t qsgw_probe_peak(int32_t kind, double* out_tflops, double* out_ms);
+
 /* Introspection (host side, no device work). */
 const char* qsgw_last_error(const qsgw_ctx* ctx);       /* "" if none; valid until next call   */
 const char* qsgw_last_create_error(void);               /* error text of a failed qsgw_create  */

@@ -74,6 +74,8 @@ def lib() -> C.CDLL:
     L.qsgw_set_stage_timing.restype = i32
     L.qsgw_stage_time_ms.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64)]
     L.qsgw_stage_time_ms.restype = i32
+    L.qsgw_probe_peak.argtypes = [i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    L.qsgw_probe_peak.restype = i32
     L.qsgw_device_bytes.restype = C.c_size_t
     L.qsgw_device_bytes.argtypes = [vp]
     L.qsgw_n_m.argtypes = [vp]
@@ -110,6 +112,19 @@ def _ptr(t, dtype=None):
     if not t.is_contiguous():
         raise ValueError("tensor must be contiguous")
     return C.c_void_p(t.data_ptr())
+
+
+PEAK_FP64_MMA, PEAK_TF32_MMA = 0, 1
+
+
+def probe_peak(kind: int = PEAK_FP64_MMA):
+    """qsgw_probe_peak: (TFLOP/s, ms) of the register-resident MMA issue-rate loop on this device."""
+    L = lib()
+    tf, ms = C.c_double(0.0), C.c_double(0.0)
+    rc = L.qsgw_probe_peak(int(kind), C.byref(tf), C.byref(ms))
+    if rc != 0:
+        raise QsgwError(rc, L.qsgw_last_create_error().decode())
+    return float(tf.value), float(ms.value)
 
 
 class Chi0Context:

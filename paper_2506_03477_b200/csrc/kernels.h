@@ -67,6 +67,9 @@ constexpr int kChi0F64KP = 16;  // pairs per pipeline stage (box rows of the ten
 cudaError_t launch_chi0_f64(const Chi0F64Args& a, cudaStream_t s);
 cudaError_t chi0_f64_configure();   // sets the dynamic shared-memory attribute once
 
+// issue-rate probes (probe_kernels.cu): measured MMA-pipe peaks for the roofline denominators
+cudaError_t probe_fp64_mma(cudaStream_t s, double* out_tflops, double* out_ms);
+
 cudaError_t launch_finalize(const double* acc_re, const double* acc_im, int n_m, int n_m_pad, int n_freq,
                             double inv_nk, double2* out, cudaStream_t s);
 

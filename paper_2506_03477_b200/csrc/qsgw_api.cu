@@ -212,6 +212,20 @@ size_t qsgw_device_bytes(const qsgw_ctx* ctx) { return ctx ? ctx->device_bytes :
 int32_t qsgw_n_m(const qsgw_ctx* ctx) { return ctx ? ctx->n_m : 0; }
 int32_t qsgw_n_b(const qsgw_ctx* ctx) { return ctx ? ctx->n_b : 0; }
 
+int32_t qsgw_probe_peak(int32_t kind, double* out_tflops, double* out_ms) {
+  g_create_error.clear();
+  if (!out_tflops) { g_create_error = "out_tflops is NULL"; return QSGW_ERR_INVALID_ARG; }
+  if (kind != QSGW_PEAK_FP64_MMA && kind != QSGW_PEAK_TF32_MMA) { g_create_error = "bad peak kind"; return QSGW_ERR_INVALID_ARG; }
+  cudaStream_t st = nullptr;
+  cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = cudaGetErrorString(e); return QSGW_ERR_UNSUPPORTED; }
+  if (kind == QSGW_PEAK_FP64_MMA) e = qsgw::probe_fp64_mma(st, out_tflops, out_ms);
+  else e = cudaErrorNotSupported;
+  cudaStreamDestroy(st);
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = cudaGetErrorString(e); return e == cudaErrorNotSupported ? QSGW_ERR_UNSUPPORTED : QSGW_ERR_CUDA; }
+  return QSGW_OK;
+}
+
 int32_t qsgw_set_stage_timing(qsgw_ctx* ctx, int32_t enable) {
   if (!ctx) return QSGW_ERR_INVALID_ARG;
   ev_harvest(ctx, true);
