@@ -286,7 +286,13 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
         peak_src = f"measured in this run: qsgw_probe_peak({dkey}) register/TMEM-resident MMA issue-rate loop"
     except q.QsgwError:
         peak, peak_src = ratio_peak, None
-    roofline = {"bound": "tensor", "kernel": "chi0_f64_kernel" if dkey == "f64" else "chi0_tf32_kernel",
+    # tensor-pipe flops the kernel executes per credited flop (full tiles, no padding counted):
+    # FP64 4M = 1; 3xTF32 = 3 products per term; single TF32 = 1
+    passes = {q.PREC_FP64: 1, q.PREC_MIXED: 3, q.PREC_MIXED_TF32X1: 1}[precision]
+    roofline = {"bound": "tensor", "kernel": "chi0_f64_kernel" if dkey == "f64" else f"chi0_tf32_kernel<{passes}>",
+                "tensor_products_per_term": passes,
+                "achieved_executed": (ach * passes) if ach else None,
+                "frac_executed": (ach * passes / peak) if ach else None,
                 "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": (ach / peak) if ach else None,
                 "traffic": None,
                 "peak_source": peak_src or f"{src} bf16 burst x nominal {dkey}/bf16 ratio",
@@ -354,7 +360,9 @@ def main_cuda(args):
     prob = generate(cfg, n_k=args.n_k or None)
 
     modes = {"fp64": [("fp64", q.PREC_FP64)], "mixed": [("mixed", q.PREC_MIXED)],
-             "both": [("fp64", q.PREC_FP64), ("mixed", q.PREC_MIXED)]}[args.mode]
+             "mixed_x1": [("mixed_x1", q.PREC_MIXED_TF32X1)],
+             "both": [("fp64", q.PREC_FP64), ("mixed", q.PREC_MIXED)],
+             "all": [("fp64", q.PREC_FP64), ("mixed", q.PREC_MIXED), ("mixed_x1", q.PREC_MIXED_TF32X1)]}[args.mode]
     if args.mode == "both" and cfg.precision == "mixed":
         modes = modes[::-1]
     res = []
@@ -371,7 +379,7 @@ def main_cuda(args):
     main = next(r for r in res if "value" in r)
     line = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if main["mode"] == "fp64" else "tf32+f64acc",
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if main["mode"] == "fp64" else "tf32 (z fp32) + f64 accumulate",
             "data": "synthetic",
             "config": {"workload": cfg.name, "mode": main["mode"], "n_m": cfg.n_m, "n_b": cfg.n_b, "n_k": cfg.n_k,
                        "n_spin": cfg.n_spin, "n_o": cfg.n_o, "n_u": cfg.n_u, "n_freq": cfg.n_freq,
@@ -405,7 +413,7 @@ def parse_args(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
-    ap.add_argument("--mode", default="both", choices=["fp64", "mixed", "both"])
+    ap.add_argument("--mode", default="both", choices=["fp64", "mixed", "mixed_x1", "both", "all"])
     ap.add_argument("--max-n-o", type=int, default=0, help="band batch (default: whole O side)")
     ap.add_argument("--max-n-u", type=int, default=0, help="band batch (default: whole U side)")
     ap.add_argument("--e2e-steps", type=int, default=2)

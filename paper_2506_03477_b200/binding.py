@@ -11,7 +11,7 @@ from typing import Optional, Sequence
 
 from .build import LIB_PATH
 
-PREC_FP64, PREC_MIXED = 0, 1
+PREC_FP64, PREC_MIXED, PREC_MIXED_TF32X1 = 0, 1, 2
 STAGE_ZMEL, STAGE_WEIGHTS, STAGE_CHI0, STAGE_FINALIZE = 0, 1, 2, 3
 _STATUS = {0: "QSGW_OK", 1: "QSGW_ERR_INVALID_ARG", 2: "QSGW_ERR_SHAPE", 3: "QSGW_ERR_STATE",
            4: "QSGW_ERR_ALLOC", 5: "QSGW_ERR_CUDA", 6: "QSGW_ERR_UNSUPPORTED"}

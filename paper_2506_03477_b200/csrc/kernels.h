@@ -5,6 +5,12 @@
 //       column group cg = I / 16 ("CG"), pair row p = n_local * n_u + n'_local, 16 doubles = 128 B.
 //       One 4-D TMA box {16, KP, 4, 2} then brings a 64-column x KP-pair tile of both planes into
 //       shared memory as [plane][cg][row][128 B] with the 128-byte swizzle.
+//   z workspace, mixed mode: float zws32[4 planes][n_m_pad][kpad]   (K-major: pair index contiguous)
+//       plane 0/1 = Re/Im of z in FP32.  planes 2/3: 3xTF32 mode = Re/Im of z minus its TF32
+//       truncation (the "lo" split part; the tensor core truncates plane 0/1 itself); 1xTF32 mode =
+//       Re/Im of z rounded to nearest TF32.  n_m_pad = ceil128(N_M); rows >= N_M stay zero.
+//       3-D TMA boxes {32 pairs, 128 rows, 2|4 planes} with the 128-byte swizzle give K-major
+//       UMMA operand tiles.  Weight table (mixed): float wtab32[n_freq][kpad].
 //   weight table:            double wtab[n_freq][kpad]        (zero beyond the batch's pairs)
 //   accumulators:            double acc_re/acc_im[n_freq][n_m_pad][n_m_pad], n_m_pad = ceil64(N_M);
 //       only tiles with tile_i <= tile_j are touched.
@@ -66,6 +72,36 @@ struct Chi0F64Args {
 constexpr int kChi0F64KP = 16;  // pairs per pipeline stage (box rows of the tensor map)
 cudaError_t launch_chi0_f64(const Chi0F64Args& a, cudaStream_t s);
 cudaError_t chi0_f64_configure();   // sets the dynamic shared-memory attribute once
+
+// ---- mixed mode (chi0_tf32_kernels.cu) -------------------------------------------------------------
+constexpr int kTileMx = 128;       // stage (b) CTA tile edge in mixed mode (UMMA M = N = 128)
+constexpr int kPairStage = 32;     // pairs per pipeline stage (one 128-byte swizzle row of floats)
+
+struct Chi0Tf32Args {
+  CUtensorMap tmap2;     // 3-D FLOAT32 {kpad, n_m_pad, 4}, box {32, 128, 2}, SWIZZLE_128B
+  CUtensorMap tmap4;     // same tensor, box {32, 128, 4}
+  const float* wtab32;   // [n_freq][kpad]
+  long long kpad;
+  double* acc_re;
+  double* acc_im;
+  int n_m_pad;           // multiple of 128
+  int n_freq;
+  int n_stages;          // ceil(n_pairs / 32)
+  const int2* d_tiles;   // 128x128 tiles, tile_i <= tile_j
+  int n_tiles;
+};
+cudaError_t chi0_tf32_configure();
+cudaError_t launch_chi0_tf32(const Chi0Tf32Args& a, int n_pass /*1 or 3*/, cudaStream_t s);
+
+// stage (a) with FP32 plane output (arithmetic in FP64, one rounding to FP32 on store)
+cudaError_t launch_zmel_mixed(const ZmelArgs& a, float* zws32, int n_m_pad, int split_lo, cudaStream_t s);
+cudaError_t launch_z_export32(const float* zws32, long long kpad, int n_m_pad, int n_m, long long n_pairs,
+                              double2* out, cudaStream_t s);
+cudaError_t launch_planes32_from_ws(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs,
+                                    float* zws32, int n_m_pad, int split_lo, cudaStream_t s);
+cudaError_t launch_weights_to_f32(const double* wtab, float* wtab32, long long kpad, long long n_pad, int n_freq,
+                                  cudaStream_t s);
+cudaError_t probe_tf32_mma(cudaStream_t s, double* out_tflops, double* out_ms);
 
 // issue-rate probes (probe_kernels.cu): measured MMA-pipe peaks for the roofline denominators
 cudaError_t probe_fp64_mma(cudaStream_t s, double* out_tflops, double* out_ms);

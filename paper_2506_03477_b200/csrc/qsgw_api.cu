@@ -60,6 +60,10 @@ struct qsgw_ctx {
   long long p_elems = 0;
   double* d_zws = nullptr;
   double* d_wtab = nullptr;
+  float* d_zws32 = nullptr;     // mixed mode: FP32 K-major planes (kernels.h)
+  float* d_wtab32 = nullptr;
+  int n_pass = 0;               // mixed mode: TF32 products per complex term (3 = 3xTF32, 1 = single)
+  CUtensorMap tmap2, tmap4;
   double* d_acc_re = nullptr;
   double* d_acc_im = nullptr;
   size_t device_bytes = 0;
@@ -114,6 +118,8 @@ void free_all(qsgw_ctx* c) {
   cudaFree(c->d_P);
   cudaFree(c->d_zws);
   cudaFree(c->d_wtab);
+  cudaFree(c->d_zws32);
+  cudaFree(c->d_wtab32);
   cudaFree(c->d_acc_re);
   cudaFree(c->d_acc_im);
 }
@@ -184,7 +190,7 @@ int create_fail(qsgw_ctx* c, int code, const std::string& msg) {
 int validate_desc(const qsgw_desc* d, std::string& why) {
   if (!d) { why = "desc is NULL"; return QSGW_ERR_INVALID_ARG; }
   if (!d->h_orb_per_site || !d->h_pb_per_site || !d->h_omega) { why = "NULL array in desc"; return QSGW_ERR_INVALID_ARG; }
-  if (d->precision != QSGW_PREC_FP64 && d->precision != QSGW_PREC_MIXED) { why = "bad precision enum"; return QSGW_ERR_INVALID_ARG; }
+  if (d->precision != QSGW_PREC_FP64 && d->precision != QSGW_PREC_MIXED && d->precision != QSGW_PREC_MIXED_TF32X1) { why = "bad precision enum"; return QSGW_ERR_INVALID_ARG; }
   if (d->n_sites < 1 || d->n_freq < 1 || d->n_k < 1 || d->max_n_o < 1 || d->max_n_u < 1) {
     why = "non-positive extent in desc"; return QSGW_ERR_SHAPE;
   }
@@ -220,7 +226,7 @@ int32_t qsgw_probe_peak(int32_t kind, double* out_tflops, double* out_ms) {
   cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = cudaGetErrorString(e); return QSGW_ERR_UNSUPPORTED; }
   if (kind == QSGW_PEAK_FP64_MMA) e = qsgw::probe_fp64_mma(st, out_tflops, out_ms);
-  else e = cudaErrorNotSupported;
+  else e = qsgw::probe_tf32_mma(st, out_tflops, out_ms);
   cudaStreamDestroy(st);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = cudaGetErrorString(e); return e == cudaErrorNotSupported ? QSGW_ERR_UNSUPPORTED : QSGW_ERR_CUDA; }
   return QSGW_OK;
@@ -253,9 +259,6 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   std::string why;
   int rc = validate_desc(desc, why);
   if (rc != QSGW_OK) return create_fail(nullptr, rc, why);
-  if (desc->precision == QSGW_PREC_MIXED)
-    return create_fail(nullptr, QSGW_ERR_UNSUPPORTED, "mixed precision is not built yet");
-
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return create_fail(nullptr, QSGW_ERR_UNSUPPORTED, std::string("no CUDA device: ") + cudaGetErrorString(e));
@@ -296,17 +299,22 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     for (int I = pb_off[s]; I < pb_off[s + 1]; ++I) pb_site[I] = s;
 
   c->ncg = (c->n_m + qsgw::kCG - 1) / qsgw::kCG;
-  c->n_m_pad = (int)round_up(c->n_m, qsgw::kTile);
+  const bool mixed = c->precision != QSGW_PREC_FP64;
+  c->n_pass = c->precision == QSGW_PREC_MIXED ? 3 : (c->precision == QSGW_PREC_MIXED_TF32X1 ? 1 : 0);
+  const int tile_edge = mixed ? qsgw::kTileMx : qsgw::kTile;
+  c->n_m_pad = (int)round_up(c->n_m, tile_edge);
   const long long max_pairs = (long long)c->max_n_o * c->max_n_u;
   c->kpad = round_up(max_pairs, qsgw::kPairAlign);
-  const size_t z_bytes = (size_t)2 * c->ncg * c->kpad * qsgw::kCG * sizeof(double);
+  const size_t z64_bytes = (size_t)2 * c->ncg * c->kpad * qsgw::kCG * sizeof(double);
+  const size_t z32_elems = mixed ? (size_t)4 * c->n_m_pad * c->kpad : 0;
+  const size_t z_bytes = z64_bytes + z32_elems * sizeof(float);
   if (desc->workspace_bytes != 0 && z_bytes > desc->workspace_bytes) {
     char buf[256];
     snprintf(buf, sizeof(buf), "z workspace for %d x %d band pairs needs %zu bytes > workspace_bytes cap %zu; "
              "pass smaller max_n_o/max_n_u", c->max_n_o, c->max_n_u, z_bytes, desc->workspace_bytes);
     return create_fail(c, QSGW_ERR_ALLOC, buf);
   }
-  const int nt = c->n_m_pad / qsgw::kTile;
+  const int nt = c->n_m_pad / tile_edge;
   std::vector<int2> tiles;
   for (int tj = 0; tj < nt; ++tj)
     for (int ti = 0; ti <= tj; ++ti) tiles.push_back(make_int2(ti, tj));
@@ -328,7 +336,11 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_tiles, tiles.size()));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_omega, (size_t)c->n_freq));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_P, (size_t)c->p_elems));
-  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zws, z_bytes / sizeof(double)));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zws, z64_bytes / sizeof(double)));
+  if (mixed) {
+    QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zws32, z32_elems));
+    QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab32, (size_t)c->n_freq * c->kpad));
+  }
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab, (size_t)c->n_freq * c->kpad));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_acc_re, acc_elems));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_acc_im, acc_elems));
@@ -347,7 +359,12 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_p_off, p_off.data(), sizeof(long long) * c->n_sites, cudaMemcpyHostToDevice, st));
   QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_tiles, tiles.data(), sizeof(int2) * tiles.size(), cudaMemcpyHostToDevice, st));
   QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_omega, c->omega.data(), sizeof(double) * c->n_freq, cudaMemcpyHostToDevice, st));
-  QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zws, 0, z_bytes, st));
+  QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zws, 0, z64_bytes, st));
+  if (mixed) {
+    QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zws32, 0, z32_elems * sizeof(float), st));
+    QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wtab32, 0, sizeof(float) * c->n_freq * c->kpad, st));
+    QSGW_TRY_CUDA(qsgw::chi0_tf32_configure());
+  }
   QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wtab, 0, sizeof(double) * c->n_freq * c->kpad, st));
   QSGW_TRY_CUDA(cudaMemsetAsync(c->d_acc_re, 0, sizeof(double) * acc_elems, st));
   QSGW_TRY_CUDA(cudaMemsetAsync(c->d_acc_im, 0, sizeof(double) * acc_elems, st));
@@ -370,6 +387,22 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
       char buf[128];
       snprintf(buf, sizeof(buf), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
       return create_fail(c, QSGW_ERR_CUDA, buf);
+    }
+  }
+  if (mixed) {
+    const cuuint64_t gdim[3] = {(cuuint64_t)c->kpad, (cuuint64_t)c->n_m_pad, 4};
+    const cuuint64_t gstr[2] = {(cuuint64_t)c->kpad * 4, (cuuint64_t)c->n_m_pad * c->kpad * 4};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    for (int np = 2; np <= 4; np += 2) {
+      const cuuint32_t box[3] = {(cuuint32_t)qsgw::kPairStage, (cuuint32_t)qsgw::kTileMx, (cuuint32_t)np};
+      CUresult r = enc(np == 2 ? &c->tmap2 : &c->tmap4, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, c->d_zws32, gdim, gstr, box,
+                       estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (r != CUDA_SUCCESS) {
+        char buf[128];
+        snprintf(buf, sizeof(buf), "cuTensorMapEncodeTiled (mixed, %d planes) failed with CUresult %d", np, (int)r);
+        return create_fail(c, QSGW_ERR_CUDA, buf);
+      }
     }
   }
   c->state = ST_CREATED;
@@ -456,12 +489,17 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   cudaError_t e;
   {
     StageScope ts(ctx, QSGW_STAGE_ZMEL);
-    e = qsgw::launch_zmel_f64(a, ctx->stream);
+    if (ctx->n_pass) e = qsgw::launch_zmel_mixed(a, ctx->d_zws32, ctx->n_m_pad, ctx->n_pass == 3 ? 1 : 0, ctx->stream);
+    else e = qsgw::launch_zmel_f64(a, ctx->stream);
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "zmel kernel launch");
-  ctx->launches += 1;
+  ctx->launches += ctx->n_pass ? 2 : 1;
   if (d_z_out) {
-    e = qsgw::launch_z_export(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u,
+    if (ctx->n_pass)
+      e = qsgw::launch_z_export32(ctx->d_zws32, ctx->kpad, ctx->n_m_pad, ctx->n_m, (long long)n_o * n_u,
+                                  static_cast<double2*>(d_z_out), ctx->stream);
+    else
+      e = qsgw::launch_z_export(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u,
                               static_cast<double2*>(d_z_out), ctx->stream);
     if (e != cudaSuccess) return ctx->cuda_fail(e, "z export kernel launch");
     ctx->launches += 1;
@@ -485,6 +523,11 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
   if (d_z) {
     e = qsgw::launch_z_import(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, static_cast<const double2*>(d_z),
                               ctx->stream);
+    if (e == cudaSuccess && ctx->n_pass) {
+      e = qsgw::launch_planes32_from_ws(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, ctx->d_zws32, ctx->n_m_pad,
+                                        ctx->n_pass == 3 ? 1 : 0, ctx->stream);
+      ctx->launches += 1;
+    }
     if (e != cudaSuccess) return ctx->cuda_fail(e, "z import kernel launch");
     ctx->launches += 1;
     ctx->last_n_o = n_o;
@@ -503,6 +546,36 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "pair weights kernel launch");
   ctx->launches += 1;
+  if (ctx->n_pass) {
+    const long long n_pad32 = round_up(n_pairs, qsgw::kPairStage);
+    {
+      StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
+      e = qsgw::launch_weights_to_f32(ctx->d_wtab, ctx->d_wtab32, ctx->kpad, n_pad32, ctx->n_freq, ctx->stream);
+    }
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "weight conversion kernel launch");
+    qsgw::Chi0Tf32Args m;
+    m.tmap2 = ctx->tmap2;
+    m.tmap4 = ctx->tmap4;
+    m.wtab32 = ctx->d_wtab32;
+    m.kpad = ctx->kpad;
+    m.acc_re = ctx->d_acc_re;
+    m.acc_im = ctx->d_acc_im;
+    m.n_m_pad = ctx->n_m_pad;
+    m.n_freq = ctx->n_freq;
+    m.n_stages = (int)(n_pad32 / qsgw::kPairStage);
+    m.d_tiles = ctx->d_tiles;
+    m.n_tiles = ctx->n_tiles;
+    {
+      StageScope ts(ctx, QSGW_STAGE_CHI0);
+      e = qsgw::launch_chi0_tf32(m, ctx->n_pass, ctx->stream);
+    }
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 (mixed) kernel launch");
+    ctx->launches += 2;
+    ctx->pairs += n_pairs;
+    ctx->state = ST_READY;
+    ctx->err.clear();
+    return QSGW_OK;
+  }
 
   qsgw::Chi0F64Args a;
   a.tmap_z = ctx->tmap_z;

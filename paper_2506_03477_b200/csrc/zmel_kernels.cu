@@ -167,6 +167,78 @@ __global__ void pair_weights_kernel(const double* __restrict__ eps_k, const doub
   }
 }
 
+// Mixed mode: FP64 z batch (column-group layout) -> FP32 K-major planes (kernels.h).  One block = one
+// column group (16 product functions) x 128 pairs, transposed through shared memory so that both the
+// reads ([p][16] doubles) and the writes (128 consecutive pairs of one I) are coalesced.
+//   split_lo = 1: planes 2/3 = z - trunc_tf32(z)   (3xTF32 split; the tensor core truncates planes 0/1)
+//   split_lo = 0: planes 2/3 = rna_tf32(z)         (single-pass TF32 operand)
+__global__ void __launch_bounds__(256) z_to_planes32_kernel(const double* __restrict__ zws, long long kpad, int ncg,
+                                                            int n_m, long long n_pairs, float* __restrict__ out,
+                                                            int n_m_pad, int split_lo) {
+  __shared__ float tx[kCG][129], ty[kCG][129];
+  const int cg = blockIdx.y;
+  const long long p0 = (long long)blockIdx.x * 128;
+  const long long plane = (long long)ncg * kpad * kCG;
+  const double* src = zws + ((long long)cg * kpad + p0) * kCG;
+  for (int idx = threadIdx.x; idx < 128 * kCG; idx += 256) {
+    const int pl = idx / kCG, col = idx % kCG;
+    float x = 0.f, y = 0.f;
+    if (p0 + pl < n_pairs) {
+      x = (float)src[idx];
+      y = (float)src[plane + idx];
+    }
+    tx[col][pl] = x;
+    ty[col][pl] = y;
+  }
+  __syncthreads();
+  const long long oplane = (long long)n_m_pad * kpad;
+  for (int idx = threadIdx.x; idx < 128 * kCG; idx += 256) {
+    const int col = idx / 128, pl = idx % 128;
+    const int I = cg * kCG + col;
+    if (I >= n_m || p0 + pl >= kpad) continue;
+    const float x = tx[col][pl], y = ty[col][pl];
+    float x2, y2;
+    if (split_lo) {
+      x2 = x - __uint_as_float(__float_as_uint(x) & 0xFFFFE000u);
+      y2 = y - __uint_as_float(__float_as_uint(y) & 0xFFFFE000u);
+    } else {
+      uint32_t rx, ry;
+      asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(rx) : "f"(x));
+      asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(ry) : "f"(y));
+      x2 = __uint_as_float(rx);
+      y2 = __uint_as_float(ry);
+    }
+    const long long o = (long long)I * kpad + p0 + pl;
+    out[o] = x;
+    out[oplane + o] = y;
+    out[2 * oplane + o] = x2;
+    out[3 * oplane + o] = y2;
+  }
+}
+
+__global__ void z_export32_kernel(const float* __restrict__ z32, long long kpad, int n_m_pad, int n_m,
+                                  long long n_pairs, double2* __restrict__ out) {
+  const long long total = n_pairs * n_m;
+  const long long oplane = (long long)n_m_pad * kpad;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total;
+       e += (long long)gridDim.x * blockDim.x) {
+    const long long p = e / n_m;
+    const int I = (int)(e - p * n_m);
+    const long long o = (long long)I * kpad + p;
+    out[e] = make_double2((double)z32[o], (double)z32[oplane + o]);
+  }
+}
+
+__global__ void weights_to_f32_kernel(const double* __restrict__ wtab, float* __restrict__ w32, long long kpad,
+                                      long long n_pad, int n_freq) {
+  const long long total = n_pad * n_freq;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total;
+       e += (long long)gridDim.x * blockDim.x) {
+    const long long j = e / n_pad, p = e - j * n_pad;
+    w32[j * kpad + p] = (float)wtab[j * kpad + p];
+  }
+}
+
 }  // namespace
 
 cudaError_t launch_zmel_f64(const ZmelArgs& a, cudaStream_t s) {
@@ -208,6 +280,35 @@ cudaError_t launch_pair_weights(const double* eps_k, const double* f_k, const do
                                 cudaStream_t s) {
   pair_weights_kernel<<<grid_for(n_pairs_padded, 128), 128, 0, s>>>(eps_k, f_k, eps_kq, f_kq, n_o, n_u, d_omega,
                                                                    n_freq, occ_tol, wtab, kpad, n_pairs_padded);
+  return cudaGetLastError();
+}
+
+// mixed mode: FP64 stage (a) into the FP64 workspace, then one conversion/transposition pass
+cudaError_t launch_zmel_mixed(const ZmelArgs& a, float* zws32, int n_m_pad, int split_lo, cudaStream_t s) {
+  cudaError_t e = launch_zmel_f64(a, s);
+  if (e != cudaSuccess) return e;
+  const long long n_pairs = (long long)a.n_o * a.n_u;
+  dim3 grid((unsigned)((a.kpad + 127) / 128), a.ncg);
+  z_to_planes32_kernel<<<grid, 256, 0, s>>>(a.zws, a.kpad, a.ncg, a.st.n_m, n_pairs, zws32, n_m_pad, split_lo);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_z_export32(const float* zws32, long long kpad, int n_m_pad, int n_m, long long n_pairs,
+                              double2* out, cudaStream_t s) {
+  z_export32_kernel<<<grid_for(n_pairs * n_m, 256), 256, 0, s>>>(zws32, kpad, n_m_pad, n_m, n_pairs, out);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_planes32_from_ws(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs,
+                                    float* zws32, int n_m_pad, int split_lo, cudaStream_t s) {
+  dim3 grid((unsigned)((kpad + 127) / 128), ncg);
+  z_to_planes32_kernel<<<grid, 256, 0, s>>>(zws, kpad, ncg, n_m, n_pairs, zws32, n_m_pad, split_lo);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_weights_to_f32(const double* wtab, float* wtab32, long long kpad, long long n_pad, int n_freq,
+                                  cudaStream_t s) {
+  weights_to_f32_kernel<<<grid_for(n_pad * n_freq, 256), 256, 0, s>>>(wtab, wtab32, kpad, n_pad, n_freq);
   return cudaGetLastError();
 }
 

@@ -1,0 +1,101 @@
+"""GPU parity of the mixed mode (FP32-complex z on the TF32 tensor pipe, FP64 accumulation) against
+the FP64 oracle on the same FP64 inputs.  Tolerance (BASELINE.json:north_star): relative Frobenius
+error per frequency <= 2e-5.  QSGW_PREC_MIXED is the 3xTF32 split; QSGW_PREC_MIXED_TF32X1 (one TF32
+product per term) is checked against its own error model."""
+import numpy as np
+import pytest
+
+import oracle
+from qsgw_synth import generate, get_config
+from gpu_helpers import rel_fro_per_freq, run_cuda, sites_of
+from test_gpu_parity import RAGGED, check_hermitian, oracle_chi
+
+pytestmark = pytest.mark.gpu
+
+TOL_MIXED = 2e-5
+MIXED, MIXED_X1 = 1, 2
+
+
+@pytest.mark.parametrize("idx", [0, 1])
+def test_full_config_mixed(idx):
+    prob = generate(get_config(idx))
+    got = run_cuda(prob, precision=MIXED)
+    err = rel_fro_per_freq(got, oracle_chi(prob))
+    assert err.max() <= TOL_MIXED, err
+    assert err.max() > 1e-12          # really the FP32 path, not the FP64 kernels
+    check_hermitian(got)
+
+
+def test_ragged_sites_and_pair_tail_mixed():
+    """N_M = 99 (one ragged 128-tile), 45 pairs per k (ragged 32-pair stage), unequal sites."""
+    prob = generate(RAGGED)
+    got = run_cuda(prob, precision=MIXED)
+    assert rel_fro_per_freq(got, oracle_chi(prob)).max() <= TOL_MIXED
+    check_hermitian(got)
+
+
+@pytest.mark.parametrize("mo,mu", [(2, 9), (5, 4), (1, 1)])
+def test_band_batching_mixed(mo, mu):
+    prob = generate(RAGGED)
+    got = run_cuda(prob, precision=MIXED, max_n_o=mo, max_n_u=mu)
+    assert rel_fro_per_freq(got, oracle_chi(prob)).max() <= TOL_MIXED
+
+
+def test_cfg3_reduced_k_both_spins_mixed():
+    """cfg 3 = the metal in mixed mode (occupation filter, both signs of D), 5 of 216 k-points."""
+    cfg = get_config(3)
+    prob = generate(cfg, n_k=5)
+    for spin in range(cfg.n_spin):
+        got = run_cuda(prob, spin=spin, precision=MIXED, n_k_norm=cfg.n_k)
+        ref = oracle_chi(prob, spin=spin, n_k_norm=cfg.n_k)
+        assert rel_fro_per_freq(got, ref).max() <= TOL_MIXED
+
+
+def test_cfg4_one_kpoint_mixed():
+    """cfg 4 extents (19 tile rows, 672 stages of 32 pairs, many drain windows), two frequencies
+    of the full 2400^2 oracle."""
+    cfg = get_config(4)
+    prob = generate(cfg, n_k=1)
+    got = run_cuda(prob, precision=MIXED, n_k_norm=cfg.n_k)
+    sp = prob.spins[0]
+    sel = [0, 9]
+    chi = oracle.chi0_ref(sites_of(prob), sp.Ck, sp.Ckq, sp.eps_k, sp.f_k, sp.eps_kq, sp.f_kq,
+                          prob.omega[sel], n_k_norm=cfg.n_k)
+    ref = oracle.hermitian_finalize_ref(chi)
+    assert rel_fro_per_freq(got[sel], ref).max() <= TOL_MIXED
+
+
+def test_single_pass_tf32_error_model():
+    """One TF32 product per term: error ~ 2.9e-4 * sqrt(N_M / K_eff); must stay within
+    3x of the model on cfg 1 and be far above the 3xTF32 error."""
+    prob = generate(get_config(1))
+    ref = oracle_chi(prob)
+    e1 = rel_fro_per_freq(run_cuda(prob, precision=MIXED_X1), ref).max()
+    e3 = rel_fro_per_freq(run_cuda(prob, precision=MIXED), ref).max()
+    assert e3 < e1 <= 3e-4, (e1, e3)
+
+
+def test_mixed_zmel_export_and_import():
+    import torch
+    import paper_2506_03477_b200 as q
+    prob = generate(RAGGED)
+    cfg, sp = prob.cfg, prob.spins[0]
+    ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, cfg.n_k, cfg.n_o, cfg.n_u, precision=MIXED)
+    ctx.set_product_tensor(torch.from_numpy(prob.P).cuda())
+    for k in range(cfg.n_k):
+        z = torch.empty((cfg.n_o, cfg.n_u, cfg.n_m), dtype=torch.complex128, device="cuda")
+        ctx.zmel_build(torch.from_numpy(sp.Ck[k]).cuda(), torch.from_numpy(sp.Ckq[k]).cuda(), 0, cfg.n_o, 0, cfg.n_u,
+                       d_z_out=z)
+        zref = oracle.zmel_ref(sites_of(prob), sp.Ck[k], sp.Ckq[k])
+        zg = z.cpu().numpy()
+        assert np.abs(zg - zref).max() <= 1e-7 * np.abs(zref).max()      # FP32 storage
+        assert np.array_equal(zg, zg.astype(np.complex64).astype(np.complex128))
+    ctx.reset()
+    for k in range(cfg.n_k):
+        zref = torch.from_numpy(oracle.zmel_ref(sites_of(prob), sp.Ck[k], sp.Ckq[k])).cuda()
+        ctx.chi0_accumulate(torch.from_numpy(sp.eps_k[k]).cuda(), torch.from_numpy(sp.f_k[k]).cuda(),
+                            torch.from_numpy(sp.eps_kq[k]).cuda(), torch.from_numpy(sp.f_kq[k]).cuda(),
+                            cfg.n_o, cfg.n_u, d_z=zref)
+    got = ctx.chi0_finalize().cpu().numpy()
+    assert rel_fro_per_freq(got, oracle_chi(prob)).max() <= TOL_MIXED
+    ctx.destroy()
