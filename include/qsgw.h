@@ -52,11 +52,14 @@ enum {
   QSGW_ERR_UNSUPPORTED = 6  /* no sm_100 device, or feature not built                   */
 };
 
-/* QSGW_PREC_MIXED: z stored and multiplied as FP32 complex on the TF32 tensor pipe with the 3xTF32 split
- *   (hi*hi + lo*hi + hi*lo: FP32-grade products), FP32 window sums, FP64 accumulation across batches and k.
- * QSGW_PREC_MIXED_TF32X1: same data path with ONE TF32 product per term (operands rounded to nearest
- *   TF32; relative Frobenius error ~ 3e-4 * sqrt(N_M / pairs summed)). */
-enum { QSGW_PREC_FP64 = 0, QSGW_PREC_MIXED = 1, QSGW_PREC_MIXED_TF32X1 = 2 };
+/* QSGW_PREC_MIXED: z held as FP32 complex and multiplied with FP32-grade products on the 5th-generation
+ *   tensor cores: every FP32 operand v (scaled by a power of two) is carried as fp16 pieces v = h + l
+ *   (22 significant bits) and a*b is formed as a_h*b_h + a_l*b_h + a_h*b_l by three exact FP16 MMAs
+ *   (tcgen05 kind::f16, twice the TF32 rate); FP32 window sums, FP64 accumulation across batches and k.
+ * QSGW_PREC_MIXED_TF32X3: the same split on the TF32 pipe (hi*hi + lo*hi + hi*lo), half the speed.
+ * QSGW_PREC_MIXED_TF32X1: ONE TF32 product per term (operands rounded to nearest TF32; relative
+ *   Frobenius error ~ 3e-4 * sqrt(N_M / pairs summed): above the 2e-5 bar on cfg 3/4). */
+enum { QSGW_PREC_FP64 = 0, QSGW_PREC_MIXED = 1, QSGW_PREC_MIXED_TF32X1 = 2, QSGW_PREC_MIXED_TF32X3 = 3 };
 
 /* Problem descriptor (host memory; copied by qsgw_create). */
 typedef struct {
@@ -67,7 +70,7 @@ typedef struct {
   const double* h_omega;         /* imaginary frequencies omega_j >= 0, strictly increasing    */
   int32_t n_k;                   /* N_k >= 1: the 1/N_k normalisation applied by finalize      */
   int32_t max_n_o, max_n_u;      /* largest band batch (n_o, n_u) any zmel_build call passes   */
-  int32_t precision;             /* QSGW_PREC_FP64 | QSGW_PREC_MIXED | QSGW_PREC_MIXED_TF32X1  */
+  int32_t precision;             /* QSGW_PREC_FP64 | QSGW_PREC_MIXED | QSGW_PREC_MIXED_TF32X*  */
   double occ_tol;                /* pair kept iff f_n*(1-f_n') > occ_tol; <0 selects 1e-12     */
   size_t workspace_bytes;        /* cap on the z workspace; 0 = no cap.  If max_n_o*max_n_u    */
                                  /* pairs do not fit, create fails with QSGW_ERR_ALLOC         */
@@ -152,10 +155,10 @@ int32_t qsgw_stage_time_ms(qsgw_ctx* ctx, int32_t stage, double* out_ms, int64_t
 /* Roofline denominators measured on this device (MEASURED_PEAKS.json has no FP64 / TF32 tensor
  * figure): an issue-rate loop of register-resident MMAs with no memory traffic, timed with CUDA
  * events on a private stream (synchronous; a few tens of ms).  kind = QSGW_PEAK_FP64_MMA: FP64
- * tensor pipe (DMMA.8x8x4); QSGW_PEAK_TF32_MMA: tcgen05.mma kind::tf32 128x128x8, A in TMEM, B in
- * shared memory.  *out_tflops = real TFLOP/s (2 flop per FMA).  Does no work of the
- * method. */
-enum { QSGW_PEAK_FP64_MMA = 0, QSGW_PEAK_TF32_MMA = 1 };
+ * tensor pipe (DMMA.8x8x4); QSGW_PEAK_TF32_MMA / QSGW_PEAK_F16_MMA: tcgen05.mma kind::tf32 128x128x8 /
+ * kind::f16 128x128x16, A in TMEM, B in shared memory.  *out_tflops = real TFLOP/s (2 flop per FMA).
+ * Does no work of the method. */
+enum { QSGW_PEAK_FP64_MMA = 0, QSGW_PEAK_TF32_MMA = 1, QSGW_PEAK_F16_MMA = 2 };
 int32_t qsgw_probe_peak(int32_t kind, double* out_tflops, double* out_ms);
 
 /* Introspection (host side, no device work). */

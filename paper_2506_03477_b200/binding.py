@@ -11,7 +11,7 @@ from typing import Optional, Sequence
 
 from .build import LIB_PATH
 
-PREC_FP64, PREC_MIXED, PREC_MIXED_TF32X1 = 0, 1, 2
+PREC_FP64, PREC_MIXED, PREC_MIXED_TF32X1, PREC_MIXED_TF32X3 = 0, 1, 2, 3
 STAGE_ZMEL, STAGE_WEIGHTS, STAGE_CHI0, STAGE_FINALIZE = 0, 1, 2, 3
 _STATUS = {0: "QSGW_OK", 1: "QSGW_ERR_INVALID_ARG", 2: "QSGW_ERR_SHAPE", 3: "QSGW_ERR_STATE",
            4: "QSGW_ERR_ALLOC", 5: "QSGW_ERR_CUDA", 6: "QSGW_ERR_UNSUPPORTED"}
@@ -114,7 +114,7 @@ def _ptr(t, dtype=None):
     return C.c_void_p(t.data_ptr())
 
 
-PEAK_FP64_MMA, PEAK_TF32_MMA = 0, 1
+PEAK_FP64_MMA, PEAK_TF32_MMA, PEAK_F16_MMA = 0, 1, 2
 
 
 def probe_peak(kind: int = PEAK_FP64_MMA):

@@ -1,0 +1,386 @@
+// Stage (b), mixed mode (default): acc_j[I,J] += sum_p conj(z[p,I]) w_j(p) z[p,J] for one 128x128 tile and
+// one frequency per CTA (Eq. 14; Alg. 1 lines 16-21) on the 5th-generation
+// tensor cores with FP32-grade products built from FP16 pieces: tcgen05.mma kind::f16, FP32 accumulators in
+// TMEM, FP64 accumulation across batches and k.
+//
+//   An FP32 value v (scaled by a power of two into the FP16 range) is carried as v = h + l with
+//   h = fp16(v), l = fp16(v - h): 22 significant bits.  With A = w_j * (x_I, y_I) and B = (x_J, y_J):
+//     a b ~= a_h b_h + a_l b_h + a_h b_l          (three exact FP16 products, the dropped a_l b_l is 2^-22)
+//     Re += A_x B_x + A_y B_y,     Im += A_x B_y - A_y B_x      ("4M"; the minus is the a_negate bit)
+//   = 12 MMAs of 128x128x16 per 16 band pairs, on the tensor pipe that runs at twice the TF32 rate (and
+//   about half the energy per product): 2x the throughput of the 3xTF32 split at the same accuracy.
+//
+//   z tiles ("hl16" planes, kernels.h) are K-major FP16: one 128-byte swizzled row = h[32 pairs] | l[32
+//   pairs], written to shared memory by TMA and read by the MMA as the B operand; the frequency-scaled
+//   operand A is formed in registers (w * (h + l), re-split) and stored to TENSOR MEMORY (tcgen05.st).
+//
+//   The CSZ CTAs of a thread-block cluster work on the same tile at CSZ consecutive frequencies: every z
+//   box is fetched from L2 once per cluster and multicast to all CTAs (the 16 frequency CTAs of a tile
+//   otherwise re-read the same boxes; at this MMA rate that is the ~6300 B/clk L2 limit, profiles/r01_mixed_*).
+//
+//   The tensor core accumulates FP32 with truncation (bias ~ -4e-8 x MMA steps into one accumulator on
+//   same-sign sums), so D is drained every WIN stages into FP32 register accumulators with round-to-nearest
+//   adds; those go to the FP64 accumulators in HBM once per launch, rescaled by 2^(-2S) / sigma_j.
+//
+// Roles (384 threads): warp 0 = TMA producer, warp 1 = MMA issuer (one thread) + TMEM allocator,
+// warps 4-11 = scale + drain ("SA") warps: thread <-> tile row I; warps 4-7 own Re, 8-11 own Im.
+#include <cuda_fp16.h>
+
+#include "kernels.h"
+#include "ptx.cuh"
+
+namespace qsgw {
+
+namespace {
+
+constexpr int kThreadsH = 384;
+constexpr int kPlaneTileH = 128 * 128;   // bytes of one 128-row x (32 h | 32 l) operand tile
+constexpr int kBoxBytes = 64 * 128;      // one TMA box: 64 rows x 128 B
+
+struct HCfg {
+  static constexpr int STAGES = 3;
+  static constexpr int B_BYTES = 2 * kPlaneTileH;
+  static constexpr int A_BYTES = 2 * kPlaneTileH;
+  static constexpr int W_BYTES = kPairStage * 4;
+  static constexpr int STAGE_BYTES = B_BYTES + A_BYTES + 1024;   // w slot padded: tiles stay 1024-B aligned
+  static constexpr int TSLOT_COLS = 64;                          // h_x, h_y, l_x, l_y: 16 columns each
+  static constexpr int TSLOTS = 4;
+  static constexpr int WIN = 8;                                  // stages per drain window (96 MMA steps)
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256 + 1024 /*align slack*/;
+};
+
+template <int CSZ>
+__global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_constant__ Chi0F16Args a) {
+  using C = HCfg;
+  extern __shared__ unsigned char smem_dyn[];
+  const uint32_t raw = smem_u32(smem_dyn);
+  const uint32_t base = (raw + 1023u) & ~1023u;
+  unsigned char* sm = smem_dyn + (base - raw);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::STAGES * C::STAGE_BYTES);
+  uint64_t* full = bars;
+  uint64_t* empty = full + C::STAGES;
+  uint64_t* a_full = empty + C::STAGES;
+  uint64_t* a_empty = a_full + C::TSLOTS;
+  uint64_t* d_full = a_empty + C::TSLOTS;
+  uint64_t* d_empty = d_full + 1;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(d_empty + 1);
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int j = blockIdx.x % a.n_freq;               // the CSZ CTAs of a cluster: same tile, consecutive j
+  const int2 tt = a.d_tiles[blockIdx.x / a.n_freq];
+  const bool need_a = (tt.x != tt.y);                // diagonal tile: the A source is the B tile
+  const int n_stages = a.n_stages;
+  const uint32_t rank = CSZ > 1 ? cluster_ctarank() : 0u;
+  constexpr uint16_t kMask = (uint16_t)((1u << CSZ) - 1u);
+
+  if (tid == 0) {
+    tma_prefetch_desc(&a.tmap);
+    for (int s = 0; s < C::STAGES; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], 9 * CSZ);   // (8 SA warps + the MMA commit) of every CTA of the cluster
+    }
+    for (int s = 0; s < C::TSLOTS; ++s) {
+      mbar_init(&a_full[s], 8);
+      mbar_init(&a_empty[s], 1);
+    }
+    mbar_init(d_full, 1);
+    mbar_init(d_empty, 8);
+    mbar_fence_init();
+  }
+  if (warp == 1) tmem_alloc(tmem_slot, 512);
+  tc_fence_before();
+  __syncthreads();
+  if (CSZ > 1) cluster_sync_all();     // every CTA's barriers exist before any remote arrive / multicast
+  tc_fence_after();
+  const uint32_t tbase = *tmem_slot;
+  const uint32_t d_re = tbase, d_im = tbase + 128, a_ring = tbase + 256;
+
+  if (warp < 4) {
+    setmaxnreg_dec<56>();
+    if (warp == 0 && lane == 0) {
+      // ------------------------------------------------------------------ TMA producer
+      const float* wrow = a.wtab32 + (long long)j * a.kpad;
+      const uint32_t bytes = C::B_BYTES + C::W_BYTES + (need_a ? C::A_BYTES : 0);
+      const int n_box = need_a ? 8 : 4;
+      for (int s = 0; s < n_stages; ++s) {
+        const int st = s % C::STAGES, u = s / C::STAGES;
+        if (u > 0) mbar_wait(&empty[st], (u - 1) & 1);
+        unsigned char* sb = sm + st * C::STAGE_BYTES;
+        mbar_arrive_expect_tx(&full[st], bytes);
+        // box i: operand (B | A source), plane (x | y), row half; box i is fetched by CTA i % CSZ
+        for (int i = (int)rank; i < n_box; i += CSZ) {
+          const int plane = (i >> 1) & 1, rh = i & 1, op = i >> 2;
+          unsigned char* dst = sb + op * C::B_BYTES + plane * kPlaneTileH + rh * kBoxBytes;
+          const int row0 = (op ? tt.x : tt.y) * kTileMx + rh * 64;
+          if (CSZ > 1) tma_load_3d_mc(dst, &a.tmap, &full[st], s * 64, row0, plane, kMask);
+          else tma_load_3d(dst, &a.tmap, &full[st], s * 64, row0, plane);
+        }
+        bulk_load_1d(sb + C::B_BYTES + C::A_BYTES, wrow + (long long)s * kPairStage, C::W_BYTES, &full[st]);
+      }
+    } else if (warp == 1 && lane == 0) {
+      // ------------------------------------------------------------------ MMA issuer
+      const uint32_t idesc = umma_idesc_f16(128, 128, 0), idesc_neg = umma_idesc_f16(128, 128, 1);
+      for (int s = 0; s < n_stages; ++s) {
+        const int st = s % C::STAGES, u = s / C::STAGES, ts = s % C::TSLOTS, tu = s / C::TSLOTS;
+        const bool win_first = (s % C::WIN) == 0;
+        if (win_first && s > 0) mbar_wait(d_empty, ((s / C::WIN) - 1) & 1);
+        mbar_wait(&full[st], u & 1);
+        mbar_wait(&a_full[ts], tu & 1);
+        tc_fence_after();
+        const uint32_t sb = base + st * C::STAGE_BYTES;
+        const uint64_t bx = umma_desc_k_sw128(sb), by = umma_desc_k_sw128(sb + kPlaneTileH);
+        const uint32_t ab = a_ring + ts * C::TSLOT_COLS;
+#pragma unroll
+        for (int g = 0; g < 2; ++g) {                       // 16 pairs = one K step of kind::f16
+          const uint32_t acc0 = (win_first && g == 0) ? 0u : 1u;
+          const uint64_t kh = (uint64_t)(2 * g);            // 16 halves = 32 B along K inside the swizzle row
+          const uint64_t kl = (uint64_t)(4 + 2 * g);        // the l half of the row starts at byte 64
+          const uint32_t ahx = ab + 8 * g, ahy = ab + 16 + 8 * g, alx = ab + 32 + 8 * g, aly = ab + 48 + 8 * g;
+          umma_f16_ts(d_re, ahx, bx + kh, idesc, acc0);
+          umma_f16_ts(d_im, ahx, by + kh, idesc, acc0);
+          umma_f16_ts(d_re, ahy, by + kh, idesc, 1u);
+          umma_f16_ts(d_im, ahy, bx + kh, idesc_neg, 1u);
+          umma_f16_ts(d_re, alx, bx + kh, idesc, 1u);
+          umma_f16_ts(d_im, alx, by + kh, idesc, 1u);
+          umma_f16_ts(d_re, aly, by + kh, idesc, 1u);
+          umma_f16_ts(d_im, aly, bx + kh, idesc_neg, 1u);
+          umma_f16_ts(d_re, ahx, bx + kl, idesc, 1u);
+          umma_f16_ts(d_im, ahx, by + kl, idesc, 1u);
+          umma_f16_ts(d_re, ahy, by + kl, idesc, 1u);
+          umma_f16_ts(d_im, ahy, bx + kl, idesc_neg, 1u);
+        }
+        if (CSZ > 1) umma_commit_mc(&empty[st], kMask);
+        else umma_commit(&empty[st]);
+        umma_commit(&a_empty[ts]);
+        if (((s + 1) % C::WIN) == 0 || s == n_stages - 1) umma_commit(d_full);
+      }
+    }
+  } else {
+    // -------------------------------------------------------------------- scale + drain warps
+    setmaxnreg_inc<224>();
+    const int q = warp & 3, h = (warp - 4) >> 2;       // TMEM lane quarter; pair half / Re-Im owner
+    const int row = 32 * q + lane;
+    const uint32_t lane_base = (uint32_t)(32 * q) << 16;
+    const uint32_t sw = (uint32_t)(row & 7);
+    float racc[128];
+#pragma unroll
+    for (int i = 0; i < 128; ++i) racc[i] = 0.f;
+    uint32_t empty_remote[CSZ];
+#pragma unroll
+    for (int r = 0; r < CSZ; ++r) empty_remote[r] = CSZ > 1 ? mapa_shared(smem_u32(&empty[0]), (uint32_t)r) : 0u;
+
+    auto drain = [&](int widx) {
+      mbar_wait(d_full, widx & 1);
+      tc_fence_after();
+      const uint32_t dcol = (h ? d_im : d_re) + lane_base;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        uint32_t v[32];
+        tmem_ld32(dcol + 32 * c, v);
+        tmem_wait_ld();
+#pragma unroll
+        for (int i = 0; i < 32; ++i) racc[32 * c + i] += __uint_as_float(v[i]);
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(d_empty);
+    };
+
+    for (int s = 0; s < n_stages; ++s) {
+      const int st = s % C::STAGES, u = s / C::STAGES, ts = s % C::TSLOTS, tu = s / C::TSLOTS;
+      mbar_wait(&full[st], u & 1);
+      if (tu > 0) mbar_wait(&a_empty[ts], (tu - 1) & 1);
+      tc_fence_after();
+      const uint32_t sb = base + st * C::STAGE_BYTES;
+      const uint32_t src = (need_a ? sb + C::B_BYTES : sb) + (uint32_t)row * 128u;
+      const uint32_t swp = sb + C::B_BYTES + C::A_BYTES + 64u * (uint32_t)h;   // this thread's 16 pairs
+      const uint32_t tdst = a_ring + ts * C::TSLOT_COLS + 8 * h + lane_base;
+      float w[16];
+#pragma unroll
+      for (int cc = 0; cc < 4; ++cc) {
+        const float4 t = ld_shared_f4(swp + 16 * cc);
+        w[4 * cc] = t.x; w[4 * cc + 1] = t.y; w[4 * cc + 2] = t.z; w[4 * cc + 3] = t.w;
+      }
+#pragma unroll
+      for (int xy = 0; xy < 2; ++xy) {
+        uint32_t hv[8], lv[8], ah[8], al[8];
+#pragma unroll
+        for (int cc = 0; cc < 2; ++cc) {
+          const uint4 th = ld_shared_u4(src + xy * kPlaneTileH + ((((uint32_t)(2 * h + cc)) ^ sw) << 4));
+          const uint4 tl = ld_shared_u4(src + xy * kPlaneTileH + ((((uint32_t)(4 + 2 * h + cc)) ^ sw) << 4));
+          hv[4 * cc] = th.x; hv[4 * cc + 1] = th.y; hv[4 * cc + 2] = th.z; hv[4 * cc + 3] = th.w;
+          lv[4 * cc] = tl.x; lv[4 * cc + 1] = tl.y; lv[4 * cc + 2] = tl.z; lv[4 * cc + 3] = tl.w;
+        }
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {                  // pairs 2e, 2e+1 of this thread's 16
+          const float2 zh = __half22float2(*reinterpret_cast<const __half2*>(&hv[e]));
+          const float2 zl = __half22float2(*reinterpret_cast<const __half2*>(&lv[e]));
+          const float a0 = w[2 * e] * (zh.x + zl.x), a1 = w[2 * e + 1] * (zh.y + zl.y);
+          const __half2 hh = __floats2half2_rn(a0, a1);
+          const float2 hf = __half22float2(hh);
+          const __half2 ll = __floats2half2_rn(a0 - hf.x, a1 - hf.y);
+          ah[e] = *reinterpret_cast<const uint32_t*>(&hh);
+          al[e] = *reinterpret_cast<const uint32_t*>(&ll);
+        }
+        tmem_st8(tdst + 16 * xy, ah);
+        tmem_st8(tdst + 32 + 16 * xy, al);
+      }
+      tmem_wait_st();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) {
+        mbar_arrive(&a_full[ts]);
+        if (CSZ > 1) {
+#pragma unroll
+          for (int r = 0; r < CSZ; ++r) mbar_arrive_cluster(empty_remote[r] + 8u * (uint32_t)st);
+        } else {
+          mbar_arrive(&empty[st]);
+        }
+      }
+      if (s >= 1 && (s % C::WIN) == 0) drain(s / C::WIN - 1);   // stage s-1 closed a window
+    }
+    drain((n_stages - 1) / C::WIN);
+
+    // FP32 window sums (in units 2^(2S) sigma_j) -> FP64 accumulators (exclusive owner of (tile, j))
+    const double sc = a.wscale[j] * exp2(-2.0 * (double)f16_scale_exp(*a.zmax));
+    const long long plane = (long long)a.n_m_pad * a.n_m_pad;
+    double* dst = (h ? a.acc_im : a.acc_re) + (long long)j * plane +
+                  (long long)(tt.x * kTileMx + row) * a.n_m_pad + tt.y * kTileMx;
+#pragma unroll
+    for (int c = 0; c < 64; ++c) {
+      double2 v = *reinterpret_cast<double2*>(dst + 2 * c);
+      v.x += sc * (double)racc[2 * c];
+      v.y += sc * (double)racc[2 * c + 1];
+      *reinterpret_cast<double2*>(dst + 2 * c) = v;
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (CSZ > 1) cluster_sync_all();     // no CTA leaves while a peer may still arrive on its barriers
+  if (warp == 1) tmem_dealloc(tbase, 512);
+}
+
+// Issue-rate probe of the FP16 tensor pipe: back-to-back 128x128x16 MMAs (A in TMEM, B in shared memory).
+__global__ void __launch_bounds__(128, 1) f16_peak_kernel(int iters) {
+  extern __shared__ unsigned char smem_dyn[];
+  const uint32_t raw = smem_u32(smem_dyn);
+  const uint32_t base = (raw + 1023u) & ~1023u;
+  unsigned char* sm = smem_dyn + (base - raw);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(sm + kPlaneTileH);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bar + 1);
+  const int tid = threadIdx.x, warp = tid >> 5;
+  for (int i = tid; i < kPlaneTileH / 2; i += 128) reinterpret_cast<__half*>(sm)[i] = __float2half(1.0f + 0.001f * (i & 255));
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    mbar_fence_init();
+  }
+  if (warp == 0) tmem_alloc(tmem_slot, 512);
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tbase = *tmem_slot;
+  uint32_t v[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    const __half2 t = __floats2half2_rn(0.5f + 0.01f * i, 0.25f + 0.01f * i);
+    v[i] = *reinterpret_cast<const uint32_t*>(&t);
+  }
+  tmem_st16(tbase + 256 + ((uint32_t)(32 * warp) << 16), v);
+  tmem_st16(tbase + 272 + ((uint32_t)(32 * warp) << 16), v);
+  tmem_wait_st();
+  tc_fence_before();
+  __syncthreads();
+  if (tid == 0) {
+    tc_fence_after();
+    const uint32_t idesc = umma_idesc_f16(128, 128, 0);
+    const uint64_t bd = umma_desc_k_sw128(base);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+      for (int g = 0; g < 4; ++g) {
+        umma_f16_ts(tbase, tbase + 256 + 8 * g, bd + (uint64_t)(2 * g), idesc, (it | g) ? 1u : 0u);
+        umma_f16_ts(tbase + 128, tbase + 256 + 8 * g, bd + (uint64_t)(2 * g), idesc, (it | g) ? 1u : 0u);
+      }
+    }
+    umma_commit(bar);
+    mbar_wait(bar, 0);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tbase, 512);
+}
+
+template <int CSZ>
+cudaError_t launch_cluster(const Chi0F16Args& a, cudaStream_t s) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(a.n_tiles * a.n_freq));
+  cfg.blockDim = dim3(kThreadsH);
+  cfg.dynamicSmemBytes = HCfg::SMEM_BYTES;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = CSZ;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, chi0_f16_kernel<CSZ>, a);
+}
+
+}  // namespace
+
+cudaError_t chi0_f16_configure() {
+  cudaError_t e = cudaFuncSetAttribute(chi0_f16_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(chi0_f16_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(chi0_f16_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(f16_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 20480);
+}
+
+cudaError_t launch_chi0_f16(const Chi0F16Args& a, int cluster, cudaStream_t s) {
+  if (a.n_stages <= 0 || a.n_tiles <= 0) return cudaSuccess;
+  if (cluster > 1 && a.n_freq % cluster != 0) cluster = (a.n_freq % 2 == 0) ? 2 : 1;
+  if (cluster >= 4) return launch_cluster<4>(a, s);
+  if (cluster >= 2) return launch_cluster<2>(a, s);
+  chi0_f16_kernel<1><<<dim3((unsigned)(a.n_tiles * a.n_freq)), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t probe_f16_mma(cudaStream_t s, double* out_tflops, double* out_ms) {
+  int dev = 0, n_sm = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) return e;
+  e = chi0_f16_configure();
+  if (e != cudaSuccess) return e;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  const int iters = 40000;
+  f16_peak_kernel<<<n_sm, 128, 20480, s>>>(iters / 4);
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0, s);
+    f16_peak_kernel<<<n_sm, 128, 20480, s>>>(iters);
+    cudaEventRecord(e1, s);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (e != cudaSuccess) return e;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const double flop = 2.0 * 128.0 * 128.0 * 16.0 * 8.0 * (double)iters * n_sm;
+  if (out_tflops) *out_tflops = flop / (best * 1e-3) / 1e12;
+  if (out_ms) *out_ms = best;
+  return cudaSuccess;
+}
+
+}  // namespace qsgw

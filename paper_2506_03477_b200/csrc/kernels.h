@@ -45,13 +45,14 @@ struct ZmelArgs {
   double* zws;           // FP64 workspace (see above)
   long long kpad;
   int ncg;
+  float* zmax = nullptr; // optional: atomicMax of |Re z|, |Im z| over the batch (FP16-split mixed mode)
 };
 
 cudaError_t launch_zmel_f64(const ZmelArgs& a, cudaStream_t s);
 cudaError_t launch_z_export(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs,
                             double2* out, cudaStream_t s);
 cudaError_t launch_z_import(double* zws, long long kpad, int ncg, int n_m, long long n_pairs,
-                            const double2* in, cudaStream_t s);
+                            const double2* in, float* zmax /*optional*/, cudaStream_t s);
 cudaError_t launch_pair_weights(const double* eps_k, const double* f_k, const double* eps_kq,
                                 const double* f_kq, int n_o, int n_u, const double* d_omega, int n_freq,
                                 double occ_tol, double* wtab, long long kpad, long long n_pairs_padded,
@@ -102,6 +103,36 @@ cudaError_t launch_planes32_from_ws(const double* zws, long long kpad, int ncg, 
 cudaError_t launch_weights_to_f32(const double* wtab, float* wtab32, long long kpad, long long n_pad, int n_freq,
                                   cudaStream_t s);
 cudaError_t probe_tf32_mma(cudaStream_t s, double* out_tflops, double* out_ms);
+
+// ---- mixed mode, FP16 split (chi0_f16_kernels.cu) ---------------------------------------------------
+//   z workspace "hl16": __half zhl[2 planes (Re,Im)][n_m_pad][kpad/32][64]: per product function I and
+//   32-pair stage one 128-byte row  h[32] | l[32],  v = fp32(z * 2^S) = h + l (h = fp16(v), l = fp16(v-h)),
+//   S = f16_scale_exp(*zmax) from the batch maximum.  3-D TMA boxes {64 halves, 64 rows, 1 plane} with the
+//   128-byte swizzle give K-major UMMA operand tiles.  wtab32[j][p] = fp32(w_j(p) / wscale[j]), wscale[j]
+//   a power of two with max_p |wtab32[j][p]| in (1/2, 1].
+struct Chi0F16Args {
+  CUtensorMap tmap;      // 3-D FLOAT16 {2*kpad, n_m_pad, 2}, box {64, 64, 1}, SWIZZLE_128B
+  const float* wtab32;   // [n_freq][kpad]
+  const double* wscale;  // [n_freq]
+  const float* zmax;     // batch maximum of |Re z|, |Im z|
+  long long kpad;
+  double* acc_re;
+  double* acc_im;
+  int n_m_pad;           // multiple of 128
+  int n_freq;
+  int n_stages;          // ceil(n_pairs / 32)
+  const int2* d_tiles;   // 128x128 tiles, tile_i <= tile_j
+  int n_tiles;
+};
+cudaError_t chi0_f16_configure();
+cudaError_t launch_chi0_f16(const Chi0F16Args& a, int cluster /*CTAs sharing a tile: 1, 2 or 4*/, cudaStream_t s);
+cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs, void* zhl,
+                             int n_m_pad, const float* zmax, cudaStream_t s);
+cudaError_t launch_z_export_hl16(const void* zhl, long long kpad, int n_m_pad, int n_m, long long n_pairs,
+                                 const float* zmax, double2* out, cudaStream_t s);
+cudaError_t launch_weights_scale_f32(const double* wtab, float* wtab32, double* wscale, long long kpad, long long n_pad,
+                                     int n_freq, cudaStream_t s);
+cudaError_t probe_f16_mma(cudaStream_t s, double* out_tflops, double* out_ms);
 
 // issue-rate probes (probe_kernels.cu): measured MMA-pipe peaks for the roofline denominators
 cudaError_t probe_fp64_mma(cudaStream_t s, double* out_tflops, double* out_ms);

@@ -5,6 +5,7 @@
 
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -62,8 +63,14 @@ struct qsgw_ctx {
   double* d_wtab = nullptr;
   float* d_zws32 = nullptr;     // mixed mode: FP32 K-major planes (kernels.h)
   float* d_wtab32 = nullptr;
-  int n_pass = 0;               // mixed mode: TF32 products per complex term (3 = 3xTF32, 1 = single)
+  int n_pass = 0;               // TF32 mixed modes: products per complex term (3 = 3xTF32, 1 = single)
   CUtensorMap tmap2, tmap4;
+  bool f16 = false;             // QSGW_PREC_MIXED: FP16-split planes (kernels.h "hl16")
+  void* d_zhl = nullptr;
+  double* d_wscale = nullptr;
+  float* d_zmax = nullptr;
+  int cluster = 1;              // CTAs of a cluster sharing one tile's z boxes (1, 2 or 4)
+  CUtensorMap tmap_h;
   double* d_acc_re = nullptr;
   double* d_acc_im = nullptr;
   size_t device_bytes = 0;
@@ -120,6 +127,9 @@ void free_all(qsgw_ctx* c) {
   cudaFree(c->d_wtab);
   cudaFree(c->d_zws32);
   cudaFree(c->d_wtab32);
+  cudaFree(c->d_zhl);
+  cudaFree(c->d_wscale);
+  cudaFree(c->d_zmax);
   cudaFree(c->d_acc_re);
   cudaFree(c->d_acc_im);
 }
@@ -190,7 +200,7 @@ int create_fail(qsgw_ctx* c, int code, const std::string& msg) {
 int validate_desc(const qsgw_desc* d, std::string& why) {
   if (!d) { why = "desc is NULL"; return QSGW_ERR_INVALID_ARG; }
   if (!d->h_orb_per_site || !d->h_pb_per_site || !d->h_omega) { why = "NULL array in desc"; return QSGW_ERR_INVALID_ARG; }
-  if (d->precision != QSGW_PREC_FP64 && d->precision != QSGW_PREC_MIXED && d->precision != QSGW_PREC_MIXED_TF32X1) { why = "bad precision enum"; return QSGW_ERR_INVALID_ARG; }
+  if (d->precision < QSGW_PREC_FP64 || d->precision > QSGW_PREC_MIXED_TF32X3) { why = "bad precision enum"; return QSGW_ERR_INVALID_ARG; }
   if (d->n_sites < 1 || d->n_freq < 1 || d->n_k < 1 || d->max_n_o < 1 || d->max_n_u < 1) {
     why = "non-positive extent in desc"; return QSGW_ERR_SHAPE;
   }
@@ -221,12 +231,13 @@ int32_t qsgw_n_b(const qsgw_ctx* ctx) { return ctx ? ctx->n_b : 0; }
 int32_t qsgw_probe_peak(int32_t kind, double* out_tflops, double* out_ms) {
   g_create_error.clear();
   if (!out_tflops) { g_create_error = "out_tflops is NULL"; return QSGW_ERR_INVALID_ARG; }
-  if (kind != QSGW_PEAK_FP64_MMA && kind != QSGW_PEAK_TF32_MMA) { g_create_error = "bad peak kind"; return QSGW_ERR_INVALID_ARG; }
+  if (kind < QSGW_PEAK_FP64_MMA || kind > QSGW_PEAK_F16_MMA) { g_create_error = "bad peak kind"; return QSGW_ERR_INVALID_ARG; }
   cudaStream_t st = nullptr;
   cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = cudaGetErrorString(e); return QSGW_ERR_UNSUPPORTED; }
   if (kind == QSGW_PEAK_FP64_MMA) e = qsgw::probe_fp64_mma(st, out_tflops, out_ms);
-  else e = qsgw::probe_tf32_mma(st, out_tflops, out_ms);
+  else if (kind == QSGW_PEAK_TF32_MMA) e = qsgw::probe_tf32_mma(st, out_tflops, out_ms);
+  else e = qsgw::probe_f16_mma(st, out_tflops, out_ms);
   cudaStreamDestroy(st);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = cudaGetErrorString(e); return e == cudaErrorNotSupported ? QSGW_ERR_UNSUPPORTED : QSGW_ERR_CUDA; }
   return QSGW_OK;
@@ -300,14 +311,20 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
 
   c->ncg = (c->n_m + qsgw::kCG - 1) / qsgw::kCG;
   const bool mixed = c->precision != QSGW_PREC_FP64;
-  c->n_pass = c->precision == QSGW_PREC_MIXED ? 3 : (c->precision == QSGW_PREC_MIXED_TF32X1 ? 1 : 0);
+  c->n_pass = c->precision == QSGW_PREC_MIXED_TF32X3 ? 3 : (c->precision == QSGW_PREC_MIXED_TF32X1 ? 1 : 0);
+  c->f16 = c->precision == QSGW_PREC_MIXED;
+  if (const char* ev = getenv("QSGW_F16_CLUSTER")) {   // tuning knob: CTAs per cluster sharing a tile (1, 2, 4)
+    const int v = atoi(ev);
+    if (v == 1 || v == 2 || v == 4) c->cluster = v;
+  }
   const int tile_edge = mixed ? qsgw::kTileMx : qsgw::kTile;
   c->n_m_pad = (int)round_up(c->n_m, tile_edge);
   const long long max_pairs = (long long)c->max_n_o * c->max_n_u;
   c->kpad = round_up(max_pairs, qsgw::kPairAlign);
   const size_t z64_bytes = (size_t)2 * c->ncg * c->kpad * qsgw::kCG * sizeof(double);
-  const size_t z32_elems = mixed ? (size_t)4 * c->n_m_pad * c->kpad : 0;
-  const size_t z_bytes = z64_bytes + z32_elems * sizeof(float);
+  const size_t z32_elems = c->n_pass ? (size_t)4 * c->n_m_pad * c->kpad : 0;
+  const size_t zhl_bytes = c->f16 ? (size_t)2 * c->n_m_pad * c->kpad * 2 * sizeof(uint16_t) : 0;
+  const size_t z_bytes = z64_bytes + z32_elems * sizeof(float) + zhl_bytes;
   if (desc->workspace_bytes != 0 && z_bytes > desc->workspace_bytes) {
     char buf[256];
     snprintf(buf, sizeof(buf), "z workspace for %d x %d band pairs needs %zu bytes > workspace_bytes cap %zu; "
@@ -337,9 +354,12 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_omega, (size_t)c->n_freq));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_P, (size_t)c->p_elems));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zws, z64_bytes / sizeof(double)));
-  if (mixed) {
-    QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zws32, z32_elems));
-    QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab32, (size_t)c->n_freq * c->kpad));
+  if (c->n_pass) QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zws32, z32_elems));
+  if (mixed) QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab32, (size_t)c->n_freq * c->kpad));
+  if (c->f16) {
+    QSGW_TRY_ALLOC(dev_alloc(c, reinterpret_cast<unsigned char**>(&c->d_zhl), zhl_bytes));
+    QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wscale, (size_t)c->n_freq));
+    QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zmax, (size_t)1));
   }
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab, (size_t)c->n_freq * c->kpad));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_acc_re, acc_elems));
@@ -360,10 +380,16 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_tiles, tiles.data(), sizeof(int2) * tiles.size(), cudaMemcpyHostToDevice, st));
   QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_omega, c->omega.data(), sizeof(double) * c->n_freq, cudaMemcpyHostToDevice, st));
   QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zws, 0, z64_bytes, st));
-  if (mixed) {
+  if (mixed) QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wtab32, 0, sizeof(float) * c->n_freq * c->kpad, st));
+  if (c->n_pass) {
     QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zws32, 0, z32_elems * sizeof(float), st));
-    QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wtab32, 0, sizeof(float) * c->n_freq * c->kpad, st));
     QSGW_TRY_CUDA(qsgw::chi0_tf32_configure());
+  }
+  if (c->f16) {
+    QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zhl, 0, zhl_bytes, st));
+    QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wscale, 0, sizeof(double) * c->n_freq, st));
+    QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zmax, 0, sizeof(float), st));
+    QSGW_TRY_CUDA(qsgw::chi0_f16_configure());
   }
   QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wtab, 0, sizeof(double) * c->n_freq * c->kpad, st));
   QSGW_TRY_CUDA(cudaMemsetAsync(c->d_acc_re, 0, sizeof(double) * acc_elems, st));
@@ -389,7 +415,21 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
       return create_fail(c, QSGW_ERR_CUDA, buf);
     }
   }
-  if (mixed) {
+  if (c->f16) {
+    const cuuint64_t gdim[3] = {(cuuint64_t)c->kpad * 2, (cuuint64_t)c->n_m_pad, 2};
+    const cuuint64_t gstr[2] = {(cuuint64_t)c->kpad * 4, (cuuint64_t)c->n_m_pad * c->kpad * 4};
+    const cuuint32_t box[3] = {64, 64, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = enc(&c->tmap_h, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, c->d_zhl, gdim, gstr, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+      char buf[128];
+      snprintf(buf, sizeof(buf), "cuTensorMapEncodeTiled (mixed, hl16 planes) failed with CUresult %d", (int)r);
+      return create_fail(c, QSGW_ERR_CUDA, buf);
+    }
+  }
+  if (c->n_pass) {
     const cuuint64_t gdim[3] = {(cuuint64_t)c->kpad, (cuuint64_t)c->n_m_pad, 4};
     const cuuint64_t gstr[2] = {(cuuint64_t)c->kpad * 4, (cuuint64_t)c->n_m_pad * c->kpad * 4};
     const cuuint32_t estr[3] = {1, 1, 1};
@@ -487,15 +527,26 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   a.kpad = ctx->kpad;
   a.ncg = ctx->ncg;
   cudaError_t e;
+  if (ctx->f16) {
+    a.zmax = ctx->d_zmax;
+    e = cudaMemsetAsync(ctx->d_zmax, 0, sizeof(float), ctx->stream);
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "reset of the batch maximum");
+  }
   {
     StageScope ts(ctx, QSGW_STAGE_ZMEL);
     if (ctx->n_pass) e = qsgw::launch_zmel_mixed(a, ctx->d_zws32, ctx->n_m_pad, ctx->n_pass == 3 ? 1 : 0, ctx->stream);
     else e = qsgw::launch_zmel_f64(a, ctx->stream);
+    if (e == cudaSuccess && ctx->f16)
+      e = qsgw::launch_z_to_hl16(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u, ctx->d_zhl,
+                                 ctx->n_m_pad, ctx->d_zmax, ctx->stream);
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "zmel kernel launch");
-  ctx->launches += ctx->n_pass ? 2 : 1;
+  ctx->launches += (ctx->n_pass || ctx->f16) ? 2 : 1;
   if (d_z_out) {
-    if (ctx->n_pass)
+    if (ctx->f16)
+      e = qsgw::launch_z_export_hl16(ctx->d_zhl, ctx->kpad, ctx->n_m_pad, ctx->n_m, (long long)n_o * n_u, ctx->d_zmax,
+                                     static_cast<double2*>(d_z_out), ctx->stream);
+    else if (ctx->n_pass)
       e = qsgw::launch_z_export32(ctx->d_zws32, ctx->kpad, ctx->n_m_pad, ctx->n_m, (long long)n_o * n_u,
                                   static_cast<double2*>(d_z_out), ctx->stream);
     else
@@ -521,8 +572,15 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
   const long long n_pairs = (long long)n_o * n_u;
   cudaError_t e;
   if (d_z) {
-    e = qsgw::launch_z_import(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, static_cast<const double2*>(d_z),
-                              ctx->stream);
+    e = ctx->f16 ? cudaMemsetAsync(ctx->d_zmax, 0, sizeof(float), ctx->stream) : cudaSuccess;
+    if (e == cudaSuccess)
+      e = qsgw::launch_z_import(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, static_cast<const double2*>(d_z),
+                                ctx->f16 ? ctx->d_zmax : nullptr, ctx->stream);
+    if (e == cudaSuccess && ctx->f16) {
+      e = qsgw::launch_z_to_hl16(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, ctx->d_zhl, ctx->n_m_pad,
+                                 ctx->d_zmax, ctx->stream);
+      ctx->launches += 1;
+    }
     if (e == cudaSuccess && ctx->n_pass) {
       e = qsgw::launch_planes32_from_ws(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, ctx->d_zws32, ctx->n_m_pad,
                                         ctx->n_pass == 3 ? 1 : 0, ctx->stream);
@@ -546,6 +604,38 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "pair weights kernel launch");
   ctx->launches += 1;
+  if (ctx->f16) {
+    const long long n_pad32 = round_up(n_pairs, qsgw::kPairStage);
+    {
+      StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
+      e = qsgw::launch_weights_scale_f32(ctx->d_wtab, ctx->d_wtab32, ctx->d_wscale, ctx->kpad, n_pad32, ctx->n_freq,
+                                         ctx->stream);
+    }
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "weight scaling kernel launch");
+    qsgw::Chi0F16Args m;
+    m.tmap = ctx->tmap_h;
+    m.wtab32 = ctx->d_wtab32;
+    m.wscale = ctx->d_wscale;
+    m.zmax = ctx->d_zmax;
+    m.kpad = ctx->kpad;
+    m.acc_re = ctx->d_acc_re;
+    m.acc_im = ctx->d_acc_im;
+    m.n_m_pad = ctx->n_m_pad;
+    m.n_freq = ctx->n_freq;
+    m.n_stages = (int)(n_pad32 / qsgw::kPairStage);
+    m.d_tiles = ctx->d_tiles;
+    m.n_tiles = ctx->n_tiles;
+    {
+      StageScope ts(ctx, QSGW_STAGE_CHI0);
+      e = qsgw::launch_chi0_f16(m, ctx->cluster, ctx->stream);
+    }
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 (mixed, FP16 split) kernel launch");
+    ctx->launches += 2;
+    ctx->pairs += n_pairs;
+    ctx->state = ST_READY;
+    ctx->err.clear();
+    return QSGW_OK;
+  }
   if (ctx->n_pass) {
     const long long n_pad32 = round_up(n_pairs, qsgw::kPairStage);
     {

@@ -1,6 +1,9 @@
 // Stage (a): muffin-tin product-basis matrix elements (Eq. 8 with Eq. 4), plus
 // the export/import of the z batch in the boundary layout and the pair-weight table (Eq. 14).
+#include <cuda_fp16.h>
+
 #include "kernels.h"
+#include "ptx.cuh"
 
 namespace qsgw {
 
@@ -32,6 +35,7 @@ __global__ void __launch_bounds__(kZmelThreads) zmel_kernel(ZmelArgs a) {
   T* zx = reinterpret_cast<T*>(a.zws);
   const long long plane = (long long)a.ncg * a.kpad * kCG;
   T* zy = zx + plane;
+  float zmx = 0.f;     // max |Re z|, |Im z| of this thread (FP16-split mixed mode: batch scale)
 
   int I = I0;
   while (I < I1) {
@@ -102,12 +106,18 @@ __global__ void __launch_bounds__(kZmelThreads) zmel_kernel(ZmelArgs a) {
             const long long off = ((long long)cg * a.kpad + pair) * kCG + col;
             zx[off] = ar[n];
             zy[off] = ai[n];
+            zmx = fmaxf(zmx, fmaxf(fabsf((float)ar[n]), fabsf((float)ai[n])));
           }
         }
       }
     }
     __syncthreads();
     I = seg_end;
+  }
+  if (a.zmax) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) zmx = fmaxf(zmx, __shfl_xor_sync(0xffffffffu, zmx, o));
+    if ((tid & 31) == 0 && zmx > 0.f) atomicMax(reinterpret_cast<unsigned int*>(a.zmax), __float_as_uint(zmx));
   }
 }
 
@@ -125,9 +135,10 @@ __global__ void z_export_kernel(const double* __restrict__ zws, long long kpad, 
 }
 
 __global__ void z_import_kernel(double* __restrict__ zws, long long kpad, int ncg, int n_m, long long n_pairs,
-                                const double2* __restrict__ in) {
+                                const double2* __restrict__ in, float* __restrict__ zmax) {
   const long long total = n_pairs * n_m;
   const long long plane = (long long)ncg * kpad * kCG;
+  float zmx = 0.f;
   for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total;
        e += (long long)gridDim.x * blockDim.x) {
     const long long p = e / n_m;
@@ -136,6 +147,12 @@ __global__ void z_import_kernel(double* __restrict__ zws, long long kpad, int nc
     const double2 v = in[e];
     zws[off] = v.x;
     zws[plane + off] = v.y;
+    zmx = fmaxf(zmx, fmaxf(fabsf((float)v.x), fabsf((float)v.y)));
+  }
+  if (zmax) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) zmx = fmaxf(zmx, __shfl_xor_sync(0xffffffffu, zmx, o));
+    if ((threadIdx.x & 31) == 0 && zmx > 0.f) atomicMax(reinterpret_cast<unsigned int*>(zmax), __float_as_uint(zmx));
   }
 }
 
@@ -239,6 +256,87 @@ __global__ void weights_to_f32_kernel(const double* __restrict__ wtab, float* __
   }
 }
 
+// Mixed mode, FP16 split: FP64 z batch (column-group layout) -> "hl16" planes (kernels.h): per product
+// function I and 32-pair stage one 128-byte row  h[32] | l[32]  with v = fp32(z * 2^S), h = fp16(v),
+// l = fp16(v - h);  S = f16_scale_exp(max |z| of the batch) keeps every h below 2^14.  Same transposition
+// through shared memory as z_to_planes32_kernel; rows of pairs beyond the batch are written as zeros.
+__global__ void __launch_bounds__(256) z_to_hl16_kernel(const double* __restrict__ zws, long long kpad, int ncg,
+                                                        int n_m, long long n_pairs, __half* __restrict__ out,
+                                                        int n_m_pad, const float* __restrict__ zmax) {
+  __shared__ float tx[kCG][129], ty[kCG][129];
+  const int cg = blockIdx.y;
+  const long long p0 = (long long)blockIdx.x * 128;
+  const long long plane = (long long)ncg * kpad * kCG;
+  const double scale = exp2((double)f16_scale_exp(*zmax));
+  const double* src = zws + ((long long)cg * kpad + p0) * kCG;
+  for (int idx = threadIdx.x; idx < 128 * kCG; idx += 256) {
+    const int pl = idx / kCG, col = idx % kCG;
+    float x = 0.f, y = 0.f;
+    if (p0 + pl < n_pairs) {
+      x = (float)(src[idx] * scale);
+      y = (float)(src[plane + idx] * scale);
+    }
+    tx[col][pl] = x;
+    ty[col][pl] = y;
+  }
+  __syncthreads();
+  const long long oplane = (long long)n_m_pad * kpad * 2;     // halves per plane
+  for (int idx = threadIdx.x; idx < 128 * kCG; idx += 256) {
+    const int col = idx / 128, pl = idx % 128;
+    const int I = cg * kCG + col;
+    if (I >= n_m || p0 + pl >= kpad) continue;
+    const float x = tx[col][pl], y = ty[col][pl];
+    const __half hx = __float2half_rn(x), hy = __float2half_rn(y);
+    const __half lx = __float2half_rn(x - __half2float(hx)), ly = __float2half_rn(y - __half2float(hy));
+    const long long p = p0 + pl;
+    const long long o = (long long)I * kpad * 2 + (p >> 5) * 64 + (p & 31);
+    out[o] = hx;
+    out[o + 32] = lx;
+    out[oplane + o] = hy;
+    out[oplane + o + 32] = ly;
+  }
+}
+
+__global__ void z_export_hl16_kernel(const __half* __restrict__ zhl, long long kpad, int n_m_pad, int n_m,
+                                     long long n_pairs, const float* __restrict__ zmax, double2* __restrict__ out) {
+  const long long total = n_pairs * n_m;
+  const long long oplane = (long long)n_m_pad * kpad * 2;
+  const double inv = exp2(-(double)f16_scale_exp(*zmax));
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total;
+       e += (long long)gridDim.x * blockDim.x) {
+    const long long p = e / n_m;
+    const int I = (int)(e - p * n_m);
+    const long long o = (long long)I * kpad * 2 + (p >> 5) * 64 + (p & 31);
+    const float x = __half2float(zhl[o]) + __half2float(zhl[o + 32]);
+    const float y = __half2float(zhl[oplane + o]) + __half2float(zhl[oplane + o + 32]);
+    out[e] = make_double2((double)x * inv, (double)y * inv);
+  }
+}
+
+// FP32 weights scaled per frequency into (1/2, 1]:  w32[j][p] = fp32(w_j(p) * sigma_j), sigma_j = 2^-e with
+// max_p |w_j(p)| = m 2^e, m in [1/2, 1);  wscale[j] = 1 / sigma_j.  One block per frequency.
+__global__ void __launch_bounds__(1024) weights_scale_f32_kernel(const double* __restrict__ wtab, float* __restrict__ w32,
+                                                                 double* __restrict__ wscale, long long kpad,
+                                                                 long long n_pad) {
+  __shared__ double red[32];
+  const int j = blockIdx.x;
+  const double* wr = wtab + (long long)j * kpad;
+  double m = 0.0;
+  for (long long p = threadIdx.x; p < n_pad; p += blockDim.x) m = fmax(m, fabs(wr[p]));
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  m = red[0];
+  for (int i = 1; i < (int)(blockDim.x >> 5); ++i) m = fmax(m, red[i]);
+  int e = 0;
+  if (m > 0.0 && m < 1e300) (void)frexp(m, &e);
+  const double sigma = exp2((double)-e);
+  if (threadIdx.x == 0) wscale[j] = exp2((double)e);
+  float* o = w32 + (long long)j * kpad;
+  for (long long p = threadIdx.x; p < n_pad; p += blockDim.x) o[p] = (float)(wr[p] * sigma);
+}
+
 }  // namespace
 
 cudaError_t launch_zmel_f64(const ZmelArgs& a, cudaStream_t s) {
@@ -269,8 +367,8 @@ cudaError_t launch_z_export(const double* zws, long long kpad, int ncg, int n_m,
 }
 
 cudaError_t launch_z_import(double* zws, long long kpad, int ncg, int n_m, long long n_pairs,
-                            const double2* in, cudaStream_t s) {
-  z_import_kernel<<<grid_for(n_pairs * n_m, 256), 256, 0, s>>>(zws, kpad, ncg, n_m, n_pairs, in);
+                            const double2* in, float* zmax, cudaStream_t s) {
+  z_import_kernel<<<grid_for(n_pairs * n_m, 256), 256, 0, s>>>(zws, kpad, ncg, n_m, n_pairs, in, zmax);
   return cudaGetLastError();
 }
 
@@ -309,6 +407,26 @@ cudaError_t launch_planes32_from_ws(const double* zws, long long kpad, int ncg, 
 cudaError_t launch_weights_to_f32(const double* wtab, float* wtab32, long long kpad, long long n_pad, int n_freq,
                                   cudaStream_t s) {
   weights_to_f32_kernel<<<grid_for(n_pad * n_freq, 256), 256, 0, s>>>(wtab, wtab32, kpad, n_pad, n_freq);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs, void* zhl,
+                             int n_m_pad, const float* zmax, cudaStream_t s) {
+  dim3 grid((unsigned)((kpad + 127) / 128), ncg);
+  z_to_hl16_kernel<<<grid, 256, 0, s>>>(zws, kpad, ncg, n_m, n_pairs, static_cast<__half*>(zhl), n_m_pad, zmax);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_z_export_hl16(const void* zhl, long long kpad, int n_m_pad, int n_m, long long n_pairs,
+                                 const float* zmax, double2* out, cudaStream_t s) {
+  z_export_hl16_kernel<<<grid_for(n_pairs * n_m, 256), 256, 0, s>>>(static_cast<const __half*>(zhl), kpad, n_m_pad,
+                                                                   n_m, n_pairs, zmax, out);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_weights_scale_f32(const double* wtab, float* wtab32, double* wscale, long long kpad, long long n_pad,
+                                     int n_freq, cudaStream_t s) {
+  weights_scale_f32_kernel<<<n_freq, 1024, 0, s>>>(wtab, wtab32, wscale, kpad, n_pad);
   return cudaGetLastError();
 }
 
