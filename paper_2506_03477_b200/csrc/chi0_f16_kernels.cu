@@ -12,7 +12,9 @@
 //
 //   z tiles ("hl16" planes, kernels.h) are K-major FP16: one 128-byte swizzled row = h[32 pairs] | l[32
 //   pairs], written to shared memory by TMA and read by the MMA as the B operand; the frequency-scaled
-//   operand A is formed in registers (w * (h + l), re-split) and stored to TENSOR MEMORY (tcgen05.st).
+//   operand A is formed in registers and stored to TENSOR MEMORY (tcgen05.st).  The scaling itself runs in
+//   packed FP16 arithmetic with an exact-residual FMA (no conversions): with w = w_h + w_l,
+//     a_h = w_h (x) z_h,   a_l = fma(w_h, z_h, -a_h) + w_h z_l + w_l z_h        (a_h + a_l = w z to 2^-22).
 //
 //   The CSZ CTAs of a thread-block cluster work on the same tile at CSZ consecutive frequencies: every z
 //   box is fetched from L2 once per cluster and multicast to all CTAs (the 16 frequency CTAs of a tile
@@ -41,11 +43,10 @@ struct HCfg {
   static constexpr int STAGES = 3;
   static constexpr int B_BYTES = 2 * kPlaneTileH;
   static constexpr int A_BYTES = 2 * kPlaneTileH;
-  static constexpr int W_BYTES = kPairStage * 4;
+  static constexpr int W_BYTES = kPairStage * 4;                 // w_h[32] | w_l[32] halves
   static constexpr int STAGE_BYTES = B_BYTES + A_BYTES + 1024;   // w slot padded: tiles stay 1024-B aligned
   static constexpr int TSLOT_COLS = 64;                          // h_x, h_y, l_x, l_y: 16 columns each
   static constexpr int TSLOTS = 4;
-  static constexpr int WIN = 8;                                  // stages per drain window (96 MMA steps)
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256 + 1024 /*align slack*/;
 };
 
@@ -69,7 +70,7 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   const int j = blockIdx.x % a.n_freq;               // the CSZ CTAs of a cluster: same tile, consecutive j
   const int2 tt = a.d_tiles[blockIdx.x / a.n_freq];
   const bool need_a = (tt.x != tt.y);                // diagonal tile: the A source is the B tile
-  const int n_stages = a.n_stages;
+  const int n_stages = a.n_stages, win = a.win;
   const uint32_t rank = CSZ > 1 ? cluster_ctarank() : 0u;
   constexpr uint16_t kMask = (uint16_t)((1u << CSZ) - 1u);
 
@@ -99,7 +100,7 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
     setmaxnreg_dec<56>();
     if (warp == 0 && lane == 0) {
       // ------------------------------------------------------------------ TMA producer
-      const float* wrow = a.wtab32 + (long long)j * a.kpad;
+      const __half* wrow = a.wtab16 + (long long)j * a.kpad * 2;
       const uint32_t bytes = C::B_BYTES + C::W_BYTES + (need_a ? C::A_BYTES : 0);
       const int n_box = need_a ? 8 : 4;
       for (int s = 0; s < n_stages; ++s) {
@@ -115,15 +116,15 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
           if (CSZ > 1) tma_load_3d_mc(dst, &a.tmap, &full[st], s * 64, row0, plane, kMask);
           else tma_load_3d(dst, &a.tmap, &full[st], s * 64, row0, plane);
         }
-        bulk_load_1d(sb + C::B_BYTES + C::A_BYTES, wrow + (long long)s * kPairStage, C::W_BYTES, &full[st]);
+        bulk_load_1d(sb + C::B_BYTES + C::A_BYTES, wrow + (long long)s * 64, C::W_BYTES, &full[st]);
       }
     } else if (warp == 1 && lane == 0) {
       // ------------------------------------------------------------------ MMA issuer
       const uint32_t idesc = umma_idesc_f16(128, 128, 0), idesc_neg = umma_idesc_f16(128, 128, 1);
       for (int s = 0; s < n_stages; ++s) {
         const int st = s % C::STAGES, u = s / C::STAGES, ts = s % C::TSLOTS, tu = s / C::TSLOTS;
-        const bool win_first = (s % C::WIN) == 0;
-        if (win_first && s > 0) mbar_wait(d_empty, ((s / C::WIN) - 1) & 1);
+        const bool win_first = (s % win) == 0;
+        if (win_first && s > 0) mbar_wait(d_empty, ((s / win) - 1) & 1);
         mbar_wait(&full[st], u & 1);
         mbar_wait(&a_full[ts], tu & 1);
         tc_fence_after();
@@ -152,7 +153,7 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
         if (CSZ > 1) umma_commit_mc(&empty[st], kMask);
         else umma_commit(&empty[st]);
         umma_commit(&a_empty[ts]);
-        if (((s + 1) % C::WIN) == 0 || s == n_stages - 1) umma_commit(d_full);
+        if (((s + 1) % win) == 0 || s == n_stages - 1) umma_commit(d_full);
       }
     }
   } else {
@@ -193,13 +194,14 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
       tc_fence_after();
       const uint32_t sb = base + st * C::STAGE_BYTES;
       const uint32_t src = (need_a ? sb + C::B_BYTES : sb) + (uint32_t)row * 128u;
-      const uint32_t swp = sb + C::B_BYTES + C::A_BYTES + 64u * (uint32_t)h;   // this thread's 16 pairs
+      const uint32_t swp = sb + C::B_BYTES + C::A_BYTES + 32u * (uint32_t)h;   // this thread's 16 pairs
       const uint32_t tdst = a_ring + ts * C::TSLOT_COLS + 8 * h + lane_base;
-      float w[16];
+      uint32_t wh[8], wl[8];
 #pragma unroll
-      for (int cc = 0; cc < 4; ++cc) {
-        const float4 t = ld_shared_f4(swp + 16 * cc);
-        w[4 * cc] = t.x; w[4 * cc + 1] = t.y; w[4 * cc + 2] = t.z; w[4 * cc + 3] = t.w;
+      for (int cc = 0; cc < 2; ++cc) {
+        const uint4 t = ld_shared_u4(swp + 16 * cc), u4 = ld_shared_u4(swp + 64 + 16 * cc);
+        wh[4 * cc] = t.x; wh[4 * cc + 1] = t.y; wh[4 * cc + 2] = t.z; wh[4 * cc + 3] = t.w;
+        wl[4 * cc] = u4.x; wl[4 * cc + 1] = u4.y; wl[4 * cc + 2] = u4.z; wl[4 * cc + 3] = u4.w;
       }
 #pragma unroll
       for (int xy = 0; xy < 2; ++xy) {
@@ -213,14 +215,14 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
         }
 #pragma unroll
         for (int e = 0; e < 8; ++e) {                  // pairs 2e, 2e+1 of this thread's 16
-          const float2 zh = __half22float2(*reinterpret_cast<const __half2*>(&hv[e]));
-          const float2 zl = __half22float2(*reinterpret_cast<const __half2*>(&lv[e]));
-          const float a0 = w[2 * e] * (zh.x + zl.x), a1 = w[2 * e + 1] * (zh.y + zl.y);
-          const __half2 hh = __floats2half2_rn(a0, a1);
-          const float2 hf = __half22float2(hh);
-          const __half2 ll = __floats2half2_rn(a0 - hf.x, a1 - hf.y);
-          ah[e] = *reinterpret_cast<const uint32_t*>(&hh);
-          al[e] = *reinterpret_cast<const uint32_t*>(&ll);
+          const __half2 zh = *reinterpret_cast<const __half2*>(&hv[e]), zl = *reinterpret_cast<const __half2*>(&lv[e]);
+          const __half2 w_h = *reinterpret_cast<const __half2*>(&wh[e]), w_l = *reinterpret_cast<const __half2*>(&wl[e]);
+          const __half2 p = __hmul2(w_h, zh);
+          __half2 r = __hfma2(w_h, zh, __hneg2(p));    // exact: the rounding error of p
+          r = __hfma2(w_h, zl, r);
+          r = __hfma2(w_l, zh, r);
+          ah[e] = *reinterpret_cast<const uint32_t*>(&p);
+          al[e] = *reinterpret_cast<const uint32_t*>(&r);
         }
         tmem_st8(tdst + 16 * xy, ah);
         tmem_st8(tdst + 32 + 16 * xy, al);
@@ -237,9 +239,9 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
           mbar_arrive(&empty[st]);
         }
       }
-      if (s >= 1 && (s % C::WIN) == 0) drain(s / C::WIN - 1);   // stage s-1 closed a window
+      if (s >= 1 && (s % win) == 0) drain(s / win - 1);   // stage s-1 closed a window
     }
-    drain((n_stages - 1) / C::WIN);
+    drain((n_stages - 1) / win);
 
     // FP32 window sums (in units 2^(2S) sigma_j) -> FP64 accumulators (exclusive owner of (tile, j))
     const double sc = a.wscale[j] * exp2(-2.0 * (double)f16_scale_exp(*a.zmax));

@@ -17,6 +17,7 @@
 #pragma once
 #include <cstdint>
 #include <cuda.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
 namespace qsgw {
@@ -71,7 +72,7 @@ struct Chi0F64Args {
   int n_tiles;
 };
 constexpr int kChi0F64KP = 16;  // pairs per pipeline stage (box rows of the tensor map)
-cudaError_t launch_chi0_f64(const Chi0F64Args& a, cudaStream_t s);
+cudaError_t launch_chi0_f64(const Chi0F64Args& a, bool three_m /*3M complex product (default) or 4M*/, cudaStream_t s);
 cudaError_t chi0_f64_configure();   // sets the dynamic shared-memory attribute once
 
 // ---- mixed mode (chi0_tf32_kernels.cu) -------------------------------------------------------------
@@ -108,11 +109,12 @@ cudaError_t probe_tf32_mma(cudaStream_t s, double* out_tflops, double* out_ms);
 //   z workspace "hl16": __half zhl[2 planes (Re,Im)][n_m_pad][kpad/32][64]: per product function I and
 //   32-pair stage one 128-byte row  h[32] | l[32],  v = fp32(z * 2^S) = h + l (h = fp16(v), l = fp16(v-h)),
 //   S = f16_scale_exp(*zmax) from the batch maximum.  3-D TMA boxes {64 halves, 64 rows, 1 plane} with the
-//   128-byte swizzle give K-major UMMA operand tiles.  wtab32[j][p] = fp32(w_j(p) / wscale[j]), wscale[j]
-//   a power of two with max_p |wtab32[j][p]| in (1/2, 1].
+//   128-byte swizzle give K-major UMMA operand tiles.  Weights: __half wtab16[n_freq][kpad/32][64], per 32-pair
+//   stage  w_h[32] | w_l[32]  with w_h + w_l = fp32(w_j(p) / wscale[j]), wscale[j] a power of two such that
+//   max_p |w_j(p)| / wscale[j] is in (1/2, 1].
 struct Chi0F16Args {
   CUtensorMap tmap;      // 3-D FLOAT16 {2*kpad, n_m_pad, 2}, box {64, 64, 1}, SWIZZLE_128B
-  const float* wtab32;   // [n_freq][kpad]
+  const __half* wtab16;  // [n_freq][kpad/32][64]
   const double* wscale;  // [n_freq]
   const float* zmax;     // batch maximum of |Re z|, |Im z|
   long long kpad;
@@ -121,6 +123,7 @@ struct Chi0F16Args {
   int n_m_pad;           // multiple of 128
   int n_freq;
   int n_stages;          // ceil(n_pairs / 32)
+  int win;               // stages per drain window (12 MMA steps into each accumulator per stage)
   const int2* d_tiles;   // 128x128 tiles, tile_i <= tile_j
   int n_tiles;
 };
@@ -130,8 +133,8 @@ cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m
                              int n_m_pad, const float* zmax, cudaStream_t s);
 cudaError_t launch_z_export_hl16(const void* zhl, long long kpad, int n_m_pad, int n_m, long long n_pairs,
                                  const float* zmax, double2* out, cudaStream_t s);
-cudaError_t launch_weights_scale_f32(const double* wtab, float* wtab32, double* wscale, long long kpad, long long n_pad,
-                                     int n_freq, cudaStream_t s);
+cudaError_t launch_weights_scale_hl16(const double* wtab, void* wtab16, double* wscale, long long kpad, long long n_pad,
+                                      int n_freq, cudaStream_t s);
 cudaError_t probe_f16_mma(cudaStream_t s, double* out_tflops, double* out_ms);
 
 // issue-rate probes (probe_kernels.cu): measured MMA-pipe peaks for the roofline denominators

@@ -70,6 +70,8 @@ struct qsgw_ctx {
   double* d_wscale = nullptr;
   float* d_zmax = nullptr;
   int cluster = 1;              // CTAs of a cluster sharing one tile's z boxes (1, 2 or 4)
+  int win = 8;                  // stages per TMEM drain window
+  bool f64_3m = true;           // FP64 mode: 3M complex product (QSGW_F64_4M=1 selects the 4M kernel)
   CUtensorMap tmap_h;
   double* d_acc_re = nullptr;
   double* d_acc_im = nullptr;
@@ -316,6 +318,11 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   if (const char* ev = getenv("QSGW_F16_CLUSTER")) {   // tuning knob: CTAs per cluster sharing a tile (1, 2, 4)
     const int v = atoi(ev);
     if (v == 1 || v == 2 || v == 4) c->cluster = v;
+  }
+  if (const char* ev = getenv("QSGW_F64_4M")) c->f64_3m = atoi(ev) == 0;   // A/B knob for profiles
+  if (const char* ev = getenv("QSGW_F16_WIN")) {       // tuning knob: stages per drain window
+    const int v = atoi(ev);
+    if (v >= 1 && v <= 64) c->win = v;
   }
   const int tile_edge = mixed ? qsgw::kTileMx : qsgw::kTile;
   c->n_m_pad = (int)round_up(c->n_m, tile_edge);
@@ -608,14 +615,15 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
     const long long n_pad32 = round_up(n_pairs, qsgw::kPairStage);
     {
       StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
-      e = qsgw::launch_weights_scale_f32(ctx->d_wtab, ctx->d_wtab32, ctx->d_wscale, ctx->kpad, n_pad32, ctx->n_freq,
-                                         ctx->stream);
+      e = qsgw::launch_weights_scale_hl16(ctx->d_wtab, ctx->d_wtab32, ctx->d_wscale, ctx->kpad, n_pad32, ctx->n_freq,
+                                          ctx->stream);
     }
     if (e != cudaSuccess) return ctx->cuda_fail(e, "weight scaling kernel launch");
     qsgw::Chi0F16Args m;
     m.tmap = ctx->tmap_h;
-    m.wtab32 = ctx->d_wtab32;
+    m.wtab16 = reinterpret_cast<const __half*>(ctx->d_wtab32);   // same bytes per pair as the FP32 table
     m.wscale = ctx->d_wscale;
+    m.win = ctx->win;
     m.zmax = ctx->d_zmax;
     m.kpad = ctx->kpad;
     m.acc_re = ctx->d_acc_re;
@@ -680,7 +688,7 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
   a.n_tiles = ctx->n_tiles;
   {
     StageScope ts(ctx, QSGW_STAGE_CHI0);
-    e = qsgw::launch_chi0_f64(a, ctx->stream);
+    e = qsgw::launch_chi0_f64(a, ctx->f64_3m, ctx->stream);
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 kernel launch");
   ctx->launches += 1;

@@ -313,11 +313,12 @@ __global__ void z_export_hl16_kernel(const __half* __restrict__ zhl, long long k
   }
 }
 
-// FP32 weights scaled per frequency into (1/2, 1]:  w32[j][p] = fp32(w_j(p) * sigma_j), sigma_j = 2^-e with
-// max_p |w_j(p)| = m 2^e, m in [1/2, 1);  wscale[j] = 1 / sigma_j.  One block per frequency.
-__global__ void __launch_bounds__(1024) weights_scale_f32_kernel(const double* __restrict__ wtab, float* __restrict__ w32,
-                                                                 double* __restrict__ wscale, long long kpad,
-                                                                 long long n_pad) {
+// Weights scaled per frequency into (1/2, 1] and split into fp16 pieces:  v = fp32(w_j(p) * sigma_j),
+// sigma_j = 2^-e with max_p |w_j(p)| = m 2^e, m in [1/2, 1);  w_h = fp16(v), w_l = fp16(v - w_h), stored per
+// 32-pair stage as  w_h[32] | w_l[32];  wscale[j] = 1 / sigma_j.  One block per frequency.
+__global__ void __launch_bounds__(1024) weights_scale_hl16_kernel(const double* __restrict__ wtab,
+                                                                  __half* __restrict__ w16, double* __restrict__ wscale,
+                                                                  long long kpad, long long n_pad) {
   __shared__ double red[32];
   const int j = blockIdx.x;
   const double* wr = wtab + (long long)j * kpad;
@@ -333,8 +334,13 @@ __global__ void __launch_bounds__(1024) weights_scale_f32_kernel(const double* _
   if (m > 0.0 && m < 1e300) (void)frexp(m, &e);
   const double sigma = exp2((double)-e);
   if (threadIdx.x == 0) wscale[j] = exp2((double)e);
-  float* o = w32 + (long long)j * kpad;
-  for (long long p = threadIdx.x; p < n_pad; p += blockDim.x) o[p] = (float)(wr[p] * sigma);
+  __half* o = w16 + (long long)j * kpad * 2;
+  for (long long p = threadIdx.x; p < n_pad; p += blockDim.x) {
+    const float v = (float)(wr[p] * sigma);
+    const __half h = __float2half_rn(v);
+    o[(p >> 5) * 64 + (p & 31)] = h;
+    o[(p >> 5) * 64 + 32 + (p & 31)] = __float2half_rn(v - __half2float(h));
+  }
 }
 
 }  // namespace
@@ -424,9 +430,9 @@ cudaError_t launch_z_export_hl16(const void* zhl, long long kpad, int n_m_pad, i
   return cudaGetLastError();
 }
 
-cudaError_t launch_weights_scale_f32(const double* wtab, float* wtab32, double* wscale, long long kpad, long long n_pad,
-                                     int n_freq, cudaStream_t s) {
-  weights_scale_f32_kernel<<<n_freq, 1024, 0, s>>>(wtab, wtab32, wscale, kpad, n_pad);
+cudaError_t launch_weights_scale_hl16(const double* wtab, void* wtab16, double* wscale, long long kpad, long long n_pad,
+                                      int n_freq, cudaStream_t s) {
+  weights_scale_hl16_kernel<<<n_freq, 1024, 0, s>>>(wtab, static_cast<__half*>(wtab16), wscale, kpad, n_pad);
   return cudaGetLastError();
 }
 

@@ -30,6 +30,38 @@ def _sampled_and_sketch(prob, spin, got, tol):
     assert (np.abs(got[:, rows, cols] - E) / scale).max() <= tol
 
 
+TOL_MIXED = 2e-5      # BASELINE.json:north_star, relative Frobenius error per frequency (mixed mode)
+
+
+def test_cfg3_full_size_mixed():
+    """cfg 3 = the metal in mixed mode, all 216 k-points, both spin channels (two contexts)."""
+    cfg = get_config(3)
+    prob = generate(cfg)
+    for spin in range(cfg.n_spin):
+        got = run_cuda(prob, spin=spin, precision=1)
+        _sampled_and_sketch(prob, spin, got, TOL_MIXED)
+
+
+def test_cfg4_full_size_mixed():
+    """cfg 4 in mixed mode, the launch configuration bench.py times (one batch per k-point)."""
+    cfg = get_config(4)
+    prob = generate(cfg)
+    got = run_cuda(prob, precision=1)
+    _sampled_and_sketch(prob, 0, got, TOL_MIXED)
+
+
+def test_cfg4_full_size_mixed_band_batches():
+    """cfg 4 in mixed mode with the O side split into 4 band batches (z workspace a quarter the size):
+    every batch carries its own FP16 scale, the result must not depend on the batching."""
+    cfg = get_config(4)
+    prob = generate(cfg, n_k=2)
+    a = run_cuda(prob, precision=1, n_k_norm=cfg.n_k)
+    b = run_cuda(prob, precision=1, max_n_o=16, n_k_norm=cfg.n_k)
+    num = np.linalg.norm((a - b).reshape(a.shape[0], -1), axis=1)
+    den = np.linalg.norm(a.reshape(a.shape[0], -1), axis=1)
+    assert (num / den).max() <= TOL_MIXED
+
+
 def test_cfg2_full_size_fp64():
     cfg = get_config(2)
     prob = generate(cfg)
