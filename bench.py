@@ -289,18 +289,25 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
     ratio_txt = f"x nominal {dkey}/bf16 ratio ({NOMINAL_TF[dkey]:g}/{NOMINAL_TF['bf16']:g})"
     if dkey == "f64":
         # MEASURED_PEAKS.json has no FP64 figure and the bf16-derived one is power-capped while FP64 is not
-        # (the kernel exceeds it): the denominator is the DMMA issue-rate probe.
-        peak = probe or burst_peak
-        peak_src = ("measured in this run: qsgw_probe_peak(f64) register-resident DMMA issue-rate loop" if probe
-                    else f"{src} bf16 burst {ratio_txt}")
+        # (the kernel exceeds it): the denominator is the DMMA pipe's issue rate, 64 FP64 FMA/clk/SM x SMs x
+        # max SM clock, which the register-resident probe reproduces when it is not throttled.
+        props = torch.cuda.get_device_properties(dev)
+        derived = 2.0 * 64.0 * props.multi_processor_count * props.clock_rate * 1e3 / 1e12
+        peak = max(derived, probe or 0.0)
+        peak_src = (f"DMMA issue rate: 64 FP64 FMA/clk/SM x {props.multi_processor_count} SMs x "
+                    f"{props.clock_rate / 1e3:.0f} MHz (qsgw_probe_peak(f64) measured {probe and round(probe, 2)} in this run)")
     else:
         # tcgen05 kernels run power-capped inside a seconds-long step: MEASURED_PEAKS.json sustained figure
         peak = sust_peak
         peak_src = f"{src} bf16 cuBLAS sustained (MEASURED_PEAKS.json) {ratio_txt}"
     # tensor-pipe flops the kernel executes per credited flop (full tiles, no padding counted):
     # FP64 4M = 1; FP16 split and 3xTF32 = 3 products per term; single TF32 = 1
-    passes = {q.PREC_FP64: 1, q.PREC_MIXED: 3, q.PREC_MIXED_TF32X3: 3, q.PREC_MIXED_TF32X1: 1}[precision]
-    kname = {"f64": "chi0_f64_kernel", "f16": "chi0_f16_kernel", "tf32": f"chi0_tf32_kernel<{passes}>"}[dkey]
+    # FP64: the 3M kernel executes 3 real products per complex one (0.75 of the credited 4); QSGW_F64_4M=1 = 4M
+    f64_4m = os.environ.get("QSGW_F64_4M", "0") not in ("", "0")
+    passes = {q.PREC_FP64: 1.0 if f64_4m else 0.75, q.PREC_MIXED: 3, q.PREC_MIXED_TF32X3: 3,
+              q.PREC_MIXED_TF32X1: 1}[precision]
+    kname = {"f64": "chi0_f64_kernel" if f64_4m else "chi0_f64_3m_kernel", "f16": "chi0_f16_kernel",
+             "tf32": f"chi0_tf32_kernel<{passes}>"}[dkey]
     roofline = {"bound": "tensor", "kernel": kname, "tensor_pipe": dkey,
                 "tensor_products_per_term": passes,
                 "achieved_executed": (ach * passes) if ach else None,
