@@ -56,6 +56,9 @@ enum {
  *   tensor cores: every FP32 operand v (scaled by a power of two) is carried as fp16 pieces v = h + l
  *   (22 significant bits) and a*b is formed as a_h*b_h + a_l*b_h + a_h*b_l by three exact FP16 MMAs
  *   (tcgen05 kind::f16, twice the TF32 rate); FP32 window sums, FP64 accumulation across batches and k.
+ *   When the job sums at least 64 band pairs per product function (n_k * max_n_o * max_n_u >= 64 * N_M, taken
+ *   from the descriptor) the two correction products a_l*b_h + a_h*b_l run in E5M2 (kind::f8f6f4): they need
+ *   ~3 significant bits; the added error ~4e-5 * sqrt(N_M / pairs summed) stays well inside the 2e-5 bar.
  * QSGW_PREC_MIXED_TF32X3: the same split on the TF32 pipe (hi*hi + lo*hi + hi*lo), half the speed.
  * QSGW_PREC_MIXED_TF32X1: ONE TF32 product per term (operands rounded to nearest TF32; relative
  *   Frobenius error ~ 3e-4 * sqrt(N_M / pairs summed): above the 2e-5 bar on cfg 3/4). */

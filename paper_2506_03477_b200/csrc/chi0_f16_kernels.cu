@@ -50,7 +50,9 @@ struct HCfg {
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256 + 1024 /*align slack*/;
 };
 
-template <int CSZ>
+// FP8 = true: the two correction products run on kind::f8f6f4 (E5M2) -- 8 f16 + 8 fp8 MMAs per 32 pairs
+// instead of 24 f16 MMAs; B rows come from the "hb8" workspace, the A source stays the full-precision hl16 rows.
+template <int CSZ, bool FP8>
 __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_constant__ Chi0F16Args a) {
   using C = HCfg;
   extern __shared__ unsigned char smem_dyn[];
@@ -69,7 +71,7 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int j = blockIdx.x % a.n_freq;               // the CSZ CTAs of a cluster: same tile, consecutive j
   const int2 tt = a.d_tiles[blockIdx.x / a.n_freq];
-  const bool need_a = (tt.x != tt.y);                // diagonal tile: the A source is the B tile
+  const bool need_a = FP8 || (tt.x != tt.y);         // f16 split, diagonal tile: the A source is the B tile
   const int n_stages = a.n_stages, win = a.win;
   const uint32_t rank = CSZ > 1 ? cluster_ctarank() : 0u;
   constexpr uint16_t kMask = (uint16_t)((1u << CSZ) - 1u);
@@ -113,14 +115,17 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
           const int plane = (i >> 1) & 1, rh = i & 1, op = i >> 2;
           unsigned char* dst = sb + op * C::B_BYTES + plane * kPlaneTileH + rh * kBoxBytes;
           const int row0 = (op ? tt.x : tt.y) * kTileMx + rh * 64;
-          if (CSZ > 1) tma_load_3d_mc(dst, &a.tmap, &full[st], s * 64, row0, plane, kMask);
-          else tma_load_3d(dst, &a.tmap, &full[st], s * 64, row0, plane);
+          const CUtensorMap* tm = (FP8 && !op) ? &a.tmap_b : &a.tmap;       // hb8 rows are addressed in bytes
+          const int c0 = (FP8 && !op) ? s * 128 : s * 64;
+          if (CSZ > 1) tma_load_3d_mc(dst, tm, &full[st], c0, row0, plane, kMask);
+          else tma_load_3d(dst, tm, &full[st], c0, row0, plane);
         }
         bulk_load_1d(sb + C::B_BYTES + C::A_BYTES, wrow + (long long)s * 64, C::W_BYTES, &full[st]);
       }
     } else if (warp == 1 && lane == 0) {
       // ------------------------------------------------------------------ MMA issuer
       const uint32_t idesc = umma_idesc_f16(128, 128, 0), idesc_neg = umma_idesc_f16(128, 128, 1);
+      const uint32_t idesc8 = umma_idesc_e5m2(128, 128, 0), idesc8_neg = umma_idesc_e5m2(128, 128, 1);
       for (int s = 0; s < n_stages; ++s) {
         const int st = s % C::STAGES, u = s / C::STAGES, ts = s % C::TSLOTS, tu = s / C::TSLOTS;
         const bool win_first = (s % win) == 0;
@@ -131,8 +136,30 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
         const uint32_t sb = base + st * C::STAGE_BYTES;
         const uint64_t bx = umma_desc_k_sw128(sb), by = umma_desc_k_sw128(sb + kPlaneTileH);
         const uint32_t ab = a_ring + ts * C::TSLOT_COLS;
+        if (FP8) {
 #pragma unroll
-        for (int g = 0; g < 2; ++g) {                       // 16 pairs = one K step of kind::f16
+          for (int g = 0; g < 2; ++g) {                     // main products: a_h b_h
+            const uint32_t acc0 = (win_first && g == 0) ? 0u : 1u;
+            const uint64_t kh = (uint64_t)(2 * g);
+            const uint32_t ahx = ab + 8 * g, ahy = ab + 16 + 8 * g;
+            umma_f16_ts(d_re, ahx, bx + kh, idesc, acc0);
+            umma_f16_ts(d_im, ahx, by + kh, idesc, acc0);
+            umma_f16_ts(d_re, ahy, by + kh, idesc, 1u);
+            umma_f16_ts(d_im, ahy, bx + kh, idesc_neg, 1u);
+          }
+          // corrections a_l8 b_8 + a_8 b_l8: one K = 32 step; b_8 at byte 64, b_l8 at byte 96 of the row
+          const uint32_t a8x = ab + 32, a8y = ab + 40, l8x = ab + 48, l8y = ab + 56;
+          umma_f8_ts(d_re, l8x, bx + 4, idesc8, 1u);
+          umma_f8_ts(d_im, l8x, by + 4, idesc8, 1u);
+          umma_f8_ts(d_re, l8y, by + 4, idesc8, 1u);
+          umma_f8_ts(d_im, l8y, bx + 4, idesc8_neg, 1u);
+          umma_f8_ts(d_re, a8x, bx + 6, idesc8, 1u);
+          umma_f8_ts(d_im, a8x, by + 6, idesc8, 1u);
+          umma_f8_ts(d_re, a8y, by + 6, idesc8, 1u);
+          umma_f8_ts(d_im, a8y, bx + 6, idesc8_neg, 1u);
+        }
+#pragma unroll
+        for (int g = 0; g < (FP8 ? 0 : 2); ++g) {           // 16 pairs = one K step of kind::f16
           const uint32_t acc0 = (win_first && g == 0) ? 0u : 1u;
           const uint64_t kh = (uint64_t)(2 * g);            // 16 halves = 32 B along K inside the swizzle row
           const uint64_t kl = (uint64_t)(4 + 2 * g);        // the l half of the row starts at byte 64
@@ -225,7 +252,19 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
           al[e] = *reinterpret_cast<const uint32_t*>(&r);
         }
         tmem_st8(tdst + 16 * xy, ah);
-        tmem_st8(tdst + 32 + 16 * xy, al);
+        if (FP8) {
+          uint32_t a8[4], l8[4];
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            a8[c] = cvt_e5m2x2_f16x2(ah[2 * c]) | (cvt_e5m2x2_f16x2(ah[2 * c + 1]) << 16);
+            l8[c] = cvt_e5m2x2_f16x2(al[2 * c]) | (cvt_e5m2x2_f16x2(al[2 * c + 1]) << 16);
+          }
+          const uint32_t t8 = a_ring + ts * C::TSLOT_COLS + 32 + 4 * h + lane_base;
+          tmem_st4(t8 + 8 * xy, a8);
+          tmem_st4(t8 + 16 + 8 * xy, l8);
+        } else {
+          tmem_st8(tdst + 32 + 16 * xy, al);
+        }
       }
       tmem_wait_st();
       tc_fence_before();
@@ -326,27 +365,33 @@ cudaError_t launch_cluster(const Chi0F16Args& a, cudaStream_t s) {
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, chi0_f16_kernel<CSZ>, a);
+  return cudaLaunchKernelEx(&cfg, chi0_f16_kernel<CSZ, false>, a);
 }
 
 }  // namespace
 
 cudaError_t chi0_f16_configure() {
-  cudaError_t e = cudaFuncSetAttribute(chi0_f16_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
+  cudaError_t e = cudaFuncSetAttribute(chi0_f16_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(chi0_f16_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
+  e = cudaFuncSetAttribute(chi0_f16_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(chi0_f16_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
+  e = cudaFuncSetAttribute(chi0_f16_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(chi0_f16_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(f16_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 20480);
 }
 
-cudaError_t launch_chi0_f16(const Chi0F16Args& a, int cluster, cudaStream_t s) {
+cudaError_t launch_chi0_f16(const Chi0F16Args& a, int cluster, bool fp8, cudaStream_t s) {
   if (a.n_stages <= 0 || a.n_tiles <= 0) return cudaSuccess;
+  if (fp8) {   // the FP8-corrected variant is built for single-CTA launches only
+    chi0_f16_kernel<1, true><<<dim3((unsigned)(a.n_tiles * a.n_freq)), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
+    return cudaGetLastError();
+  }
   if (cluster > 1 && a.n_freq % cluster != 0) cluster = (a.n_freq % 2 == 0) ? 2 : 1;
   if (cluster >= 4) return launch_cluster<4>(a, s);
   if (cluster >= 2) return launch_cluster<2>(a, s);
-  chi0_f16_kernel<1><<<dim3((unsigned)(a.n_tiles * a.n_freq)), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
+  chi0_f16_kernel<1, false><<<dim3((unsigned)(a.n_tiles * a.n_freq)), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
   return cudaGetLastError();
 }
 

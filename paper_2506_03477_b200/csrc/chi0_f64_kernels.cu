@@ -170,14 +170,21 @@ __global__ void __launch_bounds__(kThreads, 2) chi0_f64_kernel(const __grid_cons
 // 8 warps (2 along I x 4 along J), each a 32x16 complex sub-tile = 3 x 16 FP64 accumulator pairs; per 4 pairs a
 // warp loads 12 operand doubles and issues 24 DMMAs.  Normwise error ~1e-15 (the parity bar is 1e-11).
 constexpr int kThreads3M = 256;
+constexpr int KP3 = kChi0F64KP3M;     // pairs per stage of the 3M kernel (1 CTA/SM: twice the 4M kernel's stage)
+constexpr int OPER_BYTES3 = 2 * 4 * KP3 * 128;
+constexpr int PLANE_BYTES3 = 4 * KP3 * 128;
+constexpr int CGRP_BYTES3 = KP3 * 128;
+constexpr int W_BYTES3 = KP3 * 8;
+constexpr int SMEM_OPERANDS3 = STAGES * 2 * OPER_BYTES3;
+constexpr int SMEM_BYTES3 = SMEM_OPERANDS3 + STAGES * W_BYTES3 + 2 * STAGES * 8 + 1024 /*align slack*/;
 
 __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid_constant__ Chi0F64Args a) {
   extern __shared__ unsigned char smem_dyn[];
   const uint32_t raw = smem_u32(smem_dyn);
   const uint32_t base = (raw + 1023u) & ~1023u;
   unsigned char* sm = smem_dyn + (base - raw);
-  double* wsm = reinterpret_cast<double*>(sm + SMEM_OPERANDS);
-  uint64_t* full = reinterpret_cast<uint64_t*>(sm + SMEM_OPERANDS + STAGES * W_BYTES);
+  double* wsm = reinterpret_cast<double*>(sm + SMEM_OPERANDS3);
+  uint64_t* full = reinterpret_cast<uint64_t*>(sm + SMEM_OPERANDS3 + STAGES * W_BYTES3);
   uint64_t* empty = full + STAGES;
 
   const int tid = threadIdx.x;
@@ -189,7 +196,7 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
   const int tile = blockIdx.x / a.n_freq;
   const int2 tt = a.d_tiles[tile];
   const bool diag = (tt.x == tt.y);
-  const int n_iter = (int)(a.n_pairs_padded / KP);
+  const int n_iter = (int)(a.n_pairs_padded / KP3);
   const double* wrow = a.wtab + (long long)j * a.kpad;
 
   if (tid == 0) {
@@ -202,13 +209,13 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
   }
   __syncthreads();
 
-  const uint32_t stage_bytes = (diag ? OPER_BYTES : 2 * OPER_BYTES) + W_BYTES;
+  const uint32_t stage_bytes = (diag ? OPER_BYTES3 : 2 * OPER_BYTES3) + W_BYTES3;
   auto issue = [&](int slot, int it) {
-    unsigned char* dstA = sm + slot * (2 * OPER_BYTES);
+    unsigned char* dstA = sm + slot * (2 * OPER_BYTES3);
     mbar_arrive_expect_tx(&full[slot], stage_bytes);
-    tma_load_4d(dstA, &a.tmap_z, &full[slot], 0, it * KP, tt.x * 4, 0);
-    if (!diag) tma_load_4d(dstA + OPER_BYTES, &a.tmap_z, &full[slot], 0, it * KP, tt.y * 4, 0);
-    bulk_load_1d(wsm + slot * KP, wrow + (long long)it * KP, W_BYTES, &full[slot]);
+    tma_load_4d(dstA, &a.tmap_z, &full[slot], 0, it * KP3, tt.x * 4, 0);
+    if (!diag) tma_load_4d(dstA + OPER_BYTES3, &a.tmap_z, &full[slot], 0, it * KP3, tt.y * 4, 0);
+    bulk_load_1d(wsm + slot * KP3, wrow + (long long)it * KP3, W_BYTES3, &full[slot]);
   };
 
   if (tid == 0) {
@@ -244,27 +251,27 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
     __syncwarp();
     mbar_wait(&full[slot], (it / STAGES) & 1);
 
-    const uint32_t aBase = base + slot * (2 * OPER_BYTES) + (2 * wm) * CGRP_BYTES;
-    const uint32_t bBase = base + slot * (2 * OPER_BYTES) + (diag ? 0 : OPER_BYTES) + wn * CGRP_BYTES;
-    const uint32_t wBase = base + SMEM_OPERANDS + slot * W_BYTES;
+    const uint32_t aBase = base + slot * (2 * OPER_BYTES3) + (2 * wm) * CGRP_BYTES3;
+    const uint32_t bBase = base + slot * (2 * OPER_BYTES3) + (diag ? 0 : OPER_BYTES3) + wn * CGRP_BYTES3;
+    const uint32_t wBase = base + SMEM_OPERANDS3 + slot * W_BYTES3;
 
 #pragma unroll
-    for (int q = 0; q < KP / 4; ++q) {
+    for (int q = 0; q < KP3 / 4; ++q) {
       const uint32_t rq = (uint32_t)((q >> 1) * 1024);
       const double w = ld_shared_f64(wBase + (uint32_t)((8 * (q >> 1) + 2 * t + (q & 1)) * 8));
       double ax[4], ay[4], as[4], bx[2], by[2], bd[2];
 #pragma unroll
       for (int mi = 0; mi < 4; ++mi) {
-        const uint32_t ad = aBase + (mi >> 1) * CGRP_BYTES + rq + thr_off[q & 1][mi & 1];
+        const uint32_t ad = aBase + (mi >> 1) * CGRP_BYTES3 + rq + thr_off[q & 1][mi & 1];
         ax[mi] = ld_shared_f64(ad);
-        ay[mi] = ld_shared_f64(ad + PLANE_BYTES);
+        ay[mi] = ld_shared_f64(ad + PLANE_BYTES3);
         as[mi] = ax[mi] + ay[mi];
       }
 #pragma unroll
       for (int ni = 0; ni < 2; ++ni) {
         const uint32_t ad = bBase + rq + thr_off[q & 1][ni];
         bx[ni] = w * ld_shared_f64(ad);
-        by[ni] = w * ld_shared_f64(ad + PLANE_BYTES);
+        by[ni] = w * ld_shared_f64(ad + PLANE_BYTES3);
         bd[ni] = by[ni] - bx[ni];
       }
 #pragma unroll
@@ -349,13 +356,13 @@ __global__ void __launch_bounds__(256) finalize_kernel(const double* __restrict_
 cudaError_t chi0_f64_configure() {
   cudaError_t e = cudaFuncSetAttribute(chi0_f64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(chi0_f64_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  return cudaFuncSetAttribute(chi0_f64_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES3);
 }
 
 cudaError_t launch_chi0_f64(const Chi0F64Args& a, bool three_m, cudaStream_t s) {
   if (a.n_pairs_padded <= 0 || a.n_tiles <= 0) return cudaSuccess;
   dim3 grid((unsigned)(a.n_tiles * a.n_freq));
-  if (three_m) chi0_f64_3m_kernel<<<grid, kThreads3M, SMEM_BYTES, s>>>(a);
+  if (three_m) chi0_f64_3m_kernel<<<grid, kThreads3M, SMEM_BYTES3, s>>>(a);
   else chi0_f64_kernel<<<grid, kThreads, SMEM_BYTES, s>>>(a);
   return cudaGetLastError();
 }

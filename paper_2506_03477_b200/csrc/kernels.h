@@ -71,7 +71,8 @@ struct Chi0F64Args {
   const int2* d_tiles;        // (tile_i, tile_j), tile_i <= tile_j
   int n_tiles;
 };
-constexpr int kChi0F64KP = 16;  // pairs per pipeline stage (box rows of the tensor map)
+constexpr int kChi0F64KP = 16;    // pairs per pipeline stage of the 4M kernel (box rows of its tensor map)
+constexpr int kChi0F64KP3M = 32;  // same for the 3M kernel
 cudaError_t launch_chi0_f64(const Chi0F64Args& a, bool three_m /*3M complex product (default) or 4M*/, cudaStream_t s);
 cudaError_t chi0_f64_configure();   // sets the dynamic shared-memory attribute once
 
@@ -112,8 +113,12 @@ cudaError_t probe_tf32_mma(cudaStream_t s, double* out_tflops, double* out_ms);
 //   128-byte swizzle give K-major UMMA operand tiles.  Weights: __half wtab16[n_freq][kpad/32][64], per 32-pair
 //   stage  w_h[32] | w_l[32]  with w_h + w_l = fp32(w_j(p) / wscale[j]), wscale[j] a power of two such that
 //   max_p |w_j(p)| / wscale[j] is in (1/2, 1].
+//   FP8-corrected variant: a second workspace "hb8" with rows  h[32] halves | e5m2(v)[32] | e5m2(v - h)[32]
+//   feeds the B operand (same 128 bytes per 32 pairs): a b ~= a_h b_h (kind::f16) + a_l8 b_8 + a_8 b_l8
+//   (kind::f8f6f4, E5M2): the two correction products need only ~3 significant bits.
 struct Chi0F16Args {
   CUtensorMap tmap;      // 3-D FLOAT16 {2*kpad, n_m_pad, 2}, box {64, 64, 1}, SWIZZLE_128B
+  CUtensorMap tmap_b;    // FP8 variant: 3-D UINT8 {4*kpad, n_m_pad, 2}, box {128, 64, 1}, SWIZZLE_128B
   const __half* wtab16;  // [n_freq][kpad/32][64]
   const double* wscale;  // [n_freq]
   const float* zmax;     // batch maximum of |Re z|, |Im z|
@@ -128,9 +133,11 @@ struct Chi0F16Args {
   int n_tiles;
 };
 cudaError_t chi0_f16_configure();
-cudaError_t launch_chi0_f16(const Chi0F16Args& a, int cluster /*CTAs sharing a tile: 1, 2 or 4*/, cudaStream_t s);
+cudaError_t launch_chi0_f16(const Chi0F16Args& a, int cluster /*CTAs sharing a tile: 1, 2 or 4*/, bool fp8,
+                            cudaStream_t s);
 cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs, void* zhl,
-                             int n_m_pad, const float* zmax, cudaStream_t s);
+                             void* zhb8 /*optional FP8-variant B rows*/, int n_m_pad, const float* zmax,
+                             cudaStream_t s);
 cudaError_t launch_z_export_hl16(const void* zhl, long long kpad, int n_m_pad, int n_m, long long n_pairs,
                                  const float* zmax, double2* out, cudaStream_t s);
 cudaError_t launch_weights_scale_hl16(const double* wtab, void* wtab16, double* wscale, long long kpad, long long n_pad,

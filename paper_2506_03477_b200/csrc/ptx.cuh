@@ -168,6 +168,32 @@ __device__ __forceinline__ uint4 ld_shared_u4(uint32_t addr) {
   return v;
 }
 
+// ---- kind::f8f6f4 with E5M2 operands (FP32 accumulate), K = 32 bytes ------------------------------------
+__device__ __forceinline__ uint32_t umma_idesc_e5m2(int m, int n, int neg_a) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)neg_a << 13) | ((uint32_t)(n >> 3) << 17) |
+         ((uint32_t)(m >> 4) << 24);
+}
+// D[tmem] (+)= A[tmem] * B[smem]; A: lane = row, 8 columns, column c = bytes k = 4c .. 4c+3
+__device__ __forceinline__ void umma_f8_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc,
+                                           uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t (&v)[4]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(taddr), "r"(v[0]), "r"(v[1]),
+               "r"(v[2]), "r"(v[3])
+               : "memory");
+}
+// two halves (packed) -> two E5M2 bytes in the low 16 bits (byte 0 = low half), round to nearest, saturating
+__device__ __forceinline__ uint32_t cvt_e5m2x2_f16x2(uint32_t h2) {
+  uint16_t r;
+  asm("cvt.rn.satfinite.e5m2x2.f16x2 %0, %1;" : "=h"(r) : "r"(h2));
+  return (uint32_t)r;
+}
+
 // ---- thread-block clusters: multicast TMA, remote mbarrier arrive ---------------------------------
 __device__ __forceinline__ uint32_t cluster_ctarank() {
   uint32_t r;

@@ -67,6 +67,9 @@ struct qsgw_ctx {
   CUtensorMap tmap2, tmap4;
   bool f16 = false;             // QSGW_PREC_MIXED: FP16-split planes (kernels.h "hl16")
   void* d_zhl = nullptr;
+  void* d_zhb8 = nullptr;        // FP8-corrected variant: B rows h | e5m2(v) | e5m2(v-h)
+  bool fp8 = false;
+  CUtensorMap tmap_hb8;
   double* d_wscale = nullptr;
   float* d_zmax = nullptr;
   int cluster = 1;              // CTAs of a cluster sharing one tile's z boxes (1, 2 or 4)
@@ -130,6 +133,7 @@ void free_all(qsgw_ctx* c) {
   cudaFree(c->d_zws32);
   cudaFree(c->d_wtab32);
   cudaFree(c->d_zhl);
+  cudaFree(c->d_zhb8);
   cudaFree(c->d_wscale);
   cudaFree(c->d_zmax);
   cudaFree(c->d_acc_re);
@@ -320,6 +324,11 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     if (v == 1 || v == 2 || v == 4) c->cluster = v;
   }
   if (const char* ev = getenv("QSGW_F64_4M")) c->f64_3m = atoi(ev) == 0;   // A/B knob for profiles
+  // Correction products in E5M2 when enough pairs are summed per output element: the extra error is
+  // ~4e-5 * sqrt(N_M / pairs summed over the job); below 64 pairs per product function the
+  // three-FP16-product form is used.  QSGW_F16_FP8=0/1 overrides (A/B knob for profiles).
+  c->fp8 = c->f16 && (double)c->n_k * c->max_n_o * c->max_n_u >= 64.0 * c->n_m;
+  if (const char* ev = getenv("QSGW_F16_FP8")) c->fp8 = c->f16 && atoi(ev) != 0;
   if (const char* ev = getenv("QSGW_F16_WIN")) {       // tuning knob: stages per drain window
     const int v = atoi(ev);
     if (v >= 1 && v <= 64) c->win = v;
@@ -331,7 +340,7 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   const size_t z64_bytes = (size_t)2 * c->ncg * c->kpad * qsgw::kCG * sizeof(double);
   const size_t z32_elems = c->n_pass ? (size_t)4 * c->n_m_pad * c->kpad : 0;
   const size_t zhl_bytes = c->f16 ? (size_t)2 * c->n_m_pad * c->kpad * 2 * sizeof(uint16_t) : 0;
-  const size_t z_bytes = z64_bytes + z32_elems * sizeof(float) + zhl_bytes;
+  const size_t z_bytes = z64_bytes + z32_elems * sizeof(float) + zhl_bytes * (c->fp8 ? 2 : 1);
   if (desc->workspace_bytes != 0 && z_bytes > desc->workspace_bytes) {
     char buf[256];
     snprintf(buf, sizeof(buf), "z workspace for %d x %d band pairs needs %zu bytes > workspace_bytes cap %zu; "
@@ -365,6 +374,7 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   if (mixed) QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab32, (size_t)c->n_freq * c->kpad));
   if (c->f16) {
     QSGW_TRY_ALLOC(dev_alloc(c, reinterpret_cast<unsigned char**>(&c->d_zhl), zhl_bytes));
+    if (c->fp8) QSGW_TRY_ALLOC(dev_alloc(c, reinterpret_cast<unsigned char**>(&c->d_zhb8), zhl_bytes));
     QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wscale, (size_t)c->n_freq));
     QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zmax, (size_t)1));
   }
@@ -394,6 +404,7 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   }
   if (c->f16) {
     QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zhl, 0, zhl_bytes, st));
+    if (c->fp8) QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zhb8, 0, zhl_bytes, st));
     QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wscale, 0, sizeof(double) * c->n_freq, st));
     QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zmax, 0, sizeof(float), st));
     QSGW_TRY_CUDA(qsgw::chi0_f16_configure());
@@ -411,7 +422,7 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     const cuuint64_t gdim[4] = {(cuuint64_t)qsgw::kCG, (cuuint64_t)c->kpad, (cuuint64_t)c->ncg, 2};
     const cuuint64_t gstr[3] = {(cuuint64_t)qsgw::kCG * 8, (cuuint64_t)c->kpad * qsgw::kCG * 8,
                                 (cuuint64_t)c->ncg * c->kpad * qsgw::kCG * 8};
-    const cuuint32_t box[4] = {(cuuint32_t)qsgw::kCG, (cuuint32_t)qsgw::kChi0F64KP, 4, 2};
+    const cuuint32_t box[4] = {(cuuint32_t)qsgw::kCG, (cuuint32_t)(c->f64_3m ? qsgw::kChi0F64KP3M : qsgw::kChi0F64KP), 4, 2};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     CUresult r = enc(&c->tmap_z, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->d_zws, gdim, gstr, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -434,6 +445,18 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
       char buf[128];
       snprintf(buf, sizeof(buf), "cuTensorMapEncodeTiled (mixed, hl16 planes) failed with CUresult %d", (int)r);
       return create_fail(c, QSGW_ERR_CUDA, buf);
+    }
+    if (c->fp8) {
+      const cuuint64_t gdim8[3] = {(cuuint64_t)c->kpad * 4, (cuuint64_t)c->n_m_pad, 2};
+      const cuuint32_t box8[3] = {128, 64, 1};
+      r = enc(&c->tmap_hb8, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, c->d_zhb8, gdim8, gstr, box8, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (r != CUDA_SUCCESS) {
+        char buf[128];
+        snprintf(buf, sizeof(buf), "cuTensorMapEncodeTiled (mixed, hb8 planes) failed with CUresult %d", (int)r);
+        return create_fail(c, QSGW_ERR_CUDA, buf);
+      }
     }
   }
   if (c->n_pass) {
@@ -545,7 +568,7 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
     else e = qsgw::launch_zmel_f64(a, ctx->stream);
     if (e == cudaSuccess && ctx->f16)
       e = qsgw::launch_z_to_hl16(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u, ctx->d_zhl,
-                                 ctx->n_m_pad, ctx->d_zmax, ctx->stream);
+                                 ctx->d_zhb8, ctx->n_m_pad, ctx->d_zmax, ctx->stream);
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "zmel kernel launch");
   ctx->launches += (ctx->n_pass || ctx->f16) ? 2 : 1;
@@ -584,8 +607,8 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
       e = qsgw::launch_z_import(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, static_cast<const double2*>(d_z),
                                 ctx->f16 ? ctx->d_zmax : nullptr, ctx->stream);
     if (e == cudaSuccess && ctx->f16) {
-      e = qsgw::launch_z_to_hl16(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, ctx->d_zhl, ctx->n_m_pad,
-                                 ctx->d_zmax, ctx->stream);
+      e = qsgw::launch_z_to_hl16(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, ctx->d_zhl, ctx->d_zhb8,
+                                 ctx->n_m_pad, ctx->d_zmax, ctx->stream);
       ctx->launches += 1;
     }
     if (e == cudaSuccess && ctx->n_pass) {
@@ -621,6 +644,7 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
     if (e != cudaSuccess) return ctx->cuda_fail(e, "weight scaling kernel launch");
     qsgw::Chi0F16Args m;
     m.tmap = ctx->tmap_h;
+    m.tmap_b = ctx->fp8 ? ctx->tmap_hb8 : ctx->tmap_h;
     m.wtab16 = reinterpret_cast<const __half*>(ctx->d_wtab32);   // same bytes per pair as the FP32 table
     m.wscale = ctx->d_wscale;
     m.win = ctx->win;
@@ -635,7 +659,7 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
     m.n_tiles = ctx->n_tiles;
     {
       StageScope ts(ctx, QSGW_STAGE_CHI0);
-      e = qsgw::launch_chi0_f16(m, ctx->cluster, ctx->stream);
+      e = qsgw::launch_chi0_f16(m, ctx->cluster, ctx->fp8, ctx->stream);
     }
     if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 (mixed, FP16 split) kernel launch");
     ctx->launches += 2;

@@ -1,6 +1,7 @@
 // Stage (a): muffin-tin product-basis matrix elements (Eq. 8 with Eq. 4), plus
 // the export/import of the z batch in the boundary layout and the pair-weight table (Eq. 14).
 #include <cuda_fp16.h>
+#include <cuda_fp8.h>
 
 #include "kernels.h"
 #include "ptx.cuh"
@@ -262,7 +263,8 @@ __global__ void weights_to_f32_kernel(const double* __restrict__ wtab, float* __
 // through shared memory as z_to_planes32_kernel; rows of pairs beyond the batch are written as zeros.
 __global__ void __launch_bounds__(256) z_to_hl16_kernel(const double* __restrict__ zws, long long kpad, int ncg,
                                                         int n_m, long long n_pairs, __half* __restrict__ out,
-                                                        int n_m_pad, const float* __restrict__ zmax) {
+                                                        unsigned char* __restrict__ out8, int n_m_pad,
+                                                        const float* __restrict__ zmax) {
   __shared__ float tx[kCG][129], ty[kCG][129];
   const int cg = blockIdx.y;
   const long long p0 = (long long)blockIdx.x * 128;
@@ -294,6 +296,17 @@ __global__ void __launch_bounds__(256) z_to_hl16_kernel(const double* __restrict
     out[o + 32] = lx;
     out[oplane + o] = hy;
     out[oplane + o + 32] = ly;
+    if (out8) {   // FP8-variant B rows: h[32] halves | e5m2(v)[32] | e5m2(v - h)[32]   (128 B per 32 pairs)
+      const long long ob = 2 * ((long long)I * kpad * 2 + (p >> 5) * 64) + (p & 31);      // byte offset in plane
+      unsigned char* bx = out8 + ob;
+      unsigned char* by = out8 + 2 * oplane + ob;
+      reinterpret_cast<__half*>(out8)[o] = hx;
+      reinterpret_cast<__half*>(out8)[oplane + o] = hy;
+      bx[64] = (unsigned char)__nv_cvt_float_to_fp8(x, __NV_SATFINITE, __NV_E5M2);
+      bx[96] = (unsigned char)__nv_cvt_float_to_fp8(x - __half2float(hx), __NV_SATFINITE, __NV_E5M2);
+      by[64] = (unsigned char)__nv_cvt_float_to_fp8(y, __NV_SATFINITE, __NV_E5M2);
+      by[96] = (unsigned char)__nv_cvt_float_to_fp8(y - __half2float(hy), __NV_SATFINITE, __NV_E5M2);
+    }
   }
 }
 
@@ -417,9 +430,10 @@ cudaError_t launch_weights_to_f32(const double* wtab, float* wtab32, long long k
 }
 
 cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs, void* zhl,
-                             int n_m_pad, const float* zmax, cudaStream_t s) {
+                             void* zhb8, int n_m_pad, const float* zmax, cudaStream_t s) {
   dim3 grid((unsigned)((kpad + 127) / 128), ncg);
-  z_to_hl16_kernel<<<grid, 256, 0, s>>>(zws, kpad, ncg, n_m, n_pairs, static_cast<__half*>(zhl), n_m_pad, zmax);
+  z_to_hl16_kernel<<<grid, 256, 0, s>>>(zws, kpad, ncg, n_m, n_pairs, static_cast<__half*>(zhl),
+                                        static_cast<unsigned char*>(zhb8), n_m_pad, zmax);
   return cudaGetLastError();
 }
 

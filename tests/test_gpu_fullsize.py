@@ -42,6 +42,15 @@ def test_cfg3_full_size_mixed():
         _sampled_and_sketch(prob, spin, got, TOL_MIXED)
 
 
+def test_cfg3_full_size_mixed_band_batches():
+    """cfg 3 spin 0, all k-points, O x U split into 16 x 32 band batches: the FP8-corrected products are
+    still selected (216 * 16 * 32 >= 64 * 600) and every batch carries its own scale."""
+    cfg = get_config(3)
+    prob = generate(cfg)
+    got = run_cuda(prob, spin=0, precision=1, max_n_o=16, max_n_u=32)
+    _sampled_and_sketch(prob, 0, got, TOL_MIXED)
+
+
 def test_cfg4_full_size_mixed():
     """cfg 4 in mixed mode, the launch configuration bench.py times (one batch per k-point)."""
     cfg = get_config(4)
@@ -55,8 +64,8 @@ def test_cfg4_full_size_mixed_band_batches():
     every batch carries its own FP16 scale, the result must not depend on the batching."""
     cfg = get_config(4)
     prob = generate(cfg, n_k=2)
-    a = run_cuda(prob, precision=1, n_k_norm=cfg.n_k)
-    b = run_cuda(prob, precision=1, max_n_o=16, n_k_norm=cfg.n_k)
+    a = run_cuda(prob, precision=1)
+    b = run_cuda(prob, precision=1, max_n_o=16)
     num = np.linalg.norm((a - b).reshape(a.shape[0], -1), axis=1)
     den = np.linalg.norm(a.reshape(a.shape[0], -1), axis=1)
     assert (num / den).max() <= TOL_MIXED

@@ -59,11 +59,11 @@ def test_cfg4_one_kpoint_mixed():
     of the full 2400^2 oracle."""
     cfg = get_config(4)
     prob = generate(cfg, n_k=1)
-    got = run_cuda(prob, precision=MIXED, n_k_norm=cfg.n_k)
+    got = run_cuda(prob, precision=MIXED)          # declared N_k = 1: 9 pairs per product function -> FP16 products
     sp = prob.spins[0]
     sel = [0, 9]
     chi = oracle.chi0_ref(sites_of(prob), sp.Ck, sp.Ckq, sp.eps_k, sp.f_k, sp.eps_kq, sp.f_kq,
-                          prob.omega[sel], n_k_norm=cfg.n_k)
+                          prob.omega[sel])
     ref = oracle.hermitian_finalize_ref(chi)
     assert rel_fro_per_freq(got[sel], ref).max() <= TOL_MIXED
 
