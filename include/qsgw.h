@@ -172,6 +172,8 @@ int64_t qsgw_pairs_accumulated(const qsgw_ctx* ctx);    /* band pairs passed to 
 size_t qsgw_device_bytes(const qsgw_ctx* ctx);          /* device memory owned by the context  */
 int32_t qsgw_n_m(const qsgw_ctx* ctx);                  /* N_M                                 */
 int32_t qsgw_n_b(const qsgw_ctx* ctx);                  /* N_b                                 */
+int32_t qsgw_mixed_fp8(const qsgw_ctx* ctx);            /* 1 if QSGW_PREC_MIXED runs its two    */
+                                                        /* correction products in E5M2          */
 const char* qsgw_version(void);
 
 #ifdef __cplusplus

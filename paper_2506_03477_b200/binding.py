@@ -62,7 +62,7 @@ def lib() -> C.CDLL:
                                      C.POINTER(i64)]
     for name in ("qsgw_create", "qsgw_set_product_tensor", "qsgw_zmel_build", "qsgw_chi0_accumulate",
                  "qsgw_chi0_add_kpoint", "qsgw_chi0_finalize", "qsgw_reset", "qsgw_sync",
-                 "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b"):
+                 "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_mixed_fp8"):
         getattr(L, name).restype = i32
     for name in ("qsgw_last_error", "qsgw_last_create_error", "qsgw_version"):
         getattr(L, name).restype = C.c_char_p
@@ -80,6 +80,7 @@ def lib() -> C.CDLL:
     L.qsgw_device_bytes.argtypes = [vp]
     L.qsgw_n_m.argtypes = [vp]
     L.qsgw_n_b.argtypes = [vp]
+    L.qsgw_mixed_fp8.argtypes = [vp]
     _lib = L
     return L
 
@@ -149,6 +150,7 @@ class Chi0Context:
             raise QsgwError(rc, self._L.qsgw_last_create_error().decode())
         self.n_m = self._L.qsgw_n_m(self._h)
         self.n_b = self._L.qsgw_n_b(self._h)
+        self.mixed_fp8 = bool(self._L.qsgw_mixed_fp8(self._h))
 
     def _check(self, rc: int):
         if rc != 0:

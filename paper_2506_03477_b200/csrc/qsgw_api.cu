@@ -233,6 +233,7 @@ int64_t qsgw_pairs_accumulated(const qsgw_ctx* ctx) { return ctx ? ctx->pairs : 
 size_t qsgw_device_bytes(const qsgw_ctx* ctx) { return ctx ? ctx->device_bytes : 0; }
 int32_t qsgw_n_m(const qsgw_ctx* ctx) { return ctx ? ctx->n_m : 0; }
 int32_t qsgw_n_b(const qsgw_ctx* ctx) { return ctx ? ctx->n_b : 0; }
+int32_t qsgw_mixed_fp8(const qsgw_ctx* ctx) { return (ctx && ctx->fp8) ? 1 : 0; }
 
 int32_t qsgw_probe_peak(int32_t kind, double* out_tflops, double* out_ms) {
   g_create_error.clear();
