@@ -47,9 +47,12 @@ struct ZmelArgs {
   long long kpad;
   int ncg;
   float* zmax = nullptr; // optional: atomicMax of |Re z|, |Im z| over the batch (FP16-split mixed mode)
+  int kt = 0;            // DMMA kernel: padded contraction length, max over column groups of sum_seg pad4(b_seg)
 };
 
-cudaError_t launch_zmel_f64(const ZmelArgs& a, cudaStream_t s);
+cudaError_t launch_zmel_f64(const ZmelArgs& a, cudaStream_t s);    // CUDA-core fallback
+cudaError_t launch_zmel_dmma(const ZmelArgs& a, cudaStream_t s);   // step 2 on the FP64 tensor pipe (default)
+size_t zmel_dmma_smem_bytes(int b_max, int kt);
 cudaError_t launch_z_export(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs,
                             double2* out, cudaStream_t s);
 cudaError_t launch_z_import(double* zws, long long kpad, int ncg, int n_m, long long n_pairs,

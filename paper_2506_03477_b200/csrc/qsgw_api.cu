@@ -74,6 +74,7 @@ struct qsgw_ctx {
   float* d_zmax = nullptr;
   int cluster = 1;              // CTAs of a cluster sharing one tile's z boxes (1, 2 or 4)
   int win = 8;                  // stages per TMEM drain window
+  int zmel_kt = 0;              // stage (a) DMMA kernel: padded contraction length (0 = CUDA-core fallback)
   bool f64_3m = true;           // FP64 mode: 3M complex product (QSGW_F64_4M=1 selects the 4M kernel)
   CUtensorMap tmap_h;
   double* d_acc_re = nullptr;
@@ -317,6 +318,17 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     for (int I = pb_off[s]; I < pb_off[s + 1]; ++I) pb_site[I] = s;
 
   c->ncg = (c->n_m + qsgw::kCG - 1) / qsgw::kCG;
+  {   // contraction length of the DMMA stage (a) kernel: column groups may straddle sites
+    int kt = 0;
+    for (int cg = 0; cg < c->ncg; ++cg) {
+      int sum = 0, last = -1;
+      for (int I = cg * qsgw::kCG; I < c->n_m && I < (cg + 1) * qsgw::kCG; ++I)
+        if (pb_site[I] != last) { last = pb_site[I]; sum += (c->orb[last] + 3) & ~3; }
+      if (sum > kt) kt = sum;
+    }
+    const char* ev = getenv("QSGW_ZMEL_DMMA");   // A/B knob: 0 selects the CUDA-core kernel
+    if (qsgw::zmel_dmma_smem_bytes(c->b_max, kt) <= 200 * 1024 && !(ev && atoi(ev) == 0)) c->zmel_kt = kt;
+  }
   const bool mixed = c->precision != QSGW_PREC_FP64;
   c->n_pass = c->precision == QSGW_PREC_MIXED_TF32X3 ? 3 : (c->precision == QSGW_PREC_MIXED_TF32X1 ? 1 : 0);
   c->f16 = c->precision == QSGW_PREC_MIXED;
@@ -557,6 +569,7 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   a.zws = ctx->d_zws;
   a.kpad = ctx->kpad;
   a.ncg = ctx->ncg;
+  a.kt = ctx->zmel_kt;
   cudaError_t e;
   if (ctx->f16) {
     a.zmax = ctx->d_zmax;
@@ -566,7 +579,7 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   {
     StageScope ts(ctx, QSGW_STAGE_ZMEL);
     if (ctx->n_pass) e = qsgw::launch_zmel_mixed(a, ctx->d_zws32, ctx->n_m_pad, ctx->n_pass == 3 ? 1 : 0, ctx->stream);
-    else e = qsgw::launch_zmel_f64(a, ctx->stream);
+    else e = ctx->zmel_kt ? qsgw::launch_zmel_dmma(a, ctx->stream) : qsgw::launch_zmel_f64(a, ctx->stream);
     if (e == cudaSuccess && ctx->f16)
       e = qsgw::launch_z_to_hl16(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u, ctx->d_zhl,
                                  ctx->d_zhb8, ctx->n_m_pad, ctx->d_zmax, ctx->stream);

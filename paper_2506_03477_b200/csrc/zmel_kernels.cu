@@ -402,7 +402,7 @@ cudaError_t launch_pair_weights(const double* eps_k, const double* f_k, const do
 
 // mixed mode: FP64 stage (a) into the FP64 workspace, then one conversion/transposition pass
 cudaError_t launch_zmel_mixed(const ZmelArgs& a, float* zws32, int n_m_pad, int split_lo, cudaStream_t s) {
-  cudaError_t e = launch_zmel_f64(a, s);
+  cudaError_t e = a.kt ? launch_zmel_dmma(a, s) : launch_zmel_f64(a, s);
   if (e != cudaSuccess) return e;
   const long long n_pairs = (long long)a.n_o * a.n_u;
   dim3 grid((unsigned)((a.kpad + 127) / 128), a.ncg);
