@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
     drain((n_stages - 1) / win);
 
     // FP32 window sums (in units 2^(2S) sigma_j) -> FP64 accumulators (exclusive owner of (tile, j))
-    const double sc = a.wscale[j] * exp2(-2.0 * (double)f16_scale_exp(*a.zmax));
+    const double sc = a.wscale[j];     // the batches' 2^(-2S) are folded into the weights (pair_weights_kernel)
     const long long plane = (long long)a.n_m_pad * a.n_m_pad;
     double* dst = (h ? a.acc_im : a.acc_re) + (long long)j * plane +
                   (long long)(tt.x * kTileMx + row) * a.n_m_pad + tt.y * kTileMx;

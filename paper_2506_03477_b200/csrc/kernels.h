@@ -60,7 +60,7 @@ cudaError_t launch_z_import(double* zws, long long kpad, int ncg, int n_m, long 
 cudaError_t launch_pair_weights(const double* eps_k, const double* f_k, const double* eps_kq,
                                 const double* f_kq, int n_o, int n_u, const double* d_omega, int n_freq,
                                 double occ_tol, double* wtab, long long kpad, long long n_pairs_padded,
-                                cudaStream_t s);
+                                const float* zmax /*optional: fold 2^(-2S) of the batch's FP16 scale*/, cudaStream_t s);
 
 struct Chi0F64Args {
   CUtensorMap tmap_z;    // 4-D FLOAT64 {16, kpad, ncg, 2}, box {16, KP, 4, 2}, SWIZZLE_128B

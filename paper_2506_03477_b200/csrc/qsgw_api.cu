@@ -49,7 +49,8 @@ struct qsgw_ctx {
   cudaStream_t stream = nullptr;
   // derived
   int ncg = 0, n_m_pad = 0, n_tiles = 0;
-  long long kpad = 0;
+  long long kpad = 0;           // pair capacity of the z workspace (multiple of 32): several band batches are
+  long long fill = 0;           // staged back to back ([0, fill) is pending) and accumulated by ONE stage (b) launch
   // device
   int* d_pb_site = nullptr;
   int* d_pb_off = nullptr;
@@ -349,11 +350,23 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   const int tile_edge = mixed ? qsgw::kTileMx : qsgw::kTile;
   c->n_m_pad = (int)round_up(c->n_m, tile_edge);
   const long long max_pairs = (long long)c->max_n_o * c->max_n_u;
-  c->kpad = round_up(max_pairs, qsgw::kPairAlign);
-  const size_t z64_bytes = (size_t)2 * c->ncg * c->kpad * qsgw::kCG * sizeof(double);
-  const size_t z32_elems = c->n_pass ? (size_t)4 * c->n_m_pad * c->kpad : 0;
-  const size_t zhl_bytes = c->f16 ? (size_t)2 * c->n_m_pad * c->kpad * 2 * sizeof(uint16_t) : 0;
-  const size_t z_bytes = z64_bytes + z32_elems * sizeof(float) + zhl_bytes * (c->fp8 ? 2 : 1);
+  // Workspace = room for `mult` padded band batches (about 32 Ki pairs): small batches (few bands, many k-points)
+  // are staged back to back and stage (b) runs once per full workspace instead of once per batch.
+  const long long batch_pad = round_up(max_pairs, qsgw::kPairAlign);
+  long long mult = c->n_pass ? 1 : (32768 + batch_pad - 1) / batch_pad;
+  if (const char* ev = getenv("QSGW_STAGE_BATCHES")) {   // A/B knob: batches per stage (b) launch
+    const int v = atoi(ev);
+    if (v >= 1 && !c->n_pass) mult = v;
+  }
+  size_t z64_bytes = 0, z32_elems = 0, zhl_bytes = 0, z_bytes = 0;
+  for (;; --mult) {
+    c->kpad = batch_pad * mult;
+    z64_bytes = (size_t)2 * c->ncg * c->kpad * qsgw::kCG * sizeof(double);
+    z32_elems = c->n_pass ? (size_t)4 * c->n_m_pad * c->kpad : 0;
+    zhl_bytes = c->f16 ? (size_t)2 * c->n_m_pad * c->kpad * 2 * sizeof(uint16_t) : 0;
+    z_bytes = z64_bytes + z32_elems * sizeof(float) + zhl_bytes * (c->fp8 ? 2 : 1);
+    if (mult == 1 || desc->workspace_bytes == 0 || z_bytes <= desc->workspace_bytes) break;
+  }
   if (desc->workspace_bytes != 0 && z_bytes > desc->workspace_bytes) {
     char buf[256];
     snprintf(buf, sizeof(buf), "z workspace for %d x %d band pairs needs %zu bytes > workspace_bytes cap %zu; "
@@ -500,8 +513,12 @@ void qsgw_destroy(qsgw_ctx* ctx) {
   delete ctx;
 }
 
+static int flush_pending(qsgw_ctx* ctx);
+
 int32_t qsgw_sync(qsgw_ctx* ctx) {
   if (!ctx) return QSGW_ERR_INVALID_ARG;
+  int rc = flush_pending(ctx);     // staged band batches are accumulated before the wait
+  if (rc != QSGW_OK) return rc;
   cudaError_t e = cudaStreamSynchronize(ctx->stream);
   if (e != cudaSuccess) return ctx->cuda_fail(e, "cudaStreamSynchronize");
   return QSGW_OK;
@@ -525,9 +542,16 @@ int32_t qsgw_reset(qsgw_ctx* ctx) {
   if (e != cudaSuccess) return ctx->cuda_fail(e, "reset");
   if (ctx->state != ST_CREATED) ctx->state = ST_READY;
   ctx->pairs = 0;
+  ctx->fill = 0;                   // staged, not yet accumulated batches are dropped with the accumulator
   ctx->err.clear();
   return QSGW_OK;
 }
+
+// hl16 / hb8 rows of the staging slot at pair offset `off` (128 bytes per product function and 32 pairs)
+static void* hl_slot(void* base, long long off) {
+  return base ? static_cast<unsigned char*>(base) + (off / qsgw::kPairStage) * 128 : nullptr;
+}
+static int stage_slot(qsgw_ctx* ctx, long long n_pairs, long long* off);
 
 static int check_batch(qsgw_ctx* ctx, int n_o, int n_u) {
   if (n_o < 1 || n_u < 1) return ctx->fail(QSGW_ERR_SHAPE, "band batch must be non-empty (n_o=%d, n_u=%d)", n_o, n_u);
@@ -548,6 +572,9 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   int rc = check_batch(ctx, n_o, n_u);
   if (rc != QSGW_OK) return rc;
 
+  long long off = 0;
+  rc = stage_slot(ctx, (long long)n_o * n_u, &off);
+  if (rc != QSGW_OK) return rc;
   qsgw::ZmelArgs a;
   a.st.n_sites = ctx->n_sites;
   a.st.n_b = ctx->n_b;
@@ -566,7 +593,7 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   a.n_o = n_o;
   a.np_begin = np_begin;
   a.n_u = n_u;
-  a.zws = ctx->d_zws;
+  a.zws = ctx->d_zws + off * qsgw::kCG;
   a.kpad = ctx->kpad;
   a.ncg = ctx->ncg;
   a.kt = ctx->zmel_kt;
@@ -581,20 +608,21 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
     if (ctx->n_pass) e = qsgw::launch_zmel_mixed(a, ctx->d_zws32, ctx->n_m_pad, ctx->n_pass == 3 ? 1 : 0, ctx->stream);
     else e = ctx->zmel_kt ? qsgw::launch_zmel_dmma(a, ctx->stream) : qsgw::launch_zmel_f64(a, ctx->stream);
     if (e == cudaSuccess && ctx->f16)
-      e = qsgw::launch_z_to_hl16(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u, ctx->d_zhl,
-                                 ctx->d_zhb8, ctx->n_m_pad, ctx->d_zmax, ctx->stream);
+      e = qsgw::launch_z_to_hl16(a.zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u,
+                                 hl_slot(ctx->d_zhl, off), hl_slot(ctx->d_zhb8, off), ctx->n_m_pad, ctx->d_zmax,
+                                 ctx->stream);
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "zmel kernel launch");
   ctx->launches += (ctx->n_pass || ctx->f16) ? 2 : 1;
   if (d_z_out) {
     if (ctx->f16)
-      e = qsgw::launch_z_export_hl16(ctx->d_zhl, ctx->kpad, ctx->n_m_pad, ctx->n_m, (long long)n_o * n_u, ctx->d_zmax,
+      e = qsgw::launch_z_export_hl16(hl_slot(ctx->d_zhl, off), ctx->kpad, ctx->n_m_pad, ctx->n_m, (long long)n_o * n_u, ctx->d_zmax,
                                      static_cast<double2*>(d_z_out), ctx->stream);
     else if (ctx->n_pass)
       e = qsgw::launch_z_export32(ctx->d_zws32, ctx->kpad, ctx->n_m_pad, ctx->n_m, (long long)n_o * n_u,
                                   static_cast<double2*>(d_z_out), ctx->stream);
     else
-      e = qsgw::launch_z_export(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u,
+      e = qsgw::launch_z_export(a.zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u,
                               static_cast<double2*>(d_z_out), ctx->stream);
     if (e != cudaSuccess) return ctx->cuda_fail(e, "z export kernel launch");
     ctx->launches += 1;
@@ -606,6 +634,73 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   return QSGW_OK;
 }
 
+// Stage (b) over the staged pairs [0, fill): one launch for all band batches accumulated since the last flush.
+static int flush_pending(qsgw_ctx* ctx) {
+  if (ctx->fill == 0) return QSGW_OK;
+  const long long n_pad = ctx->fill;
+  ctx->fill = 0;
+  cudaError_t e;
+  if (ctx->f16) {
+    {
+      StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
+      e = qsgw::launch_weights_scale_hl16(ctx->d_wtab, ctx->d_wtab32, ctx->d_wscale, ctx->kpad, n_pad, ctx->n_freq,
+                                          ctx->stream);
+    }
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "weight scaling kernel launch");
+    qsgw::Chi0F16Args m;
+    m.tmap = ctx->tmap_h;
+    m.tmap_b = ctx->fp8 ? ctx->tmap_hb8 : ctx->tmap_h;
+    m.wtab16 = reinterpret_cast<const __half*>(ctx->d_wtab32);   // same bytes per pair as the FP32 table
+    m.wscale = ctx->d_wscale;
+    m.win = ctx->win;
+    m.zmax = ctx->d_zmax;
+    m.kpad = ctx->kpad;
+    m.acc_re = ctx->d_acc_re;
+    m.acc_im = ctx->d_acc_im;
+    m.n_m_pad = ctx->n_m_pad;
+    m.n_freq = ctx->n_freq;
+    m.n_stages = (int)(n_pad / qsgw::kPairStage);
+    m.d_tiles = ctx->d_tiles;
+    m.n_tiles = ctx->n_tiles;
+    {
+      StageScope ts(ctx, QSGW_STAGE_CHI0);
+      e = qsgw::launch_chi0_f16(m, ctx->cluster, ctx->fp8, ctx->stream);
+    }
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 (mixed, FP16 split) kernel launch");
+    ctx->launches += 2;
+    return QSGW_OK;
+  }
+  qsgw::Chi0F64Args a;
+  a.tmap_z = ctx->tmap_z;
+  a.wtab = ctx->d_wtab;
+  a.kpad = ctx->kpad;
+  a.acc_re = ctx->d_acc_re;
+  a.acc_im = ctx->d_acc_im;
+  a.n_m_pad = ctx->n_m_pad;
+  a.n_freq = ctx->n_freq;
+  a.n_pairs_padded = n_pad;
+  a.d_tiles = ctx->d_tiles;
+  a.n_tiles = ctx->n_tiles;
+  {
+    StageScope ts(ctx, QSGW_STAGE_CHI0);
+    e = qsgw::launch_chi0_f64(a, ctx->f64_3m, ctx->stream);
+  }
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 kernel launch");
+  ctx->launches += 1;
+  return QSGW_OK;
+}
+
+// Slot of the next band batch in the workspace; flushes the staged batches first when it would not fit.
+static int stage_slot(qsgw_ctx* ctx, long long n_pairs, long long* off) {
+  const long long n_pad = round_up(n_pairs, qsgw::kPairAlign);
+  if (ctx->fill + n_pad > ctx->kpad) {
+    int rc = flush_pending(ctx);
+    if (rc != QSGW_OK) return rc;
+  }
+  *off = ctx->fill;
+  return QSGW_OK;
+}
+
 int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps_k, const double* d_f_k,
                              const double* d_eps_kq, const double* d_f_kq, int32_t n_o, int32_t n_u) {
   if (!ctx) return QSGW_ERR_INVALID_ARG;
@@ -614,15 +709,20 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
   int rc = check_batch(ctx, n_o, n_u);
   if (rc != QSGW_OK) return rc;
   const long long n_pairs = (long long)n_o * n_u;
+  const long long n_pad = round_up(n_pairs, qsgw::kPairAlign);
+  long long off = ctx->fill;       // the slot the last zmel_build wrote
   cudaError_t e;
   if (d_z) {
+    rc = stage_slot(ctx, n_pairs, &off);
+    if (rc != QSGW_OK) return rc;
     e = ctx->f16 ? cudaMemsetAsync(ctx->d_zmax, 0, sizeof(float), ctx->stream) : cudaSuccess;
     if (e == cudaSuccess)
-      e = qsgw::launch_z_import(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, static_cast<const double2*>(d_z),
-                                ctx->f16 ? ctx->d_zmax : nullptr, ctx->stream);
+      e = qsgw::launch_z_import(ctx->d_zws + off * qsgw::kCG, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs,
+                                static_cast<const double2*>(d_z), ctx->f16 ? ctx->d_zmax : nullptr, ctx->stream);
     if (e == cudaSuccess && ctx->f16) {
-      e = qsgw::launch_z_to_hl16(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, ctx->d_zhl, ctx->d_zhb8,
-                                 ctx->n_m_pad, ctx->d_zmax, ctx->stream);
+      e = qsgw::launch_z_to_hl16(ctx->d_zws + off * qsgw::kCG, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs,
+                                 hl_slot(ctx->d_zhl, off), hl_slot(ctx->d_zhb8, off), ctx->n_m_pad, ctx->d_zmax,
+                                 ctx->stream);
       ctx->launches += 1;
     }
     if (e == cudaSuccess && ctx->n_pass) {
@@ -640,49 +740,23 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
       return ctx->fail(QSGW_ERR_SHAPE, "batch %d x %d differs from the last zmel_build (%d x %d)", n_o, n_u,
                        ctx->last_n_o, ctx->last_n_u);
   }
-  const long long n_pad = round_up(n_pairs, qsgw::kPairAlign);
   {
     StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
     e = qsgw::launch_pair_weights(d_eps_k, d_f_k, d_eps_kq, d_f_kq, n_o, n_u, ctx->d_omega, ctx->n_freq,
-                                  ctx->occ_tol, ctx->d_wtab, ctx->kpad, n_pad, ctx->stream);
+                                  ctx->occ_tol, ctx->d_wtab + off, ctx->kpad, n_pad,
+                                  ctx->f16 ? ctx->d_zmax : nullptr, ctx->stream);
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "pair weights kernel launch");
   ctx->launches += 1;
-  if (ctx->f16) {
-    const long long n_pad32 = round_up(n_pairs, qsgw::kPairStage);
-    {
-      StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
-      e = qsgw::launch_weights_scale_hl16(ctx->d_wtab, ctx->d_wtab32, ctx->d_wscale, ctx->kpad, n_pad32, ctx->n_freq,
-                                          ctx->stream);
-    }
-    if (e != cudaSuccess) return ctx->cuda_fail(e, "weight scaling kernel launch");
-    qsgw::Chi0F16Args m;
-    m.tmap = ctx->tmap_h;
-    m.tmap_b = ctx->fp8 ? ctx->tmap_hb8 : ctx->tmap_h;
-    m.wtab16 = reinterpret_cast<const __half*>(ctx->d_wtab32);   // same bytes per pair as the FP32 table
-    m.wscale = ctx->d_wscale;
-    m.win = ctx->win;
-    m.zmax = ctx->d_zmax;
-    m.kpad = ctx->kpad;
-    m.acc_re = ctx->d_acc_re;
-    m.acc_im = ctx->d_acc_im;
-    m.n_m_pad = ctx->n_m_pad;
-    m.n_freq = ctx->n_freq;
-    m.n_stages = (int)(n_pad32 / qsgw::kPairStage);
-    m.d_tiles = ctx->d_tiles;
-    m.n_tiles = ctx->n_tiles;
-    {
-      StageScope ts(ctx, QSGW_STAGE_CHI0);
-      e = qsgw::launch_chi0_f16(m, ctx->cluster, ctx->fp8, ctx->stream);
-    }
-    if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 (mixed, FP16 split) kernel launch");
-    ctx->launches += 2;
-    ctx->pairs += n_pairs;
-    ctx->state = ST_READY;
-    ctx->err.clear();
+  ctx->pairs += n_pairs;
+  ctx->state = ST_READY;   // the batch is staged (or, TF32 variants, consumed below)
+  ctx->err.clear();
+  if (!ctx->n_pass) {
+    ctx->fill = off + n_pad;
     return QSGW_OK;
   }
-  if (ctx->n_pass) {
+  // TF32 variants: one batch per launch, no staging
+  {
     const long long n_pad32 = round_up(n_pairs, qsgw::kPairStage);
     {
       StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
@@ -707,32 +781,7 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
     }
     if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 (mixed) kernel launch");
     ctx->launches += 2;
-    ctx->pairs += n_pairs;
-    ctx->state = ST_READY;
-    ctx->err.clear();
-    return QSGW_OK;
   }
-
-  qsgw::Chi0F64Args a;
-  a.tmap_z = ctx->tmap_z;
-  a.wtab = ctx->d_wtab;
-  a.kpad = ctx->kpad;
-  a.acc_re = ctx->d_acc_re;
-  a.acc_im = ctx->d_acc_im;
-  a.n_m_pad = ctx->n_m_pad;
-  a.n_freq = ctx->n_freq;
-  a.n_pairs_padded = n_pad;
-  a.d_tiles = ctx->d_tiles;
-  a.n_tiles = ctx->n_tiles;
-  {
-    StageScope ts(ctx, QSGW_STAGE_CHI0);
-    e = qsgw::launch_chi0_f64(a, ctx->f64_3m, ctx->stream);
-  }
-  if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 kernel launch");
-  ctx->launches += 1;
-  ctx->pairs += n_pairs;
-  ctx->state = ST_READY;   // the batch has been consumed
-  ctx->err.clear();
   return QSGW_OK;
 }
 
@@ -759,6 +808,8 @@ int32_t qsgw_chi0_finalize(qsgw_ctx* ctx, void* d_chi0_out) {
   if (!ctx) return QSGW_ERR_INVALID_ARG;
   if (ctx->state == ST_CREATED) return ctx->fail(QSGW_ERR_STATE, "nothing accumulated: set_product_tensor not called");
   if (!d_chi0_out) return ctx->fail(QSGW_ERR_INVALID_ARG, "d_chi0_out is NULL");
+  int rc = flush_pending(ctx);
+  if (rc != QSGW_OK) return rc;
   cudaError_t e;
   {
     StageScope ts(ctx, QSGW_STAGE_FINALIZE);

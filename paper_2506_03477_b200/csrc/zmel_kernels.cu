@@ -163,8 +163,10 @@ __global__ void pair_weights_kernel(const double* __restrict__ eps_k, const doub
                                     const double* __restrict__ eps_kq, const double* __restrict__ f_kq,
                                     int n_o, int n_u, const double* __restrict__ omega, int n_freq,
                                     double occ_tol, double* __restrict__ wtab, long long kpad,
-                                    long long n_pairs_padded) {
+                                    long long n_pairs_padded, const float* __restrict__ zmax) {
   const long long n_pairs = (long long)n_o * n_u;
+  // FP16-split mixed mode: this batch's z is staged as z * 2^S, so its weights carry 2^(-2S) (exact)
+  const double zfac = zmax ? exp2(-2.0 * (double)f16_scale_exp(*zmax)) : 1.0;
   for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < n_pairs_padded;
        p += (long long)gridDim.x * blockDim.x) {
     double num = 0.0, d2 = 0.0;
@@ -174,7 +176,7 @@ __global__ void pair_weights_kernel(const double* __restrict__ eps_k, const doub
       const double D = eps_kq[np] - eps_k[n];
       const double occ = f_k[n] * (1.0 - f_kq[np]);
       keep = occ > occ_tol;
-      num = -2.0 * occ * D;
+      num = -2.0 * occ * D * zfac;
       d2 = D * D;
     }
     for (int j = 0; j < n_freq; ++j) {
@@ -264,7 +266,7 @@ __global__ void weights_to_f32_kernel(const double* __restrict__ wtab, float* __
 __global__ void __launch_bounds__(256) z_to_hl16_kernel(const double* __restrict__ zws, long long kpad, int ncg,
                                                         int n_m, long long n_pairs, __half* __restrict__ out,
                                                         unsigned char* __restrict__ out8, int n_m_pad,
-                                                        const float* __restrict__ zmax) {
+                                                        const float* __restrict__ zmax, long long n_rows) {
   __shared__ float tx[kCG][129], ty[kCG][129];
   const int cg = blockIdx.y;
   const long long p0 = (long long)blockIdx.x * 128;
@@ -286,7 +288,7 @@ __global__ void __launch_bounds__(256) z_to_hl16_kernel(const double* __restrict
   for (int idx = threadIdx.x; idx < 128 * kCG; idx += 256) {
     const int col = idx / 128, pl = idx % 128;
     const int I = cg * kCG + col;
-    if (I >= n_m || p0 + pl >= kpad) continue;
+    if (I >= n_m || p0 + pl >= n_rows) continue;
     const float x = tx[col][pl], y = ty[col][pl];
     const __half hx = __float2half_rn(x), hy = __float2half_rn(y);
     const __half lx = __float2half_rn(x - __half2float(hx)), ly = __float2half_rn(y - __half2float(hy));
@@ -394,9 +396,9 @@ cudaError_t launch_z_import(double* zws, long long kpad, int ncg, int n_m, long 
 cudaError_t launch_pair_weights(const double* eps_k, const double* f_k, const double* eps_kq,
                                 const double* f_kq, int n_o, int n_u, const double* d_omega, int n_freq,
                                 double occ_tol, double* wtab, long long kpad, long long n_pairs_padded,
-                                cudaStream_t s) {
+                                const float* zmax, cudaStream_t s) {
   pair_weights_kernel<<<grid_for(n_pairs_padded, 128), 128, 0, s>>>(eps_k, f_k, eps_kq, f_kq, n_o, n_u, d_omega,
-                                                                   n_freq, occ_tol, wtab, kpad, n_pairs_padded);
+                                                                   n_freq, occ_tol, wtab, kpad, n_pairs_padded, zmax);
   return cudaGetLastError();
 }
 
@@ -431,9 +433,10 @@ cudaError_t launch_weights_to_f32(const double* wtab, float* wtab32, long long k
 
 cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs, void* zhl,
                              void* zhb8, int n_m_pad, const float* zmax, cudaStream_t s) {
-  dim3 grid((unsigned)((kpad + 127) / 128), ncg);
+  const long long n_rows = (n_pairs + kPairStage - 1) / kPairStage * kPairStage;   // this batch's padded rows
+  dim3 grid((unsigned)((n_rows + 127) / 128), ncg);
   z_to_hl16_kernel<<<grid, 256, 0, s>>>(zws, kpad, ncg, n_m, n_pairs, static_cast<__half*>(zhl),
-                                        static_cast<unsigned char*>(zhb8), n_m_pad, zmax);
+                                        static_cast<unsigned char*>(zhb8), n_m_pad, zmax, n_rows);
   return cudaGetLastError();
 }
 
