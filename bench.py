@@ -39,6 +39,11 @@ UNIT = "TFLOP/s"
 
 # Nominal dense B200 tensor peaks (guide: B200_PROFILING.md / blackwell_cuda_programming.md) used
 # only as RATIOS to the measured bf16 peak of MEASURED_PEAKS.json.
+# dram__bytes_read.sum + dram__bytes_write.sum of the stage (b) kernel for ONE cfg-4 k-point (21504 pairs), from the
+# `ncu --set full` captures under profiles/ (r01_*_full.md); a launch covers the k-points staged in the workspace.
+NCU_DRAM_BYTES_PER_KPOINT_CFG4 = {"chi0_f64_3m_kernel": 19.889e9 + 0.777e9, "chi0_f64_kernel": 17.107e9 + 0.768e9,
+                                  "chi0_f16_kernel<1,fp8>": 5.826e9 + 0.820e9, "chi0_f16_kernel": 5.537e9 + 0.802e9}
+
 NOMINAL_TF = {"bf16": 2250.0, "f16": 2250.0, "tf32": 1100.0, "f64": 40.0}
 
 
@@ -325,7 +330,10 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
                 "achieved_executed": (ach * passes) if ach else None,
                 "frac_executed": roof_exec_frac,
                 "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": (ach / peak) if ach else None,
-                "traffic": None,
+                "traffic": (NCU_DRAM_BYTES_PER_KPOINT_CFG4[kname] * n_k * n_spin * args.steps / max(chi_n, 1)
+                            if (cfg.index == 4 and kname in NCU_DRAM_BYTES_PER_KPOINT_CFG4 and chi_n) else None),
+                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per cfg-4 k-point (profiles/) x "
+                                  "k-points staged per launch; bytes",
                 "peak_source": peak_src,
                 "peak_probe": probe, "frac_executed_of_probe": (ach * passes / probe) if (ach and probe) else None,
                 "peak_burst": burst_peak, "peak_burst_source": f"{src} bf16 burst {ratio_txt}",
