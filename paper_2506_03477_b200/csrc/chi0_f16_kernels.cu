@@ -22,7 +22,14 @@
 //
 //   The tensor core accumulates FP32 with truncation (bias ~ -4e-8 x MMA steps into one accumulator on
 //   same-sign sums), so D is drained every WIN stages into FP32 register accumulators with round-to-nearest
-//   adds; those go to the FP64 accumulators in HBM once per launch, rescaled by 2^(-2S) / sigma_j.
+//   adds; those go to the FP64 accumulators in HBM once per launch, rescaled by 1 / sigma_j (the 2^(-2S) of each
+//   staged band batch is folded into that batch's weights).
+//
+//   FP8 = true (the default when the job sums >= 64 pairs per product function): the two correction products
+//   a_l b_h + a_h b_l are 2^-11 of the main one and need ~3 significant bits, so each runs as ONE kind::f8f6f4
+//   MMA of K = 32 on E5M2 operands (FP16's exponent range: no rescaling) into the same TMEM accumulators:
+//   8 + 8 instead of 24 MMAs per 32 pairs.  B rows then come from the "hb8" workspace
+//   (h[32] halves | e5m2(v)[32] | e5m2(v - h)[32]: the same 128 bytes, K offsets +64 B and +96 B).
 //
 // Roles (384 threads): warp 0 = TMA producer, warp 1 = MMA issuer (one thread) + TMEM allocator,
 // warps 4-11 = scale + drain ("SA") warps: thread <-> tile row I; warps 4-7 own Re, 8-11 own Im.
