@@ -102,3 +102,35 @@ def test_mixed_zmel_export_and_import():
     got = ctx.chi0_finalize().cpu().numpy()
     assert rel_fro_per_freq(got, oracle_chi(prob)).max() <= TOL_MIXED
     ctx.destroy()
+
+
+def test_mixed_unnormalised_inputs_and_dynamic_range():
+    """The FP16 pieces carry a power-of-two scale taken from each batch's max |z| and from each frequency's
+    max |w|: eigenvectors that are not normalised (x 37, x 1e-3), a large product tensor (x 250) and a
+    frequency grid spanning 0 ... 1e4 Ha must not cost accuracy (no overflow, no flush to zero)."""
+    import dataclasses
+    prob = generate(get_config(1), n_k=6)
+    sp = prob.spins[0]
+    sp2 = dataclasses.replace(sp, Ck=sp.Ck * 37.0, Ckq=sp.Ckq * 1e-3)
+    prob2 = dataclasses.replace(prob, P=prob.P * 250.0, spins=[sp2],
+                                omega=np.array([0.0, 1e-3, 0.3, 7.0, 1e4]))
+    got = run_cuda(prob2, precision=MIXED)
+    assert np.all(np.isfinite(got))
+    assert rel_fro_per_freq(got, oracle_chi(prob2)).max() <= TOL_MIXED
+
+
+def test_mixed_degenerate_batches():
+    """An all-zero z batch (P = 0: batch maximum 0, scale exponent 0) and a batch whose pairs are all dropped by
+    the occupation filter (max |w| = 0) give exact zeros, not NaN."""
+    import torch
+    import paper_2506_03477_b200 as q
+    prob = generate(RAGGED)
+    cfg, sp = prob.cfg, prob.spins[0]
+    for P, f_kq in ((prob.P * 0.0, sp.f_kq), (prob.P, np.ones_like(sp.f_kq))):
+        ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, cfg.n_k, cfg.n_o, cfg.n_u, precision=MIXED)
+        ctx.set_product_tensor(torch.from_numpy(P).cuda())
+        for k in range(cfg.n_k):
+            ctx.chi0_add_kpoint(*[torch.from_numpy(a[k]).cuda() for a in (sp.Ck, sp.Ckq, sp.eps_k, sp.f_k, sp.eps_kq, f_kq)])
+        got = ctx.chi0_finalize().cpu().numpy()
+        ctx.destroy()
+        assert np.all(got == 0.0)
