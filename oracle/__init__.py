@@ -2,5 +2,7 @@
 from .chi0_oracle import (chi0_accumulate_ref, chi0_entries_ref, chi0_ref, chi0_ref_naive,
                           chi0_sketch_ref, hermitian_finalize_ref, pair_weights, zmel_ref)
 
-__all__ = ["chi0_accumulate_ref", "chi0_entries_ref", "chi0_ref", "chi0_ref_naive",
+from .wc_oracle import dielectric_ref, wc_ref
+
+__all__ = ["dielectric_ref", "wc_ref", "chi0_accumulate_ref", "chi0_entries_ref", "chi0_ref", "chi0_ref_naive",
            "chi0_sketch_ref", "hermitian_finalize_ref", "pair_weights", "zmel_ref"]

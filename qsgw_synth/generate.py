@@ -107,3 +107,14 @@ def generate(cfg: WorkloadConfig, seed_offset: int = 0, n_k: int | None = None) 
             eps_k[k], f_k[k], eps_kq[k], f_kq[k] = e_o, fo, e_u, fu
         spins.append(SpinChannel(Ck, Ckq, eps_k, f_k, eps_kq, f_kq))
     return Problem(cfg=cfg, P=P, omega=omega_grid(cfg), spins=spins)
+
+
+def coulomb_eigenvalues(cfg: WorkloadConfig, seed_offset: int = 0) -> np.ndarray:
+    """Synthetic Coulomb eigenvalues v_mu > 0 of the product basis (inputs of Eqs. 10/19):
+    a 4 pi / |q+G|^2-like decaying spectrum, v_mu = 4 pi / (0.3 + 0.05 mu) Ha, jittered by a seeded factor in
+    [0.8, 1.25] and shuffled over the product functions.  The paper's real v_mu(q) come from its Coulomb-matrix
+    diagonalisation (Eq. 7), which needs data only a full code provides; these keep the dynamic range (~1e2)."""
+    rng = np.random.default_rng(BASE_SEED + 1000 + cfg.index + seed_offset)
+    mu = np.arange(cfg.n_m, dtype=np.float64)
+    v = 4.0 * np.pi / (0.3 + 0.05 * mu) * np.exp(rng.uniform(np.log(0.8), np.log(1.25), cfg.n_m))
+    return rng.permutation(v)
