@@ -148,6 +148,19 @@ int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h
                            const double* h_eps_kq, const double* h_f_kq, int32_t n_o,
                            int32_t n_u, void* h_chi0_out, int64_t* out_kernel_launches);
 
+/* Screened Coulomb interaction on the imaginary axis from the polarization (the step after the chi0 build):
+ *   eps_j = 1 - sqrt(v) chi0_j sqrt(v)                    Eq. (10)
+ *   W^c_j = sqrt(v) (eps_j^-1 - 1) sqrt(v)                Eq. (19)
+ * for every frequency j, FP64.  eps_j must be Hermitian positive definite (it is for chi0(i omega) <= 0,
+ * PAPER.md:161); the inverse is formed by a blocked Cholesky factorisation on the FP64 tensor pipe.
+ *   d_chi0   : complex128 [n_freq][N_M][N_M], row-major, full Hermitian (what qsgw_chi0_finalize writes)
+ *   d_v      : float64 [N_M], Coulomb eigenvalues v_mu > 0
+ *   d_wc_out : complex128 [n_freq][N_M][N_M], full Hermitian; may not alias d_chi0
+ *   d_info   : int32 on the device: 0, or 1 + the index of the first non-positive pivot (result then undefined)
+ * Stream-ordered on `cuda_stream` (workspace from the stream-ordered allocator); does not synchronise. */
+int32_t qsgw_wc_from_chi0(int32_t n_m, int32_t n_freq, const void* d_chi0, const double* d_v, void* d_wc_out,
+                          int32_t* d_info, void* cuda_stream);
+
 /* Per-stage device timing, for roofline measurement.  While enabled, every kernel launch of
  * the path is bracketed by CUDA events on the context's stream (Eq. 8 / Eq. 14 stages:
  * QSGW_STAGE_ZMEL, _WEIGHTS, _CHI0, _FINALIZE).  qsgw_stage_time_ms synchronises the stream,

@@ -62,7 +62,7 @@ def lib() -> C.CDLL:
                                      C.POINTER(i64)]
     for name in ("qsgw_create", "qsgw_set_product_tensor", "qsgw_zmel_build", "qsgw_chi0_accumulate",
                  "qsgw_chi0_add_kpoint", "qsgw_chi0_finalize", "qsgw_reset", "qsgw_sync",
-                 "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_mixed_fp8"):
+                 "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_mixed_fp8", "qsgw_wc_from_chi0"):
         getattr(L, name).restype = i32
     for name in ("qsgw_last_error", "qsgw_last_create_error", "qsgw_version"):
         getattr(L, name).restype = C.c_char_p
@@ -81,6 +81,7 @@ def lib() -> C.CDLL:
     L.qsgw_n_m.argtypes = [vp]
     L.qsgw_n_b.argtypes = [vp]
     L.qsgw_mixed_fp8.argtypes = [vp]
+    L.qsgw_wc_from_chi0.argtypes = [i32, i32, vp, vp, vp, vp, vp]
     _lib = L
     return L
 
@@ -229,6 +230,25 @@ class Chi0Context:
             self.destroy()
         except Exception:
             pass
+
+
+def wc_from_chi0(chi0, v, out=None, info=None):
+    """qsgw_wc_from_chi0: W^c[j] = sqrt(v) ((1 - sqrt(v) chi0[j] sqrt(v))^-1 - 1) sqrt(v) on the current
+    torch stream.  chi0: complex128 CUDA tensor [n_freq][N_M][N_M]; v: float64 CUDA tensor [N_M].
+    Returns (W^c, info) -- info is an int32 CUDA tensor (0 = all pivots positive), not synchronised."""
+    import torch
+    L = lib()
+    n_freq, n_m = int(chi0.shape[0]), int(chi0.shape[1])
+    if out is None:
+        out = torch.empty_like(chi0)
+    if info is None:
+        info = torch.zeros(1, dtype=torch.int32, device=chi0.device)
+    stream = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    rc = L.qsgw_wc_from_chi0(n_m, n_freq, _ptr(chi0, torch.complex128), _ptr(v, torch.float64),
+                             _ptr(out, torch.complex128), _ptr(info, torch.int32), stream)
+    if rc != 0:
+        raise QsgwError(rc, L.qsgw_last_create_error().decode())
+    return out, info
 
 
 def chi0_run_host(orb_per_site, pb_per_site, omega, P, Ck, Ckq, eps_k, f_k, eps_kq, f_kq,

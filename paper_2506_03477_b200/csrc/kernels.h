@@ -147,6 +147,23 @@ cudaError_t launch_weights_scale_hl16(const double* wtab, void* wtab16, double* 
                                       int n_freq, cudaStream_t s);
 cudaError_t probe_f16_mma(cudaStream_t s, double* out_tflops, double* out_ms);
 
+// ---- screened Coulomb interaction W^c (wc_kernels.cu) ---------------------------------------------------
+struct ZgemmArgs {       // batched complex FP64 GEMM on 64x64 tiles (see zgemm_dmma_kernel)
+  const double2* A; const double2* B; double2* C;
+  long long lda, ldb, ldc;      // leading dimensions in complex elements
+  long long sA, sB, sC;         // batch strides in complex elements
+  int k;                        // contraction length (multiple of 16)
+  double alpha;                 // real scale
+  int beta_one;                 // 1: C += ..., 0: C = ...
+  int tri;                      // 0 all tiles | 1 lower tiles only | 2 lower tiles and k starts at 64*max(ti,tj)
+};
+// W^c[j] = sqrt(v) ((1 - sqrt(v) chi0[j] sqrt(v))^-1 - 1) sqrt(v) for all frequencies, stream-ordered.
+// work: n_freq * (2 * n_pad^2 + 64 * n_pad + nb * 64 * 64) complex elements, n_pad = ceil64(n_m), nb = n_pad / 64.
+// d_info: 0, or 1 + index of the first non-positive Cholesky pivot (eps not positive definite).
+size_t wc_work_elems(int n_m, int n_freq);
+cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const double* v, double2* wc_out,
+                                double2* work, int* d_info, cudaStream_t s);
+
 // issue-rate probes (probe_kernels.cu): measured MMA-pipe peaks for the roofline denominators
 cudaError_t probe_fp64_mma(cudaStream_t s, double* out_tflops, double* out_ms);
 

@@ -1,0 +1,364 @@
+// Screened Coulomb interaction on the imaginary axis:
+//   eps_j = 1 - sqrt(v) chi0_j sqrt(v)   (Eq. 10),   W^c_j = sqrt(v) (eps_j^-1 - 1) sqrt(v)   (Eq. 19,
+//   PAPER.md:179-182; the paper inverts with a library routine).
+// eps_j is Hermitian positive definite (chi0(i omega) is negative semidefinite), so the inverse goes
+// through a blocked Cholesky factorisation eps = L L^H, X = L^-1, eps^-1 = X^H X, all frequencies batched:
+//   - zgemm_dmma_kernel: complex FP64 GEMM on the FP64 tensor pipe (DMMA.8x8x4), 3M complex product, 64x64 tiles,
+//     operands staged through shared memory; it carries the panel solve, the trailing update (lower tiles only),
+//     the triangular inverse and X^H X (zero blocks of the triangular factor skipped);
+//   - potrf_inv_kernel: Cholesky factor of one 64x64 diagonal block and its triangular inverse in shared memory;
+//   - element-wise kernels for eps and W^c.
+#include "kernels.h"
+#include "ptx.cuh"
+
+namespace qsgw {
+
+namespace {
+
+constexpr int kGT = 64;        // GEMM tile edge
+constexpr int kGK = 16;        // contraction depth per stage
+constexpr int kGLD = 68;       // doubles per shared-memory row (64 + 4: conflict-free DMMA fragment loads)
+constexpr int kGThreads = 256;
+constexpr int kGPlane = kGK * kGLD;                    // doubles of one real plane of one operand stage
+constexpr int kGSmem = 2 * 2 * 2 * kGPlane * 8;        // buffers x operands x (re, im)
+
+// C (+)= alpha * opA(A) opB(B) for one 64x64 tile; all extents multiples of 64 (k: of 16).
+//   A_KC:  A(i,k) = Ap[i*lda + k]            else  A(i,k) = conj(Ap[k*lda + i])   (conjugate transpose)
+//   B_KC:  B(k,j) = conj(Bp[j*ldb + k])      else  B(k,j) = Bp[k*ldb + j]
+// tri: 1 = only tiles with tj <= ti (lower triangle); 2 = additionally start the contraction at 64*max(ti,tj)
+//   (X^H X with X lower triangular: rows k < max(i,j) of X are zero in those columns); 3 = all tiles, contraction
+//   starts at 64*tj (B lower triangular).
+template <bool A_KC, bool B_KC>
+__global__ void __launch_bounds__(kGThreads) zgemm_dmma_kernel(ZgemmArgs a) {
+  const int tj = blockIdx.x, ti = blockIdx.y;
+  if ((a.tri == 1 || a.tri == 2) && tj > ti) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* sm = reinterpret_cast<double*>(smem_raw);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int g = lane >> 2, t = lane & 3;
+  const int wm = warp >> 2, wn = warp & 3;
+  const double2* Ap = a.A + (long long)blockIdx.z * a.sA;
+  const double2* Bp = a.B + (long long)blockIdx.z * a.sB;
+  double2* Cp = a.C + (long long)blockIdx.z * a.sC;
+  const int k0 = (a.tri == 2) ? kGT * max(ti, tj) : (a.tri == 3 ? kGT * tj : 0);
+  const int n_it = (a.k - k0) / kGK;
+
+  // loader mapping: 4 consecutive elements along the contiguous direction per thread
+  const int lr = A_KC ? (tid >> 2) : (tid & 15) * 4;      // A: row i (k-contiguous) | first of 4 rows i
+  const int lk = A_KC ? (tid & 3) * 4 : (tid >> 4);       //    first of 4 k         | k
+  const int br = B_KC ? (tid >> 2) : (tid & 15) * 4;
+  const int bk = B_KC ? (tid & 3) * 4 : (tid >> 4);
+  double2 ra[4], rb[4];
+  auto gload = [&](int it) {
+    const int kk = k0 + it * kGK;
+    if (A_KC) {
+      const double2* p = Ap + (long long)(ti * kGT + lr) * a.lda + kk + lk;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) ra[e] = p[e];
+    } else {
+      const double2* p = Ap + (long long)(kk + lk) * a.lda + ti * kGT + lr;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) ra[e] = p[e];
+    }
+    if (B_KC) {
+      const double2* p = Bp + (long long)(tj * kGT + br) * a.ldb + kk + bk;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) rb[e] = p[e];
+    } else {
+      const double2* p = Bp + (long long)(kk + bk) * a.ldb + tj * kGT + br;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) rb[e] = p[e];
+    }
+  };
+  auto sstore = [&](int buf) {
+    double* ax = sm + buf * 4 * kGPlane;
+    double* ay = ax + kGPlane;
+    double* bx = ay + kGPlane;
+    double* by = bx + kGPlane;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const int ka = A_KC ? lk + e : lk, ia = A_KC ? lr : lr + e;
+      ax[ka * kGLD + ia] = ra[e].x;
+      ay[ka * kGLD + ia] = A_KC ? ra[e].y : -ra[e].y;
+      const int kb = B_KC ? bk + e : bk, jb = B_KC ? br : br + e;
+      bx[kb * kGLD + jb] = rb[e].x;
+      by[kb * kGLD + jb] = B_KC ? -rb[e].y : rb[e].y;
+    }
+  };
+
+  double t1[4][2][2], t2[4][2][2], t3[4][2][2];
+#pragma unroll
+  for (int mi = 0; mi < 4; ++mi)
+#pragma unroll
+    for (int ni = 0; ni < 2; ++ni)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) t1[mi][ni][e] = t2[mi][ni][e] = t3[mi][ni][e] = 0.0;
+
+  if (n_it > 0) {
+    gload(0);
+    sstore(0);
+  }
+  __syncthreads();
+  for (int it = 0; it < n_it; ++it) {
+    const int buf = it & 1;
+    if (it + 1 < n_it) gload(it + 1);
+    const double* ax = sm + buf * 4 * kGPlane;
+    const double* ay = ax + kGPlane;
+    const double* bx = ay + kGPlane;
+    const double* by = bx + kGPlane;
+#pragma unroll
+    for (int q = 0; q < kGK / 4; ++q) {
+      const int ro = (4 * q + t) * kGLD + g;
+      double fx[4], fy[4], fs[4], hx[2], hy[2], hs[2];
+#pragma unroll
+      for (int mi = 0; mi < 4; ++mi) {
+        fx[mi] = ax[ro + 32 * wm + 8 * mi];
+        fy[mi] = ay[ro + 32 * wm + 8 * mi];
+        fs[mi] = fx[mi] + fy[mi];
+      }
+#pragma unroll
+      for (int ni = 0; ni < 2; ++ni) {
+        hx[ni] = bx[ro + 16 * wn + 8 * ni];
+        hy[ni] = by[ro + 16 * wn + 8 * ni];
+        hs[ni] = hx[ni] + hy[ni];
+      }
+#pragma unroll
+      for (int mi = 0; mi < 4; ++mi)
+#pragma unroll
+        for (int ni = 0; ni < 2; ++ni) {
+          dmma884(t1[mi][ni][0], t1[mi][ni][1], fx[mi], hx[ni]);
+          dmma884(t2[mi][ni][0], t2[mi][ni][1], fy[mi], hy[ni]);
+          dmma884(t3[mi][ni][0], t3[mi][ni][1], fs[mi], hs[ni]);
+        }
+    }
+    if (it + 1 < n_it) sstore(buf ^ 1);
+    __syncthreads();
+  }
+
+  // (x + i y)(u + i v): Re = xu - yv = T1 - T2,  Im = (x + y)(u + v) - xu - yv = T3 - T1 - T2
+#pragma unroll
+  for (int mi = 0; mi < 4; ++mi) {
+    const int row = ti * kGT + 32 * wm + 8 * mi + g;
+#pragma unroll
+    for (int ni = 0; ni < 2; ++ni) {
+      const int col = tj * kGT + 16 * wn + 8 * ni + 2 * t;
+      double2* c = Cp + (long long)row * a.ldc + col;
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        double2 v = make_double2(a.alpha * (t1[mi][ni][e] - t2[mi][ni][e]),
+                                 a.alpha * (t3[mi][ni][e] - t1[mi][ni][e] - t2[mi][ni][e]));
+        if (a.beta_one) {
+          const double2 o = c[e];
+          v.x += o.x;
+          v.y += o.y;
+        }
+        c[e] = v;
+      }
+    }
+  }
+}
+
+}  // namespace
+
+namespace {
+
+constexpr int kPB = 64;          // diagonal block edge
+constexpr int kPLD = kPB + 1;
+
+// One CTA per frequency: Cholesky factor L of the 64x64 diagonal block (in place, lower triangle; the strict
+// upper triangle is zeroed) and Linv = L^-1 (lower triangular, dense 64x64 with zero upper part).
+// Unblocked right-looking factorisation and forward substitution in shared memory.
+__global__ void __launch_bounds__(256) potrf_inv_kernel(double2* A, long long lda, long long sA, double2* Linv,
+                                                        long long sL, int block_index, int* info) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  typedef double Plane[kPLD];
+  Plane* lr = reinterpret_cast<Plane*>(smem_raw);      // L (lower), row-major [64][65]
+  Plane* li = lr + kPB;
+  Plane* xr = li + kPB;                                // Linv
+  Plane* xi = xr + kPB;
+  __shared__ double dinv;
+  double2* Ab = A + (long long)blockIdx.x * sA;
+  double2* Lb = Linv + (long long)blockIdx.x * sL;
+  const int tid = threadIdx.x;
+  for (int e = tid; e < kPB * kPB; e += 256) {
+    const int i = e / kPB, j = e % kPB;
+    const double2 v = Ab[(long long)i * lda + j];
+    lr[i][j] = v.x;
+    li[i][j] = (i == j) ? 0.0 : v.y;
+    xr[i][j] = 0.0;
+    xi[i][j] = 0.0;
+  }
+  __syncthreads();
+  for (int c = 0; c < kPB; ++c) {
+    if (tid == 0) {
+      const double d = lr[c][c];
+      if (!(d > 0.0)) {
+        atomicCAS(info, 0, 1 + block_index * kPB + c);
+        dinv = 0.0;
+      } else {
+        const double sd = sqrt(d);
+        lr[c][c] = sd;
+        dinv = 1.0 / sd;
+      }
+    }
+    __syncthreads();
+    const double s = dinv;
+    for (int i = c + 1 + tid; i < kPB; i += 256) {
+      lr[i][c] *= s;
+      li[i][c] *= s;
+    }
+    __syncthreads();
+    // trailing update of the lower triangle: A[i][j] -= L[i][c] conj(L[j][c]),  c < j <= i
+    const int m = kPB - c - 1;
+    for (int e = tid; e < m * m; e += 256) {
+      const int i = c + 1 + e / m, j = c + 1 + e % m;
+      if (j <= i) {
+        const double ar = lr[i][c], ai = li[i][c], br = lr[j][c], bi = li[j][c];
+        lr[i][j] -= ar * br + ai * bi;
+        li[i][j] -= ai * br - ar * bi;
+      }
+    }
+    __syncthreads();
+  }
+  // Linv: column c of X solves L x = e_c (forward substitution), one thread per column
+  if (tid < kPB) {
+    const int c = tid;
+    for (int i = c; i < kPB; ++i) {
+      double sr = (i == c) ? 1.0 : 0.0, si = 0.0;
+      for (int k = c; k < i; ++k) {
+        const double ar = lr[i][k], ai = li[i][k], br = xr[k][c], bi = xi[k][c];
+        sr -= ar * br - ai * bi;
+        si -= ar * bi + ai * br;
+      }
+      const double d = lr[i][i];
+      xr[i][c] = d > 0.0 ? sr / d : 0.0;
+      xi[i][c] = d > 0.0 ? si / d : 0.0;
+    }
+  }
+  __syncthreads();
+  for (int e = tid; e < kPB * kPB; e += 256) {
+    const int i = e / kPB, j = e % kPB;
+    Ab[(long long)i * lda + j] = (j <= i) ? make_double2(lr[i][j], li[i][j]) : make_double2(0.0, 0.0);
+    Lb[(long long)i * kPB + j] = make_double2(xr[i][j], xi[i][j]);
+  }
+}
+
+// eps = 1 - sqrt(v) chi0 sqrt(v) into the padded work matrix (identity in the padding)   (Eq. 10)
+__global__ void wc_form_eps_kernel(const double2* __restrict__ chi0, const double* __restrict__ v, int n_m, int n_pad,
+                                   double2* __restrict__ eps) {
+  const long long total = (long long)n_pad * n_pad;
+  const double2* c = chi0 + (long long)blockIdx.y * n_m * n_m;
+  double2* o = eps + (long long)blockIdx.y * total;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(e / n_pad), j = (int)(e % n_pad);
+    double2 r = make_double2(i == j ? 1.0 : 0.0, 0.0);
+    if (i < n_m && j < n_m) {
+      const double s = sqrt(v[i]) * sqrt(v[j]);
+      const double2 x = c[(long long)i * n_m + j];
+      r.x -= s * x.x;
+      r.y = (i == j) ? 0.0 : -s * x.y;
+    }
+    o[e] = r;
+  }
+}
+
+// 64x64 block copy: X[i-block, i-block] = Linv_ii
+__global__ void wc_copy_block_kernel(const double2* __restrict__ src, long long s_src, double2* __restrict__ dst,
+                                     long long ldd, long long s_dst) {
+  const double2* a = src + (long long)blockIdx.x * s_src;
+  double2* d = dst + (long long)blockIdx.x * s_dst;
+  for (int e = threadIdx.x; e < kPB * kPB; e += blockDim.x) d[(long long)(e / kPB) * ldd + e % kPB] = a[e];
+}
+
+// W^c = sqrt(v) (eps^-1 - 1) sqrt(v) from the lower triangle of eps^-1 (Hermitian mirror, real diagonal)  (Eq. 19)
+__global__ void wc_finish_kernel(const double2* __restrict__ inv, const double* __restrict__ v, int n_m, int n_pad,
+                                 double2* __restrict__ wc) {
+  const long long total = (long long)n_m * n_m;
+  const double2* a = inv + (long long)blockIdx.y * n_pad * n_pad;
+  double2* o = wc + (long long)blockIdx.y * total;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(e / n_m), j = (int)(e % n_m);
+    const double s = sqrt(v[i]) * sqrt(v[j]);
+    double2 x;
+    if (i == j) x = make_double2(a[(long long)i * n_pad + i].x - 1.0, 0.0);
+    else if (j < i) x = a[(long long)i * n_pad + j];
+    else { x = a[(long long)j * n_pad + i]; x.y = -x.y; }
+    o[e] = make_double2(s * x.x, s * x.y);
+  }
+}
+
+template <bool A_KC, bool B_KC>
+cudaError_t zgemm(const ZgemmArgs& a, int m_tiles, int n_tiles, int batch, cudaStream_t s) {
+  if (m_tiles <= 0 || n_tiles <= 0 || a.k <= 0) return cudaSuccess;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(zgemm_dmma_kernel<A_KC, B_KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGSmem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  zgemm_dmma_kernel<A_KC, B_KC><<<dim3(n_tiles, m_tiles, batch), kGThreads, kGSmem, s>>>(a);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+size_t wc_work_elems(int n_m, int n_freq) {
+  const size_t n = (size_t)(n_m + 63) / 64 * 64, nb = n / 64;
+  return (size_t)n_freq * (2 * n * n + 64 * n + nb * 64 * 64);
+}
+
+cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const double* v, double2* wc_out,
+                                double2* work, int* d_info, cudaStream_t s) {
+  const int N = (n_m + 63) / 64 * 64, nb = N / 64;
+  const long long sM = (long long)N * N, sT = 64LL * N, sL = (long long)nb * 4096;
+  double2* Abuf = work;
+  double2* Xbuf = Abuf + (long long)n_freq * sM;
+  double2* Tbuf = Xbuf + (long long)n_freq * sM;
+  double2* Linv = Tbuf + (long long)n_freq * sT;
+  constexpr int kPotrfSmem = 4 * kPB * kPLD * 8;
+  static bool configured = false;
+  cudaError_t e;
+  if (!configured) {
+    e = cudaFuncSetAttribute(potrf_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPotrfSmem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+#define WC_TRY(expr) do { e = (expr); if (e != cudaSuccess) return e; } while (0)
+  WC_TRY(cudaMemsetAsync(d_info, 0, sizeof(int), s));
+  WC_TRY(cudaMemsetAsync(Xbuf, 0, sizeof(double2) * n_freq * sM, s));
+  wc_form_eps_kernel<<<dim3(592, n_freq), 256, 0, s>>>(chi0, v, n_m, N, Abuf);
+  WC_TRY(cudaGetLastError());
+
+  // blocked Cholesky eps = L L^H (right-looking), L in the lower triangle of Abuf
+  for (int j = 0; j < nb; ++j) {
+    double2* Ajj = Abuf + (long long)j * 64 * N + j * 64;
+    potrf_inv_kernel<<<n_freq, 256, kPotrfSmem, s>>>(Ajj, N, sM, Linv + (long long)j * 4096, sL, j, d_info);
+    WC_TRY(cudaGetLastError());
+    const int m = nb - j - 1;
+    if (m == 0) break;
+    double2* panel = Abuf + (long long)(j + 1) * 64 * N + j * 64;
+    ZgemmArgs p{panel, Linv + (long long)j * 4096, panel, N, 64, N, sM, sL, sM, 64, 1.0, 0, 0};
+    WC_TRY((zgemm<true, true>(p, m, 1, n_freq, s)));                       // L21 = A21 Linv_jj^H
+    ZgemmArgs h{panel, panel, Abuf + (long long)(j + 1) * 64 * N + (j + 1) * 64, N, N, N, sM, sM, sM, 64, -1.0, 1, 1};
+    WC_TRY((zgemm<true, true>(h, m, m, n_freq, s)));                       // A22 -= L21 L21^H (lower tiles)
+  }
+  // X = L^-1, row block by row block:  X_ii = Linv_ii,  X[i,0:i] = -Linv_ii (L[i,0:i] X[0:i,0:i])
+  for (int i = 0; i < nb; ++i) {
+    wc_copy_block_kernel<<<n_freq, 256, 0, s>>>(Linv + (long long)i * 4096, sL, Xbuf + (long long)i * 64 * N + i * 64, N, sM);
+    WC_TRY(cudaGetLastError());
+    if (i == 0) continue;
+    ZgemmArgs t{Abuf + (long long)i * 64 * N, Xbuf, Tbuf, N, N, N, sM, sM, sT, 64 * i, 1.0, 0, 3};
+    WC_TRY((zgemm<true, false>(t, 1, i, n_freq, s)));
+    ZgemmArgs x{Linv + (long long)i * 4096, Tbuf, Xbuf + (long long)i * 64 * N, 64, N, N, sL, sT, sM, 64, -1.0, 0, 0};
+    WC_TRY((zgemm<true, false>(x, 1, i, n_freq, s)));
+  }
+  // eps^-1 = X^H X (lower tiles into Abuf), then W^c
+  ZgemmArgs g{Xbuf, Xbuf, Abuf, N, N, N, sM, sM, sM, N, 1.0, 0, 2};
+  WC_TRY((zgemm<false, false>(g, nb, nb, n_freq, s)));
+  wc_finish_kernel<<<dim3(592, n_freq), 256, 0, s>>>(Abuf, v, n_m, N, wc_out);
+  WC_TRY(cudaGetLastError());
+#undef WC_TRY
+  return cudaSuccess;
+}
+
+}  // namespace qsgw
