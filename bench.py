@@ -278,6 +278,29 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
     stage = {nm: ctx.stage_time_ms(i) for i, nm in enumerate(("zmel", "weights", "chi0", "finalize"))}
     ctx.set_stage_timing(False)
     ctx.destroy()
+    # next row of the scope table, reported beside the step, not inside `value`: W^c(i omega) from
+    # the chi0 just built (Eqs. 10, 19): blocked Cholesky inverse of N_omega matrices of order N_M on the GPU.
+    wc = None
+    if precision == q.PREC_FP64 and not args.no_wc and rank == 0:
+        from qsgw_synth import coulomb_eigenvalues
+        d_v = torch.from_numpy(coulomb_eigenvalues(cfg)).to(dev)
+        w_out = torch.empty_like(out)
+        info = torch.zeros(1, dtype=torch.int32, device=dev)
+        q.wc_from_chi0(out, d_v, out=w_out, info=info)                       # warm-up
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 3
+        torch.cuda.synchronize(dev)
+        e0.record()
+        for _ in range(reps):
+            q.wc_from_chi0(out, d_v, out=w_out, info=info)
+        e1.record()
+        torch.cuda.synchronize(dev)
+        wc_ms = e0.elapsed_time(e1) / reps
+        wc_flop = 8.0 * n_f * float(cfg.n_m) ** 3       # n^3 complex multiply-adds per frequency (factor + inverse)
+        wc = {"ms": wc_ms, "value": wc_flop / (wc_ms * 1e-3) / 1e12, "unit": UNIT, "info": int(info.item()),
+              "credited_flop": wc_flop, "what": "qsgw_wc_from_chi0 on the FP64 chi0 of this run (spin 0 / last spin), "
+              "credited n^3/3 (Cholesky) + n^3/3 (triangular inverse) + n^3/3 (X^H X) complex multiply-adds per frequency"}
+        del w_out, d_v
     del d_in, out
     torch.cuda.empty_cache()
 
@@ -373,7 +396,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
 
     return {"mode": mode_name, "value": value, "ms_per_step": ms_total / args.steps, "launches": launches,
             "roofline": roofline, "e2e": e2e, "clocks": clocks, "flops_step": flops_step,
-            "flops_stage_a": fa, "flops_stage_b": fb, "pairs_kept": pairs}
+            "flops_stage_a": fa, "flops_stage_b": fb, "pairs_kept": pairs, "wc": wc}
 
 
 def main_cuda(args):
@@ -433,6 +456,8 @@ def main_cuda(args):
                if args.n_k else {}), "gpu_launches": main["launches"],
             "clocks": main["clocks"]}
     for r in res:
+        if r.get("wc"):
+            line["wc"] = r["wc"]
         if r is not main:
             line[r["mode"]] = r
     if world == 1 and not args.no_cpu:
@@ -464,6 +489,7 @@ def parse_args(argv=None):
                          "the line is then marked config.subset and is not a bench value")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-wc", action="store_true", help="skip the W^c(i omega) leg reported beside the FP64 step")
     return ap.parse_args(argv)
 
 

@@ -84,3 +84,26 @@ def test_cfg4_full_size_fp64():
     prob = generate(cfg)
     got = run_cuda(prob)
     _sampled_and_sketch(prob, 0, got, 1e-11)
+
+
+def test_wc_full_size_cfg4():
+    """W^c at cfg-4 size (N_M = 2400: 38 diagonal blocks, ragged last block) from the ORACLE's chi0 of one
+    k-point at three frequencies (the full-k oracle chi0 is unaffordable; the inverse does not care)."""
+    import torch
+    import paper_2506_03477_b200 as q
+    from qsgw_synth import coulomb_eigenvalues
+    cfg = get_config(4)
+    prob = generate(cfg, n_k=1)
+    sp = prob.spins[0]
+    sel = [0, 8, 15]
+    chi = oracle.hermitian_finalize_ref(oracle.chi0_ref(sites_of(prob), sp.Ck, sp.Ckq, sp.eps_k, sp.f_k, sp.eps_kq,
+                                                        sp.f_kq, prob.omega[sel]))
+    v = coulomb_eigenvalues(cfg)
+    w, info = q.wc_from_chi0(torch.from_numpy(chi).cuda(), torch.from_numpy(v).cuda())
+    torch.cuda.synchronize()
+    got = w.cpu().numpy()
+    ref = oracle.wc_ref(chi, v)
+    assert int(info.item()) == 0
+    num = np.linalg.norm((got - ref).reshape(len(sel), -1), axis=1)
+    den = np.linalg.norm(ref.reshape(len(sel), -1), axis=1)
+    assert (num / den).max() <= 1e-10, num / den
