@@ -157,7 +157,8 @@ int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h
  *   d_v      : float64 [N_M], Coulomb eigenvalues v_mu > 0
  *   d_wc_out : complex128 [n_freq][N_M][N_M], full Hermitian; may not alias d_chi0
  *   d_info   : int32 on the device: 0, or 1 + the index of the first non-positive pivot (result then undefined)
- * Stream-ordered on `cuda_stream` (workspace from the stream-ordered allocator); does not synchronise. */
+ * Stream-ordered on `cuda_stream` (workspace from the stream-ordered allocator); does not synchronise.
+ * On failure the text is in qsgw_last_create_error(). */
 int32_t qsgw_wc_from_chi0(int32_t n_m, int32_t n_freq, const void* d_chi0, const double* d_v, void* d_wc_out,
                           int32_t* d_info, void* cuda_stream);
 
