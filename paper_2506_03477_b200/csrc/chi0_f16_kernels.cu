@@ -76,10 +76,14 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(d_empty + 1);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int j = blockIdx.x % a.n_freq;               // the CSZ CTAs of a cluster: same tile, consecutive j
-  const int2 tt = a.d_tiles[blockIdx.x / a.n_freq];
+  // blockIdx.x = ((tile * n_freq) + j) * split + chunk: the `split` CTAs of a (tile, j) share the staged pairs
+  // (few-tile problems: fills the SMs; their partial sums meet in the FP64 accumulator by atomic adds)
+  const int chunk = blockIdx.x % a.split, bid = blockIdx.x / a.split;
+  const int j = bid % a.n_freq;                      // the CSZ CTAs of a cluster: same tile, consecutive j
+  const int2 tt = a.d_tiles[bid / a.n_freq];
   const bool need_a = FP8 || (tt.x != tt.y);         // f16 split, diagonal tile: the A source is the B tile
-  const int n_stages = a.n_stages, win = a.win;
+  const int s_base = (int)((long long)a.n_stages * chunk / a.split);          // first global stage of this CTA
+  const int n_stages = (int)((long long)a.n_stages * (chunk + 1) / a.split) - s_base, win = a.win;
   const uint32_t rank = CSZ > 1 ? cluster_ctarank() : 0u;
   constexpr uint16_t kMask = (uint16_t)((1u << CSZ) - 1u);
 
@@ -123,11 +127,11 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
           unsigned char* dst = sb + op * C::B_BYTES + plane * kPlaneTileH + rh * kBoxBytes;
           const int row0 = (op ? tt.x : tt.y) * kTileMx + rh * 64;
           const CUtensorMap* tm = (FP8 && !op) ? &a.tmap_b : &a.tmap;       // hb8 rows are addressed in bytes
-          const int c0 = (FP8 && !op) ? s * 128 : s * 64;
+          const int c0 = (FP8 && !op) ? (s_base + s) * 128 : (s_base + s) * 64;
           if (CSZ > 1) tma_load_3d_mc(dst, tm, &full[st], c0, row0, plane, kMask);
           else tma_load_3d(dst, tm, &full[st], c0, row0, plane);
         }
-        bulk_load_1d(sb + C::B_BYTES + C::A_BYTES, wrow + (long long)s * 64, C::W_BYTES, &full[st]);
+        bulk_load_1d(sb + C::B_BYTES + C::A_BYTES, wrow + (long long)(s_base + s) * 64, C::W_BYTES, &full[st]);
       }
     } else if (warp == 1 && lane == 0) {
       // ------------------------------------------------------------------ MMA issuer
@@ -294,12 +298,17 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
     const long long plane = (long long)a.n_m_pad * a.n_m_pad;
     double* dst = (h ? a.acc_im : a.acc_re) + (long long)j * plane +
                   (long long)(tt.x * kTileMx + row) * a.n_m_pad + tt.y * kTileMx;
+    if (a.split > 1) {
 #pragma unroll
-    for (int c = 0; c < 64; ++c) {
-      double2 v = *reinterpret_cast<double2*>(dst + 2 * c);
-      v.x += sc * (double)racc[2 * c];
-      v.y += sc * (double)racc[2 * c + 1];
-      *reinterpret_cast<double2*>(dst + 2 * c) = v;
+      for (int c = 0; c < 128; ++c) atomicAdd(dst + c, sc * (double)racc[c]);
+    } else {
+#pragma unroll
+      for (int c = 0; c < 64; ++c) {
+        double2 v = *reinterpret_cast<double2*>(dst + 2 * c);
+        v.x += sc * (double)racc[2 * c];
+        v.y += sc * (double)racc[2 * c + 1];
+        *reinterpret_cast<double2*>(dst + 2 * c) = v;
+      }
     }
   }
   tc_fence_before();
@@ -389,16 +398,32 @@ cudaError_t chi0_f16_configure() {
   return cudaFuncSetAttribute(f16_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 20480);
 }
 
-cudaError_t launch_chi0_f16(const Chi0F16Args& a, int cluster, bool fp8, cudaStream_t s) {
-  if (a.n_stages <= 0 || a.n_tiles <= 0) return cudaSuccess;
+cudaError_t launch_chi0_f16(const Chi0F16Args& a_in, int cluster, bool fp8, cudaStream_t s) {
+  if (a_in.n_stages <= 0 || a_in.n_tiles <= 0) return cudaSuccess;
+  Chi0F16Args a = a_in;
+  // Few (tile, frequency) work items: split the staged pairs over 2..4 CTAs each, choosing the split that
+  // minimises rounds(CTAs / SMs) / split; every CTA keeps >= 32 stages.  Single-CTA launches only.
+  a.split = 1;
+  if (cluster <= 1) {
+    int n_sm = 148;
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+    const long long items = (long long)a.n_tiles * a.n_freq;
+    double best = (double)((items + n_sm - 1) / n_sm);
+    for (int sp = 2; sp <= 4; ++sp) {
+      if (a.n_stages < 32 * sp || items * sp > 8LL * n_sm) break;
+      const double cost = (double)((items * sp + n_sm - 1) / n_sm) / sp;
+      if (cost < 0.95 * best) { best = cost; a.split = sp; }
+    }
+  }
+  const unsigned grid = (unsigned)(a.n_tiles * a.n_freq * a.split);
   if (fp8) {   // the FP8-corrected variant is built for single-CTA launches only
-    chi0_f16_kernel<1, true><<<dim3((unsigned)(a.n_tiles * a.n_freq)), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
+    chi0_f16_kernel<1, true><<<dim3(grid), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
     return cudaGetLastError();
   }
   if (cluster > 1 && a.n_freq % cluster != 0) cluster = (a.n_freq % 2 == 0) ? 2 : 1;
   if (cluster >= 4) return launch_cluster<4>(a, s);
   if (cluster >= 2) return launch_cluster<2>(a, s);
-  chi0_f16_kernel<1, false><<<dim3((unsigned)(a.n_tiles * a.n_freq)), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
+  chi0_f16_kernel<1, false><<<dim3(grid), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
   return cudaGetLastError();
 }
 

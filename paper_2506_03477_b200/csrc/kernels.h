@@ -132,6 +132,7 @@ struct Chi0F16Args {
   int n_freq;
   int n_stages;          // ceil(n_pairs / 32)
   int win;               // stages per drain window (12 MMA steps into each accumulator per stage)
+  int split = 1;         // CTAs sharing the staged pairs of one (tile, frequency); set by launch_chi0_f16
   const int2* d_tiles;   // 128x128 tiles, tile_i <= tile_j
   int n_tiles;
 };
