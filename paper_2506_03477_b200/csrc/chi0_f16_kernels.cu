@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   // blockIdx.x = ((tile * n_freq) + j) * split + chunk: the `split` CTAs of a (tile, j) share the staged pairs
   // (few-tile problems: fills the SMs; their partial sums meet in the FP64 accumulator by atomic adds)
   const int chunk = blockIdx.x % a.split, bid = blockIdx.x / a.split;
-  const int j = bid % a.n_freq;                      // the CSZ CTAs of a cluster: same tile, consecutive j
+  const int j = a.j0 + bid % a.n_freq;                    // the CSZ CTAs of a cluster: same tile, consecutive j
   const int2 tt = a.d_tiles[bid / a.n_freq];
   const bool need_a = FP8 || (tt.x != tt.y);         // f16 split, diagonal tile: the A source is the B tile
   const int s_base = (int)((long long)a.n_stages * chunk / a.split);          // first global stage of this CTA

@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(kThreads, 2) chi0_f64_kernel(const __grid_cons
   const int g = lane >> 2, t = lane & 3;
   const int wm = warp >> 1, wn = warp & 1;
 
-  const int j = blockIdx.x % a.n_freq;
+  const int j = a.j0 + blockIdx.x % a.n_freq;
   const int tile = blockIdx.x / a.n_freq;
   const int2 tt = a.d_tiles[tile];
   const bool diag = (tt.x == tt.y);
@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
   const int g = lane >> 2, t = lane & 3;
   const int wm = warp >> 2, wn = warp & 3;
 
-  const int j = blockIdx.x % a.n_freq;
+  const int j = a.j0 + blockIdx.x % a.n_freq;
   const int tile = blockIdx.x / a.n_freq;
   const int2 tt = a.d_tiles[tile];
   const bool diag = (tt.x == tt.y);

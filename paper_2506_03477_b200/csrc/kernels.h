@@ -69,7 +69,8 @@ struct Chi0F64Args {
   double* acc_re;
   double* acc_im;
   int n_m_pad;
-  int n_freq;
+  int n_freq;                 // frequencies of this launch: j0 .. j0 + n_freq - 1
+  int j0 = 0;
   long long n_pairs_padded;   // multiple of kPairAlign
   const int2* d_tiles;        // (tile_i, tile_j), tile_i <= tile_j
   int n_tiles;
@@ -132,6 +133,7 @@ struct Chi0F16Args {
   int n_freq;
   int n_stages;          // ceil(n_pairs / 32)
   int win;               // stages per drain window (12 MMA steps into each accumulator per stage)
+  int j0 = 0;            // first frequency of this launch (n_freq = count)
   int split = 1;         // CTAs sharing the staged pairs of one (tile, frequency); set by launch_chi0_f16
   const int2* d_tiles;   // 128x128 tiles, tile_i <= tile_j
   int n_tiles;

@@ -635,18 +635,21 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
 }
 
 // Stage (b) over the staged pairs [0, fill): one launch for all band batches accumulated since the last flush.
-static int flush_pending(qsgw_ctx* ctx) {
+// (frequencies j0 .. j0+nj-1; `first`/`last` mark the first/last frequency group of one flush: the host-buffer
+// driver flushes the last workspace group by group so that the device-to-host copy overlaps the kernels)
+static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
   if (ctx->fill == 0) return QSGW_OK;
   const long long n_pad = ctx->fill;
-  ctx->fill = 0;
+  if (last) ctx->fill = 0;
   cudaError_t e;
   if (ctx->f16) {
-    {
+    if (first) {
       StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
       e = qsgw::launch_weights_scale_hl16(ctx->d_wtab, ctx->d_wtab32, ctx->d_wscale, ctx->kpad, n_pad, ctx->n_freq,
                                           ctx->stream);
+      if (e != cudaSuccess) return ctx->cuda_fail(e, "weight scaling kernel launch");
+      ctx->launches += 1;
     }
-    if (e != cudaSuccess) return ctx->cuda_fail(e, "weight scaling kernel launch");
     qsgw::Chi0F16Args m;
     m.tmap = ctx->tmap_h;
     m.tmap_b = ctx->fp8 ? ctx->tmap_hb8 : ctx->tmap_h;
@@ -658,7 +661,8 @@ static int flush_pending(qsgw_ctx* ctx) {
     m.acc_re = ctx->d_acc_re;
     m.acc_im = ctx->d_acc_im;
     m.n_m_pad = ctx->n_m_pad;
-    m.n_freq = ctx->n_freq;
+    m.n_freq = nj;
+    m.j0 = j0;
     m.n_stages = (int)(n_pad / qsgw::kPairStage);
     m.d_tiles = ctx->d_tiles;
     m.n_tiles = ctx->n_tiles;
@@ -667,7 +671,7 @@ static int flush_pending(qsgw_ctx* ctx) {
       e = qsgw::launch_chi0_f16(m, ctx->cluster, ctx->fp8, ctx->stream);
     }
     if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 (mixed, FP16 split) kernel launch");
-    ctx->launches += 2;
+    ctx->launches += 1;
     return QSGW_OK;
   }
   qsgw::Chi0F64Args a;
@@ -677,7 +681,8 @@ static int flush_pending(qsgw_ctx* ctx) {
   a.acc_re = ctx->d_acc_re;
   a.acc_im = ctx->d_acc_im;
   a.n_m_pad = ctx->n_m_pad;
-  a.n_freq = ctx->n_freq;
+  a.n_freq = nj;
+  a.j0 = j0;
   a.n_pairs_padded = n_pad;
   a.d_tiles = ctx->d_tiles;
   a.n_tiles = ctx->n_tiles;
@@ -689,6 +694,8 @@ static int flush_pending(qsgw_ctx* ctx) {
   ctx->launches += 1;
   return QSGW_OK;
 }
+
+static int flush_pending(qsgw_ctx* ctx) { return flush_range(ctx, 0, ctx->n_freq, true, true); }
 
 // Slot of the next band batch in the workspace; flushes the staged batches first when it would not fit.
 static int stage_slot(qsgw_ctx* ctx, long long n_pairs, long long* off) {
@@ -905,10 +912,37 @@ int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h
     if (rc != QSGW_OK) { g_create_error = c->err; cleanup(); return rc; }
     QSGW_H(cudaEventRecord(done[b], st));
   }
-  rc = qsgw_chi0_finalize(c, dOut);
-  if (rc != QSGW_OK) { g_create_error = c->err; cleanup(); return rc; }
-  QSGW_H(cudaMemcpyAsync(h_chi0_out, dOut, sizeof(double2) * out_e, cudaMemcpyDeviceToHost, st));
-  QSGW_H(cudaStreamSynchronize(st));
+  // The batches still staged are accumulated frequency group by frequency group; each group is finalized and
+  // copied to the host on a second stream while the next group's kernel runs (the 16 N_M^2 result is the one
+  // large transfer of the job).
+  {
+    const int ng = c->n_freq >= 4 ? 4 : 1;
+    cudaStream_t cp = nullptr;
+    cudaEvent_t ready[4] = {nullptr, nullptr, nullptr, nullptr};
+    QSGW_H(cudaStreamCreateWithFlags(&cp, cudaStreamNonBlocking));
+    const size_t plane_pad = (size_t)c->n_m_pad * c->n_m_pad, plane_out = (size_t)nm * nm;
+    cudaError_t ce = cudaSuccess;
+    for (int g = 0; g < ng && rc == QSGW_OK && ce == cudaSuccess; ++g) {
+      const int j0 = (int)((long long)c->n_freq * g / ng), j1 = (int)((long long)c->n_freq * (g + 1) / ng);
+      rc = flush_range(c, j0, j1 - j0, g == 0, g == ng - 1);
+      if (rc != QSGW_OK) break;
+      ce = qsgw::launch_finalize(c->d_acc_re + j0 * plane_pad, c->d_acc_im + j0 * plane_pad, nm, c->n_m_pad, j1 - j0,
+                                 1.0 / (double)c->n_k, dOut + j0 * plane_out, st);
+      c->launches += 1;
+      if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&ready[g], cudaEventDisableTiming);
+      if (ce == cudaSuccess) ce = cudaEventRecord(ready[g], st);
+      if (ce == cudaSuccess) ce = cudaStreamWaitEvent(cp, ready[g], 0);
+      if (ce == cudaSuccess)
+        ce = cudaMemcpyAsync(static_cast<double2*>(h_chi0_out) + j0 * plane_out, dOut + j0 * plane_out,
+                             sizeof(double2) * (j1 - j0) * plane_out, cudaMemcpyDeviceToHost, cp);
+    }
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(cp);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+    for (int g = 0; g < 4; ++g) if (ready[g]) cudaEventDestroy(ready[g]);
+    cudaStreamDestroy(cp);
+    if (rc != QSGW_OK) { g_create_error = c->err; cleanup(); return rc; }
+    if (ce != cudaSuccess) { g_create_error = std::string("result copy: ") + cudaGetErrorString(ce); cleanup(); return QSGW_ERR_CUDA; }
+  }
 #undef QSGW_H
   if (out_kernel_launches) *out_kernel_launches = c->launches;
   cleanup();
