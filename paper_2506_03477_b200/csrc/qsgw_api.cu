@@ -916,7 +916,11 @@ int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h
   // copied to the host on a second stream while the next group's kernel runs (the 16 N_M^2 result is the one
   // large transfer of the job).
   {
-    const int ng = c->n_freq >= 4 ? 4 : 1;
+    int ng = c->n_freq >= 4 ? 4 : 1;
+    if (const char* ev = getenv("QSGW_E2E_GROUPS")) {      // A/B knob: frequency groups of the last flush
+      const int v = atoi(ev);
+      if (v >= 1 && v <= 4 && v <= c->n_freq) ng = v;
+    }
     cudaStream_t cp = nullptr;
     cudaEvent_t ready[4] = {nullptr, nullptr, nullptr, nullptr};
     QSGW_H(cudaStreamCreateWithFlags(&cp, cudaStreamNonBlocking));
