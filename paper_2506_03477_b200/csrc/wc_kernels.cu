@@ -329,18 +329,28 @@ cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const 
   wc_form_eps_kernel<<<dim3(592, n_freq), 256, 0, s>>>(chi0, v, n_m, N, Abuf);
   WC_TRY(cudaGetLastError());
 
-  // blocked Cholesky eps = L L^H (right-looking), L in the lower triangle of Abuf
-  for (int j = 0; j < nb; ++j) {
-    double2* Ajj = Abuf + (long long)j * 64 * N + j * 64;
-    potrf_inv_kernel<<<n_freq, 256, kPotrfSmem, s>>>(Ajj, N, sM, Linv + (long long)j * 4096, sL, j, d_info);
+  // blocked Cholesky eps = L L^H (right-looking), L in the lower triangle of Abuf.  Two 64-column blocks j0, j1 are
+  // factored per step (j1 after a narrow K = 64 update of its own block column), so that the trailing update runs
+  // with K = 128 and touches every C tile half as often.
+  auto block = [&](int r, int c) { return Abuf + (long long)r * 64 * N + (long long)c * 64; };
+  for (int j0 = 0; j0 < nb; j0 += 2) {
+    const int j1 = j0 + 1;
+    potrf_inv_kernel<<<n_freq, 256, kPotrfSmem, s>>>(block(j0, j0), N, sM, Linv + (long long)j0 * 4096, sL, j0, d_info);
     WC_TRY(cudaGetLastError());
-    const int m = nb - j - 1;
-    if (m == 0) break;
-    double2* panel = Abuf + (long long)(j + 1) * 64 * N + j * 64;
-    ZgemmArgs p{panel, Linv + (long long)j * 4096, panel, N, 64, N, sM, sL, sM, 64, 1.0, 0, 0};
-    WC_TRY((zgemm<true, true>(p, m, 1, n_freq, s)));                       // L21 = A21 Linv_jj^H
-    ZgemmArgs h{panel, panel, Abuf + (long long)(j + 1) * 64 * N + (j + 1) * 64, N, N, N, sM, sM, sM, 64, -1.0, 1, 1};
-    WC_TRY((zgemm<true, true>(h, m, m, n_freq, s)));                       // A22 -= L21 L21^H (lower tiles)
+    if (j1 >= nb) break;
+    const int m0 = nb - j1;                                                  // block rows j1 .. nb-1
+    ZgemmArgs p0{block(j1, j0), Linv + (long long)j0 * 4096, block(j1, j0), N, 64, N, sM, sL, sM, 64, 1.0, 0, 0};
+    WC_TRY((zgemm<true, true>(p0, m0, 1, n_freq, s)));                      // L[j1.., j0] = A[j1.., j0] Linv_j0^H
+    ZgemmArgs u0{block(j1, j0), block(j1, j0), block(j1, j1), N, N, N, sM, sM, sM, 64, -1.0, 1, 0};
+    WC_TRY((zgemm<true, true>(u0, m0, 1, n_freq, s)));                      // A[j1.., j1] -= L[j1.., j0] L[j1, j0]^H
+    potrf_inv_kernel<<<n_freq, 256, kPotrfSmem, s>>>(block(j1, j1), N, sM, Linv + (long long)j1 * 4096, sL, j1, d_info);
+    WC_TRY(cudaGetLastError());
+    const int m1 = nb - j1 - 1;                                              // block rows j1+1 .. nb-1
+    if (m1 == 0) break;
+    ZgemmArgs p1{block(j1 + 1, j1), Linv + (long long)j1 * 4096, block(j1 + 1, j1), N, 64, N, sM, sL, sM, 64, 1.0, 0, 0};
+    WC_TRY((zgemm<true, true>(p1, m1, 1, n_freq, s)));                      // L[j1+1.., j1] = A[j1+1.., j1] Linv_j1^H
+    ZgemmArgs h{block(j1 + 1, j0), block(j1 + 1, j0), block(j1 + 1, j1 + 1), N, N, N, sM, sM, sM, 128, -1.0, 1, 1};
+    WC_TRY((zgemm<true, true>(h, m1, m1, n_freq, s)));                      // A22 -= L[.., j0:j1] L[.., j0:j1]^H
   }
   // X = L^-1, row block by row block:  X_ii = Linv_ii,  X[i,0:i] = -Linv_ii (L[i,0:i] X[0:i,0:i])
   for (int i = 0; i < nb; ++i) {
