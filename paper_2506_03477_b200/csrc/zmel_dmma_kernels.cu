@@ -16,10 +16,11 @@ namespace qsgw {
 namespace {
 
 constexpr int kZdThreads = 256;
-constexpr int kZdNB = 4;          // bands n per CTA
+constexpr int kZdNBMax = 6;       // bands n per CTA: template parameter NB in 4..6, chosen per launch (fewest rounds)
 constexpr int kZdRow = 20;        // doubles per T row (16 columns + 4 padding: conflict-free fragment loads)
 constexpr int kZdMaxSeg = 16;     // a 16-column group touches at most 16 sites
 
+template <int kZdNB>
 __global__ void __launch_bounds__(kZdThreads, 2) zmel_dmma_kernel(ZmelArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int bmax = a.st.b_max, kt = a.kt;
@@ -159,22 +160,41 @@ __global__ void __launch_bounds__(kZdThreads, 2) zmel_dmma_kernel(ZmelArgs a) {
 }  // namespace
 
 // Shared memory the DMMA kernel needs for a contraction length kt (padded, summed over a column group's
-// segments); the caller falls back to the CUDA-core kernel when this exceeds the per-CTA limit.
-size_t zmel_dmma_smem_bytes(int b_max, int kt) {
-  return sizeof(double) * ((size_t)2 * kZdNB * b_max + (size_t)2 * kZdNB * kt * kZdRow);
+// segments) at the largest band block; the caller falls back to the CUDA-core kernel when this exceeds the limit.
+static size_t smem_for(int nb, int b_max, int kt) {
+  return sizeof(double) * ((size_t)2 * nb * b_max + (size_t)2 * nb * kt * kZdRow);
 }
+size_t zmel_dmma_smem_bytes(int b_max, int kt) { return smem_for(kZdNBMax, b_max, kt); }
 
-cudaError_t launch_zmel_dmma(const ZmelArgs& a, cudaStream_t s) {
-  const size_t smem = zmel_dmma_smem_bytes(a.st.b_max, a.kt);
+template <int NB>
+static cudaError_t launch_nb(const ZmelArgs& a, cudaStream_t s) {
+  const size_t smem = smem_for(NB, a.st.b_max, a.kt);
   static size_t configured = 0;
   if (smem > 48 * 1024 && smem > configured) {
-    cudaError_t e = cudaFuncSetAttribute(zmel_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(zmel_dmma_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = smem;
   }
-  dim3 grid(a.ncg, (a.n_o + kZdNB - 1) / kZdNB);
-  zmel_dmma_kernel<<<grid, kZdThreads, smem, s>>>(a);
+  dim3 grid(a.ncg, (a.n_o + NB - 1) / NB);
+  zmel_dmma_kernel<NB><<<grid, kZdThreads, smem, s>>>(a);
   return cudaGetLastError();
+}
+
+cudaError_t launch_zmel_dmma(const ZmelArgs& a, cudaStream_t s) {
+  // bands per CTA: the choice with the fewest rounds x bands (2 CTAs per SM when the shared memory allows)
+  int n_sm = 148;
+  cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+  int best_nb = 4;
+  long long best = -1;
+  for (int nb = 4; nb <= kZdNBMax; ++nb) {
+    const int per_sm = smem_for(nb, a.st.b_max, a.kt) <= 110 * 1024 ? 2 : 1;
+    const long long ctas = (long long)a.ncg * ((a.n_o + nb - 1) / nb);
+    const long long cost = ((ctas + (long long)n_sm * per_sm - 1) / ((long long)n_sm * per_sm)) * nb;
+    if (best < 0 || cost < best) { best = cost; best_nb = nb; }
+  }
+  if (best_nb == 6) return launch_nb<6>(a, s);
+  if (best_nb == 5) return launch_nb<5>(a, s);
+  return launch_nb<4>(a, s);
 }
 
 }  // namespace qsgw
