@@ -192,11 +192,16 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
   const int g = lane >> 2, t = lane & 3;
   const int wm = warp >> 2, wn = warp & 3;
 
-  const int j = a.j0 + blockIdx.x % a.n_freq;
-  const int tile = blockIdx.x / a.n_freq;
+  // blockIdx.x = ((tile * n_freq) + j) * split + chunk: `split` CTAs share the staged pairs of a (tile, j) when
+  // the grid would not fill the SMs; their partial sums meet in the accumulator by atomic adds
+  const int chunk = blockIdx.x % a.split, bid = blockIdx.x / a.split;
+  const int j = a.j0 + bid % a.n_freq;
+  const int tile = bid / a.n_freq;
   const int2 tt = a.d_tiles[tile];
   const bool diag = (tt.x == tt.y);
-  const int n_iter = (int)(a.n_pairs_padded / KP3);
+  const int n_all = (int)(a.n_pairs_padded / KP3);
+  const int it_base = (int)((long long)n_all * chunk / a.split);
+  const int n_iter = (int)((long long)n_all * (chunk + 1) / a.split) - it_base;
   const double* wrow = a.wtab + (long long)j * a.kpad;
 
   if (tid == 0) {
@@ -213,9 +218,10 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
   auto issue = [&](int slot, int it) {
     unsigned char* dstA = sm + slot * (2 * OPER_BYTES3);
     mbar_arrive_expect_tx(&full[slot], stage_bytes);
-    tma_load_4d(dstA, &a.tmap_z, &full[slot], 0, it * KP3, tt.x * 4, 0);
-    if (!diag) tma_load_4d(dstA + OPER_BYTES3, &a.tmap_z, &full[slot], 0, it * KP3, tt.y * 4, 0);
-    bulk_load_1d(wsm + slot * KP3, wrow + (long long)it * KP3, W_BYTES3, &full[slot]);
+    const int gi = it_base + it;
+    tma_load_4d(dstA, &a.tmap_z, &full[slot], 0, gi * KP3, tt.x * 4, 0);
+    if (!diag) tma_load_4d(dstA + OPER_BYTES3, &a.tmap_z, &full[slot], 0, gi * KP3, tt.y * 4, 0);
+    bulk_load_1d(wsm + slot * KP3, wrow + (long long)gi * KP3, W_BYTES3, &full[slot]);
   };
 
   if (tid == 0) {
@@ -298,14 +304,24 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
     for (int ni = 0; ni < 2; ++ni) {
       const int col = tt.y * kTile + (2 * wn + ni) * 8 + 2 * t;
       const long long off = (long long)row * a.n_m_pad + col;
-      double2 r = *reinterpret_cast<double2*>(are + off);
-      r.x += t1[mi][ni][0] + t2[mi][ni][0];
-      r.y += t1[mi][ni][1] + t2[mi][ni][1];
-      *reinterpret_cast<double2*>(are + off) = r;
-      double2 m = *reinterpret_cast<double2*>(aim + off);
-      m.x += t3[mi][ni][0] + (t1[mi][ni][0] - t2[mi][ni][0]);
-      m.y += t3[mi][ni][1] + (t1[mi][ni][1] - t2[mi][ni][1]);
-      *reinterpret_cast<double2*>(aim + off) = m;
+      const double r0 = t1[mi][ni][0] + t2[mi][ni][0], r1 = t1[mi][ni][1] + t2[mi][ni][1];
+      const double m0 = t3[mi][ni][0] + (t1[mi][ni][0] - t2[mi][ni][0]);
+      const double m1 = t3[mi][ni][1] + (t1[mi][ni][1] - t2[mi][ni][1]);
+      if (a.split > 1) {
+        atomicAdd(are + off, r0);
+        atomicAdd(are + off + 1, r1);
+        atomicAdd(aim + off, m0);
+        atomicAdd(aim + off + 1, m1);
+      } else {
+        double2 r = *reinterpret_cast<double2*>(are + off);
+        r.x += r0;
+        r.y += r1;
+        *reinterpret_cast<double2*>(are + off) = r;
+        double2 m = *reinterpret_cast<double2*>(aim + off);
+        m.x += m0;
+        m.y += m1;
+        *reinterpret_cast<double2*>(aim + off) = m;
+      }
     }
   }
 }
@@ -359,9 +375,22 @@ cudaError_t chi0_f64_configure() {
   return cudaFuncSetAttribute(chi0_f64_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES3);
 }
 
-cudaError_t launch_chi0_f64(const Chi0F64Args& a, bool three_m, cudaStream_t s) {
-  if (a.n_pairs_padded <= 0 || a.n_tiles <= 0) return cudaSuccess;
-  dim3 grid((unsigned)(a.n_tiles * a.n_freq));
+cudaError_t launch_chi0_f64(const Chi0F64Args& a_in, bool three_m, cudaStream_t s) {
+  if (a_in.n_pairs_padded <= 0 || a_in.n_tiles <= 0) return cudaSuccess;
+  Chi0F64Args a = a_in;
+  a.split = 1;
+  if (three_m) {   // few (tile, frequency) items (1 CTA/SM): split the staged pairs over 2..4 CTAs (see launch_chi0_f16)
+    int n_sm = 148;
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+    const long long items = (long long)a.n_tiles * a.n_freq, n_it = a.n_pairs_padded / KP3;
+    double best = (double)((items + n_sm - 1) / n_sm);
+    for (int sp = 2; sp <= 4; ++sp) {
+      if (n_it < 16 * sp || items * sp > 8LL * n_sm) break;
+      const double cost = (double)((items * sp + n_sm - 1) / n_sm) / sp;
+      if (cost < 0.95 * best) { best = cost; a.split = sp; }
+    }
+  }
+  dim3 grid((unsigned)(a.n_tiles * a.n_freq * a.split));
   if (three_m) chi0_f64_3m_kernel<<<grid, kThreads3M, SMEM_BYTES3, s>>>(a);
   else chi0_f64_kernel<<<grid, kThreads, SMEM_BYTES, s>>>(a);
   return cudaGetLastError();

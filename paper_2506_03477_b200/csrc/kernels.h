@@ -71,6 +71,7 @@ struct Chi0F64Args {
   int n_m_pad;
   int n_freq;                 // frequencies of this launch: j0 .. j0 + n_freq - 1
   int j0 = 0;
+  int split = 1;              // CTAs sharing the staged pairs of one (tile, frequency); set by launch_chi0_f64 (3M)
   long long n_pairs_padded;   // multiple of kPairAlign
   const int2* d_tiles;        // (tile_i, tile_j), tile_i <= tile_j
   int n_tiles;
