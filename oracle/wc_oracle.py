@@ -32,3 +32,11 @@ def wc_ref(chi0: np.ndarray, v: np.ndarray) -> np.ndarray:
     for j in range(eps.shape[0]):
         out[j] = sv[:, None] * (np.linalg.inv(eps[j]) - eye) * sv[None, :]
     return out
+
+
+def rotate_to_coulomb_basis_ref(chi0: np.ndarray, U: np.ndarray) -> np.ndarray:
+    """chi0 in the orthonormal basis E_mu = sum_I M_I U[I, mu] that diagonalises the Coulomb matrix (Eq. 7,
+    PAPER.md:118; Z in terms of E_mu, Eq. 8):  z_mu = sum_I U[I, mu] z_I, hence
+    chi0_{mu nu} = sum_{IJ} conj(U[I, mu]) chi0_{IJ} U[J, nu] = (U^H chi0 U)_{mu nu}  for every frequency."""
+    U = np.asarray(U, dtype=np.complex128)
+    return np.stack([U.conj().T @ c @ U for c in np.asarray(chi0, dtype=np.complex128)])

@@ -82,3 +82,33 @@ def test_coulomb_eigenvalue_recipe():
         v = coulomb_eigenvalues(cfg)
         assert v.shape == (cfg.n_m,) and np.all(v > 0) and np.array_equal(v, coulomb_eigenvalues(cfg))
         assert 0.8 * 4 * np.pi / (0.3 + 0.05 * (cfg.n_m - 1)) <= v.min() and v.max() <= 1.25 * 4 * np.pi / 0.3
+
+
+def test_rotation_equals_rotating_z_before_accumulation():
+    """Pins the index / conjugation convention of rotate_to_coulomb_basis_ref against the definition: rotating
+    the matrix elements, z_mu = sum_I U[I, mu] z_I, and accumulating gives the same chi0 as U^H chi0 U."""
+    from qsgw_synth import haar_unitary
+    cfg = get_config(0)
+    prob = generate(cfg, n_k=2)
+    sp = prob.spins[0]
+    sites = [prob.P_site(s) for s in range(cfg.n_sites)]
+    rng = np.random.default_rng(11)
+    U = haar_unitary(rng, cfg.n_m)
+    acc_I = np.zeros((len(prob.omega), cfg.n_m, cfg.n_m), dtype=np.complex128)
+    acc_mu = np.zeros_like(acc_I)
+    for k in range(2):
+        z = oracle.zmel_ref(sites, sp.Ck[k], sp.Ckq[k])
+        w = oracle.pair_weights(sp.eps_k[k], sp.f_k[k], sp.eps_kq[k], sp.f_kq[k], prob.omega)
+        oracle.chi0_accumulate_ref(acc_I, z, w)
+        oracle.chi0_accumulate_ref(acc_mu, z @ U, w)               # z_mu[n, n', mu] = sum_I z[n, n', I] U[I, mu]
+    rot = oracle.rotate_to_coulomb_basis_ref(acc_I, U)
+    assert np.linalg.norm(rot - acc_mu) <= 1e-13 * np.linalg.norm(acc_mu)
+    # unitary invariants and the trivial cases
+    for j in (0, 3):
+        assert np.allclose(np.linalg.eigvalsh((rot[j] + rot[j].conj().T) / 2),
+                           np.linalg.eigvalsh((acc_I[j] + acc_I[j].conj().T) / 2), rtol=1e-11, atol=1e-13)
+        assert np.trace(rot[j]) == pytest.approx(np.trace(acc_I[j]), rel=1e-12)
+    assert np.array_equal(oracle.rotate_to_coulomb_basis_ref(acc_I, np.eye(cfg.n_m)), acc_I)
+    U2 = haar_unitary(rng, cfg.n_m)
+    assert np.allclose(oracle.rotate_to_coulomb_basis_ref(rot, U2), oracle.rotate_to_coulomb_basis_ref(acc_I, U @ U2),
+                       rtol=1e-11, atol=1e-14)
