@@ -162,6 +162,16 @@ int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h
 int32_t qsgw_wc_from_chi0(int32_t n_m, int32_t n_freq, const void* d_chi0, const double* d_v, void* d_wc_out,
                           int32_t* d_info, void* cuda_stream);
 
+/* chi0 in the orthonormal basis E_mu = sum_I M_I U[I, mu] that diagonalises the Coulomb matrix (Eq. 7,
+ * PAPER.md:118; Eq. 8 is written in terms of E_mu): z_mu = sum_I U[I, mu] z_I, hence
+ *   chi0_out[j] = U^H chi0[j] U        for every frequency j (two batched FP64 tensor-pipe GEMMs),
+ * the representation Eqs. (10)/(19) and qsgw_wc_from_chi0 (with the eigenvalues v_mu) are stated in.
+ *   d_chi0 : complex128 [n_freq][N_M][N_M] row-major;  d_U : complex128 [N_M][N_M] row-major, U[I][mu], unitary
+ *   d_out  : complex128 [n_freq][N_M][N_M], Hermitian (upper triangle mirrored); may not alias d_chi0
+ * Stream-ordered, no synchronisation; error text in qsgw_last_create_error(). */
+int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_chi0, const void* d_U, void* d_out,
+                                   void* cuda_stream);
+
 /* Per-stage device timing, for roofline measurement.  While enabled, every kernel launch of
  * the path is bracketed by CUDA events on the context's stream (Eq. 8 / Eq. 14 stages:
  * QSGW_STAGE_ZMEL, _WEIGHTS, _CHI0, _FINALIZE).  qsgw_stage_time_ms synchronises the stream,

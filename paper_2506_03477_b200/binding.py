@@ -62,7 +62,7 @@ def lib() -> C.CDLL:
                                      C.POINTER(i64)]
     for name in ("qsgw_create", "qsgw_set_product_tensor", "qsgw_zmel_build", "qsgw_chi0_accumulate",
                  "qsgw_chi0_add_kpoint", "qsgw_chi0_finalize", "qsgw_reset", "qsgw_sync",
-                 "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_mixed_fp8", "qsgw_wc_from_chi0"):
+                 "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_mixed_fp8", "qsgw_wc_from_chi0", "qsgw_chi0_to_coulomb_basis"):
         getattr(L, name).restype = i32
     for name in ("qsgw_last_error", "qsgw_last_create_error", "qsgw_version"):
         getattr(L, name).restype = C.c_char_p
@@ -82,6 +82,7 @@ def lib() -> C.CDLL:
     L.qsgw_n_b.argtypes = [vp]
     L.qsgw_mixed_fp8.argtypes = [vp]
     L.qsgw_wc_from_chi0.argtypes = [i32, i32, vp, vp, vp, vp, vp]
+    L.qsgw_chi0_to_coulomb_basis.argtypes = [i32, i32, vp, vp, vp, vp]
     _lib = L
     return L
 
@@ -249,6 +250,21 @@ def wc_from_chi0(chi0, v, out=None, info=None):
     if rc != 0:
         raise QsgwError(rc, L.qsgw_last_create_error().decode())
     return out, info
+
+
+def chi0_to_coulomb_basis(chi0, U, out=None):
+    """qsgw_chi0_to_coulomb_basis: U^H chi0[j] U for every frequency on the current torch stream."""
+    import torch
+    L = lib()
+    n_freq, n_m = int(chi0.shape[0]), int(chi0.shape[1])
+    if out is None:
+        out = torch.empty_like(chi0)
+    stream = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    rc = L.qsgw_chi0_to_coulomb_basis(n_m, n_freq, _ptr(chi0, torch.complex128), _ptr(U, torch.complex128),
+                                      _ptr(out, torch.complex128), stream)
+    if rc != 0:
+        raise QsgwError(rc, L.qsgw_last_create_error().decode())
+    return out
 
 
 def chi0_run_host(orb_per_site, pb_per_site, omega, P, Ck, Ckq, eps_k, f_k, eps_kq, f_kq,

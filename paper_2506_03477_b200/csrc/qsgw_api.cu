@@ -854,6 +854,31 @@ int32_t qsgw_wc_from_chi0(int32_t n_m, int32_t n_freq, const void* d_chi0, const
   return QSGW_OK;
 }
 
+int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_chi0, const void* d_U, void* d_out,
+                                   void* cuda_stream) {
+  g_create_error.clear();
+  if (!d_chi0 || !d_U || !d_out) { g_create_error = "NULL argument"; return QSGW_ERR_INVALID_ARG; }
+  if (d_chi0 == d_out) { g_create_error = "d_out aliases d_chi0"; return QSGW_ERR_INVALID_ARG; }
+  if (n_m < 1 || n_freq < 1) { g_create_error = "n_m and n_freq must be positive"; return QSGW_ERR_SHAPE; }
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    cudaGetLastError();
+    g_create_error = "no CUDA device";
+    return QSGW_ERR_UNSUPPORTED;
+  }
+  if (prop.major != 10) { g_create_error = "kernels are built for sm_100a only"; return QSGW_ERR_UNSUPPORTED; }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  double2* work = nullptr;
+  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::rotate_work_elems(n_m, n_freq), st);
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("workspace allocation failed: ") + cudaGetErrorString(e); return QSGW_ERR_ALLOC; }
+  e = qsgw::launch_rotate_basis(n_m, n_freq, static_cast<const double2*>(d_chi0), static_cast<const double2*>(d_U),
+                                static_cast<double2*>(d_out), work, st);
+  cudaFreeAsync(work, st);
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("rotation kernels: ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
+  return QSGW_OK;
+}
+
 int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h_Ck, const void* h_Ckq,
                            const double* h_eps_k, const double* h_f_k, const double* h_eps_kq, const double* h_f_kq,
                            int32_t n_o, int32_t n_u, void* h_chi0_out, int64_t* out_kernel_launches) {

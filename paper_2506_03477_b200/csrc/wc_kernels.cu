@@ -372,3 +372,62 @@ cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const 
 }
 
 }  // namespace qsgw
+
+// ---- chi0 in the Coulomb eigenbasis: chi0_{mu nu} = (U^H chi0 U)_{mu nu}  (E_mu = sum_I M_I U[I,mu]; Eqs. 7, 8) ----
+namespace qsgw {
+
+namespace {
+
+// [batch][n][n] -> [batch][N][N], zero padded (`unit_pad`: ones on the padded diagonal)
+__global__ void wc_pad_kernel(const double2* __restrict__ src, int n, int N, int unit_pad, double2* __restrict__ dst) {
+  const long long total = (long long)N * N;
+  const double2* a = src + (long long)blockIdx.y * n * n;
+  double2* o = dst + (long long)blockIdx.y * total;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(e / N), j = (int)(e % N);
+    o[e] = (i < n && j < n) ? a[(long long)i * n + j] : make_double2((unit_pad && i == j) ? 1.0 : 0.0, 0.0);
+  }
+}
+
+// [batch][N][N] -> [batch][n][n], upper triangle kept, lower = conj(upper), real diagonal
+__global__ void wc_unpad_hermitian_kernel(const double2* __restrict__ src, int n, int N, double2* __restrict__ dst) {
+  const long long total = (long long)n * n;
+  const double2* a = src + (long long)blockIdx.y * N * N;
+  double2* o = dst + (long long)blockIdx.y * total;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(e / n), j = (int)(e % n);
+    double2 x;
+    if (i == j) x = make_double2(a[(long long)i * N + i].x, 0.0);
+    else if (i < j) x = a[(long long)i * N + j];
+    else { x = a[(long long)j * N + i]; x.y = -x.y; }
+    o[e] = x;
+  }
+}
+
+}  // namespace
+
+size_t rotate_work_elems(int n_m, int n_freq) {
+  const size_t n = (size_t)(n_m + 63) / 64 * 64;
+  return (size_t)(2 * n_freq + 1) * n * n;
+}
+
+cudaError_t launch_rotate_basis(int n_m, int n_freq, const double2* chi0, const double2* U, double2* out, double2* work,
+                                cudaStream_t s) {
+  const int N = (n_m + 63) / 64 * 64, nb = N / 64;
+  const long long sM = (long long)N * N;
+  double2* Cpad = work;
+  double2* Tpad = Cpad + (long long)n_freq * sM;
+  double2* Upad = Tpad + (long long)n_freq * sM;
+  cudaError_t e;
+  wc_pad_kernel<<<dim3(592, n_freq), 256, 0, s>>>(chi0, n_m, N, 0, Cpad);
+  wc_pad_kernel<<<dim3(592, 1), 256, 0, s>>>(U, n_m, N, 1, Upad);
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  ZgemmArgs t{Cpad, Upad, Tpad, N, N, N, sM, 0, sM, N, 1.0, 0, 0};                 // T = chi0 U
+  if ((e = zgemm<true, false>(t, nb, nb, n_freq, s)) != cudaSuccess) return e;
+  ZgemmArgs r{Upad, Tpad, Cpad, N, N, N, 0, sM, sM, N, 1.0, 0, 0};                 // U^H T
+  if ((e = zgemm<false, false>(r, nb, nb, n_freq, s)) != cudaSuccess) return e;
+  wc_unpad_hermitian_kernel<<<dim3(592, n_freq), 256, 0, s>>>(Cpad, n_m, N, out);
+  return cudaGetLastError();
+}
+
+}  // namespace qsgw

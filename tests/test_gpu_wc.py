@@ -80,3 +80,24 @@ def test_wc_argument_errors():
     with pytest.raises(q.QsgwError) as ei:
         q.wc_from_chi0(chi, v, out=chi)
     assert ei.value.code == 1
+
+
+@pytest.mark.parametrize("idx", [0, 1])
+def test_rotation_to_coulomb_basis(idx):
+    """U^H chi0 U on the GPU (two batched DMMA GEMMs) against the oracle; then the chain rotate -> W^c."""
+    import torch
+    import paper_2506_03477_b200 as q
+    from qsgw_synth import haar_unitary
+    cfg = get_config(idx)
+    prob = generate(cfg, n_k=3)
+    chi = oracle_chi(prob)
+    U = haar_unitary(np.random.default_rng(21 + idx), cfg.n_m)
+    got = q.chi0_to_coulomb_basis(torch.from_numpy(chi).cuda(), torch.from_numpy(U).cuda())
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    ref = oracle.rotate_to_coulomb_basis_ref(chi, U)
+    assert rel_fro_per_freq(got, ref).max() <= 1e-12
+    assert np.array_equal(got, np.conj(np.transpose(got, (0, 2, 1))))
+    v = coulomb_eigenvalues(cfg)
+    w, info = _gpu_wc(got, v)
+    assert info == 0 and rel_fro_per_freq(w, oracle.wc_ref(ref, v)).max() <= TOL_WC
