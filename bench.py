@@ -300,7 +300,21 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
         wc = {"ms": wc_ms, "value": wc_flop / (wc_ms * 1e-3) / 1e12, "unit": UNIT, "info": int(info.item()),
               "credited_flop": wc_flop, "what": "qsgw_wc_from_chi0 on the FP64 chi0 of this run (spin 0 / last spin), "
               "credited n^3/3 (Cholesky) + n^3/3 (triangular inverse) + n^3/3 (X^H X) complex multiply-adds per frequency"}
-        del w_out, d_v
+        # chi0 in the Coulomb eigenbasis first (U^H chi0 U; the representation Eqs. 10/19 are stated in)
+        from qsgw_synth import haar_unitary
+        import numpy as _np
+        d_U = torch.from_numpy(haar_unitary(_np.random.default_rng(7), cfg.n_m)).to(dev)
+        q.chi0_to_coulomb_basis(out, d_U, out=w_out)
+        torch.cuda.synchronize(dev)
+        e0.record()
+        for _ in range(reps):
+            q.chi0_to_coulomb_basis(out, d_U, out=w_out)
+        e1.record()
+        torch.cuda.synchronize(dev)
+        rot_ms = e0.elapsed_time(e1) / reps
+        wc["rotate_ms"] = rot_ms
+        wc["rotate_value"] = 2 * 8.0 * n_f * float(cfg.n_m) ** 3 / (rot_ms * 1e-3) / 1e12   # two n^3 GEMMs per frequency
+        del w_out, d_v, d_U
     del d_in, out
     torch.cuda.empty_cache()
 
