@@ -43,31 +43,32 @@ __global__ void __launch_bounds__(kGThreads) zgemm_dmma_kernel(ZgemmArgs a) {
   const int k0 = (a.tri == 2) ? kGT * max(ti, tj) : (a.tri == 3 ? kGT * tj : 0);
   const int n_it = (a.k - k0) / kGK;
 
-  // loader mapping: 4 consecutive elements along the contiguous direction per thread
-  const int lr = A_KC ? (tid >> 2) : (tid & 15) * 4;      // A: row i (k-contiguous) | first of 4 rows i
-  const int lk = A_KC ? (tid & 3) * 4 : (tid >> 4);       //    first of 4 k         | k
-  const int br = B_KC ? (tid >> 2) : (tid & 15) * 4;
-  const int bk = B_KC ? (tid & 3) * 4 : (tid >> 4);
+  // loader mapping (4 elements per thread and operand), interleaved so that both the global loads (consecutive
+  // lanes -> consecutive 16-byte elements) and the transposing shared-memory stores (2 wavefronts per warp store,
+  // the minimum for 8-byte words) are conflict-free:
+  //   k-contiguous operand:  row = tid/4,  k = tid%4 + 4e;     mn-contiguous operand:  k = tid/16,  row = tid%16 + 16e
+  const int a_r = A_KC ? (tid >> 2) : (tid & 15), a_k = A_KC ? (tid & 3) : (tid >> 4);
+  const int b_r = B_KC ? (tid >> 2) : (tid & 15), b_k = B_KC ? (tid & 3) : (tid >> 4);
   double2 ra[4], rb[4];
   auto gload = [&](int it) {
     const int kk = k0 + it * kGK;
     if (A_KC) {
-      const double2* p = Ap + (long long)(ti * kGT + lr) * a.lda + kk + lk;
+      const double2* p = Ap + (long long)(ti * kGT + a_r) * a.lda + kk + a_k;
 #pragma unroll
-      for (int e = 0; e < 4; ++e) ra[e] = p[e];
+      for (int e = 0; e < 4; ++e) ra[e] = p[4 * e];
     } else {
-      const double2* p = Ap + (long long)(kk + lk) * a.lda + ti * kGT + lr;
+      const double2* p = Ap + (long long)(kk + a_k) * a.lda + ti * kGT + a_r;
 #pragma unroll
-      for (int e = 0; e < 4; ++e) ra[e] = p[e];
+      for (int e = 0; e < 4; ++e) ra[e] = p[16 * e];
     }
     if (B_KC) {
-      const double2* p = Bp + (long long)(tj * kGT + br) * a.ldb + kk + bk;
+      const double2* p = Bp + (long long)(tj * kGT + b_r) * a.ldb + kk + b_k;
 #pragma unroll
-      for (int e = 0; e < 4; ++e) rb[e] = p[e];
+      for (int e = 0; e < 4; ++e) rb[e] = p[4 * e];
     } else {
-      const double2* p = Bp + (long long)(kk + bk) * a.ldb + tj * kGT + br;
+      const double2* p = Bp + (long long)(kk + b_k) * a.ldb + tj * kGT + b_r;
 #pragma unroll
-      for (int e = 0; e < 4; ++e) rb[e] = p[e];
+      for (int e = 0; e < 4; ++e) rb[e] = p[16 * e];
     }
   };
   auto sstore = [&](int buf) {
@@ -77,10 +78,10 @@ __global__ void __launch_bounds__(kGThreads) zgemm_dmma_kernel(ZgemmArgs a) {
     double* by = bx + kGPlane;
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
-      const int ka = A_KC ? lk + e : lk, ia = A_KC ? lr : lr + e;
+      const int ka = A_KC ? a_k + 4 * e : a_k, ia = A_KC ? a_r : a_r + 16 * e;
       ax[ka * kGLD + ia] = ra[e].x;
       ay[ka * kGLD + ia] = A_KC ? ra[e].y : -ra[e].y;
-      const int kb = B_KC ? bk + e : bk, jb = B_KC ? br : br + e;
+      const int kb = B_KC ? b_k + 4 * e : b_k, jb = B_KC ? b_r : b_r + 16 * e;
       bx[kb * kGLD + jb] = rb[e].x;
       by[kb * kGLD + jb] = B_KC ? -rb[e].y : rb[e].y;
     }
