@@ -1,6 +1,8 @@
 """GPU parity: the CUDA path (through the C-ABI) against the oracle, element by element on the
 same seeded inputs.  Tolerances (BASELINE.json:north_star): relative Frobenius error per
 frequency <= 1e-11 in FP64 mode, <= 2e-5 in mixed mode."""
+import dataclasses
+
 import numpy as np
 import pytest
 
@@ -237,3 +239,31 @@ def test_invariants_on_gpu_output():
         ev = np.linalg.eigvalsh(got[j])
         assert ev.max() <= 1e-12 * abs(ev.min())
     assert np.all(np.diff(nrm) < 0)
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_random_small_shapes(seed):
+    """Seeded random cells: 1-6 sites with 1-14 orbitals and 1-40 product functions each (column groups that
+    straddle up to several sites, N_M below one tile or over several), 1-7 x 1-19 bands, random band batches,
+    1-6 frequencies; FP64 at 1e-11 and mixed at 2e-5 against the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    s = int(rng.integers(1, 7))
+    cfg = WorkloadConfig(name=f"rand{seed}", index=100 + seed,
+                         orb_per_site=tuple(int(x) for x in rng.integers(1, 15, s)),
+                         pb_per_site=tuple(int(x) for x in rng.integers(1, 41, s)),
+                         n_k=int(rng.integers(1, 5)), n_spin=1, n_o=1, n_u=1, n_freq=int(rng.integers(1, 7)),
+                         kind="insulator", eps_occ=(-0.45, 0.0), eps_unocc=(0.02, 1.1))
+    if sum(cfg.orb_per_site) < 2:                                    # the generator needs two bands
+        cfg = dataclasses.replace(cfg, orb_per_site=(2,) + cfg.orb_per_site[1:])
+    n_b = sum(cfg.orb_per_site)
+    n_o = int(rng.integers(1, min(7, n_b - 1) + 1))                 # the generator takes O and U from disjoint columns
+    n_u = int(rng.integers(1, min(19, n_b - n_o) + 1))
+    cfg = dataclasses.replace(cfg, n_o=n_o, n_u=n_u)
+    prob = generate(cfg)
+    ref = oracle_chi(prob)
+    mo, mu = int(rng.integers(1, n_o + 1)), int(rng.integers(1, n_u + 1))
+    for precision, tol in ((0, TOL_FP64), (1, TOL_MIXED)):
+        got = run_cuda(prob, precision=precision, max_n_o=mo, max_n_u=mu)
+        err = rel_fro_per_freq(got, ref).max()
+        assert err <= tol, (cfg, mo, mu, precision, err)
+        check_hermitian(got)
