@@ -101,3 +101,23 @@ def test_rotation_to_coulomb_basis(idx):
     v = coulomb_eigenvalues(cfg)
     w, info = _gpu_wc(got, v)
     assert info == 0 and rel_fro_per_freq(w, oracle.wc_ref(ref, v)).max() <= TOL_WC
+
+
+@pytest.mark.parametrize("n", [1, 7, 63, 64, 65, 127, 128, 130, 200])
+def test_wc_and_rotation_block_edges(n):
+    """Orders around the 64-block edges (one block, exactly full blocks, one element over, odd block counts:
+    the two-blocks-per-step Cholesky ends on a single block) with a seeded negative-semidefinite chi0."""
+    import torch
+    import paper_2506_03477_b200 as q
+    from qsgw_synth import haar_unitary
+    rng = np.random.default_rng(300 + n)
+    a = rng.standard_normal((2, n, max(1, n // 2))) + 1j * rng.standard_normal((2, n, max(1, n // 2)))
+    chi = -(a @ np.conj(np.transpose(a, (0, 2, 1)))) / n                      # rank-deficient, <= 0
+    chi[1] *= 0.01
+    v = rng.uniform(0.3, 30.0, n)
+    got, info = _gpu_wc(chi, v)
+    assert info == 0 and rel_fro_per_freq(got, oracle.wc_ref(chi, v)).max() <= TOL_WC
+    U = haar_unitary(rng, n)
+    rot = q.chi0_to_coulomb_basis(torch.from_numpy(chi).cuda(), torch.from_numpy(U).cuda())
+    torch.cuda.synchronize()
+    assert rel_fro_per_freq(rot.cpu().numpy(), oracle.rotate_to_coulomb_basis_ref(chi, U)).max() <= 1e-12
