@@ -134,3 +134,26 @@ def test_mixed_degenerate_batches():
         got = ctx.chi0_finalize().cpu().numpy()
         ctx.destroy()
         assert np.all(got == 0.0)
+
+
+@pytest.mark.parametrize("seed_offset", [0, 1, 2])
+def test_fp8_corrected_products_medium_size(seed_offset):
+    """The E5M2-corrected variant at a size the full oracle affords: N_M = 144 (two ragged 128-tiles), 16 x 40
+    bands, 16 k-points = 71 pairs per product function (>= 64: the variant is selected), three seeds.
+    Error model 4e-5 * sqrt(N_M / pairs) = 4.7e-6 plus the accumulation bias; bar 2e-5."""
+    import torch
+    import paper_2506_03477_b200 as q
+    from qsgw_synth import WorkloadConfig
+    cfg = WorkloadConfig(name="fp8mid", index=90, orb_per_site=(20, 25, 15), pb_per_site=(50, 60, 34), n_k=16,
+                         n_spin=1, n_o=16, n_u=40, n_freq=6, kind="insulator", eps_occ=(-0.45, 0.0),
+                         eps_unocc=(0.03, 1.2))
+    prob = generate(cfg, seed_offset=seed_offset)
+    ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, cfg.n_k, cfg.n_o, cfg.n_u, precision=MIXED)
+    assert ctx.mixed_fp8
+    ctx.destroy()
+    got = run_cuda(prob, precision=MIXED)
+    err = rel_fro_per_freq(got, oracle_chi(prob))
+    assert err.max() <= TOL_MIXED, err
+    small = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, 1, 4, 8, precision=MIXED)
+    assert not small.mixed_fp8                      # 32 pairs for 144 product functions: three FP16 products
+    small.destroy()
