@@ -165,6 +165,7 @@ struct ZgemmArgs {       // batched complex FP64 GEMM on 64x64 tiles (see zgemm_
 // work: n_freq * (2 * n_pad^2 + 64 * n_pad + nb * 64 * 64) complex elements, n_pad = ceil64(n_m), nb = n_pad / 64.
 // d_info: 0, or 1 + index of the first non-positive Cholesky pivot (eps not positive definite).
 size_t wc_work_elems(int n_m, int n_freq);
+cudaError_t wc_configure();
 // chi0 -> U^H chi0 U for all frequencies (work: rotate_work_elems complex elements)
 size_t rotate_work_elems(int n_m, int n_freq);
 cudaError_t launch_rotate_basis(int n_m, int n_freq, const double2* chi0, const double2* U, double2* out, double2* work,

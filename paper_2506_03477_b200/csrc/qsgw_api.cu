@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -221,6 +222,42 @@ int validate_desc(const qsgw_desc* d, std::string& why) {
     }
   }
   return QSGW_OK;
+}
+
+}  // namespace
+
+namespace {
+
+cudaError_t wc_configure_once() {
+  static std::once_flag once;
+  static cudaError_t result = cudaSuccess;
+  std::call_once(once, [] { result = qsgw::wc_configure(); });
+  return result;
+}
+
+// Internal stream and in-flight executable graphs of qsgw_wc_from_chi0 (destroyed once their event completed).
+struct WcGraphs {
+  std::mutex mu;
+  cudaStream_t stream = nullptr;
+  struct Item { cudaGraphExec_t exec; cudaEvent_t done; };
+  std::vector<Item> pending;
+  void sweep() {
+    size_t keep = 0;
+    for (size_t i = 0; i < pending.size(); ++i) {
+      if (cudaEventQuery(pending[i].done) == cudaSuccess) {
+        cudaGraphExecDestroy(pending[i].exec);
+        cudaEventDestroy(pending[i].done);
+      } else {
+        cudaGetLastError();
+        pending[keep++] = pending[i];
+      }
+    }
+    pending.resize(keep);
+  }
+};
+WcGraphs& wc_graphs() {
+  static WcGraphs* g = new WcGraphs();   // never destroyed: no CUDA calls at process exit
+  return *g;
 }
 
 }  // namespace
@@ -844,11 +881,59 @@ int32_t qsgw_wc_from_chi0(int32_t n_m, int32_t n_freq, const void* d_chi0, const
   }
   if (prop.major != 10) { g_create_error = "kernels are built for sm_100a only"; return QSGW_ERR_UNSUPPORTED; }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  cudaError_t e = wc_configure_once();
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("kernel attributes: ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
   double2* work = nullptr;
-  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::wc_work_elems(n_m, n_freq), st);
+  e = cudaMallocAsync(reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::wc_work_elems(n_m, n_freq), st);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("workspace allocation failed: ") + cudaGetErrorString(e); return QSGW_ERR_ALLOC; }
-  e = qsgw::launch_wc_from_chi0(n_m, n_freq, static_cast<const double2*>(d_chi0), d_v, static_cast<double2*>(d_wc_out),
-                                work, d_info, st);
+  // The factorisation is ~420 small dependent launches: they are captured into a CUDA graph on an internal
+  // stream (the caller's stream may be the legacy default stream, which cannot be captured) and launched as one
+  // unit between two events, so that a busy host cannot starve the GPU.  Any capture failure falls back to plain
+  // launches on the caller's stream.
+  bool done = false;
+  const char* no_graph = getenv("QSGW_WC_GRAPH");
+  if (!(no_graph && atoi(no_graph) == 0)) {
+    WcGraphs& G = wc_graphs();
+    std::lock_guard<std::mutex> lock(G.mu);
+    G.sweep();
+    cudaEvent_t ev_in = nullptr, ev_out = nullptr;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    bool ok = G.stream != nullptr || cudaStreamCreateWithFlags(&G.stream, cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&ev_in, cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&ev_out, cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaEventRecord(ev_in, st) == cudaSuccess && cudaStreamWaitEvent(G.stream, ev_in, 0) == cudaSuccess;
+    if (ok && cudaStreamBeginCapture(G.stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+      const cudaError_t le = qsgw::launch_wc_from_chi0(n_m, n_freq, static_cast<const double2*>(d_chi0), d_v,
+                                                       static_cast<double2*>(d_wc_out), work, d_info, G.stream);
+      const cudaError_t ce = cudaStreamEndCapture(G.stream, &graph);
+      ok = le == cudaSuccess && ce == cudaSuccess && graph != nullptr &&
+           cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess && cudaGraphLaunch(exec, G.stream) == cudaSuccess;
+    } else {
+      ok = false;
+    }
+    if (graph) cudaGraphDestroy(graph);
+    if (ok) {
+      ok = cudaEventRecord(ev_out, G.stream) == cudaSuccess && cudaStreamWaitEvent(st, ev_out, 0) == cudaSuccess;
+      G.pending.push_back({exec, ev_out});      // destroyed by a later sweep once ev_out has completed
+      exec = nullptr;
+      ev_out = nullptr;
+      done = ok;
+    }
+    if (exec) cudaGraphExecDestroy(exec);
+    if (ev_in) cudaEventDestroy(ev_in);
+    if (ev_out) cudaEventDestroy(ev_out);
+    if (!done) cudaGetLastError();
+  }
+  e = cudaSuccess;
+  if (!done && no_graph && atoi(no_graph) == 2) {      // QSGW_WC_GRAPH=2: the graph path is mandatory (tests)
+    cudaFreeAsync(work, st);
+    g_create_error = "CUDA graph capture of the W^c launch sequence failed";
+    return QSGW_ERR_CUDA;
+  }
+  if (!done)
+    e = qsgw::launch_wc_from_chi0(n_m, n_freq, static_cast<const double2*>(d_chi0), d_v,
+                                  static_cast<double2*>(d_wc_out), work, d_info, st);
   cudaFreeAsync(work, st);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("W^c kernels: ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
   return QSGW_OK;
@@ -870,7 +955,9 @@ int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_ch
   if (prop.major != 10) { g_create_error = "kernels are built for sm_100a only"; return QSGW_ERR_UNSUPPORTED; }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   double2* work = nullptr;
-  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::rotate_work_elems(n_m, n_freq), st);
+  cudaError_t e = wc_configure_once();
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("kernel attributes: ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
+  e = cudaMallocAsync(reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::rotate_work_elems(n_m, n_freq), st);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("workspace allocation failed: ") + cudaGetErrorString(e); return QSGW_ERR_ALLOC; }
   e = qsgw::launch_rotate_basis(n_m, n_freq, static_cast<const double2*>(d_chi0), static_cast<const double2*>(d_U),
                                 static_cast<double2*>(d_out), work, st);

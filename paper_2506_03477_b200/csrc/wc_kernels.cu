@@ -291,17 +291,21 @@ __global__ void wc_finish_kernel(const double2* __restrict__ inv, const double* 
 template <bool A_KC, bool B_KC>
 cudaError_t zgemm(const ZgemmArgs& a, int m_tiles, int n_tiles, int batch, cudaStream_t s) {
   if (m_tiles <= 0 || n_tiles <= 0 || a.k <= 0) return cudaSuccess;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(zgemm_dmma_kernel<A_KC, B_KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGSmem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
   zgemm_dmma_kernel<A_KC, B_KC><<<dim3(n_tiles, m_tiles, batch), kGThreads, kGSmem, s>>>(a);
   return cudaGetLastError();
 }
 
 }  // namespace
+
+// Function attributes of every kernel of this file (called before a stream capture: no attribute calls inside it).
+cudaError_t wc_configure() {
+  constexpr int kPotrfSmemBytes = 4 * kPB * kPLD * 8;
+  cudaError_t e = cudaFuncSetAttribute(potrf_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPotrfSmemBytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(zgemm_dmma_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(zgemm_dmma_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(zgemm_dmma_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGSmem);
+  return e;
+}
 
 size_t wc_work_elems(int n_m, int n_freq) {
   const size_t n = (size_t)(n_m + 63) / 64 * 64, nb = n / 64;
@@ -317,13 +321,7 @@ cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const 
   double2* Tbuf = Xbuf + (long long)n_freq * sM;
   double2* Linv = Tbuf + (long long)n_freq * sT;
   constexpr int kPotrfSmem = 4 * kPB * kPLD * 8;
-  static bool configured = false;
-  cudaError_t e;
-  if (!configured) {
-    e = cudaFuncSetAttribute(potrf_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPotrfSmem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  cudaError_t e;   // function attributes: wc_configure(), called by the C-ABI layer
 #define WC_TRY(expr) do { e = (expr); if (e != cudaSuccess) return e; } while (0)
   WC_TRY(cudaMemsetAsync(d_info, 0, sizeof(int), s));
   WC_TRY(cudaMemsetAsync(Xbuf, 0, sizeof(double2) * n_freq * sM, s));

@@ -121,3 +121,26 @@ def test_wc_and_rotation_block_edges(n):
     rot = q.chi0_to_coulomb_basis(torch.from_numpy(chi).cuda(), torch.from_numpy(U).cuda())
     torch.cuda.synchronize()
     assert rel_fro_per_freq(rot.cpu().numpy(), oracle.rotate_to_coulomb_basis_ref(chi, U)).max() <= 1e-12
+
+
+@pytest.mark.parametrize("mode", ["2", "0"])
+def test_wc_graph_and_plain_launch_paths(monkeypatch, mode):
+    """QSGW_WC_GRAPH=2 makes the CUDA-graph path mandatory (an error if the capture fails), =0 forces plain
+    launches on the caller's stream: both give the oracle's result, also on a non-default stream."""
+    import torch
+    import paper_2506_03477_b200 as q
+    monkeypatch.setenv("QSGW_WC_GRAPH", mode)
+    cfg = get_config(1)
+    prob = generate(cfg, n_k=2)
+    chi = oracle_chi(prob)
+    v = coulomb_eigenvalues(cfg)
+    ref = oracle.wc_ref(chi, v)
+    d_chi, d_v = torch.from_numpy(chi).cuda(), torch.from_numpy(v).cuda()
+    for stream in (None, torch.cuda.Stream()):
+        with torch.cuda.stream(stream) if stream is not None else torch.cuda.stream(torch.cuda.current_stream()):
+            w, info = q.wc_from_chi0(d_chi, d_v)
+            w2, info2 = q.wc_from_chi0(d_chi, d_v)          # back to back: the first graph is still in flight
+        torch.cuda.synchronize()
+        for x, i in ((w, info), (w2, info2)):
+            assert int(i.item()) == 0
+            assert rel_fro_per_freq(x.cpu().numpy(), ref).max() <= TOL_WC
