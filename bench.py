@@ -282,36 +282,34 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
     # the chi0 just built (Eqs. 10, 19): blocked Cholesky inverse of N_omega matrices of order N_M on the GPU.
     wc = None
     if precision == q.PREC_FP64 and not args.no_wc and rank == 0:
-        from qsgw_synth import coulomb_eigenvalues
+        from qsgw_synth import coulomb_eigenvalues, haar_unitary
+        import numpy as _np
         d_v = torch.from_numpy(coulomb_eigenvalues(cfg)).to(dev)
+        d_U = torch.from_numpy(haar_unitary(_np.random.default_rng(7), cfg.n_m)).to(dev)   # host work before any timing
         w_out = torch.empty_like(out)
         info = torch.zeros(1, dtype=torch.int32, device=dev)
-        q.wc_from_chi0(out, d_v, out=w_out, info=info)                       # warm-up
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        reps = 3
-        torch.cuda.synchronize(dev)
-        e0.record()
-        for _ in range(reps):
-            q.wc_from_chi0(out, d_v, out=w_out, info=info)
-        e1.record()
-        torch.cuda.synchronize(dev)
-        wc_ms = e0.elapsed_time(e1) / reps
+        reps = 5
+
+        def timed(fn):
+            for _ in range(3):                                    # warm-up: the GPU idled during the host-side set-up
+                fn()
+            ts = []
+            for _ in range(reps):                                 # every repetition timed on its own; median
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                fn()
+                e1.record()
+                torch.cuda.synchronize(dev)
+                ts.append(e0.elapsed_time(e1))
+            return statistics.median(ts)
+
+        wc_ms = timed(lambda: q.wc_from_chi0(out, d_v, out=w_out, info=info))
         wc_flop = 8.0 * n_f * float(cfg.n_m) ** 3       # n^3 complex multiply-adds per frequency (factor + inverse)
         wc = {"ms": wc_ms, "value": wc_flop / (wc_ms * 1e-3) / 1e12, "unit": UNIT, "info": int(info.item()),
               "credited_flop": wc_flop, "what": "qsgw_wc_from_chi0 on the FP64 chi0 of this run (spin 0 / last spin), "
               "credited n^3/3 (Cholesky) + n^3/3 (triangular inverse) + n^3/3 (X^H X) complex multiply-adds per frequency"}
-        # chi0 in the Coulomb eigenbasis first (U^H chi0 U; the representation Eqs. 10/19 are stated in)
-        from qsgw_synth import haar_unitary
-        import numpy as _np
-        d_U = torch.from_numpy(haar_unitary(_np.random.default_rng(7), cfg.n_m)).to(dev)
-        q.chi0_to_coulomb_basis(out, d_U, out=w_out)
-        torch.cuda.synchronize(dev)
-        e0.record()
-        for _ in range(reps):
-            q.chi0_to_coulomb_basis(out, d_U, out=w_out)
-        e1.record()
-        torch.cuda.synchronize(dev)
-        rot_ms = e0.elapsed_time(e1) / reps
+        # chi0 in the Coulomb eigenbasis (U^H chi0 U; the representation Eqs. 10/19 are stated in)
+        rot_ms = timed(lambda: q.chi0_to_coulomb_basis(out, d_U, out=w_out))
         wc["rotate_ms"] = rot_ms
         wc["rotate_value"] = 2 * 8.0 * n_f * float(cfg.n_m) ** 3 / (rot_ms * 1e-3) / 1e12   # two n^3 GEMMs per frequency
         del w_out, d_v, d_U

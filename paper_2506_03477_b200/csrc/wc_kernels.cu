@@ -210,11 +210,10 @@ __global__ void __launch_bounds__(256) potrf_inv_kernel(double2* A, long long ld
     }
     __syncthreads();
     // trailing update of the lower triangle: A[i][j] -= L[i][c] conj(L[j][c]),  c < j <= i
-    const int m = kPB - c - 1;
-    for (int e = tid; e < m * m; e += 256) {
-      const int i = c + 1 + e / m, j = c + 1 + e % m;
-      if (j <= i) {
-        const double ar = lr[i][c], ai = li[i][c], br = lr[j][c], bi = li[j][c];
+    for (int i = c + 1 + (tid >> 4); i < kPB; i += 16) {            // 16 x 16 thread grid, no index divisions
+      const double ar = lr[i][c], ai = li[i][c];
+      for (int j = c + 1 + (tid & 15); j <= i; j += 16) {
+        const double br = lr[j][c], bi = li[j][c];
         lr[i][j] -= ar * br + ai * bi;
         li[i][j] -= ai * br - ar * bi;
       }
