@@ -13,8 +13,11 @@ the configuration the BASELINE.json targets are quoted on.
   roofline   stage (b) kernel: credited flop per launch / mean launch time (CUDA events recorded
              by the library around each launch, inside the timed region) vs the tensor-pipe peak.
   cpu_baseline  the oracle (NumPy/BLAS, FP64) on a bounded sample of the same workload.
+  accuracy   error of the TIMED outputs against the oracle (outside the timed region): full matrix where the
+             oracle finishes in seconds, the exact sketch chi0 @ V (32 columns, all frequencies) otherwise.
+  configs    the other BASELINE.json configurations (cfg 0-3), each with throughput and accuracy.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--mode fp64|mixed|both]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--mode fp64|mixed|both] [--no-configs]
   python bench.py --impl reference ...      # times the oracle on the host cores
 Multi-GPU: the path does not shard in this build ("replicas only"): each rank runs
 the same workload; value = units of all ranks / max-over-ranks time; no data-path collective.
@@ -41,8 +44,8 @@ UNIT = "TFLOP/s"
 # only as RATIOS to the measured bf16 peak of MEASURED_PEAKS.json.
 # dram__bytes_read.sum + dram__bytes_write.sum of the stage (b) kernel for ONE cfg-4 k-point (21504 pairs), from the
 # `ncu --set full` captures under profiles/ (r01_*_full.md); a launch covers the k-points staged in the workspace.
-NCU_DRAM_BYTES_PER_KPOINT_CFG4 = {"chi0_f64_3m_kernel": 19.889e9 + 0.777e9, "chi0_f64_kernel": 17.107e9 + 0.768e9,
-                                  "chi0_f16_kernel<1,fp8>": 5.826e9 + 0.820e9, "chi0_f16_kernel": 5.537e9 + 0.802e9}
+NCU_DRAM_BYTES_PER_KPOINT_CFG4 = {"chi0_f64_3m_kernel": 19.889e9 + 0.777e9,
+                                  "chi0_f16_kernel<fp8>": 5.826e9 + 0.820e9, "chi0_f16_kernel": 5.537e9 + 0.802e9}
 
 NOMINAL_TF = {"bf16": 2250.0, "f16": 2250.0, "tf32": 1100.0, "f64": 40.0}
 
@@ -190,6 +193,38 @@ def sample_text(cfg, n_k_s, fsel):
             f"full N_M={cfg.n_m} matrix, all {cfg.n_o}x{cfg.n_u} band pairs; credited flops as for the GPU")
 
 
+# ----------------------------------------------------------------------------- accuracy of the timed outputs
+def accuracy_of(cfg, prob, outs, n_k):
+    """outs: {mode: [chi0 per spin (NumPy)]}.  Relative Frobenius error per frequency against the oracle, max over
+    spins: the full matrix when the oracle costs < ~2e11 flop, else the exact sketch chi0 @ V."""
+    import numpy as np
+    import oracle
+    sites = [prob.P_site(s) for s in range(cfg.n_sites)]
+    full = 8.0 * cfg.n_o * cfg.n_u * float(cfg.n_m) ** 2 * cfg.n_freq * n_k * cfg.n_spin < 2e11
+    res = {m: np.zeros(cfg.n_freq) for m in outs}
+    t0 = time.perf_counter()
+    for s, sp in enumerate(prob.spins):
+        a = (sites, sp.Ck[:n_k], sp.Ckq[:n_k], sp.eps_k[:n_k], sp.f_k[:n_k], sp.eps_kq[:n_k], sp.f_kq[:n_k], prob.omega)
+        if full:
+            ref = oracle.hermitian_finalize_ref(oracle.chi0_ref(*a, occ_tol=cfg.occ_tol, n_k_norm=cfg.n_k))
+            proj = lambda x: x
+        else:
+            rng = np.random.default_rng(4242 + cfg.index)
+            V = (rng.standard_normal((cfg.n_m, 32)) + 1j * rng.standard_normal((cfg.n_m, 32))) / np.sqrt(2)
+            ref = oracle.chi0_sketch_ref(*a, V, occ_tol=cfg.occ_tol, n_k_norm=cfg.n_k)
+            proj = lambda x: x @ V
+        den = np.linalg.norm(ref.reshape(cfg.n_freq, -1), axis=1)
+        for m, lst in outs.items():
+            num = np.linalg.norm((proj(lst[s]) - ref).reshape(cfg.n_freq, -1), axis=1)
+            res[m] = np.maximum(res[m], num / np.where(den > 0, den, 1.0))
+    return {m: {"max_rel_frobenius_err": float(e.max()), "per_freq": [float(x) for x in e],
+                "against": ("oracle.chi0_ref, full matrix" if full else
+                            "oracle.chi0_sketch_ref: chi0 @ V, 32 seeded Gaussian columns (unbiased estimator of the "
+                            "Frobenius error ratio)"),
+                "tolerance": 1e-11 if m == "fp64" else 2e-5, "oracle_seconds": time.perf_counter() - t0}
+            for m, e in res.items()}
+
+
 # ----------------------------------------------------------------------------- reference arm
 def main_reference(args):
     rank, _, world = dist_env()
@@ -222,7 +257,8 @@ def main_reference(args):
 
 
 # ----------------------------------------------------------------------------- CUDA arm
-def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
+def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, light=False):
+    """light: one of the small side configurations (no W^c leg, no peak probes; still step, e2e and the output)."""
     import numpy as np
     import torch
     import paper_2506_03477_b200 as q
@@ -236,7 +272,6 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
 
     ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, cfg.n_k, args.max_n_o or cfg.n_o,
                         args.max_n_u or cfg.n_u, precision=precision, occ_tol=cfg.occ_tol)
-    mixed_fp8 = bool(getattr(ctx, "mixed_fp8", False))
     ctx.set_product_tensor(torch.from_numpy(prob.P).to(dev))
     d_in = [[torch.from_numpy(a).to(dev) for a in (sp.Ck, sp.Ckq, sp.eps_k, sp.f_k, sp.eps_kq, sp.f_kq)]
             for sp in prob.spins]
@@ -277,11 +312,29 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
     launches = ctx.kernel_launches - l0
     stage = {nm: ctx.stage_time_ms(i) for i, nm in enumerate(("zmel", "weights", "chi0", "finalize"))}
     ctx.set_stage_timing(False)
+    mixed_stats = None
+    if precision == q.PREC_MIXED:        # of the last step (and spin): the counters restart at every reset
+        n_l, n_l8, pe = ctx.mixed_stats()
+        mixed_stats = {"stage_b_launches": n_l, "with_e5m2_corrections": n_l8, "min_effective_pairs": pe,
+                       "min_effective_pairs_per_product_function": pe / cfg.n_m}
+    mixed_fp8 = bool(mixed_stats and mixed_stats["with_e5m2_corrections"] > 0)
+    # the timed output (last step; both spins) comes back for the accuracy check, outside the timed region
+    outs_host = None
+    if rank == 0 and not args.no_accuracy:
+        outs_host = []
+        for s in range(n_spin):
+            if n_spin > 1:               # `out` holds the last spin only: rebuild this spin once, untimed
+                ctx.reset()
+                Ck, Ckq, ek, fk, ekq, fkq = d_in[s]
+                for k in range(n_k):
+                    ctx.chi0_add_kpoint(Ck[k], Ckq[k], ek[k], fk[k], ekq[k], fkq[k])
+                ctx.chi0_finalize(out)
+            outs_host.append(out.cpu().numpy())
     ctx.destroy()
     # next row of the scope table, reported beside the step, not inside `value`: W^c(i omega) from
     # the chi0 just built (Eqs. 10, 19): blocked Cholesky inverse of N_omega matrices of order N_M on the GPU.
     wc = None
-    if precision == q.PREC_FP64 and not args.no_wc and rank == 0:
+    if precision == q.PREC_FP64 and not args.no_wc and not light and rank == 0:
         from qsgw_synth import coulomb_eigenvalues, haar_unitary
         import numpy as _np
         d_v = torch.from_numpy(coulomb_eigenvalues(cfg)).to(dev)
@@ -304,10 +357,10 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
             return statistics.median(ts)
 
         wc_ms = timed(lambda: q.wc_from_chi0(out, d_v, out=w_out, info=info))
-        wc_flop = 8.0 * n_f * float(cfg.n_m) ** 3       # n^3 complex multiply-adds per frequency (factor + inverse)
+        wc_flop = 4.0 * n_f * float(cfg.n_m) ** 3       # n^3/2 complex multiply-adds per frequency, 8 real flop each
         wc = {"ms": wc_ms, "value": wc_flop / (wc_ms * 1e-3) / 1e12, "unit": UNIT, "info": int(info.item()),
               "credited_flop": wc_flop, "what": "qsgw_wc_from_chi0 on the FP64 chi0 of this run (spin 0 / last spin), "
-              "credited n^3/3 (Cholesky) + n^3/3 (triangular inverse) + n^3/3 (X^H X) complex multiply-adds per frequency"}
+              "credited n^3/6 (Cholesky) + n^3/6 (triangular inverse) + n^3/6 (X^H X) complex multiply-adds per frequency"}
         # chi0 in the Coulomb eigenbasis (U^H chi0 U; the representation Eqs. 10/19 are stated in)
         rot_ms = timed(lambda: q.chi0_to_coulomb_basis(out, d_U, out=w_out))
         wc["rotate_ms"] = rot_ms
@@ -320,13 +373,15 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
     chi_ms, chi_n = stage["chi0"]
     # stage (b) kernel: credited flop per launch (one k-point and band batch, all frequencies)
     ach = (fb * args.steps / max(chi_n, 1)) / (chi_ms / max(chi_n, 1) * 1e-3) / 1e12 if chi_n else None
-    dkey = {q.PREC_FP64: "f64", q.PREC_MIXED: "f16"}.get(precision, "tf32")
+    dkey = {q.PREC_FP64: "f64", q.PREC_MIXED: "f16"}[precision]
     burst_peak, src = tensor_peak(dkey, sustained=False)
     sust_peak, _ = tensor_peak(dkey, sustained=True)
-    try:      # the pipe's own issue-rate peak, measured on this device in this run
-        probe, _ = q.probe_peak({"f64": q.PEAK_FP64_MMA, "tf32": q.PEAK_TF32_MMA, "f16": q.PEAK_F16_MMA}[dkey])
-    except q.QsgwError:
-        probe = None
+    probe = None
+    if not light:
+        try:      # the pipe's own issue-rate peak, measured on this device in this run
+            probe, _ = q.probe_peak({"f64": q.PEAK_FP64_MMA, "f16": q.PEAK_F16_MMA}[dkey])
+        except q.QsgwError:
+            probe = None
     ratio_txt = f"x nominal {dkey}/bf16 ratio ({NOMINAL_TF[dkey]:g}/{NOMINAL_TF['bf16']:g})"
     if dkey == "f64":
         # MEASURED_PEAKS.json has no FP64 figure and the bf16-derived one is power-capped while FP64 is not
@@ -341,23 +396,27 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
         # tcgen05 kernels run power-capped inside a seconds-long step: MEASURED_PEAKS.json sustained figure
         peak = sust_peak
         peak_src = f"{src} bf16 cuBLAS sustained (MEASURED_PEAKS.json) {ratio_txt}"
-    # tensor-pipe flops the kernel executes per credited flop (full tiles, no padding counted):
-    # FP64 4M = 1; FP16 split and 3xTF32 = 3 products per term; single TF32 = 1
-    # FP64: the 3M kernel executes 3 real products per complex one (0.75 of the credited 4); QSGW_F64_4M=1 = 4M
-    f64_4m = os.environ.get("QSGW_F64_4M", "0") not in ("", "0")
-    passes = {q.PREC_FP64: 1.0 if f64_4m else 0.75, q.PREC_MIXED: 3, q.PREC_MIXED_TF32X3: 3,
-              q.PREC_MIXED_TF32X1: 1}[precision]
-    kname = {"f64": "chi0_f64_kernel" if f64_4m else "chi0_f64_3m_kernel", "f16": "chi0_f16_kernel",
-             "tf32": f"chi0_tf32_kernel<{passes}>"}[dkey]
+    # tensor-pipe flops the kernel executes per credited flop (full tiles, no padding counted): the FP64 kernel's
+    # 3M product executes 3 real products per complex one (0.75 of the credited 4); the FP16 split 3 per term
+    passes = {q.PREC_FP64: 0.75, q.PREC_MIXED: 3}[precision]
+    kname = {"f64": "chi0_f64_3m_kernel", "f16": "chi0_f16_kernel"}[dkey]
     pipe_txt = dkey
-    if precision == q.PREC_MIXED and mixed_fp8:
-        # FP8-corrected variant: per credited product one f16 MMA product and two E5M2 ones.  Pipe time at
-        # peak per credited flop = 1/P_f16 + 2/P_fp8 with P_fp8 = 2 P_f16 (nominal 4.5 / 2.25 PF) = 2 / P_f16:
-        # `peak` becomes P_f16 / 2 in credited flops; executed flops are 3 per credited one as before.
-        peak = sust_peak / 2.0
-        peak_src += "; credited-flop peak of the f16 + 2 x e5m2 product mix = f16 peak / 2 (fp8 nominal = 2 x f16)"
-        kname, pipe_txt = "chi0_f16_kernel<1,fp8>", "f16 + e5m2"
-        roof_exec_frac = (ach / peak) if ach else None       # pipe-time fraction
+    extra = {}
+    if precision == q.PREC_MIXED:
+        # north_star's denominator for the mixed mode: the FP32/TF32 tensor peak = measured bf16 sustained x the
+        # nominal tf32/bf16 ratio ("of measured, nominal ratio").  Beside it the pipe-time view of what runs:
+        # three f16 products per term, or (E5M2 variant) one f16 + two e5m2 products = 1/P_f16 + 2/P_fp8 =
+        # 2/P_f16 of pipe time per credited flop (fp8 nominal = 2 x f16).
+        tf32_peak, _ = tensor_peak("tf32", True)
+        pipe_peak = sust_peak / (2.0 if mixed_fp8 else 3.0)
+        extra = {"peak_pipe_mix": pipe_peak, "frac_pipe_mix": (ach / pipe_peak) if ach else None,
+                 "peak_pipe_mix_source": f"{src} bf16 sustained / " + ("2 (f16 main + 2 e5m2 corrections; fp8 nominal "
+                                         "= 2 x f16)" if mixed_fp8 else "3 (three f16 products per term)")}
+        peak = tf32_peak
+        peak_src = f"{src} bf16 cuBLAS sustained (MEASURED_PEAKS.json) x nominal tf32/bf16 ratio (1100/2250)"
+        if mixed_fp8:
+            kname, pipe_txt = "chi0_f16_kernel<fp8>", "f16 + e5m2"
+        roof_exec_frac = extra["frac_pipe_mix"]
     else:
         roof_exec_frac = (ach * passes / peak) if ach else None
     roofline = {"bound": "tensor", "kernel": kname, "tensor_pipe": pipe_txt,
@@ -369,13 +428,14 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
                             if (cfg.index == 4 and kname in NCU_DRAM_BYTES_PER_KPOINT_CFG4 and chi_n) else None),
                 "note": ("credited flops count 4 real products per complex multiply-add; the 3M kernel executes 3, so "
                          "`frac` (credited / peak) can exceed 1 while `frac_executed` stays below it"
-                         if (dkey == "f64" and not f64_4m) else None),
+                         if dkey == "f64" else "frac = credited / TF32 peak (north_star denominator); frac_executed = "
+                         "tensor-pipe time fraction of the product mix that ran (peak_pipe_mix)"),
+                **extra,
                 "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per cfg-4 k-point (profiles/) x "
                                   "k-points staged per launch; bytes",
                 "peak_source": peak_src,
                 "peak_probe": probe, "frac_executed_of_probe": (ach * passes / probe) if (ach and probe) else None,
                 "peak_burst": burst_peak, "peak_burst_source": f"{src} bf16 burst {ratio_txt}",
-                "achieved_vs_tf32_sustained_peak": (ach / tensor_peak("tf32", True)[0]) if (ach and dkey != "f64") else None,
                 "avg_launch_ms": chi_ms / max(chi_n, 1), "launches_timed": chi_n,
                 "stage_ms_per_step": {nm: v[0] / args.steps for nm, v in stage.items()}}
 
@@ -389,35 +449,42 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world):
         h2d = n_spin * h_P.nbytes + sum(a.nbytes for sp in h_in for a in sp)
         d2h = n_spin * h_out.nbytes
 
+        # one context per spin, created (and its staging buffers allocated by a first call) before the clock starts
+        e_ctx = [q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, cfg.n_k, args.max_n_o or cfg.n_o,
+                               args.max_n_u or cfg.n_u, precision=precision, occ_tol=cfg.occ_tol)
+                 for _ in range(n_spin)]
+
         def e2e_step():
             n = 0
             for s in range(n_spin):
-                _, ln = q.chi0_run_host(cfg.orb_per_site, cfg.pb_per_site, prob.omega, h_P, *h_in[s],
-                                        args.max_n_o or cfg.n_o, args.max_n_u or cfg.n_u, precision=precision,
-                                        occ_tol=cfg.occ_tol, out=h_out)
+                _, ln = e_ctx[s].run_host(h_P, *h_in[s], out=h_out)
                 n += ln
             return n
-        e2e_step()
+        for _ in range(2):
+            e2e_step()
         barrier()
         n_e = max(1, min(args.steps, args.e2e_steps))
-        # every step is timed on its own (wall clock around the synchronous call, max over ranks); the value is
-        # the MEDIAN step: on these shared hosts single calls sporadically take 0.1-0.4 s longer on the host side
-        # (device time unchanged), all step times are listed
+        # every step is timed on its own: wall clock around the synchronous C-ABI call, max over ranks
         step_s = []
         for _ in range(n_e):
             t0 = time.perf_counter()
             e2e_step()
             step_s.append(max_over_ranks(time.perf_counter() - t0, world, dev))
         barrier()
+        for c in e_ctx:
+            c.destroy()
         dt = statistics.median(step_s)
         e2e = {"value": world * flops_step / dt / 1e12, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * dt, "steps": n_e,
-               "ms_steps": [round(1e3 * t, 2) for t in step_s], "statistic": "median of the timed steps",
-               "api": "qsgw_chi0_run_host (pinned host buffers, H2D + all kernels + D2H inside the timed region)"}
+               "ms_steps": [round(1e3 * t, 2) for t in step_s], "ms_min": 1e3 * min(step_s), "ms_max": 1e3 * max(step_s),
+               "statistic": "median of the timed steps",
+               "api": "qsgw_chi0_run_host on a persistent context (pinned host buffers; reset + H2D + all kernels + "
+                      "D2H inside the timed region)"}
 
     return {"mode": mode_name, "value": value, "ms_per_step": ms_total / args.steps, "launches": launches,
             "roofline": roofline, "e2e": e2e, "clocks": clocks, "flops_step": flops_step,
-            "flops_stage_a": fa, "flops_stage_b": fb, "pairs_kept": pairs, "wc": wc}
+            "flops_stage_a": fa, "flops_stage_b": fb, "pairs_kept": pairs, "wc": wc, "mixed_selection": mixed_stats,
+            "_out": outs_host}
 
 
 def main_cuda(args):
@@ -442,29 +509,47 @@ def main_cuda(args):
     prob = generate(cfg, n_k=args.n_k or None)
 
     modes = {"fp64": [("fp64", q.PREC_FP64)], "mixed": [("mixed", q.PREC_MIXED)],
-             "mixed_x1": [("mixed_x1", q.PREC_MIXED_TF32X1)],
-             "mixed_tf32x3": [("mixed_tf32x3", q.PREC_MIXED_TF32X3)],
-             "both": [("fp64", q.PREC_FP64), ("mixed", q.PREC_MIXED)],
-             "all": [("fp64", q.PREC_FP64), ("mixed", q.PREC_MIXED), ("mixed_tf32x3", q.PREC_MIXED_TF32X3),
-                     ("mixed_x1", q.PREC_MIXED_TF32X1)]}[args.mode]
+             "both": [("fp64", q.PREC_FP64), ("mixed", q.PREC_MIXED)]}[args.mode]
     if args.mode == "both" and cfg.precision == "mixed":
         modes = modes[::-1]
-    res = []
-    for name, prec in modes:
-        try:
-            res.append(run_mode(args, cfg, prob, prec, name, rank, local_rank, world))
-        except q.QsgwError as e:
-            if e.code == 6 and len(modes) > 1:       # QSGW_ERR_UNSUPPORTED: mode not built
-                res.append({"mode": name, "unavailable": str(e)})
-            else:
-                raise
+    res = [run_mode(args, cfg, prob, prec, name, rank, local_rank, world) for name, prec in modes]
+
+    # the other BASELINE.json configurations, each in the mode(s) it names: throughput, e2e and accuracy
+    side = []
+    if not args.no_configs and not args.n_k and world == 1:
+        for idx in [i for i in (0, 1, 2, 3) if i != cfg.index]:
+            c2 = get_config(idx)
+            p2 = generate(c2)
+            m2 = [("mixed", q.PREC_MIXED)] if c2.precision == "mixed" else [("fp64", q.PREC_FP64)]
+            if idx in (0, 1):
+                m2 = [("fp64", q.PREC_FP64), ("mixed", q.PREC_MIXED)]
+            a2 = argparse.Namespace(**{**vars(args), "max_n_o": 0, "max_n_u": 0, "steps": max(args.steps, 5),
+                                       "e2e_steps": 3})
+            rs = [run_mode(a2, c2, p2, prec, name, rank, local_rank, world, light=True) for name, prec in m2]
+            acc = {} if args.no_accuracy else accuracy_of(c2, p2, {r["mode"]: r["_out"] for r in rs}, c2.n_k)
+            side.append({"workload": c2.name, "n_m": c2.n_m, "n_k": c2.n_k, "n_spin": c2.n_spin,
+                         "modes": [{"mode": r["mode"], "value": r["value"], "unit": UNIT, "ms_per_step": r["ms_per_step"],
+                                    "gpu_launches": r["launches"], "credited_flop_per_step": r["flops_step"],
+                                    "stage_b_kernel_tflops": r["roofline"]["achieved"],
+                                    "stage_ms_per_step": r["roofline"]["stage_ms_per_step"],
+                                    "e2e": r["e2e"] and {k: r["e2e"][k] for k in ("value", "ms_per_step", "ms_min", "ms_max")},
+                                    "mixed_selection": r["mixed_selection"], "accuracy": acc.get(r["mode"])}
+                                   for r in rs]})
+            del p2, rs
     if rank != 0:
         return 0
-    main = next(r for r in res if "value" in r)
+    if not args.no_accuracy:
+        acc = accuracy_of(cfg, prob, {r["mode"]: r["_out"] for r in res}, prob.spins[0].Ck.shape[0])
+        for r in res:
+            r["accuracy"] = acc[r["mode"]]
+    for r in res:
+        r.pop("_out", None)
+    main = res[0]
     line = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": {"fp64": "f64", "mixed": "fp32 z as f16 pieces: f16 main + 2 e5m2 correction products (fp32-grade) + f64 accumulate"}.get(
-                main["mode"], "tf32 (z fp32) + f64 accumulate"),
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": {"fp64": "f64", "mixed": "fp32 z as f16 pieces (f16 main product + f16 or e5m2 correction products, "
+                                              "fp32-grade) + f64 accumulate"}[main["mode"]],
             "data": "synthetic",
             "config": {"workload": cfg.name, "mode": main["mode"], "n_m": cfg.n_m, "n_b": cfg.n_b, "n_k": cfg.n_k,
                        "n_spin": cfg.n_spin, "n_o": cfg.n_o, "n_u": cfg.n_u, "n_freq": cfg.n_freq,
@@ -472,7 +557,7 @@ def main_cuda(args):
                        "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": "no flush needed: accumulator + z workspace per step far exceed the 126 MB L2"
                              if cfg.n_m >= 600 else "working set fits L2 (latency-bound config)"},
-            "roofline": main["roofline"], "e2e": main["e2e"],
+            "roofline": main["roofline"], "e2e": main["e2e"], "accuracy": main.get("accuracy"),
             **({"subset": f"first {args.n_k} of {cfg.n_k} k-points (profiling run, not a bench value)"}
                if args.n_k else {}), "gpu_launches": main["launches"],
             "clocks": main["clocks"]}
@@ -481,6 +566,10 @@ def main_cuda(args):
             line["wc"] = r["wc"]
         if r is not main:
             line[r["mode"]] = r
+    if main.get("mixed_selection"):
+        line["mixed_selection"] = main["mixed_selection"]
+    if side:
+        line["configs"] = side
     if world == 1 and not args.no_cpu:
         n_k_s, fsel = oracle_sample(cfg, prob, seconds_hint=args.cpu_seconds)
         dt, fl = run_oracle_sample(cfg, prob, n_k_s, fsel)
@@ -500,7 +589,7 @@ def parse_args(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
-    ap.add_argument("--mode", default="both", choices=["fp64", "mixed", "mixed_x1", "mixed_tf32x3", "both", "all"])
+    ap.add_argument("--mode", default="both", choices=["fp64", "mixed", "both"])
     ap.add_argument("--max-n-o", type=int, default=0, help="band batch (default: whole O side)")
     ap.add_argument("--max-n-u", type=int, default=0, help="band batch (default: whole U side)")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -511,6 +600,8 @@ def parse_args(argv=None):
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-wc", action="store_true", help="skip the W^c(i omega) leg reported beside the FP64 step")
+    ap.add_argument("--no-accuracy", action="store_true", help="skip the oracle check of the timed outputs")
+    ap.add_argument("--no-configs", action="store_true", help="skip the side runs of the other configurations")
     return ap.parse_args(argv)
 
 

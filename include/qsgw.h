@@ -56,13 +56,13 @@ enum {
  *   tensor cores: every FP32 operand v (scaled by a power of two) is carried as fp16 pieces v = h + l
  *   (22 significant bits) and a*b is formed as a_h*b_h + a_l*b_h + a_h*b_l by three exact FP16 MMAs
  *   (tcgen05 kind::f16, twice the TF32 rate); FP32 window sums, FP64 accumulation across batches and k.
- *   When the job sums at least 64 band pairs per product function (n_k * max_n_o * max_n_u >= 64 * N_M, taken
- *   from the descriptor) the two correction products a_l*b_h + a_h*b_l run in E5M2 (kind::f8f6f4): they need
- *   ~3 significant bits; the added error ~4e-5 * sqrt(N_M / pairs summed) stays well inside the 2e-5 bar.
- * QSGW_PREC_MIXED_TF32X3: the same split on the TF32 pipe (hi*hi + lo*hi + hi*lo), half the speed.
- * QSGW_PREC_MIXED_TF32X1: ONE TF32 product per term (operands rounded to nearest TF32; relative
- *   Frobenius error ~ 3e-4 * sqrt(N_M / pairs summed): above the 2e-5 bar on cfg 3/4). */
-enum { QSGW_PREC_FP64 = 0, QSGW_PREC_MIXED = 1, QSGW_PREC_MIXED_TF32X1 = 2, QSGW_PREC_MIXED_TF32X3 = 3 };
+ *   The two correction products a_l*b_h + a_h*b_l need only ~3 significant bits and run in E5M2
+ *   (kind::f8f6f4) for every stage (b) launch whose staged pairs are numerous enough: the choice is made ON THE
+ *   DEVICE, per launch, from the weights of the pairs that are actually accumulated (effective pair count
+ *   P_eff = (sum w)^2 / sum w^2, minimum over the frequencies, against a multiple of N_M), never from the
+ *   descriptor; launches below the threshold use the three-FP16-product form.  Contract of the mode in either
+ *   case: relative Frobenius error <= 2e-5 per frequency against the FP64 result. */
+enum { QSGW_PREC_FP64 = 0, QSGW_PREC_MIXED = 1 };
 
 /* Problem descriptor (host memory; copied by qsgw_create). */
 typedef struct {
@@ -73,10 +73,12 @@ typedef struct {
   const double* h_omega;         /* imaginary frequencies omega_j >= 0, strictly increasing    */
   int32_t n_k;                   /* N_k >= 1: the 1/N_k normalisation applied by finalize      */
   int32_t max_n_o, max_n_u;      /* largest band batch (n_o, n_u) any zmel_build call passes   */
-  int32_t precision;             /* QSGW_PREC_FP64 | QSGW_PREC_MIXED | QSGW_PREC_MIXED_TF32X*  */
+  int32_t precision;             /* QSGW_PREC_FP64 | QSGW_PREC_MIXED                           */
   double occ_tol;                /* pair kept iff f_n*(1-f_n') > occ_tol; <0 selects 1e-12     */
-  size_t workspace_bytes;        /* cap on the z workspace; 0 = no cap.  If max_n_o*max_n_u    */
-                                 /* pairs do not fit, create fails with QSGW_ERR_ALLOC         */
+  size_t workspace_bytes;        /* cap on the z workspace; 0 = library default (room for the  */
+                                 /* larger of one band batch and ~32 Ki staged pairs).  If one */
+                                 /* max_n_o*max_n_u batch does not fit under a non-zero cap,   */
+                                 /* create fails with QSGW_ERR_ALLOC                           */
 } qsgw_desc;
 
 /* Create a context on the current CUDA device.  `cuda_stream` is a cudaStream_t (NULL =
@@ -138,15 +140,19 @@ int32_t qsgw_reset(qsgw_ctx* ctx);
 int32_t qsgw_sync(qsgw_ctx* ctx);
 void qsgw_destroy(qsgw_ctx* ctx);
 
-/* Whole job from HOST buffers (H2D copies, all k-points, D2H of the result), for end-to-end
- * timing.  Host arrays: h_P as set_product_tensor; h_Ck complex128 [n_k][n_o][N_b] (row =
- * band), h_Ckq [n_k][n_u][N_b]; h_eps_k,h_f_k float64 [n_k][n_o]; h_eps_kq,h_f_kq
- * [n_k][n_u]; h_chi0_out complex128 [n_freq][N_M][N_M].  desc->max_n_o/max_n_u give the band
- * batch.  Creates and destroys its own context and stream; synchronous. */
-int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h_Ck,
-                           const void* h_Ckq, const double* h_eps_k, const double* h_f_k,
-                           const double* h_eps_kq, const double* h_f_kq, int32_t n_o,
-                           int32_t n_u, void* h_chi0_out, int64_t* out_kernel_launches);
+/* Whole job from HOST buffers on an existing context: qsgw_reset, H2D of P and of every k-point's
+ * arrays, the band-batch loop of all n_k_points k-points, finalize, D2H of the result.  Host arrays: h_P as
+ * set_product_tensor; h_Ck complex128 [n_k_points][n_o][N_b] (row = band), h_Ckq [n_k_points][n_u][N_b];
+ * h_eps_k,h_f_k float64 [n_k_points][n_o]; h_eps_kq,h_f_kq [n_k_points][n_u]; h_chi0_out complex128
+ * [n_freq][N_M][N_M].  Pinned host memory makes the copies asynchronous; the library pins nothing itself.
+ * The device staging buffers belong to the context (allocated by the first call, reused afterwards), the
+ * copies and kernels run on the context's stream (results leave on a second stream while the last launches
+ * run).  Synchronous: returns when h_chi0_out is complete.  *out_kernel_launches = kernels launched by
+ * this call. */
+int32_t qsgw_chi0_run_host(qsgw_ctx* ctx, const void* h_P, const void* h_Ck, const void* h_Ckq,
+                           const double* h_eps_k, const double* h_f_k, const double* h_eps_kq,
+                           const double* h_f_kq, int32_t n_k_points, int32_t n_o, int32_t n_u,
+                           void* h_chi0_out, int64_t* out_kernel_launches);
 
 /* Screened Coulomb interaction on the imaginary axis from the polarization (the step after the chi0 build):
  *   eps_j = 1 - sqrt(v) chi0_j sqrt(v)                    Eq. (10)
@@ -199,9 +205,25 @@ int64_t qsgw_pairs_accumulated(const qsgw_ctx* ctx);    /* band pairs passed to 
 size_t qsgw_device_bytes(const qsgw_ctx* ctx);          /* device memory owned by the context  */
 int32_t qsgw_n_m(const qsgw_ctx* ctx);                  /* N_M                                 */
 int32_t qsgw_n_b(const qsgw_ctx* ctx);                  /* N_b                                 */
-int32_t qsgw_mixed_fp8(const qsgw_ctx* ctx);            /* 1 if QSGW_PREC_MIXED runs its two    */
-                                                        /* correction products in E5M2          */
 const char* qsgw_version(void);
+
+/* Mixed mode: what the device-side selection did since the last qsgw_reset (synchronises the stream):
+ * stage (b) launches in all, those that ran the E5M2 correction products, and the smallest effective pair
+ * count P_eff any launch saw (qsgw.h, QSGW_PREC_MIXED).  QSGW_ERR_STATE in FP64 mode. */
+int32_t qsgw_mixed_stats(qsgw_ctx* ctx, int64_t* out_launches, int64_t* out_launches_fp8,
+                         double* out_min_effective_pairs);
+
+/* Tuning and test knobs (never read from the environment).  ctx != NULL, allowed while nothing is staged:
+ *   "stage_batches"   n >= 1   band batches staged per stage (b) launch (capped by the workspace)
+ *   "zmel_dmma"       0 | 1    stage (a) step 2 on CUDA cores | on the FP64 tensor pipe (default 1)
+ *   "mixed_fp8"       0 | 1 | 2  E5M2 correction products never | always | chosen on the device (default 2)
+ *   "mixed_fp8_threshold_x100"  T*100: automatic choice takes E5M2 when P_eff >= T * N_M
+ *   "mixed_window"    1..64    pipeline stages per TMEM drain window (default 8)
+ *   "e2e_groups"      1..4     frequency groups of the last launch of qsgw_chi0_run_host (default 4)
+ * ctx == NULL, process-wide:
+ *   "wc_graph"        0 | 1 | 2  qsgw_wc_from_chi0: plain launches | CUDA graph with fallback (default) | graph or fail
+ * Unknown key or value out of range: QSGW_ERR_INVALID_ARG. */
+int32_t qsgw_set_option(qsgw_ctx* ctx, const char* key, int64_t value);
 
 #ifdef __cplusplus
 }

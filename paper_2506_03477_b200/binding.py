@@ -11,7 +11,7 @@ from typing import Optional, Sequence
 
 from .build import LIB_PATH
 
-PREC_FP64, PREC_MIXED, PREC_MIXED_TF32X1, PREC_MIXED_TF32X3 = 0, 1, 2, 3
+PREC_FP64, PREC_MIXED = 0, 1
 STAGE_ZMEL, STAGE_WEIGHTS, STAGE_CHI0, STAGE_FINALIZE = 0, 1, 2, 3
 _STATUS = {0: "QSGW_OK", 1: "QSGW_ERR_INVALID_ARG", 2: "QSGW_ERR_SHAPE", 3: "QSGW_ERR_STATE",
            4: "QSGW_ERR_ALLOC", 5: "QSGW_ERR_CUDA", 6: "QSGW_ERR_UNSUPPORTED"}
@@ -58,11 +58,13 @@ def lib() -> C.CDLL:
     L.qsgw_sync.argtypes = [vp]
     L.qsgw_destroy.argtypes = [vp]
     L.qsgw_destroy.restype = None
-    L.qsgw_chi0_run_host.argtypes = [C.POINTER(_Desc), vp, vp, vp, vp, vp, vp, vp, i32, i32, vp,
-                                     C.POINTER(i64)]
+    L.qsgw_chi0_run_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp, C.POINTER(i64)]
+    L.qsgw_set_option.argtypes = [vp, C.c_char_p, i64]
+    L.qsgw_mixed_stats.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(C.c_double)]
     for name in ("qsgw_create", "qsgw_set_product_tensor", "qsgw_zmel_build", "qsgw_chi0_accumulate",
                  "qsgw_chi0_add_kpoint", "qsgw_chi0_finalize", "qsgw_reset", "qsgw_sync",
-                 "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_mixed_fp8", "qsgw_wc_from_chi0", "qsgw_chi0_to_coulomb_basis"):
+                 "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_set_option", "qsgw_mixed_stats", "qsgw_wc_from_chi0",
+                 "qsgw_chi0_to_coulomb_basis"):
         getattr(L, name).restype = i32
     for name in ("qsgw_last_error", "qsgw_last_create_error", "qsgw_version"):
         getattr(L, name).restype = C.c_char_p
@@ -80,7 +82,6 @@ def lib() -> C.CDLL:
     L.qsgw_device_bytes.argtypes = [vp]
     L.qsgw_n_m.argtypes = [vp]
     L.qsgw_n_b.argtypes = [vp]
-    L.qsgw_mixed_fp8.argtypes = [vp]
     L.qsgw_wc_from_chi0.argtypes = [i32, i32, vp, vp, vp, vp, vp]
     L.qsgw_chi0_to_coulomb_basis.argtypes = [i32, i32, vp, vp, vp, vp]
     _lib = L
@@ -152,7 +153,6 @@ class Chi0Context:
             raise QsgwError(rc, self._L.qsgw_last_create_error().decode())
         self.n_m = self._L.qsgw_n_m(self._h)
         self.n_b = self._L.qsgw_n_b(self._h)
-        self.mixed_fp8 = bool(self._L.qsgw_mixed_fp8(self._h))
 
     def _check(self, rc: int):
         if rc != 0:
@@ -199,6 +199,30 @@ class Chi0Context:
 
     def sync(self):
         self._check(self._L.qsgw_sync(self._h))
+
+    def set_option(self, key: str, value: int):
+        self._check(self._L.qsgw_set_option(self._h, key.encode(), int(value)))
+
+    def mixed_stats(self):
+        """qsgw_mixed_stats: (stage (b) launches, launches with E5M2 corrections, smallest P_eff); synchronises."""
+        n, n8, pe = C.c_int64(0), C.c_int64(0), C.c_double(0.0)
+        self._check(self._L.qsgw_mixed_stats(self._h, C.byref(n), C.byref(n8), C.byref(pe)))
+        return int(n.value), int(n8.value), float(pe.value)
+
+    def run_host(self, P, Ck, Ckq, eps_k, f_k, eps_kq, f_kq, out=None):
+        """qsgw_chi0_run_host: whole job from HOST (NumPy) buffers on this context; returns (chi0, launches)."""
+        import numpy as np
+        n_k, n_o, _ = Ck.shape
+        n_u = Ckq.shape[1]
+        arrs = [np.ascontiguousarray(a, dtype=dt) for a, dt in
+                ((P, np.complex128), (Ck, np.complex128), (Ckq, np.complex128), (eps_k, np.float64),
+                 (f_k, np.float64), (eps_kq, np.float64), (f_kq, np.float64))]
+        if out is None:
+            out = np.empty((self.n_freq, self.n_m, self.n_m), dtype=np.complex128)
+        launches = C.c_int64(0)
+        self._check(self._L.qsgw_chi0_run_host(self._h, *[a.ctypes.data_as(C.c_void_p) for a in arrs], n_k, n_o,
+                                               n_u, out.ctypes.data_as(C.c_void_p), C.byref(launches)))
+        return out, int(launches.value)
 
     def set_stage_timing(self, enable: bool):
         self._check(self._L.qsgw_set_stage_timing(self._h, int(bool(enable))))
@@ -267,24 +291,22 @@ def chi0_to_coulomb_basis(chi0, U, out=None):
     return out
 
 
+def set_global_option(key: str, value: int):
+    """qsgw_set_option(NULL, key, value): process-wide options ("wc_graph")."""
+    L = lib()
+    rc = L.qsgw_set_option(None, key.encode(), int(value))
+    if rc != 0:
+        raise QsgwError(rc, L.qsgw_last_create_error().decode())
+
+
 def chi0_run_host(orb_per_site, pb_per_site, omega, P, Ck, Ckq, eps_k, f_k, eps_kq, f_kq,
                   max_n_o: int, max_n_u: int, precision: int = PREC_FP64, occ_tol: float = 1e-12,
                   out=None):
-    """qsgw_chi0_run_host: whole job from HOST (NumPy) buffers; returns (chi0, kernel_launches)."""
-    import numpy as np
-    L = lib()
-    n_k, n_o, _ = Ck.shape
-    n_u = Ckq.shape[1]
-    n_m = int(sum(pb_per_site))
-    arrs = [np.ascontiguousarray(a, dtype=dt) for a, dt in
-            ((P, np.complex128), (Ck, np.complex128), (Ckq, np.complex128), (eps_k, np.float64),
-             (f_k, np.float64), (eps_kq, np.float64), (f_kq, np.float64))]
-    if out is None:
-        out = np.empty((len(omega), n_m, n_m), dtype=np.complex128)
-    d = _make_desc(orb_per_site, pb_per_site, omega, n_k, max_n_o, max_n_u, precision, occ_tol, 0)
-    launches = C.c_int64(0)
-    rc = L.qsgw_chi0_run_host(C.byref(d), *[a.ctypes.data_as(C.c_void_p) for a in arrs], n_o, n_u,
-                              out.ctypes.data_as(C.c_void_p), C.byref(launches))
-    if rc != 0:
-        raise QsgwError(rc, L.qsgw_last_create_error().decode())
-    return out, int(launches.value)
+    """One-shot convenience: create a context, qsgw_chi0_run_host, destroy it; returns (chi0, kernel_launches).
+    Repeated jobs should keep a Chi0Context and call its run_host (no per-call allocation)."""
+    ctx = Chi0Context(orb_per_site, pb_per_site, omega, Ck.shape[0], max_n_o, max_n_u, precision=precision,
+                      occ_tol=occ_tol)
+    try:
+        return ctx.run_host(P, Ck, Ckq, eps_k, f_k, eps_kq, f_kq, out=out)
+    finally:
+        ctx.destroy()

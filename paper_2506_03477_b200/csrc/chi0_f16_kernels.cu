@@ -16,16 +16,13 @@
 //   packed FP16 arithmetic with an exact-residual FMA (no conversions): with w = w_h + w_l,
 //     a_h = w_h (x) z_h,   a_l = fma(w_h, z_h, -a_h) + w_h z_l + w_l z_h        (a_h + a_l = w z to 2^-22).
 //
-//   The CSZ CTAs of a thread-block cluster work on the same tile at CSZ consecutive frequencies: every z
-//   box is fetched from L2 once per cluster and multicast to all CTAs (the 16 frequency CTAs of a tile
-//   otherwise re-read the same boxes; at this MMA rate that is the ~6300 B/clk L2 limit, profiles/r01_mixed_*).
-//
 //   The tensor core accumulates FP32 with truncation (bias ~ -4e-8 x MMA steps into one accumulator on
 //   same-sign sums), so D is drained every WIN stages into FP32 register accumulators with round-to-nearest
 //   adds; those go to the FP64 accumulators in HBM once per launch, rescaled by 1 / sigma_j (the 2^(-2S) of each
 //   staged band batch is folded into that batch's weights).
 //
-//   FP8 = true (the default when the job sums >= 64 pairs per product function): the two correction products
+//   FP8 = true (selected per flush on the device from the weights of the staged pairs, kernels.h MixedCtl): the two
+//   correction products
 //   a_l b_h + a_h b_l are 2^-11 of the main one and need ~3 significant bits, so each runs as ONE kind::f8f6f4
 //   MMA of K = 32 on E5M2 operands (FP16's exponent range: no rescaling) into the same TMEM accumulators:
 //   8 + 8 instead of 24 MMAs per 32 pairs.  B rows then come from the "hb8" workspace
@@ -59,7 +56,7 @@ struct HCfg {
 
 // FP8 = true: the two correction products run on kind::f8f6f4 (E5M2) -- 8 f16 + 8 fp8 MMAs per 32 pairs
 // instead of 24 f16 MMAs; B rows come from the "hb8" workspace, the A source stays the full-precision hl16 rows.
-template <int CSZ, bool FP8>
+template <bool FP8>
 __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_constant__ Chi0F16Args a) {
   using C = HCfg;
   extern __shared__ unsigned char smem_dyn[];
@@ -75,23 +72,22 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   uint64_t* d_empty = d_full + 1;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(d_empty + 1);
 
+  if ((a.ctl->use_fp8 != 0) != FP8) return;     // the other variant of this flush runs (uniform over the grid)
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   // blockIdx.x = ((tile * n_freq) + j) * split + chunk: the `split` CTAs of a (tile, j) share the staged pairs
   // (few-tile problems: fills the SMs; their partial sums meet in the FP64 accumulator by atomic adds)
   const int chunk = blockIdx.x % a.split, bid = blockIdx.x / a.split;
-  const int j = a.j0 + bid % a.n_freq;                    // the CSZ CTAs of a cluster: same tile, consecutive j
+  const int j = a.j0 + bid % a.n_freq;
   const int2 tt = a.d_tiles[bid / a.n_freq];
   const bool need_a = FP8 || (tt.x != tt.y);         // f16 split, diagonal tile: the A source is the B tile
   const int s_base = (int)((long long)a.n_stages * chunk / a.split);          // first global stage of this CTA
   const int n_stages = (int)((long long)a.n_stages * (chunk + 1) / a.split) - s_base, win = a.win;
-  const uint32_t rank = CSZ > 1 ? cluster_ctarank() : 0u;
-  constexpr uint16_t kMask = (uint16_t)((1u << CSZ) - 1u);
 
   if (tid == 0) {
     tma_prefetch_desc(&a.tmap);
     for (int s = 0; s < C::STAGES; ++s) {
       mbar_init(&full[s], 1);
-      mbar_init(&empty[s], 9 * CSZ);   // (8 SA warps + the MMA commit) of every CTA of the cluster
+      mbar_init(&empty[s], 9);         // 8 SA warps + the MMA commit
     }
     for (int s = 0; s < C::TSLOTS; ++s) {
       mbar_init(&a_full[s], 8);
@@ -104,7 +100,6 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   if (warp == 1) tmem_alloc(tmem_slot, 512);
   tc_fence_before();
   __syncthreads();
-  if (CSZ > 1) cluster_sync_all();     // every CTA's barriers exist before any remote arrive / multicast
   tc_fence_after();
   const uint32_t tbase = *tmem_slot;
   const uint32_t d_re = tbase, d_im = tbase + 128, a_ring = tbase + 256;
@@ -121,15 +116,14 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
         if (u > 0) mbar_wait(&empty[st], (u - 1) & 1);
         unsigned char* sb = sm + st * C::STAGE_BYTES;
         mbar_arrive_expect_tx(&full[st], bytes);
-        // box i: operand (B | A source), plane (x | y), row half; box i is fetched by CTA i % CSZ
-        for (int i = (int)rank; i < n_box; i += CSZ) {
+        // box i: operand (B | A source), plane (x | y), row half
+        for (int i = 0; i < n_box; ++i) {
           const int plane = (i >> 1) & 1, rh = i & 1, op = i >> 2;
           unsigned char* dst = sb + op * C::B_BYTES + plane * kPlaneTileH + rh * kBoxBytes;
           const int row0 = (op ? tt.x : tt.y) * kTileMx + rh * 64;
           const CUtensorMap* tm = (FP8 && !op) ? &a.tmap_b : &a.tmap;       // hb8 rows are addressed in bytes
           const int c0 = (FP8 && !op) ? (s_base + s) * 128 : (s_base + s) * 64;
-          if (CSZ > 1) tma_load_3d_mc(dst, tm, &full[st], c0, row0, plane, kMask);
-          else tma_load_3d(dst, tm, &full[st], c0, row0, plane);
+          tma_load_3d(dst, tm, &full[st], c0, row0, plane);
         }
         bulk_load_1d(sb + C::B_BYTES + C::A_BYTES, wrow + (long long)(s_base + s) * 64, C::W_BYTES, &full[st]);
       }
@@ -188,8 +182,7 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
           umma_f16_ts(d_re, ahy, by + kl, idesc, 1u);
           umma_f16_ts(d_im, ahy, bx + kl, idesc_neg, 1u);
         }
-        if (CSZ > 1) umma_commit_mc(&empty[st], kMask);
-        else umma_commit(&empty[st]);
+        umma_commit(&empty[st]);
         umma_commit(&a_empty[ts]);
         if (((s + 1) % win) == 0 || s == n_stages - 1) umma_commit(d_full);
       }
@@ -204,9 +197,6 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
     float racc[128];
 #pragma unroll
     for (int i = 0; i < 128; ++i) racc[i] = 0.f;
-    uint32_t empty_remote[CSZ];
-#pragma unroll
-    for (int r = 0; r < CSZ; ++r) empty_remote[r] = CSZ > 1 ? mapa_shared(smem_u32(&empty[0]), (uint32_t)r) : 0u;
 
     auto drain = [&](int widx) {
       mbar_wait(d_full, widx & 1);
@@ -282,12 +272,7 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
       __syncwarp();
       if (lane == 0) {
         mbar_arrive(&a_full[ts]);
-        if (CSZ > 1) {
-#pragma unroll
-          for (int r = 0; r < CSZ; ++r) mbar_arrive_cluster(empty_remote[r] + 8u * (uint32_t)st);
-        } else {
-          mbar_arrive(&empty[st]);
-        }
+        mbar_arrive(&empty[st]);
       }
       if (s >= 1 && (s % win) == 0) drain(s / win - 1);   // stage s-1 closed a window
     }
@@ -313,100 +298,25 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   }
   tc_fence_before();
   __syncthreads();
-  if (CSZ > 1) cluster_sync_all();     // no CTA leaves while a peer may still arrive on its barriers
   if (warp == 1) tmem_dealloc(tbase, 512);
-}
-
-// Issue-rate probe of the FP16 tensor pipe: back-to-back 128x128x16 MMAs (A in TMEM, B in shared memory).
-__global__ void __launch_bounds__(128, 1) f16_peak_kernel(int iters) {
-  extern __shared__ unsigned char smem_dyn[];
-  const uint32_t raw = smem_u32(smem_dyn);
-  const uint32_t base = (raw + 1023u) & ~1023u;
-  unsigned char* sm = smem_dyn + (base - raw);
-  uint64_t* bar = reinterpret_cast<uint64_t*>(sm + kPlaneTileH);
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bar + 1);
-  const int tid = threadIdx.x, warp = tid >> 5;
-  for (int i = tid; i < kPlaneTileH / 2; i += 128) reinterpret_cast<__half*>(sm)[i] = __float2half(1.0f + 0.001f * (i & 255));
-  if (tid == 0) {
-    mbar_init(bar, 1);
-    mbar_fence_init();
-  }
-  if (warp == 0) tmem_alloc(tmem_slot, 512);
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tbase = *tmem_slot;
-  uint32_t v[16];
-#pragma unroll
-  for (int i = 0; i < 16; ++i) {
-    const __half2 t = __floats2half2_rn(0.5f + 0.01f * i, 0.25f + 0.01f * i);
-    v[i] = *reinterpret_cast<const uint32_t*>(&t);
-  }
-  tmem_st16(tbase + 256 + ((uint32_t)(32 * warp) << 16), v);
-  tmem_st16(tbase + 272 + ((uint32_t)(32 * warp) << 16), v);
-  tmem_wait_st();
-  tc_fence_before();
-  __syncthreads();
-  if (tid == 0) {
-    tc_fence_after();
-    const uint32_t idesc = umma_idesc_f16(128, 128, 0);
-    const uint64_t bd = umma_desc_k_sw128(base);
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-      for (int g = 0; g < 4; ++g) {
-        umma_f16_ts(tbase, tbase + 256 + 8 * g, bd + (uint64_t)(2 * g), idesc, (it | g) ? 1u : 0u);
-        umma_f16_ts(tbase + 128, tbase + 256 + 8 * g, bd + (uint64_t)(2 * g), idesc, (it | g) ? 1u : 0u);
-      }
-    }
-    umma_commit(bar);
-    mbar_wait(bar, 0);
-  }
-  tc_fence_before();
-  __syncthreads();
-  if (warp == 0) tmem_dealloc(tbase, 512);
-}
-
-template <int CSZ>
-cudaError_t launch_cluster(const Chi0F16Args& a, cudaStream_t s) {
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)(a.n_tiles * a.n_freq));
-  cfg.blockDim = dim3(kThreadsH);
-  cfg.dynamicSmemBytes = HCfg::SMEM_BYTES;
-  cfg.stream = s;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = CSZ;
-  attr[0].val.clusterDim.y = 1;
-  attr[0].val.clusterDim.z = 1;
-  cfg.attrs = attr;
-  cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, chi0_f16_kernel<CSZ, false>, a);
 }
 
 }  // namespace
 
 cudaError_t chi0_f16_configure() {
-  cudaError_t e = cudaFuncSetAttribute(chi0_f16_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
+  cudaError_t e = cudaFuncSetAttribute(chi0_f16_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(chi0_f16_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(chi0_f16_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(chi0_f16_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(f16_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 20480);
+  return cudaFuncSetAttribute(chi0_f16_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, HCfg::SMEM_BYTES);
 }
 
-cudaError_t launch_chi0_f16(const Chi0F16Args& a_in, int cluster, bool fp8, cudaStream_t s) {
+cudaError_t launch_chi0_f16(const Chi0F16Args& a_in, cudaStream_t s) {
   if (a_in.n_stages <= 0 || a_in.n_tiles <= 0) return cudaSuccess;
   Chi0F16Args a = a_in;
   // Few (tile, frequency) work items: split the staged pairs over 2..4 CTAs each, choosing the split that
-  // minimises rounds(CTAs / SMs) / split; every CTA keeps >= 32 stages.  Single-CTA launches only.
+  // minimises rounds(CTAs / SMs) / split; every CTA keeps >= 32 stages.
   a.split = 1;
-  if (cluster <= 1) {
-    int n_sm = 148;
-    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+  {
+    const int n_sm = a.n_sm;
     const long long items = (long long)a.n_tiles * a.n_freq;
     double best = (double)((items + n_sm - 1) / n_sm);
     for (int sp = 2; sp <= 4; ++sp) {
@@ -416,50 +326,11 @@ cudaError_t launch_chi0_f16(const Chi0F16Args& a_in, int cluster, bool fp8, cuda
     }
   }
   const unsigned grid = (unsigned)(a.n_tiles * a.n_freq * a.split);
-  if (fp8) {   // the FP8-corrected variant is built for single-CTA launches only
-    chi0_f16_kernel<1, true><<<dim3(grid), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
-    return cudaGetLastError();
-  }
-  if (cluster > 1 && a.n_freq % cluster != 0) cluster = (a.n_freq % 2 == 0) ? 2 : 1;
-  if (cluster >= 4) return launch_cluster<4>(a, s);
-  if (cluster >= 2) return launch_cluster<2>(a, s);
-  chi0_f16_kernel<1, false><<<dim3(grid), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
+  chi0_f16_kernel<true><<<dim3(grid), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  chi0_f16_kernel<false><<<dim3(grid), kThreadsH, HCfg::SMEM_BYTES, s>>>(a);
   return cudaGetLastError();
-}
-
-cudaError_t probe_f16_mma(cudaStream_t s, double* out_tflops, double* out_ms) {
-  int dev = 0, n_sm = 0;
-  cudaError_t e = cudaGetDevice(&dev);
-  if (e != cudaSuccess) return e;
-  e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-  if (e != cudaSuccess) return e;
-  e = chi0_f16_configure();
-  if (e != cudaSuccess) return e;
-  cudaEvent_t e0 = nullptr, e1 = nullptr;
-  cudaEventCreate(&e0);
-  cudaEventCreate(&e1);
-  const int iters = 40000;
-  f16_peak_kernel<<<n_sm, 128, 20480, s>>>(iters / 4);
-  float best = 1e30f;
-  for (int rep = 0; rep < 4; ++rep) {
-    cudaEventRecord(e0, s);
-    f16_peak_kernel<<<n_sm, 128, 20480, s>>>(iters);
-    cudaEventRecord(e1, s);
-    e = cudaEventSynchronize(e1);
-    if (e != cudaSuccess) break;
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, e0, e1);
-    if (ms < best) best = ms;
-  }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  if (e != cudaSuccess) return e;
-  e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
-  const double flop = 2.0 * 128.0 * 128.0 * 16.0 * 8.0 * (double)iters * n_sm;
-  if (out_tflops) *out_tflops = flop / (best * 1e-3) / 1e12;
-  if (out_ms) *out_ms = best;
-  return cudaSuccess;
 }
 
 }  // namespace qsgw

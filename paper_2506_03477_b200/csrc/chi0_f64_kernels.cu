@@ -2,10 +2,9 @@
 // frequency per CTA (Eq. 14; Alg. 1 lines 16-21), on the FP64 tensor
 // pipe (DMMA.8x8x4), and the finalize kernel (1/N_k, Hermitian mirror).
 //
-// z = x + i y:  Re += x_I (w x_J) + y_I (w y_J),  Im += x_I (w y_J) - y_I (w x_J)   ("4M").
-// The 64-column x KP-pair tiles of both planes arrive by one 4-D TMA box per operand with the
+// The 64-column x 32-pair tiles of both planes (z = x + i y) arrive by one 4-D TMA box per operand with the
 // 128-byte swizzle; w_j(p) for the stage arrives by a 1-D bulk copy; the frequency-scaled operand
-// w*z is formed in registers.  4 warps, each a 32x32 complex sub-tile = 64 DMMA per 4 pairs.
+// w*z is formed in registers.
 #include "kernels.h"
 #include "ptx.cuh"
 
@@ -13,164 +12,14 @@ namespace qsgw {
 
 namespace {
 
-constexpr int KP = kChi0F64KP;         // pairs per stage
 constexpr int STAGES = 3;
-constexpr int kThreads = 128;
-constexpr int OPER_BYTES = 2 * 4 * KP * 128;   // planes x column groups x rows x 128 B
-constexpr int PLANE_BYTES = 4 * KP * 128;
-constexpr int CGRP_BYTES = KP * 128;
-constexpr int W_BYTES = KP * 8;
-constexpr int SMEM_OPERANDS = STAGES * 2 * OPER_BYTES;
-constexpr int SMEM_BYTES = SMEM_OPERANDS + STAGES * W_BYTES + 2 * STAGES * 8 + 1024 /*align slack*/;
 
-static_assert(KP % 8 == 0, "swizzle atom is 8 rows");
-static_assert(CGRP_BYTES % 1024 == 0, "column-group blocks must keep the 1024 B swizzle alignment");
-
-__global__ void __launch_bounds__(kThreads, 2) chi0_f64_kernel(const __grid_constant__ Chi0F64Args a) {
-  extern __shared__ unsigned char smem_dyn[];
-  const uint32_t raw = smem_u32(smem_dyn);
-  const uint32_t base = (raw + 1023u) & ~1023u;
-  unsigned char* sm = smem_dyn + (base - raw);
-  double* wsm = reinterpret_cast<double*>(sm + SMEM_OPERANDS);
-  uint64_t* full = reinterpret_cast<uint64_t*>(sm + SMEM_OPERANDS + STAGES * W_BYTES);
-  uint64_t* empty = full + STAGES;
-
-  const int tid = threadIdx.x;
-  const int lane = tid & 31, warp = tid >> 5;
-  const int g = lane >> 2, t = lane & 3;
-  const int wm = warp >> 1, wn = warp & 1;
-
-  const int j = a.j0 + blockIdx.x % a.n_freq;
-  const int tile = blockIdx.x / a.n_freq;
-  const int2 tt = a.d_tiles[tile];
-  const bool diag = (tt.x == tt.y);
-  const int n_iter = (int)(a.n_pairs_padded / KP);
-  const double* wrow = a.wtab + (long long)j * a.kpad;
-
-  if (tid == 0) {
-    tma_prefetch_desc(&a.tmap_z);
-    for (int s = 0; s < STAGES; ++s) {
-      mbar_init(&full[s], 1);
-      mbar_init(&empty[s], kThreads / 32);
-    }
-    mbar_fence_init();
-  }
-  __syncthreads();
-
-  const uint32_t stage_bytes = (diag ? OPER_BYTES : 2 * OPER_BYTES) + W_BYTES;
-  auto issue = [&](int slot, int it) {
-    unsigned char* dstA = sm + slot * (2 * OPER_BYTES);
-    mbar_arrive_expect_tx(&full[slot], stage_bytes);
-    tma_load_4d(dstA, &a.tmap_z, &full[slot], 0, it * KP, tt.x * 4, 0);
-    if (!diag) tma_load_4d(dstA + OPER_BYTES, &a.tmap_z, &full[slot], 0, it * KP, tt.y * 4, 0);
-    bulk_load_1d(wsm + slot * KP, wrow + (long long)it * KP, W_BYTES, &full[slot]);
-  };
-
-  if (tid == 0) {
-    for (int it = 0; it < STAGES - 1 && it < n_iter; ++it) issue(it, it);
-  }
-
-  // per-thread swizzled offsets: row r = 8*(q>>1) + 2t + (q&1); 16-byte chunk ^= r&7
-  uint32_t thr_off[2][2];
-#pragma unroll
-  for (int s = 0; s < 2; ++s)
-#pragma unroll
-    for (int par = 0; par < 2; ++par)
-      thr_off[s][par] = (uint32_t)((2 * t + s) * 128 + ((((4 * par + (g >> 1)) ^ (2 * t + s)) << 4) | ((g & 1) << 3)));
-
-  double cre[4][4][2], cim[4][4][2];
-#pragma unroll
-  for (int mi = 0; mi < 4; ++mi)
-#pragma unroll
-    for (int ni = 0; ni < 4; ++ni) {
-      cre[mi][ni][0] = cre[mi][ni][1] = 0.0;
-      cim[mi][ni][0] = cim[mi][ni][1] = 0.0;
-    }
-
-  for (int it = 0; it < n_iter; ++it) {
-    const int slot = it % STAGES;
-    if (tid == 0) {
-      const int nxt = it + STAGES - 1;
-      if (nxt < n_iter) {
-        const int s2 = nxt % STAGES;
-        if (nxt >= STAGES) mbar_wait(&empty[s2], ((nxt / STAGES) - 1) & 1);
-        issue(s2, nxt);
-      }
-    }
-    __syncwarp();
-    mbar_wait(&full[slot], (it / STAGES) & 1);
-
-    const uint32_t aBase = base + slot * (2 * OPER_BYTES) + (2 * wm) * CGRP_BYTES;
-    const uint32_t bBase = base + slot * (2 * OPER_BYTES) + (diag ? 0 : OPER_BYTES) + (2 * wn) * CGRP_BYTES;
-    const uint32_t wBase = base + SMEM_OPERANDS + slot * W_BYTES;
-
-#pragma unroll
-    for (int q = 0; q < KP / 4; ++q) {
-      const uint32_t rq = (uint32_t)((q >> 1) * 1024);
-      const double w = ld_shared_f64(wBase + (uint32_t)((8 * (q >> 1) + 2 * t + (q & 1)) * 8));
-      double ax[4], ay[4], bx[4], by[4];
-#pragma unroll
-      for (int mi = 0; mi < 4; ++mi) {
-        const uint32_t ad = aBase + (mi >> 1) * CGRP_BYTES + rq + thr_off[q & 1][mi & 1];
-        ax[mi] = ld_shared_f64(ad);
-        ay[mi] = ld_shared_f64(ad + PLANE_BYTES);
-      }
-#pragma unroll
-      for (int ni = 0; ni < 4; ++ni) {
-        const uint32_t ad = bBase + (ni >> 1) * CGRP_BYTES + rq + thr_off[q & 1][ni & 1];
-        bx[ni] = w * ld_shared_f64(ad);
-        by[ni] = w * ld_shared_f64(ad + PLANE_BYTES);
-      }
-#pragma unroll
-      for (int mi = 0; mi < 4; ++mi)
-#pragma unroll
-        for (int ni = 0; ni < 4; ++ni) {
-          dmma884(cre[mi][ni][0], cre[mi][ni][1], ax[mi], bx[ni]);
-          dmma884(cim[mi][ni][0], cim[mi][ni][1], ax[mi], by[ni]);
-        }
-#pragma unroll
-      for (int ni = 0; ni < 4; ++ni) bx[ni] = -bx[ni];
-#pragma unroll
-      for (int mi = 0; mi < 4; ++mi)
-#pragma unroll
-        for (int ni = 0; ni < 4; ++ni) {
-          dmma884(cre[mi][ni][0], cre[mi][ni][1], ay[mi], by[ni]);
-          dmma884(cim[mi][ni][0], cim[mi][ni][1], ay[mi], bx[ni]);
-        }
-    }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&empty[slot]);
-  }
-
-  // epilogue: exclusive owner of (tile, j) -> plain read-modify-write
-  const long long plane = (long long)a.n_m_pad * a.n_m_pad;
-  double* are = a.acc_re + (long long)j * plane;
-  double* aim = a.acc_im + (long long)j * plane;
-#pragma unroll
-  for (int mi = 0; mi < 4; ++mi) {
-    const int row = tt.x * kTile + (4 * wm + mi) * 8 + g;
-#pragma unroll
-    for (int ni = 0; ni < 4; ++ni) {
-      const int col = tt.y * kTile + (4 * wn + ni) * 8 + 2 * t;
-      const long long off = (long long)row * a.n_m_pad + col;
-      double2 r = *reinterpret_cast<double2*>(are + off);
-      r.x += cre[mi][ni][0];
-      r.y += cre[mi][ni][1];
-      *reinterpret_cast<double2*>(are + off) = r;
-      double2 m = *reinterpret_cast<double2*>(aim + off);
-      m.x += cim[mi][ni][0];
-      m.y += cim[mi][ni][1];
-      *reinterpret_cast<double2*>(aim + off) = m;
-    }
-  }
-}
-
-// 3M form (three real products per complex one, 25 % fewer DMMAs than 4M):
+// 3M form (three real products per complex one, 25 % fewer DMMAs than the four-product form):
 //   T1 += x_I (w x_J),  T2 += y_I (w y_J),  T3 += (x_I + y_I) (w (y_J - x_J));   Re = T1 + T2,  Im = T3 + T1 - T2.
 // 8 warps (2 along I x 4 along J), each a 32x16 complex sub-tile = 3 x 16 FP64 accumulator pairs; per 4 pairs a
 // warp loads 12 operand doubles and issues 24 DMMAs.  Normwise error ~1e-15 (the parity bar is 1e-11).
 constexpr int kThreads3M = 256;
-constexpr int KP3 = kChi0F64KP3M;     // pairs per stage of the 3M kernel (1 CTA/SM: twice the 4M kernel's stage)
+constexpr int KP3 = kChi0F64KP3M;     // pairs per stage (1 CTA/SM)
 constexpr int OPER_BYTES3 = 2 * 4 * KP3 * 128;
 constexpr int PLANE_BYTES3 = 4 * KP3 * 128;
 constexpr int CGRP_BYTES3 = KP3 * 128;
@@ -370,18 +219,15 @@ __global__ void __launch_bounds__(256) finalize_kernel(const double* __restrict_
 }  // namespace
 
 cudaError_t chi0_f64_configure() {
-  cudaError_t e = cudaFuncSetAttribute(chi0_f64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-  if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(chi0_f64_3m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES3);
 }
 
-cudaError_t launch_chi0_f64(const Chi0F64Args& a_in, bool three_m, cudaStream_t s) {
+cudaError_t launch_chi0_f64(const Chi0F64Args& a_in, cudaStream_t s) {
   if (a_in.n_pairs_padded <= 0 || a_in.n_tiles <= 0) return cudaSuccess;
   Chi0F64Args a = a_in;
   a.split = 1;
-  if (three_m) {   // few (tile, frequency) items (1 CTA/SM): split the staged pairs over 2..4 CTAs (see launch_chi0_f16)
-    int n_sm = 148;
-    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+  {   // few (tile, frequency) items (1 CTA/SM): split the staged pairs over 2..4 CTAs (see launch_chi0_f16)
+    const int n_sm = a.n_sm;
     const long long items = (long long)a.n_tiles * a.n_freq, n_it = a.n_pairs_padded / KP3;
     double best = (double)((items + n_sm - 1) / n_sm);
     for (int sp = 2; sp <= 4; ++sp) {
@@ -391,8 +237,7 @@ cudaError_t launch_chi0_f64(const Chi0F64Args& a_in, bool three_m, cudaStream_t 
     }
   }
   dim3 grid((unsigned)(a.n_tiles * a.n_freq * a.split));
-  if (three_m) chi0_f64_3m_kernel<<<grid, kThreads3M, SMEM_BYTES3, s>>>(a);
-  else chi0_f64_kernel<<<grid, kThreads, SMEM_BYTES, s>>>(a);
+  chi0_f64_3m_kernel<<<grid, kThreads3M, SMEM_BYTES3, s>>>(a);
   return cudaGetLastError();
 }
 

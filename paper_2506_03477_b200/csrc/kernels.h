@@ -5,12 +5,6 @@
 //       column group cg = I / 16 ("CG"), pair row p = n_local * n_u + n'_local, 16 doubles = 128 B.
 //       One 4-D TMA box {16, KP, 4, 2} then brings a 64-column x KP-pair tile of both planes into
 //       shared memory as [plane][cg][row][128 B] with the 128-byte swizzle.
-//   z workspace, mixed mode: float zws32[4 planes][n_m_pad][kpad]   (K-major: pair index contiguous)
-//       plane 0/1 = Re/Im of z in FP32.  planes 2/3: 3xTF32 mode = Re/Im of z minus its TF32
-//       truncation (the "lo" split part; the tensor core truncates plane 0/1 itself); 1xTF32 mode =
-//       Re/Im of z rounded to nearest TF32.  n_m_pad = ceil128(N_M); rows >= N_M stay zero.
-//       3-D TMA boxes {32 pairs, 128 rows, 2|4 planes} with the 128-byte swizzle give K-major
-//       UMMA operand tiles.  Weight table (mixed): float wtab32[n_freq][kpad].
 //   weight table:            double wtab[n_freq][kpad]        (zero beyond the batch's pairs)
 //   accumulators:            double acc_re/acc_im[n_freq][n_m_pad][n_m_pad], n_m_pad = ceil64(N_M);
 //       only tiles with tile_i <= tile_j are touched.
@@ -22,6 +16,7 @@
 
 namespace qsgw {
 
+constexpr int kMaxDevices = 64; // per-device bookkeeping of kernel attributes
 constexpr int kCG = 16;         // columns per column group (128 B of doubles)
 constexpr int kTile = 64;       // stage (b) CTA tile edge (complex outputs)
 constexpr int kPairAlign = 32;  // kpad and the padded pair count are multiples of this
@@ -48,6 +43,7 @@ struct ZmelArgs {
   int ncg;
   float* zmax = nullptr; // optional: atomicMax of |Re z|, |Im z| over the batch (FP16-split mixed mode)
   int kt = 0;            // DMMA kernel: padded contraction length, max over column groups of sum_seg pad4(b_seg)
+  int n_sm = 148;        // SMs of the context's device
 };
 
 cudaError_t launch_zmel_f64(const ZmelArgs& a, cudaStream_t s);    // CUDA-core fallback
@@ -71,45 +67,18 @@ struct Chi0F64Args {
   int n_m_pad;
   int n_freq;                 // frequencies of this launch: j0 .. j0 + n_freq - 1
   int j0 = 0;
-  int split = 1;              // CTAs sharing the staged pairs of one (tile, frequency); set by launch_chi0_f64 (3M)
+  int split = 1;              // CTAs sharing the staged pairs of one (tile, frequency); set by launch_chi0_f64
+  int n_sm = 148;             // SMs of the context's device
   long long n_pairs_padded;   // multiple of kPairAlign
   const int2* d_tiles;        // (tile_i, tile_j), tile_i <= tile_j
   int n_tiles;
 };
-constexpr int kChi0F64KP = 16;    // pairs per pipeline stage of the 4M kernel (box rows of its tensor map)
-constexpr int kChi0F64KP3M = 32;  // same for the 3M kernel
-cudaError_t launch_chi0_f64(const Chi0F64Args& a, bool three_m /*3M complex product (default) or 4M*/, cudaStream_t s);
-cudaError_t chi0_f64_configure();   // sets the dynamic shared-memory attribute once
+constexpr int kChi0F64KP3M = 32;  // pairs per pipeline stage (box rows of the tensor map)
+cudaError_t launch_chi0_f64(const Chi0F64Args& a, cudaStream_t s);
+cudaError_t chi0_f64_configure();   // sets the dynamic shared-memory attribute (per device: call at context creation)
 
-// ---- mixed mode (chi0_tf32_kernels.cu) -------------------------------------------------------------
 constexpr int kTileMx = 128;       // stage (b) CTA tile edge in mixed mode (UMMA M = N = 128)
-constexpr int kPairStage = 32;     // pairs per pipeline stage (one 128-byte swizzle row of floats)
-
-struct Chi0Tf32Args {
-  CUtensorMap tmap2;     // 3-D FLOAT32 {kpad, n_m_pad, 4}, box {32, 128, 2}, SWIZZLE_128B
-  CUtensorMap tmap4;     // same tensor, box {32, 128, 4}
-  const float* wtab32;   // [n_freq][kpad]
-  long long kpad;
-  double* acc_re;
-  double* acc_im;
-  int n_m_pad;           // multiple of 128
-  int n_freq;
-  int n_stages;          // ceil(n_pairs / 32)
-  const int2* d_tiles;   // 128x128 tiles, tile_i <= tile_j
-  int n_tiles;
-};
-cudaError_t chi0_tf32_configure();
-cudaError_t launch_chi0_tf32(const Chi0Tf32Args& a, int n_pass /*1 or 3*/, cudaStream_t s);
-
-// stage (a) with FP32 plane output (arithmetic in FP64, one rounding to FP32 on store)
-cudaError_t launch_zmel_mixed(const ZmelArgs& a, float* zws32, int n_m_pad, int split_lo, cudaStream_t s);
-cudaError_t launch_z_export32(const float* zws32, long long kpad, int n_m_pad, int n_m, long long n_pairs,
-                              double2* out, cudaStream_t s);
-cudaError_t launch_planes32_from_ws(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs,
-                                    float* zws32, int n_m_pad, int split_lo, cudaStream_t s);
-cudaError_t launch_weights_to_f32(const double* wtab, float* wtab32, long long kpad, long long n_pad, int n_freq,
-                                  cudaStream_t s);
-cudaError_t probe_tf32_mma(cudaStream_t s, double* out_tflops, double* out_ms);
+constexpr int kPairStage = 32;     // pairs per pipeline stage (one 128-byte swizzle row)
 
 // ---- mixed mode, FP16 split (chi0_f16_kernels.cu) ---------------------------------------------------
 //   z workspace "hl16": __half zhl[2 planes (Re,Im)][n_m_pad][kpad/32][64]: per product function I and
@@ -121,6 +90,20 @@ cudaError_t probe_tf32_mma(cudaStream_t s, double* out_tflops, double* out_ms);
 //   FP8-corrected variant: a second workspace "hb8" with rows  h[32] halves | e5m2(v)[32] | e5m2(v - h)[32]
 //   feeds the B operand (same 128 bytes per 32 pairs): a b ~= a_h b_h (kind::f16) + a_l8 b_8 + a_8 b_l8
 //   (kind::f8f6f4, E5M2): the two correction products need only ~3 significant bits.
+// Device-side control block of the mixed mode (one per context).
+//   E5M2 correction products add a relative Frobenius error ~ c * sqrt(N_M / P_eff) with P_eff the effective number
+//   of band pairs summed per output element, P_eff = (sum_p w)^2 / sum_p w^2 (participation ratio of the weights of
+//   the staged pairs, minimum over the frequencies).  use_fp8 = mode 1, or mode 2 and P_eff >= thr_pairs.
+struct MixedCtl {
+  float peff_min;            // min over frequencies of P_eff of the flush being prepared (atomicMin on the bits)
+  int use_fp8;               // decision for the current flush
+  int mode;                  // 0 never | 1 always | 2 automatic
+  float thr_pairs;           // automatic: threshold on P_eff (pairs), = T * N_M
+  unsigned int ticket;       // last-block-done counter of weights_scale_hl16_kernel
+  unsigned long long n_flush, n_flush_fp8;   // statistics (qsgw_mixed_stats)
+  float peff_min_seen;       // smallest P_eff of any flush since the last reset
+};
+
 struct Chi0F16Args {
   CUtensorMap tmap;      // 3-D FLOAT16 {2*kpad, n_m_pad, 2}, box {64, 64, 1}, SWIZZLE_128B
   CUtensorMap tmap_b;    // FP8 variant: 3-D UINT8 {4*kpad, n_m_pad, 2}, box {128, 64, 1}, SWIZZLE_128B
@@ -136,20 +119,23 @@ struct Chi0F16Args {
   int win;               // stages per drain window (12 MMA steps into each accumulator per stage)
   int j0 = 0;            // first frequency of this launch (n_freq = count)
   int split = 1;         // CTAs sharing the staged pairs of one (tile, frequency); set by launch_chi0_f16
+  int n_sm = 148;        // SMs of the context's device
+  const MixedCtl* ctl;   // device: use_fp8 selects the variant that runs (the other one exits at once)
   const int2* d_tiles;   // 128x128 tiles, tile_i <= tile_j
   int n_tiles;
 };
 cudaError_t chi0_f16_configure();
-cudaError_t launch_chi0_f16(const Chi0F16Args& a, int cluster /*CTAs sharing a tile: 1, 2 or 4*/, bool fp8,
-                            cudaStream_t s);
+// Launches BOTH product variants (three FP16 products | FP16 main + two E5M2 correction products); each CTA reads
+// ctl->use_fp8 first and the variant that was not selected returns immediately (the selection is made on the
+// device from the weights of the staged pairs, see weights_scale_hl16_kernel: no host synchronisation).
+cudaError_t launch_chi0_f16(const Chi0F16Args& a, cudaStream_t s);
 cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs, void* zhl,
                              void* zhb8 /*optional FP8-variant B rows*/, int n_m_pad, const float* zmax,
                              cudaStream_t s);
 cudaError_t launch_z_export_hl16(const void* zhl, long long kpad, int n_m_pad, int n_m, long long n_pairs,
                                  const float* zmax, double2* out, cudaStream_t s);
 cudaError_t launch_weights_scale_hl16(const double* wtab, void* wtab16, double* wscale, long long kpad, long long n_pad,
-                                      int n_freq, cudaStream_t s);
-cudaError_t probe_f16_mma(cudaStream_t s, double* out_tflops, double* out_ms);
+                                      int n_freq, MixedCtl* ctl, cudaStream_t s);
 
 // ---- screened Coulomb interaction W^c (wc_kernels.cu) ---------------------------------------------------
 struct ZgemmArgs {       // batched complex FP64 GEMM on 64x64 tiles (see zgemm_dmma_kernel)
@@ -160,12 +146,13 @@ struct ZgemmArgs {       // batched complex FP64 GEMM on 64x64 tiles (see zgemm_
   double alpha;                 // real scale
   int beta_one;                 // 1: C += ..., 0: C = ...
   int tri;                      // 0 all tiles | 1 lower tiles only | 2 lower tiles and k starts at 64*max(ti,tj)
+                                // | 3 all tiles and k starts at 64*tj (B lower triangular)
 };
 // W^c[j] = sqrt(v) ((1 - sqrt(v) chi0[j] sqrt(v))^-1 - 1) sqrt(v) for all frequencies, stream-ordered.
 // work: n_freq * (2 * n_pad^2 + 64 * n_pad + nb * 64 * 64) complex elements, n_pad = ceil64(n_m), nb = n_pad / 64.
 // d_info: 0, or 1 + index of the first non-positive Cholesky pivot (eps not positive definite).
 size_t wc_work_elems(int n_m, int n_freq);
-cudaError_t wc_configure();
+cudaError_t wc_configure();          // kernel attributes (per device)
 // chi0 -> U^H chi0 U for all frequencies (work: rotate_work_elems complex elements)
 size_t rotate_work_elems(int n_m, int n_freq);
 cudaError_t launch_rotate_basis(int n_m, int n_freq, const double2* chi0, const double2* U, double2* out, double2* work,
@@ -175,6 +162,8 @@ cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const 
 
 // issue-rate probes (probe_kernels.cu): measured MMA-pipe peaks for the roofline denominators
 cudaError_t probe_fp64_mma(cudaStream_t s, double* out_tflops, double* out_ms);
+cudaError_t probe_tf32_mma(cudaStream_t s, double* out_tflops, double* out_ms);
+cudaError_t probe_f16_mma(cudaStream_t s, double* out_tflops, double* out_ms);
 
 cudaError_t launch_finalize(const double* acc_re, const double* acc_im, int n_m, int n_m_pad, int n_freq,
                             double inv_nk, double2* out, cudaStream_t s);

@@ -63,21 +63,24 @@ struct qsgw_ctx {
   long long p_elems = 0;
   double* d_zws = nullptr;
   double* d_wtab = nullptr;
-  float* d_zws32 = nullptr;     // mixed mode: FP32 K-major planes (kernels.h)
-  float* d_wtab32 = nullptr;
-  int n_pass = 0;               // TF32 mixed modes: products per complex term (3 = 3xTF32, 1 = single)
-  CUtensorMap tmap2, tmap4;
+  float* d_wtab32 = nullptr;    // mixed mode: fp16 weight pieces (same bytes per pair as an FP32 table)
   bool f16 = false;             // QSGW_PREC_MIXED: FP16-split planes (kernels.h "hl16")
   void* d_zhl = nullptr;
-  void* d_zhb8 = nullptr;        // FP8-corrected variant: B rows h | e5m2(v) | e5m2(v-h)
-  bool fp8 = false;
+  void* d_zhb8 = nullptr;       // B rows of the E5M2-corrected variant: h | e5m2(v) | e5m2(v-h)
   CUtensorMap tmap_hb8;
   double* d_wscale = nullptr;
   float* d_zmax = nullptr;
-  int cluster = 1;              // CTAs of a cluster sharing one tile's z boxes (1, 2 or 4)
+  qsgw::MixedCtl* d_ctl = nullptr;   // device-side choice of the product variant per flush
+  int fp8_mode = 2;             // 0 never | 1 always | 2 chosen on the device (option "mixed_fp8")
+  double fp8_thr = 2.0;         // automatic choice: E5M2 when P_eff >= fp8_thr * N_M
   int win = 8;                  // stages per TMEM drain window
-  int zmel_kt = 0;              // stage (a) DMMA kernel: padded contraction length (0 = CUDA-core fallback)
-  bool f64_3m = true;           // FP64 mode: 3M complex product (QSGW_F64_4M=1 selects the 4M kernel)
+  int zmel_kt = 0;              // stage (a) DMMA kernel: padded contraction length (0 = CUDA-core kernel)
+  int zmel_kt_avail = 0;        // ... as computed at creation (option "zmel_dmma" switches zmel_kt between 0 and this)
+  int device = 0, n_sm = 148;   // device the context lives on
+  long long batch_pad = 0;      // padded pairs of the largest band batch
+  long long stage_cap = 0;      // staged pairs that trigger a flush (<= kpad; option "stage_batches")
+  long long z_off = 0;          // workspace slot of the batch the last zmel_build wrote
+  int e2e_groups = 4;           // frequency groups of the last flush of qsgw_chi0_run_host
   CUtensorMap tmap_h;
   double* d_acc_re = nullptr;
   double* d_acc_im = nullptr;
@@ -95,6 +98,18 @@ struct qsgw_ctx {
   std::vector<cudaEvent_t> ev_free;
   double stage_ms[QSGW_N_STAGES] = {0, 0, 0, 0};
   long long stage_n[QSGW_N_STAGES] = {0, 0, 0, 0};
+  // device staging buffers of qsgw_chi0_run_host (allocated by its first call)
+  struct HostRun {
+    double2* dP = nullptr;
+    double2* dCk[2] = {nullptr, nullptr};
+    double2* dCkq[2] = {nullptr, nullptr};
+    double* dE[2] = {nullptr, nullptr};       // eps_k | f_k | eps_kq | f_kq
+    double2* dOut = nullptr;
+    size_t ck_cap = 0, ckq_cap = 0, e_cap = 0;
+    cudaEvent_t done[2] = {nullptr, nullptr};
+    cudaEvent_t ready[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaStream_t cp = nullptr;
+  } hr;
 
   int fail(int code, const char* fmt, ...) {
     char buf[512];
@@ -133,8 +148,18 @@ void free_all(qsgw_ctx* c) {
   cudaFree(c->d_P);
   cudaFree(c->d_zws);
   cudaFree(c->d_wtab);
-  cudaFree(c->d_zws32);
   cudaFree(c->d_wtab32);
+  cudaFree(c->d_ctl);
+  cudaFree(c->hr.dP);
+  cudaFree(c->hr.dOut);
+  for (int i = 0; i < 2; ++i) {
+    cudaFree(c->hr.dCk[i]);
+    cudaFree(c->hr.dCkq[i]);
+    cudaFree(c->hr.dE[i]);
+    if (c->hr.done[i]) cudaEventDestroy(c->hr.done[i]);
+  }
+  for (int i = 0; i < 4; ++i) if (c->hr.ready[i]) cudaEventDestroy(c->hr.ready[i]);
+  if (c->hr.cp) cudaStreamDestroy(c->hr.cp);
   cudaFree(c->d_zhl);
   cudaFree(c->d_zhb8);
   cudaFree(c->d_wscale);
@@ -209,7 +234,7 @@ int create_fail(qsgw_ctx* c, int code, const std::string& msg) {
 int validate_desc(const qsgw_desc* d, std::string& why) {
   if (!d) { why = "desc is NULL"; return QSGW_ERR_INVALID_ARG; }
   if (!d->h_orb_per_site || !d->h_pb_per_site || !d->h_omega) { why = "NULL array in desc"; return QSGW_ERR_INVALID_ARG; }
-  if (d->precision < QSGW_PREC_FP64 || d->precision > QSGW_PREC_MIXED_TF32X3) { why = "bad precision enum"; return QSGW_ERR_INVALID_ARG; }
+  if (d->precision != QSGW_PREC_FP64 && d->precision != QSGW_PREC_MIXED) { why = "bad precision enum"; return QSGW_ERR_INVALID_ARG; }
   if (d->n_sites < 1 || d->n_freq < 1 || d->n_k < 1 || d->max_n_o < 1 || d->max_n_u < 1) {
     why = "non-positive extent in desc"; return QSGW_ERR_SHAPE;
   }
@@ -228,17 +253,45 @@ int validate_desc(const qsgw_desc* d, std::string& why) {
 
 namespace {
 
-cudaError_t wc_configure_once() {
-  static std::once_flag once;
-  static cudaError_t result = cudaSuccess;
-  std::call_once(once, [] { result = qsgw::wc_configure(); });
-  return result;
+// Device ordinal, SM count and compute capability of the current device (cached per device; cheap attribute
+// queries instead of cudaGetDeviceProperties).
+struct DevInfo { int dev = -1, n_sm = 0, cc_major = 0; };
+cudaError_t current_device(DevInfo* out) {
+  static std::mutex mu;
+  static DevInfo cache[qsgw::kMaxDevices];
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
+  if (dev >= 0 && dev < qsgw::kMaxDevices && cache[dev].dev == dev) { *out = cache[dev]; return cudaSuccess; }
+  DevInfo d;
+  d.dev = dev;
+  e = cudaDeviceGetAttribute(&d.n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&d.cc_major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e != cudaSuccess) return e;
+  if (dev >= 0 && dev < qsgw::kMaxDevices) cache[dev] = d;
+  *out = d;
+  return cudaSuccess;
 }
 
-// Internal stream and in-flight executable graphs of qsgw_wc_from_chi0 (destroyed once their event completed).
+// Kernel attributes of wc_kernels.cu, set once per device.
+cudaError_t wc_configure_device(int dev) {
+  static std::mutex mu;
+  static bool done[qsgw::kMaxDevices] = {};
+  std::lock_guard<std::mutex> lock(mu);
+  if (dev >= 0 && dev < qsgw::kMaxDevices && done[dev]) return cudaSuccess;
+  cudaError_t e = qsgw::wc_configure();
+  if (e == cudaSuccess && dev >= 0 && dev < qsgw::kMaxDevices) done[dev] = true;
+  return e;
+}
+
+int g_wc_graph = 1;     // option "wc_graph": 0 plain launches | 1 graph with fallback | 2 graph or fail
+
+// Internal streams (one per device) and in-flight executable graphs of qsgw_wc_from_chi0 (destroyed once their
+// event completed).
 struct WcGraphs {
   std::mutex mu;
-  cudaStream_t stream = nullptr;
+  cudaStream_t stream[qsgw::kMaxDevices] = {};
   struct Item { cudaGraphExec_t exec; cudaEvent_t done; };
   std::vector<Item> pending;
   void sweep() {
@@ -264,7 +317,7 @@ WcGraphs& wc_graphs() {
 
 extern "C" {
 
-const char* qsgw_version(void) { return "qsgw-chi0 0.1 (sm_100a)"; }
+const char* qsgw_version(void) { return "qsgw-chi0 0.2 (sm_100a)"; }
 const char* qsgw_last_create_error(void) { return g_create_error.c_str(); }
 const char* qsgw_last_error(const qsgw_ctx* ctx) { return ctx ? ctx->err.c_str() : "ctx is NULL"; }
 int64_t qsgw_kernel_launches(const qsgw_ctx* ctx) { return ctx ? ctx->launches : 0; }
@@ -272,7 +325,6 @@ int64_t qsgw_pairs_accumulated(const qsgw_ctx* ctx) { return ctx ? ctx->pairs : 
 size_t qsgw_device_bytes(const qsgw_ctx* ctx) { return ctx ? ctx->device_bytes : 0; }
 int32_t qsgw_n_m(const qsgw_ctx* ctx) { return ctx ? ctx->n_m : 0; }
 int32_t qsgw_n_b(const qsgw_ctx* ctx) { return ctx ? ctx->n_b : 0; }
-int32_t qsgw_mixed_fp8(const qsgw_ctx* ctx) { return (ctx && ctx->fp8) ? 1 : 0; }
 
 int32_t qsgw_probe_peak(int32_t kind, double* out_tflops, double* out_ms) {
   g_create_error.clear();
@@ -309,6 +361,18 @@ int32_t qsgw_stage_time_ms(qsgw_ctx* ctx, int32_t stage, double* out_ms, int64_t
   return QSGW_OK;
 }
 
+static cudaError_t upload_ctl(qsgw_ctx* c) {
+  qsgw::MixedCtl h;
+  memset(&h, 0, sizeof(h));
+  h.peff_min = 3.0e38f;
+  h.peff_min_seen = 3.0e38f;
+  h.mode = c->fp8_mode;
+  h.use_fp8 = c->fp8_mode == 1;
+  h.thr_pairs = (float)(c->fp8_thr * c->n_m);
+  // pageable source: the copy is staged before the call returns
+  return cudaMemcpyAsync(c->d_ctl, &h, sizeof(h), cudaMemcpyHostToDevice, c->stream);
+}
+
 int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   g_create_error.clear();
   if (!out) return create_fail(nullptr, QSGW_ERR_INVALID_ARG, "out is NULL");
@@ -316,17 +380,16 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   std::string why;
   int rc = validate_desc(desc, why);
   if (rc != QSGW_OK) return create_fail(nullptr, rc, why);
-  int dev = 0;
-  cudaError_t e = cudaGetDevice(&dev);
-  if (e != cudaSuccess) return create_fail(nullptr, QSGW_ERR_UNSUPPORTED, std::string("no CUDA device: ") + cudaGetErrorString(e));
-  cudaDeviceProp prop;
-  e = cudaGetDeviceProperties(&prop, dev);
-  if (e != cudaSuccess) return create_fail(nullptr, QSGW_ERR_CUDA, cudaGetErrorString(e));
-  if (prop.major != 10) return create_fail(nullptr, QSGW_ERR_UNSUPPORTED, "kernels are built for sm_100a only");
+  DevInfo di;
+  cudaError_t e = current_device(&di);
+  if (e != cudaSuccess) { cudaGetLastError(); return create_fail(nullptr, QSGW_ERR_UNSUPPORTED, std::string("no CUDA device: ") + cudaGetErrorString(e)); }
+  if (di.cc_major != 10) return create_fail(nullptr, QSGW_ERR_UNSUPPORTED, "kernels are built for sm_100a only");
 
   qsgw_ctx* c = new (std::nothrow) qsgw_ctx();
   if (!c) return create_fail(nullptr, QSGW_ERR_ALLOC, "host allocation failed");
   c->stream = static_cast<cudaStream_t>(cuda_stream);
+  c->device = di.dev;
+  c->n_sm = di.n_sm;
   c->n_sites = desc->n_sites;
   c->n_freq = desc->n_freq;
   c->n_k = desc->n_k;
@@ -364,46 +427,27 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
         if (pb_site[I] != last) { last = pb_site[I]; sum += (c->orb[last] + 3) & ~3; }
       if (sum > kt) kt = sum;
     }
-    const char* ev = getenv("QSGW_ZMEL_DMMA");   // A/B knob: 0 selects the CUDA-core kernel
-    if (qsgw::zmel_dmma_smem_bytes(c->b_max, kt) <= 200 * 1024 && !(ev && atoi(ev) == 0)) c->zmel_kt = kt;
+    if (qsgw::zmel_dmma_smem_bytes(c->b_max, kt) <= 200 * 1024) c->zmel_kt_avail = kt;
+    c->zmel_kt = c->zmel_kt_avail;
   }
   const bool mixed = c->precision != QSGW_PREC_FP64;
-  c->n_pass = c->precision == QSGW_PREC_MIXED_TF32X3 ? 3 : (c->precision == QSGW_PREC_MIXED_TF32X1 ? 1 : 0);
-  c->f16 = c->precision == QSGW_PREC_MIXED;
-  if (const char* ev = getenv("QSGW_F16_CLUSTER")) {   // tuning knob: CTAs per cluster sharing a tile (1, 2, 4)
-    const int v = atoi(ev);
-    if (v == 1 || v == 2 || v == 4) c->cluster = v;
-  }
-  if (const char* ev = getenv("QSGW_F64_4M")) c->f64_3m = atoi(ev) == 0;   // A/B knob for profiles
-  // Correction products in E5M2 when enough pairs are summed per output element: the extra error is
-  // ~4e-5 * sqrt(N_M / pairs summed over the job); below 64 pairs per product function the
-  // three-FP16-product form is used.  QSGW_F16_FP8=0/1 overrides (A/B knob for profiles).
-  c->fp8 = c->f16 && (double)c->n_k * c->max_n_o * c->max_n_u >= 64.0 * c->n_m;
-  if (const char* ev = getenv("QSGW_F16_FP8")) c->fp8 = c->f16 && atoi(ev) != 0;
-  if (const char* ev = getenv("QSGW_F16_WIN")) {       // tuning knob: stages per drain window
-    const int v = atoi(ev);
-    if (v >= 1 && v <= 64) c->win = v;
-  }
+  c->f16 = mixed;
   const int tile_edge = mixed ? qsgw::kTileMx : qsgw::kTile;
   c->n_m_pad = (int)round_up(c->n_m, tile_edge);
   const long long max_pairs = (long long)c->max_n_o * c->max_n_u;
   // Workspace = room for `mult` padded band batches (about 32 Ki pairs): small batches (few bands, many k-points)
   // are staged back to back and stage (b) runs once per full workspace instead of once per batch.
-  const long long batch_pad = round_up(max_pairs, qsgw::kPairAlign);
-  long long mult = c->n_pass ? 1 : (32768 + batch_pad - 1) / batch_pad;
-  if (const char* ev = getenv("QSGW_STAGE_BATCHES")) {   // A/B knob: batches per stage (b) launch
-    const int v = atoi(ev);
-    if (v >= 1 && !c->n_pass) mult = v;
-  }
-  size_t z64_bytes = 0, z32_elems = 0, zhl_bytes = 0, z_bytes = 0;
+  c->batch_pad = round_up(max_pairs, qsgw::kPairAlign);
+  long long mult = (32768 + c->batch_pad - 1) / c->batch_pad;
+  size_t z64_bytes = 0, zhl_bytes = 0, z_bytes = 0;
   for (;; --mult) {
-    c->kpad = batch_pad * mult;
+    c->kpad = c->batch_pad * mult;
     z64_bytes = (size_t)2 * c->ncg * c->kpad * qsgw::kCG * sizeof(double);
-    z32_elems = c->n_pass ? (size_t)4 * c->n_m_pad * c->kpad : 0;
     zhl_bytes = c->f16 ? (size_t)2 * c->n_m_pad * c->kpad * 2 * sizeof(uint16_t) : 0;
-    z_bytes = z64_bytes + z32_elems * sizeof(float) + zhl_bytes * (c->fp8 ? 2 : 1);
+    z_bytes = z64_bytes + 2 * zhl_bytes;
     if (mult == 1 || desc->workspace_bytes == 0 || z_bytes <= desc->workspace_bytes) break;
   }
+  c->stage_cap = c->kpad;
   if (desc->workspace_bytes != 0 && z_bytes > desc->workspace_bytes) {
     char buf[256];
     snprintf(buf, sizeof(buf), "z workspace for %d x %d band pairs needs %zu bytes > workspace_bytes cap %zu; "
@@ -433,13 +477,13 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_omega, (size_t)c->n_freq));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_P, (size_t)c->p_elems));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zws, z64_bytes / sizeof(double)));
-  if (c->n_pass) QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zws32, z32_elems));
-  if (mixed) QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab32, (size_t)c->n_freq * c->kpad));
   if (c->f16) {
+    QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab32, (size_t)c->n_freq * c->kpad));
     QSGW_TRY_ALLOC(dev_alloc(c, reinterpret_cast<unsigned char**>(&c->d_zhl), zhl_bytes));
-    if (c->fp8) QSGW_TRY_ALLOC(dev_alloc(c, reinterpret_cast<unsigned char**>(&c->d_zhb8), zhl_bytes));
+    QSGW_TRY_ALLOC(dev_alloc(c, reinterpret_cast<unsigned char**>(&c->d_zhb8), zhl_bytes));
     QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wscale, (size_t)c->n_freq));
     QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zmax, (size_t)1));
+    QSGW_TRY_ALLOC(dev_alloc(c, &c->d_ctl, (size_t)1));
   }
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab, (size_t)c->n_freq * c->kpad));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_acc_re, acc_elems));
@@ -460,16 +504,13 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_tiles, tiles.data(), sizeof(int2) * tiles.size(), cudaMemcpyHostToDevice, st));
   QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_omega, c->omega.data(), sizeof(double) * c->n_freq, cudaMemcpyHostToDevice, st));
   QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zws, 0, z64_bytes, st));
-  if (mixed) QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wtab32, 0, sizeof(float) * c->n_freq * c->kpad, st));
-  if (c->n_pass) {
-    QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zws32, 0, z32_elems * sizeof(float), st));
-    QSGW_TRY_CUDA(qsgw::chi0_tf32_configure());
-  }
   if (c->f16) {
+    QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wtab32, 0, sizeof(float) * c->n_freq * c->kpad, st));
     QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zhl, 0, zhl_bytes, st));
-    if (c->fp8) QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zhb8, 0, zhl_bytes, st));
+    QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zhb8, 0, zhl_bytes, st));
     QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wscale, 0, sizeof(double) * c->n_freq, st));
     QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zmax, 0, sizeof(float), st));
+    QSGW_TRY_CUDA(upload_ctl(c));
     QSGW_TRY_CUDA(qsgw::chi0_f16_configure());
   }
   QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wtab, 0, sizeof(double) * c->n_freq * c->kpad, st));
@@ -485,7 +526,7 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     const cuuint64_t gdim[4] = {(cuuint64_t)qsgw::kCG, (cuuint64_t)c->kpad, (cuuint64_t)c->ncg, 2};
     const cuuint64_t gstr[3] = {(cuuint64_t)qsgw::kCG * 8, (cuuint64_t)c->kpad * qsgw::kCG * 8,
                                 (cuuint64_t)c->ncg * c->kpad * qsgw::kCG * 8};
-    const cuuint32_t box[4] = {(cuuint32_t)qsgw::kCG, (cuuint32_t)(c->f64_3m ? qsgw::kChi0F64KP3M : qsgw::kChi0F64KP), 4, 2};
+    const cuuint32_t box[4] = {(cuuint32_t)qsgw::kCG, (cuuint32_t)qsgw::kChi0F64KP3M, 4, 2};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     CUresult r = enc(&c->tmap_z, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->d_zws, gdim, gstr, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -504,38 +545,17 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     CUresult r = enc(&c->tmap_h, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, c->d_zhl, gdim, gstr, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) {
-      char buf[128];
-      snprintf(buf, sizeof(buf), "cuTensorMapEncodeTiled (mixed, hl16 planes) failed with CUresult %d", (int)r);
-      return create_fail(c, QSGW_ERR_CUDA, buf);
-    }
-    if (c->fp8) {
+    if (r == CUDA_SUCCESS) {
       const cuuint64_t gdim8[3] = {(cuuint64_t)c->kpad * 4, (cuuint64_t)c->n_m_pad, 2};
       const cuuint32_t box8[3] = {128, 64, 1};
       r = enc(&c->tmap_hb8, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, c->d_zhb8, gdim8, gstr, box8, estr,
               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-      if (r != CUDA_SUCCESS) {
-        char buf[128];
-        snprintf(buf, sizeof(buf), "cuTensorMapEncodeTiled (mixed, hb8 planes) failed with CUresult %d", (int)r);
-        return create_fail(c, QSGW_ERR_CUDA, buf);
-      }
     }
-  }
-  if (c->n_pass) {
-    const cuuint64_t gdim[3] = {(cuuint64_t)c->kpad, (cuuint64_t)c->n_m_pad, 4};
-    const cuuint64_t gstr[2] = {(cuuint64_t)c->kpad * 4, (cuuint64_t)c->n_m_pad * c->kpad * 4};
-    const cuuint32_t estr[3] = {1, 1, 1};
-    for (int np = 2; np <= 4; np += 2) {
-      const cuuint32_t box[3] = {(cuuint32_t)qsgw::kPairStage, (cuuint32_t)qsgw::kTileMx, (cuuint32_t)np};
-      CUresult r = enc(np == 2 ? &c->tmap2 : &c->tmap4, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, c->d_zws32, gdim, gstr, box,
-                       estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-      if (r != CUDA_SUCCESS) {
-        char buf[128];
-        snprintf(buf, sizeof(buf), "cuTensorMapEncodeTiled (mixed, %d planes) failed with CUresult %d", np, (int)r);
-        return create_fail(c, QSGW_ERR_CUDA, buf);
-      }
+    if (r != CUDA_SUCCESS) {
+      char buf[128];
+      snprintf(buf, sizeof(buf), "cuTensorMapEncodeTiled (mixed, hl16 / hb8 planes) failed with CUresult %d", (int)r);
+      return create_fail(c, QSGW_ERR_CUDA, buf);
     }
   }
   c->state = ST_CREATED;
@@ -546,11 +566,60 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
 void qsgw_destroy(qsgw_ctx* ctx) {
   if (!ctx) return;
   cudaStreamSynchronize(ctx->stream);
+  if (ctx->hr.cp) cudaStreamSynchronize(ctx->hr.cp);
   free_all(ctx);
   delete ctx;
 }
 
 static int flush_pending(qsgw_ctx* ctx);
+
+int32_t qsgw_set_option(qsgw_ctx* ctx, const char* key, int64_t value) {
+  if (!key) return ctx ? ctx->fail(QSGW_ERR_INVALID_ARG, "key is NULL") : QSGW_ERR_INVALID_ARG;
+  const std::string k(key);
+  if (!ctx) {
+    g_create_error.clear();
+    if (k == "wc_graph" && value >= 0 && value <= 2) { g_wc_graph = (int)value; return QSGW_OK; }
+    g_create_error = "unknown process-wide option or value out of range: " + k;
+    return QSGW_ERR_INVALID_ARG;
+  }
+  if (ctx->fill != 0) return ctx->fail(QSGW_ERR_STATE, "options can be set only while no band batch is staged");
+  if (k == "stage_batches" && value >= 1) {
+    const long long cap = ctx->batch_pad * (value > (1LL << 30) ? (1LL << 30) : value);
+    ctx->stage_cap = cap < ctx->kpad ? cap : ctx->kpad;
+  } else if (k == "zmel_dmma" && (value == 0 || value == 1)) {
+    if (value == 1 && ctx->zmel_kt_avail == 0)
+      return ctx->fail(QSGW_ERR_UNSUPPORTED, "the tensor-pipe stage (a) kernel does not fit this site structure");
+    ctx->zmel_kt = value ? ctx->zmel_kt_avail : 0;
+  } else if (k == "mixed_fp8" && value >= 0 && value <= 2 && ctx->f16) {
+    ctx->fp8_mode = (int)value;
+    if (upload_ctl(ctx) != cudaSuccess) return ctx->fail(QSGW_ERR_CUDA, "upload of the mixed-mode control block failed");
+  } else if (k == "mixed_fp8_threshold_x100" && value >= 0 && ctx->f16) {
+    ctx->fp8_thr = 0.01 * (double)value;
+    if (upload_ctl(ctx) != cudaSuccess) return ctx->fail(QSGW_ERR_CUDA, "upload of the mixed-mode control block failed");
+  } else if (k == "mixed_window" && value >= 1 && value <= 64 && ctx->f16) {
+    ctx->win = (int)value;
+  } else if (k == "e2e_groups" && value >= 1 && value <= 4) {
+    ctx->e2e_groups = (int)value;
+  } else {
+    return ctx->fail(QSGW_ERR_INVALID_ARG, "unknown option, value out of range, or option of the other precision mode: %s", key);
+  }
+  ctx->err.clear();
+  return QSGW_OK;
+}
+
+int32_t qsgw_mixed_stats(qsgw_ctx* ctx, int64_t* out_launches, int64_t* out_launches_fp8,
+                         double* out_min_effective_pairs) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  if (!ctx->f16) return ctx->fail(QSGW_ERR_STATE, "qsgw_mixed_stats: the context is in FP64 mode");
+  qsgw::MixedCtl h;
+  cudaError_t e = cudaMemcpyAsync(&h, ctx->d_ctl, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "read of the mixed-mode control block");
+  if (out_launches) *out_launches = (int64_t)h.n_flush;
+  if (out_launches_fp8) *out_launches_fp8 = (int64_t)h.n_flush_fp8;
+  if (out_min_effective_pairs) *out_min_effective_pairs = (double)h.peff_min_seen;
+  return QSGW_OK;
+}
 
 int32_t qsgw_sync(qsgw_ctx* ctx) {
   if (!ctx) return QSGW_ERR_INVALID_ARG;
@@ -576,10 +645,12 @@ int32_t qsgw_reset(qsgw_ctx* ctx) {
   const size_t acc_elems = (size_t)ctx->n_freq * ctx->n_m_pad * ctx->n_m_pad;
   cudaError_t e = cudaMemsetAsync(ctx->d_acc_re, 0, sizeof(double) * acc_elems, ctx->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_acc_im, 0, sizeof(double) * acc_elems, ctx->stream);
+  if (e == cudaSuccess && ctx->f16) e = upload_ctl(ctx);
   if (e != cudaSuccess) return ctx->cuda_fail(e, "reset");
   if (ctx->state != ST_CREATED) ctx->state = ST_READY;
   ctx->pairs = 0;
   ctx->fill = 0;                   // staged, not yet accumulated batches are dropped with the accumulator
+  ctx->z_off = 0;
   ctx->err.clear();
   return QSGW_OK;
 }
@@ -634,6 +705,7 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   a.kpad = ctx->kpad;
   a.ncg = ctx->ncg;
   a.kt = ctx->zmel_kt;
+  a.n_sm = ctx->n_sm;
   cudaError_t e;
   if (ctx->f16) {
     a.zmax = ctx->d_zmax;
@@ -642,22 +714,18 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   }
   {
     StageScope ts(ctx, QSGW_STAGE_ZMEL);
-    if (ctx->n_pass) e = qsgw::launch_zmel_mixed(a, ctx->d_zws32, ctx->n_m_pad, ctx->n_pass == 3 ? 1 : 0, ctx->stream);
-    else e = ctx->zmel_kt ? qsgw::launch_zmel_dmma(a, ctx->stream) : qsgw::launch_zmel_f64(a, ctx->stream);
+    e = ctx->zmel_kt ? qsgw::launch_zmel_dmma(a, ctx->stream) : qsgw::launch_zmel_f64(a, ctx->stream);
     if (e == cudaSuccess && ctx->f16)
       e = qsgw::launch_z_to_hl16(a.zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u,
                                  hl_slot(ctx->d_zhl, off), hl_slot(ctx->d_zhb8, off), ctx->n_m_pad, ctx->d_zmax,
                                  ctx->stream);
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "zmel kernel launch");
-  ctx->launches += (ctx->n_pass || ctx->f16) ? 2 : 1;
+  ctx->launches += ctx->f16 ? 2 : 1;
   if (d_z_out) {
     if (ctx->f16)
       e = qsgw::launch_z_export_hl16(hl_slot(ctx->d_zhl, off), ctx->kpad, ctx->n_m_pad, ctx->n_m, (long long)n_o * n_u, ctx->d_zmax,
                                      static_cast<double2*>(d_z_out), ctx->stream);
-    else if (ctx->n_pass)
-      e = qsgw::launch_z_export32(ctx->d_zws32, ctx->kpad, ctx->n_m_pad, ctx->n_m, (long long)n_o * n_u,
-                                  static_cast<double2*>(d_z_out), ctx->stream);
     else
       e = qsgw::launch_z_export(a.zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u,
                               static_cast<double2*>(d_z_out), ctx->stream);
@@ -666,6 +734,7 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   }
   ctx->last_n_o = n_o;
   ctx->last_n_u = n_u;
+  ctx->z_off = off;
   ctx->state = ST_Z_BUILT;
   ctx->err.clear();
   return QSGW_OK;
@@ -683,14 +752,14 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
     if (first) {
       StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
       e = qsgw::launch_weights_scale_hl16(ctx->d_wtab, ctx->d_wtab32, ctx->d_wscale, ctx->kpad, n_pad, ctx->n_freq,
-                                          ctx->stream);
+                                          ctx->d_ctl, ctx->stream);
       if (e != cudaSuccess) return ctx->cuda_fail(e, "weight scaling kernel launch");
       ctx->launches += 1;
     }
     qsgw::Chi0F16Args m;
     m.tmap = ctx->tmap_h;
-    m.tmap_b = ctx->fp8 ? ctx->tmap_hb8 : ctx->tmap_h;
-    m.wtab16 = reinterpret_cast<const __half*>(ctx->d_wtab32);   // same bytes per pair as the FP32 table
+    m.tmap_b = ctx->tmap_hb8;
+    m.wtab16 = reinterpret_cast<const __half*>(ctx->d_wtab32);   // same bytes per pair as an FP32 table
     m.wscale = ctx->d_wscale;
     m.win = ctx->win;
     m.zmax = ctx->d_zmax;
@@ -701,14 +770,16 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
     m.n_freq = nj;
     m.j0 = j0;
     m.n_stages = (int)(n_pad / qsgw::kPairStage);
+    m.n_sm = ctx->n_sm;
+    m.ctl = ctx->d_ctl;
     m.d_tiles = ctx->d_tiles;
     m.n_tiles = ctx->n_tiles;
     {
       StageScope ts(ctx, QSGW_STAGE_CHI0);
-      e = qsgw::launch_chi0_f16(m, ctx->cluster, ctx->fp8, ctx->stream);
+      e = qsgw::launch_chi0_f16(m, ctx->stream);
     }
     if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 (mixed, FP16 split) kernel launch");
-    ctx->launches += 1;
+    ctx->launches += 2;            // both product variants are launched, one of them exits at once
     return QSGW_OK;
   }
   qsgw::Chi0F64Args a;
@@ -721,11 +792,12 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
   a.n_freq = nj;
   a.j0 = j0;
   a.n_pairs_padded = n_pad;
+  a.n_sm = ctx->n_sm;
   a.d_tiles = ctx->d_tiles;
   a.n_tiles = ctx->n_tiles;
   {
     StageScope ts(ctx, QSGW_STAGE_CHI0);
-    e = qsgw::launch_chi0_f64(a, ctx->f64_3m, ctx->stream);
+    e = qsgw::launch_chi0_f64(a, ctx->stream);
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 kernel launch");
   ctx->launches += 1;
@@ -737,7 +809,7 @@ static int flush_pending(qsgw_ctx* ctx) { return flush_range(ctx, 0, ctx->n_freq
 // Slot of the next band batch in the workspace; flushes the staged batches first when it would not fit.
 static int stage_slot(qsgw_ctx* ctx, long long n_pairs, long long* off) {
   const long long n_pad = round_up(n_pairs, qsgw::kPairAlign);
-  if (ctx->fill + n_pad > ctx->kpad) {
+  if (ctx->fill + n_pad > ctx->stage_cap) {
     int rc = flush_pending(ctx);
     if (rc != QSGW_OK) return rc;
   }
@@ -754,8 +826,8 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
   if (rc != QSGW_OK) return rc;
   const long long n_pairs = (long long)n_o * n_u;
   const long long n_pad = round_up(n_pairs, qsgw::kPairAlign);
-  long long off = ctx->fill;       // the slot the last zmel_build wrote
-  cudaError_t e;
+  long long off = 0;
+  cudaError_t e = cudaSuccess;
   if (d_z) {
     rc = stage_slot(ctx, n_pairs, &off);
     if (rc != QSGW_OK) return rc;
@@ -769,11 +841,6 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
                                  ctx->stream);
       ctx->launches += 1;
     }
-    if (e == cudaSuccess && ctx->n_pass) {
-      e = qsgw::launch_planes32_from_ws(ctx->d_zws, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, ctx->d_zws32, ctx->n_m_pad,
-                                        ctx->n_pass == 3 ? 1 : 0, ctx->stream);
-      ctx->launches += 1;
-    }
     if (e != cudaSuccess) return ctx->cuda_fail(e, "z import kernel launch");
     ctx->launches += 1;
     ctx->last_n_o = n_o;
@@ -783,6 +850,14 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
     if (n_o != ctx->last_n_o || n_u != ctx->last_n_u)
       return ctx->fail(QSGW_ERR_SHAPE, "batch %d x %d differs from the last zmel_build (%d x %d)", n_o, n_u,
                        ctx->last_n_o, ctx->last_n_u);
+    // The batch sits where zmel_build wrote it.  A qsgw_sync / qsgw_chi0_finalize in between has flushed and
+    // released the slots below it: their weights are zeroed so that the rows [0, z_off) of this flush contribute
+    // exactly nothing (the z rows there are a stale, already accumulated batch).
+    off = ctx->z_off;
+    if (off != ctx->fill) {
+      e = cudaMemset2DAsync(ctx->d_wtab, sizeof(double) * ctx->kpad, 0, sizeof(double) * off, ctx->n_freq, ctx->stream);
+      if (e != cudaSuccess) return ctx->cuda_fail(e, "clearing the weights of released workspace slots");
+    }
   }
   {
     StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
@@ -793,39 +868,9 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
   if (e != cudaSuccess) return ctx->cuda_fail(e, "pair weights kernel launch");
   ctx->launches += 1;
   ctx->pairs += n_pairs;
-  ctx->state = ST_READY;   // the batch is staged (or, TF32 variants, consumed below)
+  ctx->state = ST_READY;   // the batch is staged
+  ctx->fill = off + n_pad;
   ctx->err.clear();
-  if (!ctx->n_pass) {
-    ctx->fill = off + n_pad;
-    return QSGW_OK;
-  }
-  // TF32 variants: one batch per launch, no staging
-  {
-    const long long n_pad32 = round_up(n_pairs, qsgw::kPairStage);
-    {
-      StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
-      e = qsgw::launch_weights_to_f32(ctx->d_wtab, ctx->d_wtab32, ctx->kpad, n_pad32, ctx->n_freq, ctx->stream);
-    }
-    if (e != cudaSuccess) return ctx->cuda_fail(e, "weight conversion kernel launch");
-    qsgw::Chi0Tf32Args m;
-    m.tmap2 = ctx->tmap2;
-    m.tmap4 = ctx->tmap4;
-    m.wtab32 = ctx->d_wtab32;
-    m.kpad = ctx->kpad;
-    m.acc_re = ctx->d_acc_re;
-    m.acc_im = ctx->d_acc_im;
-    m.n_m_pad = ctx->n_m_pad;
-    m.n_freq = ctx->n_freq;
-    m.n_stages = (int)(n_pad32 / qsgw::kPairStage);
-    m.d_tiles = ctx->d_tiles;
-    m.n_tiles = ctx->n_tiles;
-    {
-      StageScope ts(ctx, QSGW_STAGE_CHI0);
-      e = qsgw::launch_chi0_tf32(m, ctx->n_pass, ctx->stream);
-    }
-    if (e != cudaSuccess) return ctx->cuda_fail(e, "chi0 (mixed) kernel launch");
-    ctx->launches += 2;
-  }
   return QSGW_OK;
 }
 
@@ -866,59 +911,70 @@ int32_t qsgw_chi0_finalize(qsgw_ctx* ctx, void* d_chi0_out) {
   return QSGW_OK;
 }
 
+// Common checks of the context-free entry points: an sm_100 device is current, kernel attributes are set.
+static int wc_prologue(DevInfo* di) {
+  if (current_device(di) != cudaSuccess) {
+    cudaGetLastError();
+    g_create_error = "no CUDA device";
+    return QSGW_ERR_UNSUPPORTED;
+  }
+  if (di->cc_major != 10) { g_create_error = "kernels are built for sm_100a only"; return QSGW_ERR_UNSUPPORTED; }
+  cudaError_t e = wc_configure_device(di->dev);
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("kernel attributes: ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
+  return QSGW_OK;
+}
+
 int32_t qsgw_wc_from_chi0(int32_t n_m, int32_t n_freq, const void* d_chi0, const double* d_v, void* d_wc_out,
                           int32_t* d_info, void* cuda_stream) {
   g_create_error.clear();
   if (!d_chi0 || !d_v || !d_wc_out || !d_info) { g_create_error = "NULL argument"; return QSGW_ERR_INVALID_ARG; }
   if (d_chi0 == d_wc_out) { g_create_error = "d_wc_out aliases d_chi0"; return QSGW_ERR_INVALID_ARG; }
   if (n_m < 1 || n_freq < 1) { g_create_error = "n_m and n_freq must be positive"; return QSGW_ERR_SHAPE; }
-  int dev = 0;
-  cudaDeviceProp prop;
-  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
-    cudaGetLastError();
-    g_create_error = "no CUDA device";
-    return QSGW_ERR_UNSUPPORTED;
-  }
-  if (prop.major != 10) { g_create_error = "kernels are built for sm_100a only"; return QSGW_ERR_UNSUPPORTED; }
+  DevInfo di;
+  int rc = wc_prologue(&di);
+  if (rc != QSGW_OK) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  cudaError_t e = wc_configure_once();
-  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("kernel attributes: ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
   double2* work = nullptr;
-  e = cudaMallocAsync(reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::wc_work_elems(n_m, n_freq), st);
+  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::wc_work_elems(n_m, n_freq), st);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("workspace allocation failed: ") + cudaGetErrorString(e); return QSGW_ERR_ALLOC; }
-  // The factorisation is ~420 small dependent launches: they are captured into a CUDA graph on an internal
-  // stream (the caller's stream may be the legacy default stream, which cannot be captured) and launched as one
-  // unit between two events, so that a busy host cannot starve the GPU.  Any capture failure falls back to plain
-  // launches on the caller's stream.
-  bool done = false;
-  const char* no_graph = getenv("QSGW_WC_GRAPH");
-  if (!(no_graph && atoi(no_graph) == 0)) {
+  // The factorisation is a few hundred small dependent launches: they are captured into a CUDA graph on an
+  // internal stream of this device (the caller's stream may be the legacy default stream, which cannot be
+  // captured) and launched as one unit between two events, so that a busy host cannot starve the GPU.  A capture
+  // failure falls back to plain launches on the caller's stream; a failure AFTER the graph was launched does not
+  // (the graph is in flight on `work`): it is reported.
+  bool done = false, launched = false;
+  if (g_wc_graph != 0 && di.dev >= 0 && di.dev < qsgw::kMaxDevices) {
     WcGraphs& G = wc_graphs();
     std::lock_guard<std::mutex> lock(G.mu);
     G.sweep();
+    cudaStream_t& gs = G.stream[di.dev];
     cudaEvent_t ev_in = nullptr, ev_out = nullptr;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
-    bool ok = G.stream != nullptr || cudaStreamCreateWithFlags(&G.stream, cudaStreamNonBlocking) == cudaSuccess;
+    bool ok = gs != nullptr || cudaStreamCreateWithFlags(&gs, cudaStreamNonBlocking) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&ev_in, cudaEventDisableTiming) == cudaSuccess &&
          cudaEventCreateWithFlags(&ev_out, cudaEventDisableTiming) == cudaSuccess;
-    ok = ok && cudaEventRecord(ev_in, st) == cudaSuccess && cudaStreamWaitEvent(G.stream, ev_in, 0) == cudaSuccess;
-    if (ok && cudaStreamBeginCapture(G.stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+    ok = ok && cudaEventRecord(ev_in, st) == cudaSuccess && cudaStreamWaitEvent(gs, ev_in, 0) == cudaSuccess;
+    if (ok && cudaStreamBeginCapture(gs, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
       const cudaError_t le = qsgw::launch_wc_from_chi0(n_m, n_freq, static_cast<const double2*>(d_chi0), d_v,
-                                                       static_cast<double2*>(d_wc_out), work, d_info, G.stream);
-      const cudaError_t ce = cudaStreamEndCapture(G.stream, &graph);
+                                                       static_cast<double2*>(d_wc_out), work, d_info, gs);
+      const cudaError_t ce = cudaStreamEndCapture(gs, &graph);
       ok = le == cudaSuccess && ce == cudaSuccess && graph != nullptr &&
-           cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess && cudaGraphLaunch(exec, G.stream) == cudaSuccess;
+           cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess;
+      if (ok) {
+        ok = cudaGraphLaunch(exec, gs) == cudaSuccess;
+        launched = ok;
+      }
     } else {
       ok = false;
     }
     if (graph) cudaGraphDestroy(graph);
-    if (ok) {
-      ok = cudaEventRecord(ev_out, G.stream) == cudaSuccess && cudaStreamWaitEvent(st, ev_out, 0) == cudaSuccess;
-      G.pending.push_back({exec, ev_out});      // destroyed by a later sweep once ev_out has completed
+    if (launched) {
+      done = cudaEventRecord(ev_out, gs) == cudaSuccess && cudaStreamWaitEvent(st, ev_out, 0) == cudaSuccess;
+      if (!done) cudaStreamSynchronize(gs);        // the graph still owns `work`: wait for it before anything else
+      G.pending.push_back({exec, ev_out});         // destroyed by a later sweep once ev_out has completed
       exec = nullptr;
       ev_out = nullptr;
-      done = ok;
     }
     if (exec) cudaGraphExecDestroy(exec);
     if (ev_in) cudaEventDestroy(ev_in);
@@ -926,9 +982,9 @@ int32_t qsgw_wc_from_chi0(int32_t n_m, int32_t n_freq, const void* d_chi0, const
     if (!done) cudaGetLastError();
   }
   e = cudaSuccess;
-  if (!done && no_graph && atoi(no_graph) == 2) {      // QSGW_WC_GRAPH=2: the graph path is mandatory (tests)
+  if (!done && (launched || g_wc_graph == 2)) {
     cudaFreeAsync(work, st);
-    g_create_error = "CUDA graph capture of the W^c launch sequence failed";
+    g_create_error = launched ? "ordering the W^c graph after launch failed" : "CUDA graph capture of the W^c launch sequence failed";
     return QSGW_ERR_CUDA;
   }
   if (!done)
@@ -945,19 +1001,12 @@ int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_ch
   if (!d_chi0 || !d_U || !d_out) { g_create_error = "NULL argument"; return QSGW_ERR_INVALID_ARG; }
   if (d_chi0 == d_out) { g_create_error = "d_out aliases d_chi0"; return QSGW_ERR_INVALID_ARG; }
   if (n_m < 1 || n_freq < 1) { g_create_error = "n_m and n_freq must be positive"; return QSGW_ERR_SHAPE; }
-  int dev = 0;
-  cudaDeviceProp prop;
-  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
-    cudaGetLastError();
-    g_create_error = "no CUDA device";
-    return QSGW_ERR_UNSUPPORTED;
-  }
-  if (prop.major != 10) { g_create_error = "kernels are built for sm_100a only"; return QSGW_ERR_UNSUPPORTED; }
+  DevInfo di;
+  int rc = wc_prologue(&di);
+  if (rc != QSGW_OK) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   double2* work = nullptr;
-  cudaError_t e = wc_configure_once();
-  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("kernel attributes: ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
-  e = cudaMallocAsync(reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::rotate_work_elems(n_m, n_freq), st);
+  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::rotate_work_elems(n_m, n_freq), st);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("workspace allocation failed: ") + cudaGetErrorString(e); return QSGW_ERR_ALLOC; }
   e = qsgw::launch_rotate_basis(n_m, n_freq, static_cast<const double2*>(d_chi0), static_cast<const double2*>(d_U),
                                 static_cast<double2*>(d_out), work, st);
@@ -966,76 +1015,64 @@ int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_ch
   return QSGW_OK;
 }
 
-int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h_Ck, const void* h_Ckq,
-                           const double* h_eps_k, const double* h_f_k, const double* h_eps_kq, const double* h_f_kq,
+int32_t qsgw_chi0_run_host(qsgw_ctx* c, const void* h_P, const void* h_Ck, const void* h_Ckq, const double* h_eps_k,
+                           const double* h_f_k, const double* h_eps_kq, const double* h_f_kq, int32_t n_k_points,
                            int32_t n_o, int32_t n_u, void* h_chi0_out, int64_t* out_kernel_launches) {
-  g_create_error.clear();
-  if (!desc || !h_P || !h_Ck || !h_Ckq || !h_eps_k || !h_f_k || !h_eps_kq || !h_f_kq || !h_chi0_out) {
-    g_create_error = "NULL argument";
-    return QSGW_ERR_INVALID_ARG;
-  }
-  if (n_o < 1 || n_u < 1) { g_create_error = "n_o and n_u must be positive"; return QSGW_ERR_SHAPE; }
-  cudaStream_t st = nullptr;
-  cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
-  if (e != cudaSuccess) { g_create_error = cudaGetErrorString(e); return QSGW_ERR_CUDA; }
-  qsgw_ctx* c = nullptr;
-  int rc = qsgw_create(desc, st, &c);
-  if (rc != QSGW_OK) { cudaStreamDestroy(st); return rc; }
-
-  const int nb = c->n_b, nm = c->n_m, nk = c->n_k;
+  if (!c) return QSGW_ERR_INVALID_ARG;
+  if (!h_P || !h_Ck || !h_Ckq || !h_eps_k || !h_f_k || !h_eps_kq || !h_f_kq || !h_chi0_out)
+    return c->fail(QSGW_ERR_INVALID_ARG, "NULL argument");
+  if (n_o < 1 || n_u < 1 || n_k_points < 1) return c->fail(QSGW_ERR_SHAPE, "n_k_points, n_o and n_u must be positive");
+  cudaStream_t st = c->stream;
+  qsgw_ctx::HostRun& H = c->hr;
+  const int nb = c->n_b, nm = c->n_m;
   const size_t ck_e = (size_t)n_o * nb, ckq_e = (size_t)n_u * nb;
-  double2 *dP = nullptr, *dCk[2] = {nullptr, nullptr}, *dCkq[2] = {nullptr, nullptr}, *dOut = nullptr;
-  double* dE[2] = {nullptr, nullptr};   // eps_k | f_k | eps_kq | f_kq
-  cudaEvent_t done[2] = {nullptr, nullptr};
   const size_t e_len = 2 * (size_t)n_o + 2 * (size_t)n_u;
   const size_t out_e = (size_t)c->n_freq * nm * nm;
-  auto cleanup = [&]() {
-    cudaFree(dP); cudaFree(dOut);
-    for (int i = 0; i < 2; ++i) { cudaFree(dCk[i]); cudaFree(dCkq[i]); cudaFree(dE[i]); if (done[i]) cudaEventDestroy(done[i]); }
-    qsgw_destroy(c);
-    cudaStreamDestroy(st);
-  };
+  const long long launches0 = c->launches;
 #define QSGW_H(expr)                                                                   \
   do {                                                                                 \
     cudaError_t _e = (expr);                                                           \
-    if (_e != cudaSuccess) { g_create_error = std::string(#expr ": ") + cudaGetErrorString(_e); cleanup(); return QSGW_ERR_CUDA; } \
+    if (_e != cudaSuccess) { cudaGetLastError(); return c->cuda_fail(_e, #expr); }     \
   } while (0)
-  QSGW_H(cudaMalloc(&dP, sizeof(double2) * c->p_elems));
-  QSGW_H(cudaMalloc(&dOut, sizeof(double2) * out_e));
+  // staging buffers: allocated once, grown when a later call passes larger band counts
+  if (!H.dP) QSGW_H(dev_alloc(c, &H.dP, (size_t)c->p_elems));
+  if (!H.dOut) QSGW_H(dev_alloc(c, &H.dOut, out_e));
   for (int i = 0; i < 2; ++i) {
-    QSGW_H(cudaMalloc(&dCk[i], sizeof(double2) * ck_e));
-    QSGW_H(cudaMalloc(&dCkq[i], sizeof(double2) * ckq_e));
-    QSGW_H(cudaMalloc(&dE[i], sizeof(double) * e_len));
-    QSGW_H(cudaEventCreateWithFlags(&done[i], cudaEventDisableTiming));
+    if (H.ck_cap < ck_e) { cudaStreamSynchronize(st); cudaFree(H.dCk[i]); H.dCk[i] = nullptr; QSGW_H(dev_alloc(c, &H.dCk[i], ck_e)); }
+    if (H.ckq_cap < ckq_e) { cudaStreamSynchronize(st); cudaFree(H.dCkq[i]); H.dCkq[i] = nullptr; QSGW_H(dev_alloc(c, &H.dCkq[i], ckq_e)); }
+    if (H.e_cap < e_len) { cudaStreamSynchronize(st); cudaFree(H.dE[i]); H.dE[i] = nullptr; QSGW_H(dev_alloc(c, &H.dE[i], e_len)); }
+    if (!H.done[i]) QSGW_H(cudaEventCreateWithFlags(&H.done[i], cudaEventDisableTiming));
   }
-  QSGW_H(cudaMemcpyAsync(dP, h_P, sizeof(double2) * c->p_elems, cudaMemcpyHostToDevice, st));
-  rc = qsgw_set_product_tensor(c, dP);
-  if (rc != QSGW_OK) { g_create_error = c->err; cleanup(); return rc; }
-  for (int k = 0; k < nk; ++k) {
+  if (H.ck_cap < ck_e) H.ck_cap = ck_e;
+  if (H.ckq_cap < ckq_e) H.ckq_cap = ckq_e;
+  if (H.e_cap < e_len) H.e_cap = e_len;
+  for (int g = 0; g < 4; ++g)
+    if (!H.ready[g]) QSGW_H(cudaEventCreateWithFlags(&H.ready[g], cudaEventDisableTiming));
+  if (!H.cp) QSGW_H(cudaStreamCreateWithFlags(&H.cp, cudaStreamNonBlocking));
+
+  int rc = qsgw_reset(c);
+  if (rc != QSGW_OK) return rc;
+  QSGW_H(cudaMemcpyAsync(H.dP, h_P, sizeof(double2) * c->p_elems, cudaMemcpyHostToDevice, st));
+  rc = qsgw_set_product_tensor(c, H.dP);
+  if (rc != QSGW_OK) return rc;
+  for (int k = 0; k < n_k_points; ++k) {
     const int b = k & 1;
-    if (k >= 2) QSGW_H(cudaEventSynchronize(done[b]));   // buffer b free again (copies are stream-ordered anyway)
-    QSGW_H(cudaMemcpyAsync(dCk[b], static_cast<const double2*>(h_Ck) + (size_t)k * ck_e, sizeof(double2) * ck_e, cudaMemcpyHostToDevice, st));
-    QSGW_H(cudaMemcpyAsync(dCkq[b], static_cast<const double2*>(h_Ckq) + (size_t)k * ckq_e, sizeof(double2) * ckq_e, cudaMemcpyHostToDevice, st));
-    QSGW_H(cudaMemcpyAsync(dE[b], h_eps_k + (size_t)k * n_o, sizeof(double) * n_o, cudaMemcpyHostToDevice, st));
-    QSGW_H(cudaMemcpyAsync(dE[b] + n_o, h_f_k + (size_t)k * n_o, sizeof(double) * n_o, cudaMemcpyHostToDevice, st));
-    QSGW_H(cudaMemcpyAsync(dE[b] + 2 * n_o, h_eps_kq + (size_t)k * n_u, sizeof(double) * n_u, cudaMemcpyHostToDevice, st));
-    QSGW_H(cudaMemcpyAsync(dE[b] + 2 * n_o + n_u, h_f_kq + (size_t)k * n_u, sizeof(double) * n_u, cudaMemcpyHostToDevice, st));
-    rc = qsgw_chi0_add_kpoint(c, dCk[b], nb, dCkq[b], nb, dE[b], dE[b] + n_o, dE[b] + 2 * n_o, dE[b] + 2 * n_o + n_u, n_o, n_u);
-    if (rc != QSGW_OK) { g_create_error = c->err; cleanup(); return rc; }
-    QSGW_H(cudaEventRecord(done[b], st));
+    if (k >= 2) QSGW_H(cudaEventSynchronize(H.done[b]));   // keeps the host at most two k-points ahead
+    QSGW_H(cudaMemcpyAsync(H.dCk[b], static_cast<const double2*>(h_Ck) + (size_t)k * ck_e, sizeof(double2) * ck_e, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(H.dCkq[b], static_cast<const double2*>(h_Ckq) + (size_t)k * ckq_e, sizeof(double2) * ckq_e, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(H.dE[b], h_eps_k + (size_t)k * n_o, sizeof(double) * n_o, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(H.dE[b] + n_o, h_f_k + (size_t)k * n_o, sizeof(double) * n_o, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(H.dE[b] + 2 * n_o, h_eps_kq + (size_t)k * n_u, sizeof(double) * n_u, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(H.dE[b] + 2 * n_o + n_u, h_f_kq + (size_t)k * n_u, sizeof(double) * n_u, cudaMemcpyHostToDevice, st));
+    rc = qsgw_chi0_add_kpoint(c, H.dCk[b], nb, H.dCkq[b], nb, H.dE[b], H.dE[b] + n_o, H.dE[b] + 2 * n_o, H.dE[b] + 2 * n_o + n_u, n_o, n_u);
+    if (rc != QSGW_OK) return rc;
+    QSGW_H(cudaEventRecord(H.done[b], st));
   }
   // The batches still staged are accumulated frequency group by frequency group; each group is finalized and
   // copied to the host on a second stream while the next group's kernel runs (the 16 N_M^2 result is the one
   // large transfer of the job).
   {
-    int ng = c->n_freq >= 4 ? 4 : 1;
-    if (const char* ev = getenv("QSGW_E2E_GROUPS")) {      // A/B knob: frequency groups of the last flush
-      const int v = atoi(ev);
-      if (v >= 1 && v <= 4 && v <= c->n_freq) ng = v;
-    }
-    cudaStream_t cp = nullptr;
-    cudaEvent_t ready[4] = {nullptr, nullptr, nullptr, nullptr};
-    QSGW_H(cudaStreamCreateWithFlags(&cp, cudaStreamNonBlocking));
+    const int ng = c->e2e_groups <= c->n_freq ? c->e2e_groups : 1;
     const size_t plane_pad = (size_t)c->n_m_pad * c->n_m_pad, plane_out = (size_t)nm * nm;
     cudaError_t ce = cudaSuccess;
     for (int g = 0; g < ng && rc == QSGW_OK && ce == cudaSuccess; ++g) {
@@ -1043,25 +1080,24 @@ int32_t qsgw_chi0_run_host(const qsgw_desc* desc, const void* h_P, const void* h
       rc = flush_range(c, j0, j1 - j0, g == 0, g == ng - 1);
       if (rc != QSGW_OK) break;
       ce = qsgw::launch_finalize(c->d_acc_re + j0 * plane_pad, c->d_acc_im + j0 * plane_pad, nm, c->n_m_pad, j1 - j0,
-                                 1.0 / (double)c->n_k, dOut + j0 * plane_out, st);
+                                 1.0 / (double)c->n_k, H.dOut + j0 * plane_out, st);
       c->launches += 1;
-      if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&ready[g], cudaEventDisableTiming);
-      if (ce == cudaSuccess) ce = cudaEventRecord(ready[g], st);
-      if (ce == cudaSuccess) ce = cudaStreamWaitEvent(cp, ready[g], 0);
+      if (ce == cudaSuccess) ce = cudaEventRecord(H.ready[g], st);
+      if (ce == cudaSuccess) ce = cudaStreamWaitEvent(H.cp, H.ready[g], 0);
       if (ce == cudaSuccess)
-        ce = cudaMemcpyAsync(static_cast<double2*>(h_chi0_out) + j0 * plane_out, dOut + j0 * plane_out,
-                             sizeof(double2) * (j1 - j0) * plane_out, cudaMemcpyDeviceToHost, cp);
+        ce = cudaMemcpyAsync(static_cast<double2*>(h_chi0_out) + j0 * plane_out, H.dOut + j0 * plane_out,
+                             sizeof(double2) * (j1 - j0) * plane_out, cudaMemcpyDeviceToHost, H.cp);
     }
-    if (ce == cudaSuccess) ce = cudaStreamSynchronize(cp);
-    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
-    for (int g = 0; g < 4; ++g) if (ready[g]) cudaEventDestroy(ready[g]);
-    cudaStreamDestroy(cp);
-    if (rc != QSGW_OK) { g_create_error = c->err; cleanup(); return rc; }
-    if (ce != cudaSuccess) { g_create_error = std::string("result copy: ") + cudaGetErrorString(ce); cleanup(); return QSGW_ERR_CUDA; }
+    cudaError_t se = cudaStreamSynchronize(H.cp);
+    if (ce == cudaSuccess) ce = se;
+    se = cudaStreamSynchronize(st);
+    if (ce == cudaSuccess) ce = se;
+    if (rc != QSGW_OK) return rc;
+    if (ce != cudaSuccess) { cudaGetLastError(); return c->cuda_fail(ce, "result copy"); }
   }
 #undef QSGW_H
-  if (out_kernel_launches) *out_kernel_launches = c->launches;
-  cleanup();
+  if (out_kernel_launches) *out_kernel_launches = c->launches - launches0;
+  c->err.clear();
   return QSGW_OK;
 }
 

@@ -169,11 +169,14 @@ size_t zmel_dmma_smem_bytes(int b_max, int kt) { return smem_for(kZdNBMax, b_max
 template <int NB>
 static cudaError_t launch_nb(const ZmelArgs& a, cudaStream_t s) {
   const size_t smem = smem_for(NB, a.st.b_max, a.kt);
-  static size_t configured = 0;
-  if (smem > 48 * 1024 && smem > configured) {
+  static size_t configured[kMaxDevices] = {};      // the attribute is per device
+  int dev = 0;
+  cudaGetDevice(&dev);
+  dev = dev < 0 || dev >= kMaxDevices ? 0 : dev;
+  if (smem > 48 * 1024 && smem > configured[dev]) {
     cudaError_t e = cudaFuncSetAttribute(zmel_dmma_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    configured = smem;
+    configured[dev] = smem;
   }
   dim3 grid(a.ncg, (a.n_o + NB - 1) / NB);
   zmel_dmma_kernel<NB><<<grid, kZdThreads, smem, s>>>(a);
@@ -182,8 +185,7 @@ static cudaError_t launch_nb(const ZmelArgs& a, cudaStream_t s) {
 
 cudaError_t launch_zmel_dmma(const ZmelArgs& a, cudaStream_t s) {
   // bands per CTA: the choice with the fewest rounds x bands (2 CTAs per SM when the shared memory allows)
-  int n_sm = 148;
-  cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+  const int n_sm = a.n_sm;
   int best_nb = 4;
   long long best = -1;
   for (int nb = 4; nb <= kZdNBMax; ++nb) {

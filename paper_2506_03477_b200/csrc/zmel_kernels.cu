@@ -187,82 +187,11 @@ __global__ void pair_weights_kernel(const double* __restrict__ eps_k, const doub
   }
 }
 
-// Mixed mode: FP64 z batch (column-group layout) -> FP32 K-major planes (kernels.h).  One block = one
-// column group (16 product functions) x 128 pairs, transposed through shared memory so that both the
-// reads ([p][16] doubles) and the writes (128 consecutive pairs of one I) are coalesced.
-//   split_lo = 1: planes 2/3 = z - trunc_tf32(z)   (3xTF32 split; the tensor core truncates planes 0/1)
-//   split_lo = 0: planes 2/3 = rna_tf32(z)         (single-pass TF32 operand)
-__global__ void __launch_bounds__(256) z_to_planes32_kernel(const double* __restrict__ zws, long long kpad, int ncg,
-                                                            int n_m, long long n_pairs, float* __restrict__ out,
-                                                            int n_m_pad, int split_lo) {
-  __shared__ float tx[kCG][129], ty[kCG][129];
-  const int cg = blockIdx.y;
-  const long long p0 = (long long)blockIdx.x * 128;
-  const long long plane = (long long)ncg * kpad * kCG;
-  const double* src = zws + ((long long)cg * kpad + p0) * kCG;
-  for (int idx = threadIdx.x; idx < 128 * kCG; idx += 256) {
-    const int pl = idx / kCG, col = idx % kCG;
-    float x = 0.f, y = 0.f;
-    if (p0 + pl < n_pairs) {
-      x = (float)src[idx];
-      y = (float)src[plane + idx];
-    }
-    tx[col][pl] = x;
-    ty[col][pl] = y;
-  }
-  __syncthreads();
-  const long long oplane = (long long)n_m_pad * kpad;
-  for (int idx = threadIdx.x; idx < 128 * kCG; idx += 256) {
-    const int col = idx / 128, pl = idx % 128;
-    const int I = cg * kCG + col;
-    if (I >= n_m || p0 + pl >= kpad) continue;
-    const float x = tx[col][pl], y = ty[col][pl];
-    float x2, y2;
-    if (split_lo) {
-      x2 = x - __uint_as_float(__float_as_uint(x) & 0xFFFFE000u);
-      y2 = y - __uint_as_float(__float_as_uint(y) & 0xFFFFE000u);
-    } else {
-      uint32_t rx, ry;
-      asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(rx) : "f"(x));
-      asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(ry) : "f"(y));
-      x2 = __uint_as_float(rx);
-      y2 = __uint_as_float(ry);
-    }
-    const long long o = (long long)I * kpad + p0 + pl;
-    out[o] = x;
-    out[oplane + o] = y;
-    out[2 * oplane + o] = x2;
-    out[3 * oplane + o] = y2;
-  }
-}
-
-__global__ void z_export32_kernel(const float* __restrict__ z32, long long kpad, int n_m_pad, int n_m,
-                                  long long n_pairs, double2* __restrict__ out) {
-  const long long total = n_pairs * n_m;
-  const long long oplane = (long long)n_m_pad * kpad;
-  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total;
-       e += (long long)gridDim.x * blockDim.x) {
-    const long long p = e / n_m;
-    const int I = (int)(e - p * n_m);
-    const long long o = (long long)I * kpad + p;
-    out[e] = make_double2((double)z32[o], (double)z32[oplane + o]);
-  }
-}
-
-__global__ void weights_to_f32_kernel(const double* __restrict__ wtab, float* __restrict__ w32, long long kpad,
-                                      long long n_pad, int n_freq) {
-  const long long total = n_pad * n_freq;
-  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total;
-       e += (long long)gridDim.x * blockDim.x) {
-    const long long j = e / n_pad, p = e - j * n_pad;
-    w32[j * kpad + p] = (float)wtab[j * kpad + p];
-  }
-}
-
 // Mixed mode, FP16 split: FP64 z batch (column-group layout) -> "hl16" planes (kernels.h): per product
 // function I and 32-pair stage one 128-byte row  h[32] | l[32]  with v = fp32(z * 2^S), h = fp16(v),
-// l = fp16(v - h);  S = f16_scale_exp(max |z| of the batch) keeps every h below 2^14.  Same transposition
-// through shared memory as z_to_planes32_kernel; rows of pairs beyond the batch are written as zeros.
+// l = fp16(v - h);  S = f16_scale_exp(max |z| of the batch) keeps every h below 2^14.  One block = one column
+// group (16 product functions) x 128 pairs, transposed through shared memory so that both the reads ([p][16]
+// doubles) and the writes (consecutive pairs of one I) are coalesced; rows of pairs beyond the batch are zeros.
 __global__ void __launch_bounds__(256) z_to_hl16_kernel(const double* __restrict__ zws, long long kpad, int ncg,
                                                         int n_m, long long n_pairs, __half* __restrict__ out,
                                                         unsigned char* __restrict__ out8, int n_m_pad,
@@ -331,20 +260,42 @@ __global__ void z_export_hl16_kernel(const __half* __restrict__ zhl, long long k
 // Weights scaled per frequency into (1/2, 1] and split into fp16 pieces:  v = fp32(w_j(p) * sigma_j),
 // sigma_j = 2^-e with max_p |w_j(p)| = m 2^e, m in [1/2, 1);  w_h = fp16(v), w_l = fp16(v - w_h), stored per
 // 32-pair stage as  w_h[32] | w_l[32];  wscale[j] = 1 / sigma_j.  One block per frequency.
+// The same pass decides which product variant the flush runs (kernels.h, MixedCtl): P_eff_j = (sum_p w_j)^2 /
+// sum_p w_j^2 is the effective number of pairs summed per output element at frequency j; the last block to
+// finish takes the minimum over j and sets ctl->use_fp8.
 __global__ void __launch_bounds__(1024) weights_scale_hl16_kernel(const double* __restrict__ wtab,
                                                                   __half* __restrict__ w16, double* __restrict__ wscale,
-                                                                  long long kpad, long long n_pad) {
-  __shared__ double red[32];
+                                                                  long long kpad, long long n_pad, MixedCtl* ctl) {
+  __shared__ double red[3][32];
   const int j = blockIdx.x;
   const double* wr = wtab + (long long)j * kpad;
-  double m = 0.0;
-  for (long long p = threadIdx.x; p < n_pad; p += blockDim.x) m = fmax(m, fabs(wr[p]));
+  double m = 0.0, s1 = 0.0, s2 = 0.0;
+  for (long long p = threadIdx.x; p < n_pad; p += blockDim.x) {
+    const double w = wr[p];
+    m = fmax(m, fabs(w));
+    s1 += w;
+    s2 += w * w;
+  }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  for (int o = 16; o > 0; o >>= 1) {
+    m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    red[0][threadIdx.x >> 5] = m;
+    red[1][threadIdx.x >> 5] = s1;
+    red[2][threadIdx.x >> 5] = s2;
+  }
   __syncthreads();
-  m = red[0];
-  for (int i = 1; i < (int)(blockDim.x >> 5); ++i) m = fmax(m, red[i]);
+  m = red[0][0];
+  s1 = red[1][0];
+  s2 = red[2][0];
+  for (int i = 1; i < (int)(blockDim.x >> 5); ++i) {
+    m = fmax(m, red[0][i]);
+    s1 += red[1][i];
+    s2 += red[2][i];
+  }
   int e = 0;
   if (m > 0.0 && m < 1e300) (void)frexp(m, &e);
   const double sigma = exp2((double)-e);
@@ -356,18 +307,37 @@ __global__ void __launch_bounds__(1024) weights_scale_hl16_kernel(const double* 
     o[(p >> 5) * 64 + (p & 31)] = h;
     o[(p >> 5) * 64 + 32 + (p & 31)] = __float2half_rn(v - __half2float(h));
   }
+  if (threadIdx.x == 0) {
+    // all-zero rows (every pair dropped) do not constrain the choice
+    if (s2 > 0.0) atomicMin(reinterpret_cast<unsigned int*>(&ctl->peff_min), __float_as_uint((float)(s1 * s1 / s2)));
+    __threadfence();
+    if (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1) {     // last block: every frequency has contributed
+      __threadfence();
+      const float pe = *reinterpret_cast<volatile float*>(&ctl->peff_min);
+      const int use = ctl->mode == 1 || (ctl->mode == 2 && pe >= ctl->thr_pairs);
+      ctl->use_fp8 = use;
+      ctl->n_flush += 1;
+      ctl->n_flush_fp8 += use ? 1 : 0;
+      ctl->peff_min_seen = fminf(ctl->peff_min_seen, pe);
+      ctl->peff_min = 3.0e38f;                               // re-armed for the next flush
+      ctl->ticket = 0;
+    }
+  }
 }
 
 }  // namespace
 
 cudaError_t launch_zmel_f64(const ZmelArgs& a, cudaStream_t s) {
   const size_t smem = sizeof(double) * (2 * kZmelNB * a.st.b_max + 2 * kZmelNB * a.st.b_max * kCG);
-  static size_t configured = 0;
-  if (smem > 48 * 1024 && smem > configured) {
+  static size_t configured[kMaxDevices] = {};      // the attribute is per device
+  int dev = 0;
+  cudaGetDevice(&dev);
+  dev = dev < 0 || dev >= kMaxDevices ? 0 : dev;
+  if (smem > 48 * 1024 && smem > configured[dev]) {
     cudaError_t e = cudaFuncSetAttribute(zmel_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)smem);
     if (e != cudaSuccess) return e;
-    configured = smem;
+    configured[dev] = smem;
   }
   dim3 grid(a.ncg, (a.n_o + kZmelNB - 1) / kZmelNB);
   zmel_kernel<double><<<grid, kZmelThreads, smem, s>>>(a);
@@ -402,35 +372,6 @@ cudaError_t launch_pair_weights(const double* eps_k, const double* f_k, const do
   return cudaGetLastError();
 }
 
-// mixed mode: FP64 stage (a) into the FP64 workspace, then one conversion/transposition pass
-cudaError_t launch_zmel_mixed(const ZmelArgs& a, float* zws32, int n_m_pad, int split_lo, cudaStream_t s) {
-  cudaError_t e = a.kt ? launch_zmel_dmma(a, s) : launch_zmel_f64(a, s);
-  if (e != cudaSuccess) return e;
-  const long long n_pairs = (long long)a.n_o * a.n_u;
-  dim3 grid((unsigned)((a.kpad + 127) / 128), a.ncg);
-  z_to_planes32_kernel<<<grid, 256, 0, s>>>(a.zws, a.kpad, a.ncg, a.st.n_m, n_pairs, zws32, n_m_pad, split_lo);
-  return cudaGetLastError();
-}
-
-cudaError_t launch_z_export32(const float* zws32, long long kpad, int n_m_pad, int n_m, long long n_pairs,
-                              double2* out, cudaStream_t s) {
-  z_export32_kernel<<<grid_for(n_pairs * n_m, 256), 256, 0, s>>>(zws32, kpad, n_m_pad, n_m, n_pairs, out);
-  return cudaGetLastError();
-}
-
-cudaError_t launch_planes32_from_ws(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs,
-                                    float* zws32, int n_m_pad, int split_lo, cudaStream_t s) {
-  dim3 grid((unsigned)((kpad + 127) / 128), ncg);
-  z_to_planes32_kernel<<<grid, 256, 0, s>>>(zws, kpad, ncg, n_m, n_pairs, zws32, n_m_pad, split_lo);
-  return cudaGetLastError();
-}
-
-cudaError_t launch_weights_to_f32(const double* wtab, float* wtab32, long long kpad, long long n_pad, int n_freq,
-                                  cudaStream_t s) {
-  weights_to_f32_kernel<<<grid_for(n_pad * n_freq, 256), 256, 0, s>>>(wtab, wtab32, kpad, n_pad, n_freq);
-  return cudaGetLastError();
-}
-
 cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs, void* zhl,
                              void* zhb8, int n_m_pad, const float* zmax, cudaStream_t s) {
   const long long n_rows = (n_pairs + kPairStage - 1) / kPairStage * kPairStage;   // this batch's padded rows
@@ -448,8 +389,8 @@ cudaError_t launch_z_export_hl16(const void* zhl, long long kpad, int n_m_pad, i
 }
 
 cudaError_t launch_weights_scale_hl16(const double* wtab, void* wtab16, double* wscale, long long kpad, long long n_pad,
-                                      int n_freq, cudaStream_t s) {
-  weights_scale_hl16_kernel<<<n_freq, 1024, 0, s>>>(wtab, static_cast<__half*>(wtab16), wscale, kpad, n_pad);
+                                      int n_freq, MixedCtl* ctl, cudaStream_t s) {
+  weights_scale_hl16_kernel<<<n_freq, 1024, 0, s>>>(wtab, static_cast<__half*>(wtab16), wscale, kpad, n_pad, ctl);
   return cudaGetLastError();
 }
 

@@ -6,7 +6,8 @@ def sites_of(prob):
     return [prob.P_site(s) for s in range(prob.cfg.n_sites)]
 
 
-def run_cuda(prob, spin=0, precision=0, max_n_o=None, max_n_u=None, n_k_norm=None, return_ctx=False):
+def run_cuda(prob, spin=0, precision=0, max_n_o=None, max_n_u=None, n_k_norm=None, return_ctx=False, options=None,
+             stats=None):
     import torch
     import paper_2506_03477_b200 as q
     cfg = prob.cfg
@@ -17,6 +18,8 @@ def run_cuda(prob, spin=0, precision=0, max_n_o=None, max_n_u=None, n_k_norm=Non
                         n_k if n_k_norm is None else n_k_norm,
                         max_n_o or cfg.n_o, max_n_u or cfg.n_u, precision=precision,
                         occ_tol=cfg.occ_tol)
+    for key, val in (options or {}).items():
+        ctx.set_option(key, val)
     ctx.set_product_tensor(torch.from_numpy(prob.P).to(dev))
     Ck = torch.from_numpy(sp.Ck).to(dev); Ckq = torch.from_numpy(sp.Ckq).to(dev)
     ek = torch.from_numpy(sp.eps_k).to(dev); fk = torch.from_numpy(sp.f_k).to(dev)
@@ -26,6 +29,8 @@ def run_cuda(prob, spin=0, precision=0, max_n_o=None, max_n_u=None, n_k_norm=Non
     out = ctx.chi0_finalize()
     ctx.sync()
     res = out.cpu().numpy()
+    if stats is not None and precision == 1:
+        stats["launches"], stats["launches_fp8"], stats["min_eff_pairs"] = ctx.mixed_stats()
     if return_ctx:
         return res, ctx
     ctx.destroy()

@@ -88,15 +88,44 @@ def test_band_batching_equals_single_batch(mo, mu):
 
 
 @pytest.mark.parametrize("precision,tol", [(0, TOL_FP64), (1, TOL_MIXED)])
-@pytest.mark.parametrize("batches", ["1", "2", "7"])
-def test_staged_batches_per_launch(monkeypatch, precision, tol, batches):
+@pytest.mark.parametrize("batches", [1, 2, 7])
+def test_staged_batches_per_launch(precision, tol, batches):
     """Band batches are staged back to back in the z workspace and accumulated by one stage (b) launch per
     full workspace: 1, 2 or 7 batches per launch (a flush in the middle of a k-point, a partial last flush at
     finalize) must all give the oracle's result.  cfg 1 shapes, 5 k-points, 2 x 23 band batches."""
-    monkeypatch.setenv("QSGW_STAGE_BATCHES", batches)
     cfg = get_config(1)
     prob = generate(cfg, n_k=5)
-    got = run_cuda(prob, precision=precision, max_n_o=2, max_n_u=23)
+    got = run_cuda(prob, precision=precision, max_n_o=2, max_n_u=23, options={"stage_batches": batches})
+    assert rel_fro_per_freq(got, oracle_chi(prob)).max() <= tol
+
+
+@pytest.mark.parametrize("precision,tol", [(0, TOL_FP64), (1, TOL_MIXED)])
+def test_sync_between_build_and_accumulate(precision, tol):
+    """A qsgw_sync (or finalize) between zmel_build and chi0_accumulate(d_z = NULL) flushes the batches staged
+    below the one just built; the built batch must still be accumulated from the slot it was written to, and the
+    released slots must contribute nothing.  [build, accumulate] x 2, build, sync, accumulate per k-point, with
+    three batches staged per launch, against the oracle."""
+    import torch
+    import paper_2506_03477_b200 as q
+    cfg = get_config(1)
+    prob = generate(cfg, n_k=3)
+    sp = prob.spins[0]
+    ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, 3, 2, 16, precision=precision)
+    ctx.set_option("stage_batches", 3)
+    ctx.set_product_tensor(torch.from_numpy(prob.P).cuda())
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    for k in range(3):
+        Ck, Ckq = t(sp.Ck[k]), t(sp.Ckq[k])
+        batches = [(n0, u0) for n0 in (0, 2) for u0 in (0, 16, 32)]       # 2 x {16, 16, 14} bands
+        for i, (n0, u0) in enumerate(batches):
+            nu = min(16, cfg.n_u - u0)
+            ctx.zmel_build(Ck, Ckq, n0, 2, u0, nu)
+            if i % 3 == 2:
+                ctx.sync()                                              # flushes the two batches staged below
+            ctx.chi0_accumulate(t(sp.eps_k[k, n0:n0 + 2]), t(sp.f_k[k, n0:n0 + 2]), t(sp.eps_kq[k, u0:u0 + nu]),
+                                t(sp.f_kq[k, u0:u0 + nu]), 2, nu)
+    got = ctx.chi0_finalize().cpu().numpy()
+    ctx.destroy()
     assert rel_fro_per_freq(got, oracle_chi(prob)).max() <= tol
 
 

@@ -123,13 +123,13 @@ def test_wc_and_rotation_block_edges(n):
     assert rel_fro_per_freq(rot.cpu().numpy(), oracle.rotate_to_coulomb_basis_ref(chi, U)).max() <= 1e-12
 
 
-@pytest.mark.parametrize("mode", ["2", "0"])
-def test_wc_graph_and_plain_launch_paths(monkeypatch, mode):
-    """QSGW_WC_GRAPH=2 makes the CUDA-graph path mandatory (an error if the capture fails), =0 forces plain
+@pytest.mark.parametrize("mode", [2, 0])
+def test_wc_graph_and_plain_launch_paths(mode):
+    """Option "wc_graph" = 2 makes the CUDA-graph path mandatory (an error if the capture fails), = 0 forces plain
     launches on the caller's stream: both give the oracle's result, also on a non-default stream."""
     import torch
     import paper_2506_03477_b200 as q
-    monkeypatch.setenv("QSGW_WC_GRAPH", mode)
+    q.set_global_option("wc_graph", mode)
     cfg = get_config(1)
     prob = generate(cfg, n_k=2)
     chi = oracle_chi(prob)
@@ -144,3 +144,4 @@ def test_wc_graph_and_plain_launch_paths(monkeypatch, mode):
         for x, i in ((w, info), (w2, info2)):
             assert int(i.item()) == 0
             assert rel_fro_per_freq(x.cpu().numpy(), ref).max() <= TOL_WC
+    q.set_global_option("wc_graph", 1)

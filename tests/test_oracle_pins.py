@@ -299,7 +299,8 @@ def test_generator_recipe():
         assert 0.9 < v < 1.1
     p2 = generate(get_config(2), n_k=2)
     f = p2.spins[0].f_k
-    assert f.min() >= 0 and f.max() <= 1 and ((f > 1e-6) & (f < 1 - 1e-6)).any() or True
+    assert f.min() >= 0 and f.max() <= 1
+    assert ((f > 1e-6) & (f < 1 - 1e-6)).any()          # the metal has partially filled bands (kT = 1e-3 Ha)
     full = generate(get_config(0)); part = generate(get_config(0), n_k=3)
     assert np.array_equal(full.spins[0].Ck[:3], part.spins[0].Ck)
 
