@@ -217,7 +217,7 @@ int32_t qsgw_mixed_stats(qsgw_ctx* ctx, int64_t* out_launches, int64_t* out_laun
  *   "stage_batches"   n >= 1   band batches staged per stage (b) launch (capped by the workspace)
  *   "zmel_dmma"       0 | 1    stage (a) step 2 on CUDA cores | on the FP64 tensor pipe (default 1)
  *   "mixed_fp8"       0 | 1 | 2  E5M2 correction products never | always | chosen on the device (default 2)
- *   "mixed_fp8_threshold_x100"  T*100: automatic choice takes E5M2 when P_eff >= T * N_M
+ *   "mixed_fp8_threshold_x100"  T*100: automatic choice takes E5M2 when P_eff >= T * N_M (default T = 4)
  *   "mixed_window"    1..64    pipeline stages per TMEM drain window (default 8)
  *   "e2e_groups"      1..4     frequency groups of the last launch of qsgw_chi0_run_host (default 4)
  * ctx == NULL, process-wide:

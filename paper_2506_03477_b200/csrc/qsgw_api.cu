@@ -72,7 +72,8 @@ struct qsgw_ctx {
   float* d_zmax = nullptr;
   qsgw::MixedCtl* d_ctl = nullptr;   // device-side choice of the product variant per flush
   int fp8_mode = 2;             // 0 never | 1 always | 2 chosen on the device (option "mixed_fp8")
-  double fp8_thr = 2.0;         // automatic choice: E5M2 when P_eff >= fp8_thr * N_M
+  double fp8_thr = 4.0;         // automatic choice: E5M2 when P_eff >= fp8_thr * N_M (measured, DESIGN.md 4b:
+                                // 1.2e-5 at P_eff = 4.8 N_M, 1.6e-5 at 2.4 N_M, 2.2e-5 at 0.7 N_M)
   int win = 8;                  // stages per TMEM drain window
   int zmel_kt = 0;              // stage (a) DMMA kernel: padded contraction length (0 = CUDA-core kernel)
   int zmel_kt_avail = 0;        // ... as computed at creation (option "zmel_dmma" switches zmel_kt between 0 and this)

@@ -121,8 +121,8 @@ def test_cfg4_full_matrix_mixed(cfg4_case, variant):
     got = run_cuda(prob, precision=1, options={"mixed_fp8": variant}, stats=st)
     err = rel_fro_per_freq(got[CFG4_FREQS], ref)
     assert err.max() <= TOL_MIXED, (variant, st, err)
-    assert st["launches_fp8"] == (st["launches"] if variant == E5M2 else 0 if variant == FP16X3 else st["launches_fp8"])
-    if variant == AUTO:
+    assert st["launches_fp8"] == (0 if variant == FP16X3 else st["launches"]) > (-1 if variant == FP16X3 else 0)
+    if variant == AUTO:       # the bench configuration: two k-points per launch, P_eff = 9 N_M -> E5M2 in every launch
         _sampled_and_sketch(prob, 0, got, TOL_MIXED)
 
 
