@@ -178,6 +178,30 @@ int32_t qsgw_wc_from_chi0(int32_t n_m, int32_t n_freq, const void* d_chi0, const
 int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_chi0, const void* d_U, void* d_out,
                                    void* cuda_stream);
 
+/* Imaginary-axis part of the correlation self-energy for one k-point and one batch of intermediate states
+ * (the step after W^c; Eq. (22); Alg. 2 lines 11-25 and 44):
+ *   ZW^c[n', n, nu] = sum_i w^I_i(eps_qn - eps_{q-k,n'}) sum_mu z[n', n, mu] W^c[i][mu, nu]
+ *   sigc[n, m]     += -(1/N_k) sum_{n', nu} ZW^c[n', n, nu] conj(z[n', m, nu])
+ * with z[n', n, mu] = conj(Z_mu^{q-k n', q n}): the batch qsgw_zmel_build makes for d_Ck = C_{q-k} (bands n', the
+ * n_all intermediate states) and d_Ckq = C_q (bands n, the n_qp states of the self-energy matrix).
+ * Weights (Eq. 23; the paper defers to Aryasetiawan-Gunnarsson and prints no formula -- DESIGN.md reading R17):
+ *   int d omega / 2 pi X(i omega) / (dE - i omega) = int_0^inf K(dE, omega) X(i omega) d omega for even X,
+ *   K = dE / (pi (dE^2 + omega^2)), integrated exactly against the piecewise-linear interpolant of X on the context's
+ *   mesh omega_0 = 0 < omega_1 < ... (X = 0 beyond the last point); dE = 0 gives weight 0.
+ *   d_z      : NULL = the batch of the last qsgw_zmel_build (n_all = its n_o, n_qp = its n_u; in QSGW_PREC_MIXED
+ *              that batch carries FP32-grade values), else complex128 [n_all][n_qp][N_M] (the d_z_out layout)
+ *   d_eps_q  : float64 [n_qp]   eps_qn;      d_eps_qk : float64 [n_all]  eps_{q-k, n'} of the batch
+ *   d_wc     : complex128 [n_freq][N_M][N_M] row-major, W^c(k, i omega_i) on the context's mesh (what
+ *              qsgw_wc_from_chi0 writes); any matrix is accepted, Hermiticity is not assumed
+ *   d_sigc   : complex128 [n_qp][n_qp] row-major, ACCUMULATED (the caller zeroes it before the first call);
+ *              1/N_k is the context's n_k.  Not Hermitian: the weight carries eps_qn of the row index (Eq. 3
+ *              symmetrises later).
+ * FP64 arithmetic on the FP64 tensor pipe in both precision modes.  n_all <= max_n_o, n_qp <= max_n_u.  The
+ * context allocates its I^c workspace (two z-sized buffers and the weight table) at the first call.
+ * Stream-ordered, does not synchronise; does not touch the chi0 accumulator or the staged batches. */
+int32_t qsgw_sigc_imag_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps_q, const double* d_eps_qk,
+                                  const void* d_wc, int32_t n_all, int32_t n_qp, void* d_sigc);
+
 /* Per-stage device timing, for roofline measurement.  While enabled, every kernel launch of
  * the path is bracketed by CUDA events on the context's stream (Eq. 8 / Eq. 14 stages:
  * QSGW_STAGE_ZMEL, _WEIGHTS, _CHI0, _FINALIZE).  qsgw_stage_time_ms synchronises the stream,

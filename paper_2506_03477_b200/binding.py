@@ -60,10 +60,12 @@ def lib() -> C.CDLL:
     L.qsgw_destroy.restype = None
     L.qsgw_chi0_run_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp, C.POINTER(i64)]
     L.qsgw_set_option.argtypes = [vp, C.c_char_p, i64]
+    L.qsgw_sigc_imag_accumulate.argtypes = [vp, vp, dp, dp, vp, i32, i32, vp]
     L.qsgw_mixed_stats.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(C.c_double)]
     for name in ("qsgw_create", "qsgw_set_product_tensor", "qsgw_zmel_build", "qsgw_chi0_accumulate",
                  "qsgw_chi0_add_kpoint", "qsgw_chi0_finalize", "qsgw_reset", "qsgw_sync",
                  "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_set_option", "qsgw_mixed_stats", "qsgw_wc_from_chi0",
+                 "qsgw_sigc_imag_accumulate",
                  "qsgw_chi0_to_coulomb_basis"):
         getattr(L, name).restype = i32
     for name in ("qsgw_last_error", "qsgw_last_create_error", "qsgw_version"):
@@ -193,6 +195,14 @@ class Chi0Context:
                                      device="cuda")
         self._check(self._L.qsgw_chi0_finalize(self._h, _ptr(d_chi0_out, torch.complex128)))
         return d_chi0_out
+
+    def sigc_imag_accumulate(self, d_eps_q, d_eps_qk, d_wc, n_all: int, n_qp: int, d_sigc, d_z=None):
+        """I^c of Eq. (22) for one k-point and one batch of intermediate states, added into d_sigc [n_qp][n_qp]."""
+        import torch
+        f64 = torch.float64
+        self._check(self._L.qsgw_sigc_imag_accumulate(self._h, _ptr(d_z, torch.complex128), _ptr(d_eps_q, f64),
+                                                      _ptr(d_eps_qk, f64), _ptr(d_wc, torch.complex128), n_all, n_qp,
+                                                      _ptr(d_sigc, torch.complex128)))
 
     def reset(self):
         self._check(self._L.qsgw_reset(self._h))

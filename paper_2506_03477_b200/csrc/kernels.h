@@ -137,17 +137,37 @@ cudaError_t launch_z_export_hl16(const void* zhl, long long kpad, int n_m_pad, i
 cudaError_t launch_weights_scale_hl16(const double* wtab, void* wtab16, double* wscale, long long kpad, long long n_pad,
                                       int n_freq, MixedCtl* ctl, cudaStream_t s);
 
-// ---- screened Coulomb interaction W^c (wc_kernels.cu) ---------------------------------------------------
-struct ZgemmArgs {       // batched complex FP64 GEMM on 64x64 tiles (see zgemm_dmma_kernel)
+// ---- batched complex FP64 GEMM on the FP64 tensor pipe, operands staged by TMA (zgemm_tma_kernels.cu) ----------
+// C (+)= alpha * sum_{r < reps} diag(row_scale[r]) opA(A_r) opB(B_r)   on 64x64 tiles, complex128 interleaved, row-major.
+//   a_kc:  A_r(i,k) = A[r*rA + i*lda + k]              else  A_r(i,k) = conj(A[r*rA + k*lda + i])   (conjugate transpose)
+//   b_kc:  B_r(k,j) = conj(B[r*rB + j*ldb + k])        else  B_r(k,j) = B[r*rB + k*ldb + j]
+// Extents are arbitrary (ragged tiles are zero-filled by TMA, stores are guarded); batch b reads A + b*sA, B + b*sB and
+// writes C + b*sC (stride 0 = operand shared by all batches).  The repetitions are an outer contraction loop: the
+// frequencies of the I^c product (A fixed, B = W^c(i omega_r), row_scale = the quadrature weights) or the
+// intermediate states of its closing contraction.  split > 1: the repetitions are divided over `split` CTAs per tile,
+// which add their partial sums to C atomically (C must hold the value to add to: beta_one semantics).
+struct ZgemmArgs {
   const double2* A; const double2* B; double2* C;
   long long lda, ldb, ldc;      // leading dimensions in complex elements
   long long sA, sB, sC;         // batch strides in complex elements
-  int k;                        // contraction length (multiple of 16)
-  double alpha;                 // real scale
-  int beta_one;                 // 1: C += ..., 0: C = ...
-  int tri;                      // 0 all tiles | 1 lower tiles only | 2 lower tiles and k starts at 64*max(ti,tj)
+  int m, n, k;                  // C is m x n; contraction length k per repetition
+  int batch = 1;
+  double alpha = 1.0;           // real scale
+  int beta_one = 0;             // 1: C += ..., 0: C = ...
+  int tri = 0;                  // 0 all tiles | 1 lower tiles only | 2 lower tiles and k starts at 64*max(ti,tj)
                                 // | 3 all tiles and k starts at 64*tj (B lower triangular)
+  int reps = 1; long long rA = 0, rB = 0;
+  const double* row_scale = nullptr; long long ld_scale = 0;    // [reps][ld_scale], row i of C / opA
+  int split = 1;
 };
+cudaError_t launch_zgemm(bool a_kc, bool b_kc, const ZgemmArgs& a, cudaStream_t s);
+cudaError_t zgemm_configure();       // kernel attributes (per device)
+// 4-D FP64 tensor map over interleaved complex128 data: dims {2*inner, outer, d2, d3} (strides in complex elements),
+// box {16 doubles, box_rows, 1, 1}, 128-byte swizzle, zero fill out of bounds.  Defined in qsgw_api.cu.
+cudaError_t make_zmap(CUtensorMap* out, const double2* base, long long inner, long long outer, long long ld,
+                      long long d2, long long s2, long long d3, long long s3, int box_rows);
+
+// ---- screened Coulomb interaction W^c (wc_kernels.cu) ---------------------------------------------------
 // W^c[j] = sqrt(v) ((1 - sqrt(v) chi0[j] sqrt(v))^-1 - 1) sqrt(v) for all frequencies, stream-ordered.
 // work: n_freq * (2 * n_pad^2 + 64 * n_pad + nb * 64 * 64) complex elements, n_pad = ceil64(n_m), nb = n_pad / 64.
 // d_info: 0, or 1 + index of the first non-positive Cholesky pivot (eps not positive definite).
@@ -159,6 +179,14 @@ cudaError_t launch_rotate_basis(int n_m, int n_freq, const double2* chi0, const 
                                 cudaStream_t s);
 cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const double* v, double2* wc_out,
                                 double2* work, int* d_info, cudaStream_t s);
+
+// ---- imaginary-axis correlation self-energy I^c (sigc_kernels.cu; Eq. 22, Alg. 2) -------------------------------
+// w[i][p] (ld doubles per frequency) for the pairs p = n' * n_qp + n of one batch of intermediate states
+cudaError_t launch_sigc_weights(const double* eps_q, const double* eps_qk, int n_all, int n_qp, const double* d_omega,
+                                int n_freq, double* w, long long ld, cudaStream_t s);
+// z: complex128 [n_all][n_qp][n_m]; wc: [n_freq][n_m][n_m]; zw: workspace of the size of z; sigc [n_qp][n_qp] += ...
+cudaError_t launch_sigc_imag(const double2* z, const double* w, long long ld_w, const double2* wc, int n_all, int n_qp,
+                             int n_m, int n_freq, double inv_nk, double2* zw, double2* sigc, int n_sm, cudaStream_t s);
 
 // issue-rate probes (probe_kernels.cu): measured MMA-pipe peaks for the roofline denominators
 cudaError_t probe_fp64_mma(cudaStream_t s, double* out_tflops, double* out_ms);

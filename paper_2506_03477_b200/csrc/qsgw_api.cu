@@ -40,6 +40,29 @@ inline long long round_up(long long x, long long m) { return (x + m - 1) / m * m
 
 }  // namespace
 
+namespace qsgw {
+
+cudaError_t make_zmap(CUtensorMap* out, const double2* base, long long inner, long long outer, long long ld,
+                      long long d2, long long s2, long long d3, long long s3, int box_rows) {
+  EncodeTiledFn enc = get_encode_tiled();
+  if (!enc) return cudaErrorNotSupported;
+  if (inner < 1 || outer < 1 || ld < inner || d2 < 1 || d3 < 1) return cudaErrorInvalidValue;
+  // a dimension of extent 1 still needs a valid (non-zero, 16-byte multiple) stride
+  const unsigned long long plane = (unsigned long long)ld * (unsigned long long)outer * 16ull;
+  const unsigned long long st2 = (d2 > 1 && s2 > 0) ? (unsigned long long)s2 * 16ull : plane;
+  const unsigned long long st3 = (d3 > 1 && s3 > 0) ? (unsigned long long)s3 * 16ull : (st2 > plane ? st2 : plane) * (unsigned long long)d2;
+  const cuuint64_t gdim[4] = {(cuuint64_t)(2 * inner), (cuuint64_t)outer, (cuuint64_t)d2, (cuuint64_t)d3};
+  const cuuint64_t gstr[3] = {(cuuint64_t)ld * 16ull, (cuuint64_t)st2, (cuuint64_t)st3};
+  const cuuint32_t box[4] = {16, (cuuint32_t)box_rows, 1, 1};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double2*>(base), gdim, gstr, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+}  // namespace qsgw
+
 struct qsgw_ctx {
   // problem
   int n_sites = 0, n_b = 0, n_m = 0, b_max = 0, n_freq = 0, n_k = 0;
@@ -82,6 +105,10 @@ struct qsgw_ctx {
   long long stage_cap = 0;      // staged pairs that trigger a flush (<= kpad; option "stage_batches")
   long long z_off = 0;          // workspace slot of the batch the last zmel_build wrote
   int e2e_groups = 4;           // frequency groups of the last flush of qsgw_chi0_run_host
+  // I^c workspace (qsgw_sigc_imag_accumulate; allocated by its first call)
+  double2* d_sz = nullptr;      // z of the batch, complex128 [pairs][N_M]
+  double2* d_szw = nullptr;     // ZW^c, same shape
+  double* d_sw = nullptr;       // quadrature weights [n_freq][batch_pad]
   CUtensorMap tmap_h;
   double* d_acc_re = nullptr;
   double* d_acc_im = nullptr;
@@ -161,6 +188,9 @@ void free_all(qsgw_ctx* c) {
   }
   for (int i = 0; i < 4; ++i) if (c->hr.ready[i]) cudaEventDestroy(c->hr.ready[i]);
   if (c->hr.cp) cudaStreamDestroy(c->hr.cp);
+  cudaFree(c->d_sz);
+  cudaFree(c->d_szw);
+  cudaFree(c->d_sw);
   cudaFree(c->d_zhl);
   cudaFree(c->d_zhb8);
   cudaFree(c->d_wscale);
@@ -908,6 +938,57 @@ int32_t qsgw_chi0_finalize(qsgw_ctx* ctx, void* d_chi0_out) {
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "finalize kernel launch");
   ctx->launches += 1;
+  ctx->err.clear();
+  return QSGW_OK;
+}
+
+int32_t qsgw_sigc_imag_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps_q, const double* d_eps_qk,
+                                  const void* d_wc, int32_t n_all, int32_t n_qp, void* d_sigc) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  if (!d_eps_q || !d_eps_qk || !d_wc || !d_sigc) return ctx->fail(QSGW_ERR_INVALID_ARG, "NULL argument");
+  int rc = check_batch(ctx, n_all, n_qp);
+  if (rc != QSGW_OK) return rc;
+  if (!d_z) {
+    if (ctx->state != ST_Z_BUILT) return ctx->fail(QSGW_ERR_STATE, "no z batch: call zmel_build first or pass d_z");
+    if (n_all != ctx->last_n_o || n_qp != ctx->last_n_u)
+      return ctx->fail(QSGW_ERR_SHAPE, "batch %d x %d differs from the last zmel_build (%d x %d)", n_all, n_qp,
+                       ctx->last_n_o, ctx->last_n_u);
+  }
+  cudaError_t e = wc_configure_device(ctx->device);
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "kernel attributes");
+  if (!ctx->d_szw) {
+    const size_t cap = (size_t)ctx->max_n_o * ctx->max_n_u * ctx->n_m;
+    e = dev_alloc(ctx, &ctx->d_sz, cap);
+    if (e == cudaSuccess) e = dev_alloc(ctx, &ctx->d_sw, (size_t)ctx->n_freq * ctx->batch_pad);
+    if (e == cudaSuccess) e = dev_alloc(ctx, &ctx->d_szw, cap);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      cudaFree(ctx->d_sz); cudaFree(ctx->d_sw); cudaFree(ctx->d_szw);
+      ctx->d_sz = ctx->d_szw = nullptr; ctx->d_sw = nullptr;
+      return ctx->fail(QSGW_ERR_ALLOC, "I^c workspace allocation failed: %s", cudaGetErrorString(e));
+    }
+  }
+  const long long n_pairs = (long long)n_all * n_qp;
+  const double2* z = static_cast<const double2*>(d_z);
+  if (!d_z) {
+    if (ctx->f16)
+      e = qsgw::launch_z_export_hl16(hl_slot(ctx->d_zhl, ctx->z_off), ctx->kpad, ctx->n_m_pad, ctx->n_m, n_pairs,
+                                     ctx->d_zmax, ctx->d_sz, ctx->stream);
+    else
+      e = qsgw::launch_z_export(ctx->d_zws + ctx->z_off * qsgw::kCG, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, ctx->d_sz,
+                                ctx->stream);
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "z export kernel launch");
+    ctx->launches += 1;
+    z = ctx->d_sz;
+  }
+  e = qsgw::launch_sigc_weights(d_eps_q, d_eps_qk, n_all, n_qp, ctx->d_omega, ctx->n_freq, ctx->d_sw, ctx->batch_pad,
+                                ctx->stream);
+  if (e == cudaSuccess)
+    e = qsgw::launch_sigc_imag(z, ctx->d_sw, ctx->batch_pad, static_cast<const double2*>(d_wc), n_all, n_qp, ctx->n_m,
+                               ctx->n_freq, 1.0 / (double)ctx->n_k, ctx->d_szw, static_cast<double2*>(d_sigc), ctx->n_sm,
+                               ctx->stream);
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "I^c kernel launch");
+  ctx->launches += 3;
   ctx->err.clear();
   return QSGW_OK;
 }

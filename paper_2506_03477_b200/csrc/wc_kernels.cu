@@ -15,154 +15,6 @@ namespace qsgw {
 
 namespace {
 
-constexpr int kGT = 64;        // GEMM tile edge
-constexpr int kGK = 16;        // contraction depth per stage
-constexpr int kGLD = 68;       // doubles per shared-memory row (64 + 4: conflict-free DMMA fragment loads)
-constexpr int kGThreads = 256;
-constexpr int kGPlane = kGK * kGLD;                    // doubles of one real plane of one operand stage
-constexpr int kGSmem = 2 * 2 * 2 * kGPlane * 8;        // buffers x operands x (re, im)
-
-// C (+)= alpha * opA(A) opB(B) for one 64x64 tile; all extents multiples of 64 (k: of 16).
-//   A_KC:  A(i,k) = Ap[i*lda + k]            else  A(i,k) = conj(Ap[k*lda + i])   (conjugate transpose)
-//   B_KC:  B(k,j) = conj(Bp[j*ldb + k])      else  B(k,j) = Bp[k*ldb + j]
-// tri: 1 = only tiles with tj <= ti (lower triangle); 2 = additionally start the contraction at 64*max(ti,tj)
-//   (X^H X with X lower triangular: rows k < max(i,j) of X are zero in those columns); 3 = all tiles, contraction
-//   starts at 64*tj (B lower triangular).
-template <bool A_KC, bool B_KC>
-__global__ void __launch_bounds__(kGThreads) zgemm_dmma_kernel(ZgemmArgs a) {
-  const int tj = blockIdx.x, ti = blockIdx.y;
-  if ((a.tri == 1 || a.tri == 2) && tj > ti) return;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  double* sm = reinterpret_cast<double*>(smem_raw);
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int g = lane >> 2, t = lane & 3;
-  const int wm = warp >> 2, wn = warp & 3;
-  const double2* Ap = a.A + (long long)blockIdx.z * a.sA;
-  const double2* Bp = a.B + (long long)blockIdx.z * a.sB;
-  double2* Cp = a.C + (long long)blockIdx.z * a.sC;
-  const int k0 = (a.tri == 2) ? kGT * max(ti, tj) : (a.tri == 3 ? kGT * tj : 0);
-  const int n_it = (a.k - k0) / kGK;
-
-  // loader mapping (4 elements per thread and operand), interleaved so that both the global loads (consecutive
-  // lanes -> consecutive 16-byte elements) and the transposing shared-memory stores (2 wavefronts per warp store,
-  // the minimum for 8-byte words) are conflict-free:
-  //   k-contiguous operand:  row = tid/4,  k = tid%4 + 4e;     mn-contiguous operand:  k = tid/16,  row = tid%16 + 16e
-  const int a_r = A_KC ? (tid >> 2) : (tid & 15), a_k = A_KC ? (tid & 3) : (tid >> 4);
-  const int b_r = B_KC ? (tid >> 2) : (tid & 15), b_k = B_KC ? (tid & 3) : (tid >> 4);
-  double2 ra[4], rb[4];
-  auto gload = [&](int it) {
-    const int kk = k0 + it * kGK;
-    if (A_KC) {
-      const double2* p = Ap + (long long)(ti * kGT + a_r) * a.lda + kk + a_k;
-#pragma unroll
-      for (int e = 0; e < 4; ++e) ra[e] = p[4 * e];
-    } else {
-      const double2* p = Ap + (long long)(kk + a_k) * a.lda + ti * kGT + a_r;
-#pragma unroll
-      for (int e = 0; e < 4; ++e) ra[e] = p[16 * e];
-    }
-    if (B_KC) {
-      const double2* p = Bp + (long long)(tj * kGT + b_r) * a.ldb + kk + b_k;
-#pragma unroll
-      for (int e = 0; e < 4; ++e) rb[e] = p[4 * e];
-    } else {
-      const double2* p = Bp + (long long)(kk + b_k) * a.ldb + tj * kGT + b_r;
-#pragma unroll
-      for (int e = 0; e < 4; ++e) rb[e] = p[16 * e];
-    }
-  };
-  auto sstore = [&](int buf) {
-    double* ax = sm + buf * 4 * kGPlane;
-    double* ay = ax + kGPlane;
-    double* bx = ay + kGPlane;
-    double* by = bx + kGPlane;
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      const int ka = A_KC ? a_k + 4 * e : a_k, ia = A_KC ? a_r : a_r + 16 * e;
-      ax[ka * kGLD + ia] = ra[e].x;
-      ay[ka * kGLD + ia] = A_KC ? ra[e].y : -ra[e].y;
-      const int kb = B_KC ? b_k + 4 * e : b_k, jb = B_KC ? b_r : b_r + 16 * e;
-      bx[kb * kGLD + jb] = rb[e].x;
-      by[kb * kGLD + jb] = B_KC ? -rb[e].y : rb[e].y;
-    }
-  };
-
-  double t1[4][2][2], t2[4][2][2], t3[4][2][2];
-#pragma unroll
-  for (int mi = 0; mi < 4; ++mi)
-#pragma unroll
-    for (int ni = 0; ni < 2; ++ni)
-#pragma unroll
-      for (int e = 0; e < 2; ++e) t1[mi][ni][e] = t2[mi][ni][e] = t3[mi][ni][e] = 0.0;
-
-  if (n_it > 0) {
-    gload(0);
-    sstore(0);
-  }
-  __syncthreads();
-  for (int it = 0; it < n_it; ++it) {
-    const int buf = it & 1;
-    if (it + 1 < n_it) gload(it + 1);
-    const double* ax = sm + buf * 4 * kGPlane;
-    const double* ay = ax + kGPlane;
-    const double* bx = ay + kGPlane;
-    const double* by = bx + kGPlane;
-#pragma unroll
-    for (int q = 0; q < kGK / 4; ++q) {
-      const int ro = (4 * q + t) * kGLD + g;
-      double fx[4], fy[4], fs[4], hx[2], hy[2], hs[2];
-#pragma unroll
-      for (int mi = 0; mi < 4; ++mi) {
-        fx[mi] = ax[ro + 32 * wm + 8 * mi];
-        fy[mi] = ay[ro + 32 * wm + 8 * mi];
-        fs[mi] = fx[mi] + fy[mi];
-      }
-#pragma unroll
-      for (int ni = 0; ni < 2; ++ni) {
-        hx[ni] = bx[ro + 16 * wn + 8 * ni];
-        hy[ni] = by[ro + 16 * wn + 8 * ni];
-        hs[ni] = hx[ni] + hy[ni];
-      }
-#pragma unroll
-      for (int mi = 0; mi < 4; ++mi)
-#pragma unroll
-        for (int ni = 0; ni < 2; ++ni) {
-          dmma884(t1[mi][ni][0], t1[mi][ni][1], fx[mi], hx[ni]);
-          dmma884(t2[mi][ni][0], t2[mi][ni][1], fy[mi], hy[ni]);
-          dmma884(t3[mi][ni][0], t3[mi][ni][1], fs[mi], hs[ni]);
-        }
-    }
-    if (it + 1 < n_it) sstore(buf ^ 1);
-    __syncthreads();
-  }
-
-  // (x + i y)(u + i v): Re = xu - yv = T1 - T2,  Im = (x + y)(u + v) - xu - yv = T3 - T1 - T2
-#pragma unroll
-  for (int mi = 0; mi < 4; ++mi) {
-    const int row = ti * kGT + 32 * wm + 8 * mi + g;
-#pragma unroll
-    for (int ni = 0; ni < 2; ++ni) {
-      const int col = tj * kGT + 16 * wn + 8 * ni + 2 * t;
-      double2* c = Cp + (long long)row * a.ldc + col;
-#pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        double2 v = make_double2(a.alpha * (t1[mi][ni][e] - t2[mi][ni][e]),
-                                 a.alpha * (t3[mi][ni][e] - t1[mi][ni][e] - t2[mi][ni][e]));
-        if (a.beta_one) {
-          const double2 o = c[e];
-          v.x += o.x;
-          v.y += o.y;
-        }
-        c[e] = v;
-      }
-    }
-  }
-}
-
-}  // namespace
-
-namespace {
-
 constexpr int kPB = 64;          // diagonal block edge
 constexpr int kPLD = kPB + 1;
 
@@ -287,22 +139,13 @@ __global__ void wc_finish_kernel(const double2* __restrict__ inv, const double* 
   }
 }
 
-template <bool A_KC, bool B_KC>
-cudaError_t zgemm(const ZgemmArgs& a, int m_tiles, int n_tiles, int batch, cudaStream_t s) {
-  if (m_tiles <= 0 || n_tiles <= 0 || a.k <= 0) return cudaSuccess;
-  zgemm_dmma_kernel<A_KC, B_KC><<<dim3(n_tiles, m_tiles, batch), kGThreads, kGSmem, s>>>(a);
-  return cudaGetLastError();
-}
-
 }  // namespace
 
 // Function attributes of every kernel of this file (called before a stream capture: no attribute calls inside it).
 cudaError_t wc_configure() {
   constexpr int kPotrfSmemBytes = 4 * kPB * kPLD * 8;
   cudaError_t e = cudaFuncSetAttribute(potrf_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPotrfSmemBytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(zgemm_dmma_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGSmem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(zgemm_dmma_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGSmem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(zgemm_dmma_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGSmem);
+  if (e == cudaSuccess) e = zgemm_configure();
   return e;
 }
 
@@ -322,6 +165,14 @@ cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const 
   constexpr int kPotrfSmem = 4 * kPB * kPLD * 8;
   cudaError_t e;   // function attributes: wc_configure(), called by the C-ABI layer
 #define WC_TRY(expr) do { e = (expr); if (e != cudaSuccess) return e; } while (0)
+  auto gemm = [&](bool a_kc, bool b_kc, const double2* A, const double2* B, double2* C, long long lda, long long ldb,
+                  long long ldc, long long sA, long long sB, long long sC, int m, int n, int k, double alpha, int beta_one,
+                  int tri) {
+    ZgemmArgs g;
+    g.A = A; g.B = B; g.C = C; g.lda = lda; g.ldb = ldb; g.ldc = ldc; g.sA = sA; g.sB = sB; g.sC = sC;
+    g.m = m; g.n = n; g.k = k; g.batch = n_freq; g.alpha = alpha; g.beta_one = beta_one; g.tri = tri;
+    return launch_zgemm(a_kc, b_kc, g, s);
+  };
   WC_TRY(cudaMemsetAsync(d_info, 0, sizeof(int), s));
   WC_TRY(cudaMemsetAsync(Xbuf, 0, sizeof(double2) * n_freq * sM, s));
   wc_form_eps_kernel<<<dim3(592, n_freq), 256, 0, s>>>(chi0, v, n_m, N, Abuf);
@@ -337,32 +188,30 @@ cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const 
     WC_TRY(cudaGetLastError());
     if (j1 >= nb) break;
     const int m0 = nb - j1;                                                  // block rows j1 .. nb-1
-    ZgemmArgs p0{block(j1, j0), Linv + (long long)j0 * 4096, block(j1, j0), N, 64, N, sM, sL, sM, 64, 1.0, 0, 0};
-    WC_TRY((zgemm<true, true>(p0, m0, 1, n_freq, s)));                      // L[j1.., j0] = A[j1.., j0] Linv_j0^H
-    ZgemmArgs u0{block(j1, j0), block(j1, j0), block(j1, j1), N, N, N, sM, sM, sM, 64, -1.0, 1, 0};
-    WC_TRY((zgemm<true, true>(u0, m0, 1, n_freq, s)));                      // A[j1.., j1] -= L[j1.., j0] L[j1, j0]^H
+    WC_TRY(gemm(true, true, block(j1, j0), Linv + (long long)j0 * 4096, block(j1, j0), N, 64, N, sM, sL, sM,
+                64 * m0, 64, 64, 1.0, 0, 0));                               // L[j1.., j0] = A[j1.., j0] Linv_j0^H
+    WC_TRY(gemm(true, true, block(j1, j0), block(j1, j0), block(j1, j1), N, N, N, sM, sM, sM,
+                64 * m0, 64, 64, -1.0, 1, 0));                              // A[j1.., j1] -= L[j1.., j0] L[j1, j0]^H
     potrf_inv_kernel<<<n_freq, 256, kPotrfSmem, s>>>(block(j1, j1), N, sM, Linv + (long long)j1 * 4096, sL, j1, d_info);
     WC_TRY(cudaGetLastError());
     const int m1 = nb - j1 - 1;                                              // block rows j1+1 .. nb-1
     if (m1 == 0) break;
-    ZgemmArgs p1{block(j1 + 1, j1), Linv + (long long)j1 * 4096, block(j1 + 1, j1), N, 64, N, sM, sL, sM, 64, 1.0, 0, 0};
-    WC_TRY((zgemm<true, true>(p1, m1, 1, n_freq, s)));                      // L[j1+1.., j1] = A[j1+1.., j1] Linv_j1^H
-    ZgemmArgs h{block(j1 + 1, j0), block(j1 + 1, j0), block(j1 + 1, j1 + 1), N, N, N, sM, sM, sM, 128, -1.0, 1, 1};
-    WC_TRY((zgemm<true, true>(h, m1, m1, n_freq, s)));                      // A22 -= L[.., j0:j1] L[.., j0:j1]^H
+    WC_TRY(gemm(true, true, block(j1 + 1, j1), Linv + (long long)j1 * 4096, block(j1 + 1, j1), N, 64, N, sM, sL, sM,
+                64 * m1, 64, 64, 1.0, 0, 0));                               // L[j1+1.., j1] = A[j1+1.., j1] Linv_j1^H
+    WC_TRY(gemm(true, true, block(j1 + 1, j0), block(j1 + 1, j0), block(j1 + 1, j1 + 1), N, N, N, sM, sM, sM,
+                64 * m1, 64 * m1, 128, -1.0, 1, 1));                        // A22 -= L[.., j0:j1] L[.., j0:j1]^H
   }
   // X = L^-1, row block by row block:  X_ii = Linv_ii,  X[i,0:i] = -Linv_ii (L[i,0:i] X[0:i,0:i])
   for (int i = 0; i < nb; ++i) {
     wc_copy_block_kernel<<<n_freq, 256, 0, s>>>(Linv + (long long)i * 4096, sL, Xbuf + (long long)i * 64 * N + i * 64, N, sM);
     WC_TRY(cudaGetLastError());
     if (i == 0) continue;
-    ZgemmArgs t{Abuf + (long long)i * 64 * N, Xbuf, Tbuf, N, N, N, sM, sM, sT, 64 * i, 1.0, 0, 3};
-    WC_TRY((zgemm<true, false>(t, 1, i, n_freq, s)));
-    ZgemmArgs x{Linv + (long long)i * 4096, Tbuf, Xbuf + (long long)i * 64 * N, 64, N, N, sL, sT, sM, 64, -1.0, 0, 0};
-    WC_TRY((zgemm<true, false>(x, 1, i, n_freq, s)));
+    WC_TRY(gemm(true, false, Abuf + (long long)i * 64 * N, Xbuf, Tbuf, N, N, N, sM, sM, sT, 64, 64 * i, 64 * i, 1.0, 0, 3));
+    WC_TRY(gemm(true, false, Linv + (long long)i * 4096, Tbuf, Xbuf + (long long)i * 64 * N, 64, N, N, sL, sT, sM,
+                64, 64 * i, 64, -1.0, 0, 0));
   }
   // eps^-1 = X^H X (lower tiles into Abuf), then W^c
-  ZgemmArgs g{Xbuf, Xbuf, Abuf, N, N, N, sM, sM, sM, N, 1.0, 0, 2};
-  WC_TRY((zgemm<false, false>(g, nb, nb, n_freq, s)));
+  WC_TRY(gemm(false, false, Xbuf, Xbuf, Abuf, N, N, N, sM, sM, sM, N, N, N, 1.0, 0, 2));
   wc_finish_kernel<<<dim3(592, n_freq), 256, 0, s>>>(Abuf, v, n_m, N, wc_out);
   WC_TRY(cudaGetLastError());
 #undef WC_TRY
@@ -411,7 +260,7 @@ size_t rotate_work_elems(int n_m, int n_freq) {
 
 cudaError_t launch_rotate_basis(int n_m, int n_freq, const double2* chi0, const double2* U, double2* out, double2* work,
                                 cudaStream_t s) {
-  const int N = (n_m + 63) / 64 * 64, nb = N / 64;
+  const int N = (n_m + 63) / 64 * 64;
   const long long sM = (long long)N * N;
   double2* Cpad = work;
   double2* Tpad = Cpad + (long long)n_freq * sM;
@@ -420,10 +269,13 @@ cudaError_t launch_rotate_basis(int n_m, int n_freq, const double2* chi0, const 
   wc_pad_kernel<<<dim3(592, n_freq), 256, 0, s>>>(chi0, n_m, N, 0, Cpad);
   wc_pad_kernel<<<dim3(592, 1), 256, 0, s>>>(U, n_m, N, 1, Upad);
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  ZgemmArgs t{Cpad, Upad, Tpad, N, N, N, sM, 0, sM, N, 1.0, 0, 0};                 // T = chi0 U
-  if ((e = zgemm<true, false>(t, nb, nb, n_freq, s)) != cudaSuccess) return e;
-  ZgemmArgs r{Upad, Tpad, Cpad, N, N, N, 0, sM, sM, N, 1.0, 0, 0};                 // U^H T
-  if ((e = zgemm<false, false>(r, nb, nb, n_freq, s)) != cudaSuccess) return e;
+  ZgemmArgs t;                                                                     // T = chi0 U
+  t.A = Cpad; t.B = Upad; t.C = Tpad; t.lda = t.ldb = t.ldc = N; t.sA = sM; t.sB = 0; t.sC = sM;
+  t.m = t.n = t.k = N; t.batch = n_freq;
+  if ((e = launch_zgemm(true, false, t, s)) != cudaSuccess) return e;
+  ZgemmArgs r = t;                                                                 // U^H T
+  r.A = Upad; r.B = Tpad; r.C = Cpad; r.sA = 0; r.sB = sM;
+  if ((e = launch_zgemm(false, false, r, s)) != cudaSuccess) return e;
   wc_unpad_hermitian_kernel<<<dim3(592, n_freq), 256, 0, s>>>(Cpad, n_m, N, out);
   return cudaGetLastError();
 }

@@ -118,3 +118,21 @@ def coulomb_eigenvalues(cfg: WorkloadConfig, seed_offset: int = 0) -> np.ndarray
     mu = np.arange(cfg.n_m, dtype=np.float64)
     v = 4.0 * np.pi / (0.3 + 0.05 * mu) * np.exp(rng.uniform(np.log(0.8), np.log(1.25), cfg.n_m))
     return rng.permutation(v)
+
+
+def synthetic_wc(n_m: int, omega: np.ndarray, seed: int = 0, hermitian: bool = True) -> np.ndarray:
+    """Synthetic screened interaction W^c(i omega_i), complex128 [n_freq][n_m][n_m] (an INPUT of Eq. 22,
+    PAPER.md:197-205, where the paper reads it from the W task): negative semidefinite Hermitian matrices with
+    monotonic damping along the imaginary axis, W_i = -(G_i G_i^H) / (n_m (1 + omega_i^2)) with
+    G_i = G + 0.3 H_i complex Gaussian.  hermitian=False adds a general complex part (tests that must tell W from
+    its transpose)."""
+    rng = np.random.default_rng(BASE_SEED + 2000 + seed)
+    c = lambda *sh: (rng.standard_normal(sh) + 1j * rng.standard_normal(sh)) / np.sqrt(2.0)
+    G = c(n_m, n_m)
+    out = np.empty((len(omega), n_m, n_m), dtype=np.complex128)
+    for i, w in enumerate(np.asarray(omega, dtype=np.float64)):
+        Gi = G + 0.3 * c(n_m, n_m)
+        out[i] = -(Gi @ Gi.conj().T) / (n_m * (1.0 + w * w))
+        if not hermitian:
+            out[i] += 0.2 * c(n_m, n_m) / (1.0 + w * w)
+    return out
