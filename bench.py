@@ -334,6 +334,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
     # next row of the scope table, reported beside the step, not inside `value`: W^c(i omega) from
     # the chi0 just built (Eqs. 10, 19): blocked Cholesky inverse of N_omega matrices of order N_M on the GPU.
     wc = None
+    sigc = None
     if precision == q.PREC_FP64 and not args.no_wc and not light and rank == 0:
         from qsgw_synth import coulomb_eigenvalues, haar_unitary
         import numpy as _np
@@ -365,6 +366,67 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
         rot_ms = timed(lambda: q.chi0_to_coulomb_basis(out, d_U, out=w_out))
         wc["rotate_ms"] = rot_ms
         wc["rotate_value"] = 2 * 8.0 * n_f * float(cfg.n_m) ** 3 / (rot_ms * 1e-3) / 1e12   # two n^3 GEMMs per frequency
+        # next row f2: imaginary-axis correlation self-energy I^c (Eq. 22, Alg. 2) with the W^c just computed:
+        # n_qp = the O-side bands of k-point 0 (the q states), intermediate states = the U-side bands of each k-point
+        if not args.no_sigc:
+            q.wc_from_chi0(out, d_v, out=w_out, info=info)
+            sp0 = prob.spins[0]
+            n_all, n_qp, nks = cfg.n_u, cfg.n_o, min(2, n_k)
+            sctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, cfg.n_k, n_all, n_qp,
+                                 precision=q.PREC_FP64)
+            sctx.set_product_tensor(torch.from_numpy(prob.P).to(dev))
+            d_Cq = torch.from_numpy(sp0.Ck[0]).to(dev)
+            d_eq = torch.from_numpy(sp0.eps_k[0]).to(dev)
+            d_Cqk = torch.from_numpy(sp0.Ckq[:nks]).to(dev)
+            d_eqk = torch.from_numpy(sp0.eps_kq[:nks]).to(dev)
+            sig = torch.zeros((n_qp, n_qp), dtype=torch.complex128, device=dev)
+
+            def sigc_pass(n_sub=None):
+                sig.zero_()
+                na = n_sub or n_all
+                for k in range(nks):
+                    sctx.zmel_build(d_Cqk[k], d_Cq, 0, na, 0, n_qp)
+                    sctx.sigc_imag_accumulate(d_eq, d_eqk[k][:na], w_out, na, n_qp, sig)
+
+            sigc_pass()                                            # allocates the I^c workspace
+            torch.cuda.synchronize(dev)
+            l_s = sctx.kernel_launches
+            ts = []
+            for _ in range(3):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                sigc_pass()
+                e1.record()
+                torch.cuda.synchronize(dev)
+                ts.append(e0.elapsed_time(e1))
+            s_ms = statistics.median(ts)
+            s_launch = (sctx.kernel_launches - l_s) // 3
+            fl_a = 8.0 * nks * sum(m * b * n_all * (b + n_qp) for b, m in zip(cfg.orb_per_site, cfg.pb_per_site))
+            fl_zw = 8.0 * nks * n_qp * n_all * float(cfg.n_m) ** 2 * n_f
+            fl_c = 8.0 * nks * n_qp * n_qp * n_all * float(cfg.n_m)
+            sigc = {"ms": s_ms, "ms_runs": [round(t, 2) for t in ts], "value": (fl_a + fl_zw + fl_c) / (s_ms * 1e-3) / 1e12,
+                    "unit": UNIT, "k_points": nks, "n_all": n_all, "n_qp": n_qp, "gpu_launches": s_launch,
+                    "credited_flop": fl_a + fl_zw + fl_c,
+                    "what": "qsgw_zmel_build + qsgw_sigc_imag_accumulate per k-point with the W^c of this run; credited "
+                            "n_qp n_all N_M^2 n_omega (Table 1, I^c) + n_qp^2 n_all N_M (closing GEMM) + stage (a) "
+                            "complex multiply-adds, 8 real flop each"}
+            if not args.no_accuracy:
+                # accuracy of this path against the oracle on the first 8 intermediate states (bounded CPU time)
+                import oracle
+                n_sub = min(8, n_all)
+                sigc_pass(n_sub)
+                torch.cuda.synchronize(dev)
+                got = sig.cpu().numpy()
+                wc_h = w_out.cpu().numpy()
+                sites = [prob.P_site(s_) for s_ in range(cfg.n_sites)]
+                zs = [oracle.zmel_ref(sites, sp0.Ckq[k][:n_sub], sp0.Ck[0]) for k in range(nks)]
+                ref = oracle.sigc_imag_ref(zs, sp0.eps_k[0], [sp0.eps_kq[k][:n_sub] for k in range(nks)], [wc_h] * nks,
+                                           prob.omega, n_k_norm=cfg.n_k)
+                sigc["accuracy"] = {"rel_frobenius_err": float(_np.linalg.norm(got - ref) / _np.linalg.norm(ref)),
+                                    "against": f"oracle.sigc_imag_ref on the first {n_sub} intermediate states of "
+                                               f"{nks} k-points, W^c from the GPU", "tolerance": 1e-10}
+            sctx.destroy()
+            del d_Cq, d_Cqk, sig
         del w_out, d_v, d_U
     del d_in, out
     torch.cuda.empty_cache()
@@ -483,7 +545,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
 
     return {"mode": mode_name, "value": value, "ms_per_step": ms_total / args.steps, "launches": launches,
             "roofline": roofline, "e2e": e2e, "clocks": clocks, "flops_step": flops_step,
-            "flops_stage_a": fa, "flops_stage_b": fb, "pairs_kept": pairs, "wc": wc, "mixed_selection": mixed_stats,
+            "flops_stage_a": fa, "flops_stage_b": fb, "pairs_kept": pairs, "wc": wc, "sigc": sigc, "mixed_selection": mixed_stats,
             "_out": outs_host}
 
 
@@ -564,6 +626,8 @@ def main_cuda(args):
     for r in res:
         if r.get("wc"):
             line["wc"] = r["wc"]
+        if r.get("sigc"):
+            line["sigc"] = r["sigc"]
         if r is not main:
             line[r["mode"]] = r
     if main.get("mixed_selection"):
@@ -600,6 +664,7 @@ def parse_args(argv=None):
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-wc", action="store_true", help="skip the W^c(i omega) leg reported beside the FP64 step")
+    ap.add_argument("--no-sigc", action="store_true", help="skip the I^c (imaginary-axis self-energy) leg")
     ap.add_argument("--no-accuracy", action="store_true", help="skip the oracle check of the timed outputs")
     ap.add_argument("--no-configs", action="store_true", help="skip the side runs of the other configurations")
     return ap.parse_args(argv)

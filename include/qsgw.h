@@ -246,6 +246,8 @@ int32_t qsgw_mixed_stats(qsgw_ctx* ctx, int64_t* out_launches, int64_t* out_laun
  *   "e2e_groups"      1..4     frequency groups of the last launch of qsgw_chi0_run_host (default 4)
  * ctx == NULL, process-wide:
  *   "wc_graph"        0 | 1 | 2  qsgw_wc_from_chi0: plain launches | CUDA graph with fallback (default) | graph or fail
+ *   "trim_workspace"  bytes    qsgw_wc_from_chi0 / qsgw_chi0_to_coulomb_basis keep their stream-ordered workspace in a
+ *                              private memory pool between calls; this returns all but `bytes` of it to the driver
  * Unknown key or value out of range: QSGW_ERR_INVALID_ARG. */
 int32_t qsgw_set_option(qsgw_ctx* ctx, const char* key, int64_t value);
 

@@ -316,6 +316,37 @@ cudaError_t wc_configure_device(int dev) {
   return e;
 }
 
+// Stream-ordered workspace of the context-free entry points (W^c, basis rotation: ~3 GB at cfg-4 size) comes from a
+// private memory pool per device that keeps its memory between calls: the default pool hands it back to the driver
+// at every synchronisation and the next cudaMallocAsync then costs ~17 ms with the GPU idle (measured, cfg 4).
+// Option "trim_workspace" returns the memory to the driver.
+cudaMemPool_t g_work_pool[qsgw::kMaxDevices] = {};
+std::mutex g_work_pool_mu;
+cudaError_t work_alloc(int dev, void** p, size_t bytes, cudaStream_t st) {
+  cudaMemPool_t pool = nullptr;
+  if (dev >= 0 && dev < qsgw::kMaxDevices) {
+    std::lock_guard<std::mutex> lock(g_work_pool_mu);
+    if (!g_work_pool[dev]) {
+      cudaMemPoolProps props;
+      memset(&props, 0, sizeof(props));
+      props.allocType = cudaMemAllocationTypePinned;
+      props.handleTypes = cudaMemHandleTypeNone;
+      props.location.type = cudaMemLocationTypeDevice;
+      props.location.id = dev;
+      cudaMemPool_t np = nullptr;
+      if (cudaMemPoolCreate(&np, &props) == cudaSuccess) {
+        unsigned long long keep = ~0ull;
+        cudaMemPoolSetAttribute(np, cudaMemPoolAttrReleaseThreshold, &keep);
+        g_work_pool[dev] = np;
+      } else {
+        cudaGetLastError();
+      }
+    }
+    pool = g_work_pool[dev];
+  }
+  return pool ? cudaMallocFromPoolAsync(p, bytes, pool, st) : cudaMallocAsync(p, bytes, st);
+}
+
 int g_wc_graph = 1;     // option "wc_graph": 0 plain launches | 1 graph with fallback | 2 graph or fail
 
 // Internal streams (one per device) and in-flight executable graphs of qsgw_wc_from_chi0 (destroyed once their
@@ -610,6 +641,12 @@ int32_t qsgw_set_option(qsgw_ctx* ctx, const char* key, int64_t value) {
   if (!ctx) {
     g_create_error.clear();
     if (k == "wc_graph" && value >= 0 && value <= 2) { g_wc_graph = (int)value; return QSGW_OK; }
+    if (k == "trim_workspace") {     // hand the cached W^c / rotation workspace of every device back to the driver
+      std::lock_guard<std::mutex> lock(g_work_pool_mu);
+      for (int d = 0; d < qsgw::kMaxDevices; ++d)
+        if (g_work_pool[d]) cudaMemPoolTrimTo(g_work_pool[d], (size_t)(value > 0 ? value : 0));
+      return QSGW_OK;
+    }
     g_create_error = "unknown process-wide option or value out of range: " + k;
     return QSGW_ERR_INVALID_ARG;
   }
@@ -1017,7 +1054,7 @@ int32_t qsgw_wc_from_chi0(int32_t n_m, int32_t n_freq, const void* d_chi0, const
   if (rc != QSGW_OK) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   double2* work = nullptr;
-  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::wc_work_elems(n_m, n_freq), st);
+  cudaError_t e = work_alloc(di.dev, reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::wc_work_elems(n_m, n_freq), st);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("workspace allocation failed: ") + cudaGetErrorString(e); return QSGW_ERR_ALLOC; }
   // The factorisation is a few hundred small dependent launches: they are captured into a CUDA graph on an
   // internal stream of this device (the caller's stream may be the legacy default stream, which cannot be
@@ -1088,7 +1125,7 @@ int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_ch
   if (rc != QSGW_OK) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   double2* work = nullptr;
-  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::rotate_work_elems(n_m, n_freq), st);
+  cudaError_t e = work_alloc(di.dev, reinterpret_cast<void**>(&work), sizeof(double2) * qsgw::rotate_work_elems(n_m, n_freq), st);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("workspace allocation failed: ") + cudaGetErrorString(e); return QSGW_ERR_ALLOC; }
   e = qsgw::launch_rotate_basis(n_m, n_freq, static_cast<const double2*>(d_chi0), static_cast<const double2*>(d_U),
                                 static_cast<double2*>(d_out), work, st);
