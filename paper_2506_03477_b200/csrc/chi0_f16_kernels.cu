@@ -43,15 +43,22 @@ constexpr int kThreadsH = 384;
 constexpr int kPlaneTileH = 128 * 128;   // bytes of one 128-row x (32 h | 32 l) operand tile
 constexpr int kBoxBytes = 64 * 128;      // one TMA box: 64 rows x 128 B
 
+// Two shared-memory rings with their own producer threads: the B tiles (read by the MMAs, released by the MMA
+// commit) and the A-source tiles + weight rows (read by the scaling warps, released as soon as they are in
+// registers), so that the scaling warps' data runs ahead of the MMAs instead of waiting for a slot the tensor pipe
+// still reads (ncu, round 2: 25 % of the scaling warps' time was the wait for the common ring).
 struct HCfg {
-  static constexpr int STAGES = 3;
+  static constexpr int STAGES = 3;                               // B ring
+  static constexpr int ASTAGES = 3;                              // A-source ring
   static constexpr int B_BYTES = 2 * kPlaneTileH;
   static constexpr int A_BYTES = 2 * kPlaneTileH;
   static constexpr int W_BYTES = kPairStage * 4;                 // w_h[32] | w_l[32] halves
-  static constexpr int STAGE_BYTES = B_BYTES + A_BYTES + 1024;   // w slot padded: tiles stay 1024-B aligned
+  static constexpr int ASTAGE_BYTES = A_BYTES + 1024;            // w slot padded: tiles stay 1024-B aligned
+  static constexpr int A_RING_OFF = STAGES * B_BYTES;
+  static constexpr int BAR_OFF = A_RING_OFF + ASTAGES * ASTAGE_BYTES;
   static constexpr int TSLOT_COLS = 64;                          // h_x, h_y, l_x, l_y: 16 columns each
   static constexpr int TSLOTS = 4;
-  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256 + 1024 /*align slack*/;
+  static constexpr int SMEM_BYTES = BAR_OFF + 256 + 1024 /*align slack*/;
 };
 
 // FP8 = true: the two correction products run on kind::f8f6f4 (E5M2) -- 8 f16 + 8 fp8 MMAs per 32 pairs
@@ -63,10 +70,12 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   const uint32_t raw = smem_u32(smem_dyn);
   const uint32_t base = (raw + 1023u) & ~1023u;
   unsigned char* sm = smem_dyn + (base - raw);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::STAGES * C::STAGE_BYTES);
-  uint64_t* full = bars;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::BAR_OFF);
+  uint64_t* full = bars;                     // B ring
   uint64_t* empty = full + C::STAGES;
-  uint64_t* a_full = empty + C::STAGES;
+  uint64_t* s_full = empty + C::STAGES;      // A-source ring
+  uint64_t* s_empty = s_full + C::ASTAGES;
+  uint64_t* a_full = s_empty + C::ASTAGES;   // scaled operand in TMEM
   uint64_t* a_empty = a_full + C::TSLOTS;
   uint64_t* d_full = a_empty + C::TSLOTS;
   uint64_t* d_empty = d_full + 1;
@@ -79,7 +88,6 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   const int chunk = blockIdx.x % a.split, bid = blockIdx.x / a.split;
   const int j = a.j0 + bid % a.n_freq;
   const int2 tt = a.d_tiles[bid / a.n_freq];
-  const bool need_a = FP8 || (tt.x != tt.y);         // f16 split, diagonal tile: the A source is the B tile
   const int s_base = (int)((long long)a.n_stages * chunk / a.split);          // first global stage of this CTA
   const int n_stages = (int)((long long)a.n_stages * (chunk + 1) / a.split) - s_base, win = a.win;
 
@@ -87,7 +95,11 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
     tma_prefetch_desc(&a.tmap);
     for (int s = 0; s < C::STAGES; ++s) {
       mbar_init(&full[s], 1);
-      mbar_init(&empty[s], 9);         // 8 SA warps + the MMA commit
+      mbar_init(&empty[s], 1);         // the MMA commit
+    }
+    for (int s = 0; s < C::ASTAGES; ++s) {
+      mbar_init(&s_full[s], 1);
+      mbar_init(&s_empty[s], 8);       // 8 SA warps
     }
     for (int s = 0; s < C::TSLOTS; ++s) {
       mbar_init(&a_full[s], 8);
@@ -107,38 +119,50 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   if (warp < 4) {
     setmaxnreg_dec<56>();
     if (warp == 0 && lane == 0) {
-      // ------------------------------------------------------------------ TMA producer
-      const __half* wrow = a.wtab16 + (long long)j * a.kpad * 2;
-      const uint32_t bytes = C::B_BYTES + C::W_BYTES + (need_a ? C::A_BYTES : 0);
-      const int n_box = need_a ? 8 : 4;
+      // ------------------------------------------------------------------ TMA producer, B tiles
+      int st = 0, u = 0;
       for (int s = 0; s < n_stages; ++s) {
-        const int st = s % C::STAGES, u = s / C::STAGES;
         if (u > 0) mbar_wait(&empty[st], (u - 1) & 1);
-        unsigned char* sb = sm + st * C::STAGE_BYTES;
-        mbar_arrive_expect_tx(&full[st], bytes);
-        // box i: operand (B | A source), plane (x | y), row half
-        for (int i = 0; i < n_box; ++i) {
-          const int plane = (i >> 1) & 1, rh = i & 1, op = i >> 2;
-          unsigned char* dst = sb + op * C::B_BYTES + plane * kPlaneTileH + rh * kBoxBytes;
-          const int row0 = (op ? tt.x : tt.y) * kTileMx + rh * 64;
-          const CUtensorMap* tm = (FP8 && !op) ? &a.tmap_b : &a.tmap;       // hb8 rows are addressed in bytes
-          const int c0 = (FP8 && !op) ? (s_base + s) * 128 : (s_base + s) * 64;
-          tma_load_3d(dst, tm, &full[st], c0, row0, plane);
+        unsigned char* sb = sm + st * C::B_BYTES;
+        mbar_arrive_expect_tx(&full[st], C::B_BYTES);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {                  // box i: plane (x | y), row half
+          const int plane = i >> 1, rh = i & 1;
+          const CUtensorMap* tm = FP8 ? &a.tmap_b : &a.tmap;                 // hb8 rows are addressed in bytes
+          tma_load_3d(sb + plane * kPlaneTileH + rh * kBoxBytes, tm, &full[st], (s_base + s) * (FP8 ? 128 : 64),
+                      tt.y * kTileMx + rh * 64, plane);
         }
-        bulk_load_1d(sb + C::B_BYTES + C::A_BYTES, wrow + (long long)(s_base + s) * 64, C::W_BYTES, &full[st]);
+        if (++st == C::STAGES) { st = 0; ++u; }
+      }
+    } else if (warp == 2 && lane == 0) {
+      // ------------------------------------------------------------------ TMA producer, A-source tiles + weights
+      const __half* wrow = a.wtab16 + (long long)j * a.kpad * 2;
+      int st = 0, u = 0;
+      for (int s = 0; s < n_stages; ++s) {
+        if (u > 0) mbar_wait(&s_empty[st], (u - 1) & 1);
+        unsigned char* sa = sm + C::A_RING_OFF + st * C::ASTAGE_BYTES;
+        mbar_arrive_expect_tx(&s_full[st], C::A_BYTES + C::W_BYTES);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int plane = i >> 1, rh = i & 1;
+          tma_load_3d(sa + plane * kPlaneTileH + rh * kBoxBytes, &a.tmap, &s_full[st], (s_base + s) * 64,
+                      tt.x * kTileMx + rh * 64, plane);
+        }
+        bulk_load_1d(sa + C::A_BYTES, wrow + (long long)(s_base + s) * 64, C::W_BYTES, &s_full[st]);
+        if (++st == C::ASTAGES) { st = 0; ++u; }
       }
     } else if (warp == 1 && lane == 0) {
       // ------------------------------------------------------------------ MMA issuer
       const uint32_t idesc = umma_idesc_f16(128, 128, 0), idesc_neg = umma_idesc_f16(128, 128, 1);
       const uint32_t idesc8 = umma_idesc_e5m2(128, 128, 0), idesc8_neg = umma_idesc_e5m2(128, 128, 1);
+      int st = 0, u = 0, ts = 0, tu = 0, wpos = 0, widx = 0;     // ring positions / window position without divisions
       for (int s = 0; s < n_stages; ++s) {
-        const int st = s % C::STAGES, u = s / C::STAGES, ts = s % C::TSLOTS, tu = s / C::TSLOTS;
-        const bool win_first = (s % win) == 0;
-        if (win_first && s > 0) mbar_wait(d_empty, ((s / win) - 1) & 1);
+        const bool win_first = wpos == 0;
+        if (win_first && s > 0) mbar_wait(d_empty, (widx - 1) & 1);
         mbar_wait(&full[st], u & 1);
         mbar_wait(&a_full[ts], tu & 1);
         tc_fence_after();
-        const uint32_t sb = base + st * C::STAGE_BYTES;
+        const uint32_t sb = base + st * C::B_BYTES;
         const uint64_t bx = umma_desc_k_sw128(sb), by = umma_desc_k_sw128(sb + kPlaneTileH);
         const uint32_t ab = a_ring + ts * C::TSLOT_COLS;
         if (FP8) {
@@ -184,7 +208,10 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
         }
         umma_commit(&empty[st]);
         umma_commit(&a_empty[ts]);
-        if (((s + 1) % win) == 0 || s == n_stages - 1) umma_commit(d_full);
+        if (++wpos == win) { wpos = 0; ++widx; }
+        if (wpos == 0 || s == n_stages - 1) umma_commit(d_full);
+        if (++st == C::STAGES) { st = 0; ++u; }
+        if (++ts == C::TSLOTS) { ts = 0; ++tu; }
       }
     }
   } else {
@@ -215,14 +242,14 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
       if (lane == 0) mbar_arrive(d_empty);
     };
 
+    int st = 0, u = 0, ts = 0, tu = 0, wpos = 0, widx = 0;
     for (int s = 0; s < n_stages; ++s) {
-      const int st = s % C::STAGES, u = s / C::STAGES, ts = s % C::TSLOTS, tu = s / C::TSLOTS;
-      mbar_wait(&full[st], u & 1);
+      mbar_wait(&s_full[st], u & 1);
       if (tu > 0) mbar_wait(&a_empty[ts], (tu - 1) & 1);
       tc_fence_after();
-      const uint32_t sb = base + st * C::STAGE_BYTES;
-      const uint32_t src = (need_a ? sb + C::B_BYTES : sb) + (uint32_t)row * 128u;
-      const uint32_t swp = sb + C::B_BYTES + C::A_BYTES + 32u * (uint32_t)h;   // this thread's 16 pairs
+      const uint32_t sb = base + C::A_RING_OFF + st * C::ASTAGE_BYTES;
+      const uint32_t src = sb + (uint32_t)row * 128u;
+      const uint32_t swp = sb + C::A_BYTES + 32u * (uint32_t)h;                // this thread's 16 pairs
       const uint32_t tdst = a_ring + ts * C::TSLOT_COLS + 8 * h + lane_base;
       uint32_t wh[8], wl[8];
 #pragma unroll
@@ -272,11 +299,14 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
       __syncwarp();
       if (lane == 0) {
         mbar_arrive(&a_full[ts]);
-        mbar_arrive(&empty[st]);
+        mbar_arrive(&s_empty[st]);
       }
-      if (s >= 1 && (s % win) == 0) drain(s / win - 1);   // stage s-1 closed a window
+      if (s >= 1 && wpos == 0) drain(widx - 1);            // stage s-1 closed a window
+      if (++wpos == win) { wpos = 0; ++widx; }
+      if (++st == C::ASTAGES) { st = 0; ++u; }
+      if (++ts == C::TSLOTS) { ts = 0; ++tu; }
     }
-    drain((n_stages - 1) / win);
+    drain(wpos == 0 ? widx - 1 : widx);
 
     // FP32 window sums (in units 2^(2S) sigma_j) -> FP64 accumulators (exclusive owner of (tile, j))
     const double sc = a.wscale[j];     // the batches' 2^(-2S) are folded into the weights (pair_weights_kernel)
