@@ -2,8 +2,8 @@
 """bench.py -- chi0(q, i*omega) build throughput on B200 (BASELINE.json metric).
 
 A "step" is one pass of the whole hot path over one synthetic workload: for every spin channel
-and k-point {qsgw_zmel_build, qsgw_chi0_accumulate} over all band batches, then
-qsgw_chi0_finalize.  Default workload: cfg 4 (superlattice-scale cell),
+and k-point {qsgw_zmel_build, qsgw_chi0_accumulate} over all band batches (driven by
+qsgw_chi0_add_kpoints), then qsgw_chi0_finalize.  Default workload: cfg 4 (superlattice-scale cell),
 the configuration the BASELINE.json targets are quoted on.
 
   value      credited complex-arithmetic TFLOP/s (8 real flop per complex multiply-add; stage (a)
@@ -280,9 +280,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
     def step():
         for s in range(n_spin):
             ctx.reset()
-            Ck, Ckq, ek, fk, ekq, fkq = d_in[s]
-            for k in range(n_k):
-                ctx.chi0_add_kpoint(Ck[k], Ckq[k], ek[k], fk[k], ekq[k], fkq[k])
+            ctx.chi0_add_kpoints(*d_in[s])        # all k-points: one stage (a) + weight launch per workspace group
             ctx.chi0_finalize(out)
 
     def barrier():
@@ -325,9 +323,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
         for s in range(n_spin):
             if n_spin > 1:               # `out` holds the last spin only: rebuild this spin once, untimed
                 ctx.reset()
-                Ck, Ckq, ek, fk, ekq, fkq = d_in[s]
-                for k in range(n_k):
-                    ctx.chi0_add_kpoint(Ck[k], Ckq[k], ek[k], fk[k], ekq[k], fkq[k])
+                ctx.chi0_add_kpoints(*d_in[s])
                 ctx.chi0_finalize(out)
             outs_host.append(out.cpu().numpy())
     ctx.destroy()

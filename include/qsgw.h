@@ -130,6 +130,17 @@ int32_t qsgw_chi0_add_kpoint(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, cons
                              const double* d_eps_kq, const double* d_f_kq, int32_t n_o_total,
                              int32_t n_u_total);
 
+/* The same for n_kpoints k-points at once (equivalent to n_kpoints calls of qsgw_chi0_add_kpoint): k-point k reads
+ * d_Ck + k*stride_k and d_Ckq + k*stride_kq (strides in complex elements; a contiguous [k][band][orbital] array has
+ * stride n_bands*ld) and rows k of d_eps_k, d_f_k (float64 [n_kpoints][n_o_total]) and d_eps_kq, d_f_kq
+ * ([n_kpoints][n_u_total]).  When one k-point fits a band batch (n_o_total <= max_n_o, n_u_total <= max_n_u) the
+ * k-points that fit the z workspace together are built by ONE stage (a) launch and ONE weight launch: small cells with
+ * many k-points stop being bound by launch latency. */
+int32_t qsgw_chi0_add_kpoints(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, int64_t stride_k, const void* d_Ckq,
+                              int64_t ld_kq, int64_t stride_kq, const double* d_eps_k, const double* d_f_k,
+                              const double* d_eps_kq, const double* d_f_kq, int32_t n_o_total, int32_t n_u_total,
+                              int32_t n_kpoints);
+
 /* chi0[j][I][J] = acc/N_k as a full Hermitian matrix: d_chi0_out complex128
  * [n_freq][N_M][N_M], row-major.  May be called again after more accumulation. */
 int32_t qsgw_chi0_finalize(qsgw_ctx* ctx, void* d_chi0_out);

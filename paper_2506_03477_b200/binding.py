@@ -53,6 +53,7 @@ def lib() -> C.CDLL:
     L.qsgw_zmel_build.argtypes = [vp, vp, i64, vp, i64, i32, i32, i32, i32, vp]
     L.qsgw_chi0_accumulate.argtypes = [vp, vp, dp, dp, dp, dp, i32, i32]
     L.qsgw_chi0_add_kpoint.argtypes = [vp, vp, i64, vp, i64, dp, dp, dp, dp, i32, i32]
+    L.qsgw_chi0_add_kpoints.argtypes = [vp, vp, i64, i64, vp, i64, i64, dp, dp, dp, dp, i32, i32, i32]
     L.qsgw_chi0_finalize.argtypes = [vp, vp]
     L.qsgw_reset.argtypes = [vp]
     L.qsgw_sync.argtypes = [vp]
@@ -65,7 +66,7 @@ def lib() -> C.CDLL:
     for name in ("qsgw_create", "qsgw_set_product_tensor", "qsgw_zmel_build", "qsgw_chi0_accumulate",
                  "qsgw_chi0_add_kpoint", "qsgw_chi0_finalize", "qsgw_reset", "qsgw_sync",
                  "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_set_option", "qsgw_mixed_stats", "qsgw_wc_from_chi0",
-                 "qsgw_sigc_imag_accumulate",
+                 "qsgw_sigc_imag_accumulate", "qsgw_chi0_add_kpoints",
                  "qsgw_chi0_to_coulomb_basis"):
         getattr(L, name).restype = i32
     for name in ("qsgw_last_error", "qsgw_last_create_error", "qsgw_version"):
@@ -187,6 +188,18 @@ class Chi0Context:
             self._h, _ptr(d_Ck, torch.complex128), d_Ck.shape[-1], _ptr(d_Ckq, torch.complex128),
             d_Ckq.shape[-1], _ptr(d_eps_k, f64), _ptr(d_f_k, f64), _ptr(d_eps_kq, f64),
             _ptr(d_f_kq, f64), d_Ck.shape[0], d_Ckq.shape[0]))
+
+    def chi0_add_kpoints(self, d_Ck, d_Ckq, d_eps_k, d_f_k, d_eps_kq, d_f_kq):
+        """All k-points of contiguous arrays d_Ck [n_k][n_o][N_b], d_Ckq [n_k][n_u][N_b], d_eps_k/d_f_k [n_k][n_o],
+        d_eps_kq/d_f_kq [n_k][n_u] in one call."""
+        import torch
+        f64 = torch.float64
+        n_k, n_o, ld = d_Ck.shape
+        n_u = d_Ckq.shape[1]
+        self._check(self._L.qsgw_chi0_add_kpoints(
+            self._h, _ptr(d_Ck, torch.complex128), ld, n_o * ld, _ptr(d_Ckq, torch.complex128), d_Ckq.shape[2],
+            n_u * d_Ckq.shape[2], _ptr(d_eps_k, f64), _ptr(d_f_k, f64), _ptr(d_eps_kq, f64), _ptr(d_f_kq, f64),
+            n_o, n_u, n_k))
 
     def chi0_finalize(self, d_chi0_out=None):
         import torch

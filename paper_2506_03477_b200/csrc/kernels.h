@@ -41,7 +41,11 @@ struct ZmelArgs {
   double* zws;           // FP64 workspace (see above)
   long long kpad;
   int ncg;
-  float* zmax = nullptr; // optional: atomicMax of |Re z|, |Im z| over the batch (FP16-split mixed mode)
+  float* zmax = nullptr; // optional: atomicMax of |Re z|, |Im z| over the batch (FP16-split mixed mode); [n_batch]
+  // several k-points per launch (blockIdx.z): k-point b reads Ck + b*Ck_bs, Ckq + b*Ckq_bs (complex elements) and
+  // writes the workspace slot at pair offset b*z_bs
+  int n_batch = 1;
+  long long Ck_bs = 0, Ckq_bs = 0, z_bs = 0;
   int kt = 0;            // DMMA kernel: padded contraction length, max over column groups of sum_seg pad4(b_seg)
   int n_sm = 148;        // SMs of the context's device
 };
@@ -53,10 +57,13 @@ cudaError_t launch_z_export(const double* zws, long long kpad, int ncg, int n_m,
                             double2* out, cudaStream_t s);
 cudaError_t launch_z_import(double* zws, long long kpad, int ncg, int n_m, long long n_pairs,
                             const double2* in, float* zmax /*optional*/, cudaStream_t s);
+// n_batch k-points per launch: k-point b reads eps_k + b*n_o, ..., eps_kq + b*n_u, ..., zmax[b] and writes the table
+// columns [b*n_pairs_padded, (b+1)*n_pairs_padded)
 cudaError_t launch_pair_weights(const double* eps_k, const double* f_k, const double* eps_kq,
                                 const double* f_kq, int n_o, int n_u, const double* d_omega, int n_freq,
                                 double occ_tol, double* wtab, long long kpad, long long n_pairs_padded,
-                                const float* zmax /*optional: fold 2^(-2S) of the batch's FP16 scale*/, cudaStream_t s);
+                                const float* zmax /*optional: fold 2^(-2S) of the batch's FP16 scale*/, int n_batch,
+                                cudaStream_t s);
 
 struct Chi0F64Args {
   CUtensorMap tmap_z;    // 4-D FLOAT64 {16, kpad, ncg, 2}, box {16, KP, 4, 2}, SWIZZLE_128B
@@ -129,9 +136,10 @@ cudaError_t chi0_f16_configure();
 // ctl->use_fp8 first and the variant that was not selected returns immediately (the selection is made on the
 // device from the weights of the staged pairs, see weights_scale_hl16_kernel: no host synchronisation).
 cudaError_t launch_chi0_f16(const Chi0F16Args& a, cudaStream_t s);
+// n_batch batches of n_pairs pairs at pair offsets b*z_bs (a multiple of 32), scales zmax[b]
 cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs, void* zhl,
-                             void* zhb8 /*optional FP8-variant B rows*/, int n_m_pad, const float* zmax,
-                             cudaStream_t s);
+                             void* zhb8 /*optional FP8-variant B rows*/, int n_m_pad, const float* zmax, int n_batch,
+                             long long z_bs, cudaStream_t s);
 cudaError_t launch_z_export_hl16(const void* zhl, long long kpad, int n_m_pad, int n_m, long long n_pairs,
                                  const float* zmax, double2* out, cudaStream_t s);
 cudaError_t launch_weights_scale_hl16(const double* wtab, void* wtab16, double* wscale, long long kpad, long long n_pad,

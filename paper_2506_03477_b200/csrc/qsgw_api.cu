@@ -104,6 +104,8 @@ struct qsgw_ctx {
   long long batch_pad = 0;      // padded pairs of the largest band batch
   long long stage_cap = 0;      // staged pairs that trigger a flush (<= kpad; option "stage_batches")
   long long z_off = 0;          // workspace slot of the batch the last zmel_build wrote
+  int z_zi = 0;                 // ... and the index of its FP16 scale in d_zmax
+  int zslot = 0;                // batches staged since the last flush (next free index of d_zmax)
   int e2e_groups = 4;           // frequency groups of the last flush of qsgw_chi0_run_host
   // I^c workspace (qsgw_sigc_imag_accumulate; allocated by its first call)
   double2* d_sz = nullptr;      // z of the batch, complex128 [pairs][N_M]
@@ -544,7 +546,7 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     QSGW_TRY_ALLOC(dev_alloc(c, reinterpret_cast<unsigned char**>(&c->d_zhl), zhl_bytes));
     QSGW_TRY_ALLOC(dev_alloc(c, reinterpret_cast<unsigned char**>(&c->d_zhb8), zhl_bytes));
     QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wscale, (size_t)c->n_freq));
-    QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zmax, (size_t)1));
+    QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zmax, (size_t)(c->kpad / qsgw::kPairAlign + 1)));   // one scale per staged batch
     QSGW_TRY_ALLOC(dev_alloc(c, &c->d_ctl, (size_t)1));
   }
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab, (size_t)c->n_freq * c->kpad));
@@ -571,7 +573,7 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zhl, 0, zhl_bytes, st));
     QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zhb8, 0, zhl_bytes, st));
     QSGW_TRY_CUDA(cudaMemsetAsync(c->d_wscale, 0, sizeof(double) * c->n_freq, st));
-    QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zmax, 0, sizeof(float), st));
+    QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zmax, 0, sizeof(float) * (c->kpad / qsgw::kPairAlign + 1), st));
     QSGW_TRY_CUDA(upload_ctl(c));
     QSGW_TRY_CUDA(qsgw::chi0_f16_configure());
   }
@@ -718,7 +720,9 @@ int32_t qsgw_reset(qsgw_ctx* ctx) {
   if (ctx->state != ST_CREATED) ctx->state = ST_READY;
   ctx->pairs = 0;
   ctx->fill = 0;                   // staged, not yet accumulated batches are dropped with the accumulator
+  ctx->zslot = 0;
   ctx->z_off = 0;
+  ctx->z_zi = 0;
   ctx->err.clear();
   return QSGW_OK;
 }
@@ -737,6 +741,58 @@ static int check_batch(qsgw_ctx* ctx, int n_o, int n_u) {
   return QSGW_OK;
 }
 
+// Stage (a) for `n_batch` k-points of equal band batch in ONE launch (grid.z = k-point): k-point b reads
+// Ck + b*ck_bs, Ckq + b*ckq_bs and fills the workspace slot at pair offset off + b*n_pad with batch-scale index
+// zi + b.  The caller has made room ([off, off + n_batch*n_pad) <= kpad).
+static int build_batches(qsgw_ctx* ctx, const double2* Ck, long long ld_k, long long ck_bs, const double2* Ckq,
+                         long long ld_kq, long long ckq_bs, int n_begin, int n_o, int np_begin, int n_u, int n_batch,
+                         long long off, long long n_pad, int zi) {
+  qsgw::ZmelArgs a;
+  a.st.n_sites = ctx->n_sites;
+  a.st.n_b = ctx->n_b;
+  a.st.n_m = ctx->n_m;
+  a.st.b_max = ctx->b_max;
+  a.st.d_pb_site = ctx->d_pb_site;
+  a.st.d_pb_off = ctx->d_pb_off;
+  a.st.d_orb_off = ctx->d_orb_off;
+  a.st.d_p_off = ctx->d_p_off;
+  a.P = ctx->d_P;
+  a.Ck = Ck;
+  a.ld_k = ld_k;
+  a.Ckq = Ckq;
+  a.ld_kq = ld_kq;
+  a.n_begin = n_begin;
+  a.n_o = n_o;
+  a.np_begin = np_begin;
+  a.n_u = n_u;
+  a.zws = ctx->d_zws + off * qsgw::kCG;
+  a.kpad = ctx->kpad;
+  a.ncg = ctx->ncg;
+  a.kt = ctx->zmel_kt;
+  a.n_sm = ctx->n_sm;
+  a.n_batch = n_batch;
+  a.Ck_bs = ck_bs;
+  a.Ckq_bs = ckq_bs;
+  a.z_bs = n_pad;
+  cudaError_t e;
+  if (ctx->f16) {
+    a.zmax = ctx->d_zmax + zi;
+    e = cudaMemsetAsync(a.zmax, 0, sizeof(float) * n_batch, ctx->stream);
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "reset of the batch maximum");
+  }
+  {
+    StageScope ts(ctx, QSGW_STAGE_ZMEL);
+    e = ctx->zmel_kt ? qsgw::launch_zmel_dmma(a, ctx->stream) : qsgw::launch_zmel_f64(a, ctx->stream);
+    if (e == cudaSuccess && ctx->f16)
+      e = qsgw::launch_z_to_hl16(a.zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u,
+                                 hl_slot(ctx->d_zhl, off), hl_slot(ctx->d_zhb8, off), ctx->n_m_pad, a.zmax, n_batch,
+                                 n_pad, ctx->stream);
+  }
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "zmel kernel launch");
+  ctx->launches += ctx->f16 ? 2 : 1;
+  return QSGW_OK;
+}
+
 int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const void* d_Ckq, int64_t ld_kq,
                         int32_t n_begin, int32_t n_o, int32_t np_begin, int32_t n_u, void* d_z_out) {
   if (!ctx) return QSGW_ERR_INVALID_ARG;
@@ -749,60 +805,28 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
   if (rc != QSGW_OK) return rc;
 
   long long off = 0;
-  rc = stage_slot(ctx, (long long)n_o * n_u, &off);
+  const long long n_pairs = (long long)n_o * n_u;
+  rc = stage_slot(ctx, n_pairs, &off);
   if (rc != QSGW_OK) return rc;
-  qsgw::ZmelArgs a;
-  a.st.n_sites = ctx->n_sites;
-  a.st.n_b = ctx->n_b;
-  a.st.n_m = ctx->n_m;
-  a.st.b_max = ctx->b_max;
-  a.st.d_pb_site = ctx->d_pb_site;
-  a.st.d_pb_off = ctx->d_pb_off;
-  a.st.d_orb_off = ctx->d_orb_off;
-  a.st.d_p_off = ctx->d_p_off;
-  a.P = ctx->d_P;
-  a.Ck = static_cast<const double2*>(d_Ck);
-  a.ld_k = ld_k;
-  a.Ckq = static_cast<const double2*>(d_Ckq);
-  a.ld_kq = ld_kq;
-  a.n_begin = n_begin;
-  a.n_o = n_o;
-  a.np_begin = np_begin;
-  a.n_u = n_u;
-  a.zws = ctx->d_zws + off * qsgw::kCG;
-  a.kpad = ctx->kpad;
-  a.ncg = ctx->ncg;
-  a.kt = ctx->zmel_kt;
-  a.n_sm = ctx->n_sm;
+  const int zi = ctx->zslot;
+  rc = build_batches(ctx, static_cast<const double2*>(d_Ck), ld_k, 0, static_cast<const double2*>(d_Ckq), ld_kq, 0,
+                     n_begin, n_o, np_begin, n_u, 1, off, round_up(n_pairs, qsgw::kPairAlign), zi);
+  if (rc != QSGW_OK) return rc;
   cudaError_t e;
-  if (ctx->f16) {
-    a.zmax = ctx->d_zmax;
-    e = cudaMemsetAsync(ctx->d_zmax, 0, sizeof(float), ctx->stream);
-    if (e != cudaSuccess) return ctx->cuda_fail(e, "reset of the batch maximum");
-  }
-  {
-    StageScope ts(ctx, QSGW_STAGE_ZMEL);
-    e = ctx->zmel_kt ? qsgw::launch_zmel_dmma(a, ctx->stream) : qsgw::launch_zmel_f64(a, ctx->stream);
-    if (e == cudaSuccess && ctx->f16)
-      e = qsgw::launch_z_to_hl16(a.zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u,
-                                 hl_slot(ctx->d_zhl, off), hl_slot(ctx->d_zhb8, off), ctx->n_m_pad, ctx->d_zmax,
-                                 ctx->stream);
-  }
-  if (e != cudaSuccess) return ctx->cuda_fail(e, "zmel kernel launch");
-  ctx->launches += ctx->f16 ? 2 : 1;
   if (d_z_out) {
     if (ctx->f16)
-      e = qsgw::launch_z_export_hl16(hl_slot(ctx->d_zhl, off), ctx->kpad, ctx->n_m_pad, ctx->n_m, (long long)n_o * n_u, ctx->d_zmax,
-                                     static_cast<double2*>(d_z_out), ctx->stream);
+      e = qsgw::launch_z_export_hl16(hl_slot(ctx->d_zhl, off), ctx->kpad, ctx->n_m_pad, ctx->n_m, n_pairs,
+                                     ctx->d_zmax + zi, static_cast<double2*>(d_z_out), ctx->stream);
     else
-      e = qsgw::launch_z_export(a.zws, ctx->kpad, ctx->ncg, ctx->n_m, (long long)n_o * n_u,
-                              static_cast<double2*>(d_z_out), ctx->stream);
+      e = qsgw::launch_z_export(ctx->d_zws + off * qsgw::kCG, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs,
+                                static_cast<double2*>(d_z_out), ctx->stream);
     if (e != cudaSuccess) return ctx->cuda_fail(e, "z export kernel launch");
     ctx->launches += 1;
   }
   ctx->last_n_o = n_o;
   ctx->last_n_u = n_u;
   ctx->z_off = off;
+  ctx->z_zi = zi;
   ctx->state = ST_Z_BUILT;
   ctx->err.clear();
   return QSGW_OK;
@@ -814,7 +838,7 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
 static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
   if (ctx->fill == 0) return QSGW_OK;
   const long long n_pad = ctx->fill;
-  if (last) ctx->fill = 0;
+  if (last) { ctx->fill = 0; ctx->zslot = 0; }
   cudaError_t e;
   if (ctx->f16) {
     if (first) {
@@ -895,17 +919,20 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
   const long long n_pairs = (long long)n_o * n_u;
   const long long n_pad = round_up(n_pairs, qsgw::kPairAlign);
   long long off = 0;
+  int zi = 0;
   cudaError_t e = cudaSuccess;
   if (d_z) {
     rc = stage_slot(ctx, n_pairs, &off);
     if (rc != QSGW_OK) return rc;
-    e = ctx->f16 ? cudaMemsetAsync(ctx->d_zmax, 0, sizeof(float), ctx->stream) : cudaSuccess;
+    zi = ctx->zslot;
+    float* zmax = ctx->f16 ? ctx->d_zmax + zi : nullptr;
+    e = ctx->f16 ? cudaMemsetAsync(zmax, 0, sizeof(float), ctx->stream) : cudaSuccess;
     if (e == cudaSuccess)
       e = qsgw::launch_z_import(ctx->d_zws + off * qsgw::kCG, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs,
-                                static_cast<const double2*>(d_z), ctx->f16 ? ctx->d_zmax : nullptr, ctx->stream);
+                                static_cast<const double2*>(d_z), zmax, ctx->stream);
     if (e == cudaSuccess && ctx->f16) {
       e = qsgw::launch_z_to_hl16(ctx->d_zws + off * qsgw::kCG, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs,
-                                 hl_slot(ctx->d_zhl, off), hl_slot(ctx->d_zhb8, off), ctx->n_m_pad, ctx->d_zmax,
+                                 hl_slot(ctx->d_zhl, off), hl_slot(ctx->d_zhb8, off), ctx->n_m_pad, zmax, 1, n_pad,
                                  ctx->stream);
       ctx->launches += 1;
     }
@@ -922,6 +949,7 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
     // released the slots below it: their weights are zeroed so that the rows [0, z_off) of this flush contribute
     // exactly nothing (the z rows there are a stale, already accumulated batch).
     off = ctx->z_off;
+    zi = ctx->z_zi;
     if (off != ctx->fill) {
       e = cudaMemset2DAsync(ctx->d_wtab, sizeof(double) * ctx->kpad, 0, sizeof(double) * off, ctx->n_freq, ctx->stream);
       if (e != cudaSuccess) return ctx->cuda_fail(e, "clearing the weights of released workspace slots");
@@ -931,13 +959,14 @@ int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps
     StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
     e = qsgw::launch_pair_weights(d_eps_k, d_f_k, d_eps_kq, d_f_kq, n_o, n_u, ctx->d_omega, ctx->n_freq,
                                   ctx->occ_tol, ctx->d_wtab + off, ctx->kpad, n_pad,
-                                  ctx->f16 ? ctx->d_zmax : nullptr, ctx->stream);
+                                  ctx->f16 ? ctx->d_zmax + zi : nullptr, 1, ctx->stream);
   }
   if (e != cudaSuccess) return ctx->cuda_fail(e, "pair weights kernel launch");
   ctx->launches += 1;
   ctx->pairs += n_pairs;
   ctx->state = ST_READY;   // the batch is staged
   ctx->fill = off + n_pad;
+  ctx->zslot = zi + 1;
   ctx->err.clear();
   return QSGW_OK;
 }
@@ -958,6 +987,71 @@ int32_t qsgw_chi0_add_kpoint(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, cons
       if (rc != QSGW_OK) return rc;
     }
   }
+  return QSGW_OK;
+}
+
+int32_t qsgw_chi0_add_kpoints(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, int64_t stride_k, const void* d_Ckq,
+                              int64_t ld_kq, int64_t stride_kq, const double* d_eps_k, const double* d_f_k,
+                              const double* d_eps_kq, const double* d_f_kq, int32_t n_o_total, int32_t n_u_total,
+                              int32_t n_kpoints) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  if (ctx->state == ST_CREATED) return ctx->fail(QSGW_ERR_STATE, "set_product_tensor must precede chi0_add_kpoints");
+  if (n_o_total < 1 || n_u_total < 1 || n_kpoints < 1)
+    return ctx->fail(QSGW_ERR_SHAPE, "n_o_total, n_u_total and n_kpoints must be positive");
+  if (!d_Ck || !d_Ckq || !d_eps_k || !d_f_k || !d_eps_kq || !d_f_kq) return ctx->fail(QSGW_ERR_INVALID_ARG, "NULL argument");
+  if (ld_k < ctx->n_b || ld_kq < ctx->n_b)
+    return ctx->fail(QSGW_ERR_INVALID_ARG, "leading dimension smaller than N_b=%d", ctx->n_b);
+  if (stride_k < 0 || stride_kq < 0) return ctx->fail(QSGW_ERR_INVALID_ARG, "negative k-point stride");
+  const double2* Ck = static_cast<const double2*>(d_Ck);
+  const double2* Ckq = static_cast<const double2*>(d_Ckq);
+  const long long n_pairs = (long long)n_o_total * n_u_total;
+  const long long n_pad = round_up(n_pairs, qsgw::kPairAlign);
+  if (n_o_total > ctx->max_n_o || n_u_total > ctx->max_n_u || n_pad > ctx->stage_cap) {
+    // the k-point does not fit one band batch: k-point by k-point through the band-batch loop
+    for (int k = 0; k < n_kpoints; ++k) {
+      int rc = qsgw_chi0_add_kpoint(ctx, Ck + (long long)k * stride_k, ld_k, Ckq + (long long)k * stride_kq, ld_kq,
+                                    d_eps_k + (long long)k * n_o_total, d_f_k + (long long)k * n_o_total,
+                                    d_eps_kq + (long long)k * n_u_total, d_f_kq + (long long)k * n_u_total, n_o_total,
+                                    n_u_total);
+      if (rc != QSGW_OK) return rc;
+    }
+    return QSGW_OK;
+  }
+  // groups of k-points that fit the staging workspace: ONE stage (a) launch (+ conversion) and ONE weight launch each
+  for (int k0 = 0; k0 < n_kpoints;) {
+    if (ctx->fill + n_pad > ctx->stage_cap) {
+      int rc = flush_pending(ctx);
+      if (rc != QSGW_OK) return rc;
+    }
+    long long room = (ctx->stage_cap - ctx->fill) / n_pad;
+    int g = (int)(room < (long long)(n_kpoints - k0) ? room : (long long)(n_kpoints - k0));
+    if (g > 65535) g = 65535;           // grid.z
+    const long long off = ctx->fill;
+    const int zi = ctx->zslot;
+    int rc = build_batches(ctx, Ck + (long long)k0 * stride_k, ld_k, stride_k, Ckq + (long long)k0 * stride_kq, ld_kq,
+                           stride_kq, 0, n_o_total, 0, n_u_total, g, off, n_pad, zi);
+    if (rc != QSGW_OK) return rc;
+    cudaError_t e;
+    {
+      StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
+      e = qsgw::launch_pair_weights(d_eps_k + (long long)k0 * n_o_total, d_f_k + (long long)k0 * n_o_total,
+                                    d_eps_kq + (long long)k0 * n_u_total, d_f_kq + (long long)k0 * n_u_total, n_o_total,
+                                    n_u_total, ctx->d_omega, ctx->n_freq, ctx->occ_tol, ctx->d_wtab + off, ctx->kpad,
+                                    n_pad, ctx->f16 ? ctx->d_zmax + zi : nullptr, g, ctx->stream);
+    }
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "pair weights kernel launch");
+    ctx->launches += 1;
+    ctx->pairs += n_pairs * g;
+    ctx->fill = off + n_pad * g;
+    ctx->zslot = zi + g;
+    ctx->last_n_o = n_o_total;
+    ctx->last_n_u = n_u_total;
+    ctx->z_off = off + n_pad * (g - 1);
+    ctx->z_zi = zi + g - 1;
+    ctx->state = ST_READY;
+    k0 += g;
+  }
+  ctx->err.clear();
   return QSGW_OK;
 }
 
@@ -1010,7 +1104,7 @@ int32_t qsgw_sigc_imag_accumulate(qsgw_ctx* ctx, const void* d_z, const double* 
   if (!d_z) {
     if (ctx->f16)
       e = qsgw::launch_z_export_hl16(hl_slot(ctx->d_zhl, ctx->z_off), ctx->kpad, ctx->n_m_pad, ctx->n_m, n_pairs,
-                                     ctx->d_zmax, ctx->d_sz, ctx->stream);
+                                     ctx->d_zmax + ctx->z_zi, ctx->d_sz, ctx->stream);
     else
       e = qsgw::launch_z_export(ctx->d_zws + ctx->z_off * qsgw::kCG, ctx->kpad, ctx->ncg, ctx->n_m, n_pairs, ctx->d_sz,
                                 ctx->stream);
@@ -1144,8 +1238,20 @@ int32_t qsgw_chi0_run_host(qsgw_ctx* c, const void* h_P, const void* h_Ck, const
   cudaStream_t st = c->stream;
   qsgw_ctx::HostRun& H = c->hr;
   const int nb = c->n_b, nm = c->n_m;
-  const size_t ck_e = (size_t)n_o * nb, ckq_e = (size_t)n_u * nb;
-  const size_t e_len = 2 * (size_t)n_o + 2 * (size_t)n_u;
+  // k-points travel in groups: as many as one multi-k launch of qsgw_chi0_add_kpoints takes (bounded to 64 MB of
+  // staging per array), one k-point at a time when a k-point needs the band-batch loop
+  const long long n_pad1 = round_up((long long)n_o * n_u, qsgw::kPairAlign);
+  int G = 1;
+  if (n_o <= c->max_n_o && n_u <= c->max_n_u && n_pad1 <= c->stage_cap) {
+    long long g = c->stage_cap / n_pad1;
+    const long long cap = (64ll << 20) / (long long)(sizeof(double2) * (size_t)(n_o > n_u ? n_o : n_u) * nb);
+    if (g > cap) g = cap;
+    if (g > n_k_points) g = n_k_points;
+    G = (int)(g < 1 ? 1 : g);
+  }
+  const size_t ck_1 = (size_t)n_o * nb, ckq_1 = (size_t)n_u * nb;
+  const size_t ck_e = ck_1 * G, ckq_e = ckq_1 * G;
+  const size_t e_len = (2 * (size_t)n_o + 2 * (size_t)n_u) * G;
   const size_t out_e = (size_t)c->n_freq * nm * nm;
   const long long launches0 = c->launches;
 #define QSGW_H(expr)                                                                   \
@@ -1174,16 +1280,24 @@ int32_t qsgw_chi0_run_host(qsgw_ctx* c, const void* h_P, const void* h_Ck, const
   QSGW_H(cudaMemcpyAsync(H.dP, h_P, sizeof(double2) * c->p_elems, cudaMemcpyHostToDevice, st));
   rc = qsgw_set_product_tensor(c, H.dP);
   if (rc != QSGW_OK) return rc;
-  for (int k = 0; k < n_k_points; ++k) {
-    const int b = k & 1;
-    if (k >= 2) QSGW_H(cudaEventSynchronize(H.done[b]));   // keeps the host at most two k-points ahead
-    QSGW_H(cudaMemcpyAsync(H.dCk[b], static_cast<const double2*>(h_Ck) + (size_t)k * ck_e, sizeof(double2) * ck_e, cudaMemcpyHostToDevice, st));
-    QSGW_H(cudaMemcpyAsync(H.dCkq[b], static_cast<const double2*>(h_Ckq) + (size_t)k * ckq_e, sizeof(double2) * ckq_e, cudaMemcpyHostToDevice, st));
-    QSGW_H(cudaMemcpyAsync(H.dE[b], h_eps_k + (size_t)k * n_o, sizeof(double) * n_o, cudaMemcpyHostToDevice, st));
-    QSGW_H(cudaMemcpyAsync(H.dE[b] + n_o, h_f_k + (size_t)k * n_o, sizeof(double) * n_o, cudaMemcpyHostToDevice, st));
-    QSGW_H(cudaMemcpyAsync(H.dE[b] + 2 * n_o, h_eps_kq + (size_t)k * n_u, sizeof(double) * n_u, cudaMemcpyHostToDevice, st));
-    QSGW_H(cudaMemcpyAsync(H.dE[b] + 2 * n_o + n_u, h_f_kq + (size_t)k * n_u, sizeof(double) * n_u, cudaMemcpyHostToDevice, st));
-    rc = qsgw_chi0_add_kpoint(c, H.dCk[b], nb, H.dCkq[b], nb, H.dE[b], H.dE[b] + n_o, H.dE[b] + 2 * n_o, H.dE[b] + 2 * n_o + n_u, n_o, n_u);
+  int grp = 0;
+  for (int k = 0; k < n_k_points; k += G, ++grp) {
+    const int b = grp & 1;
+    const size_t g = (size_t)((n_k_points - k < G) ? n_k_points - k : G);
+    if (grp >= 2) QSGW_H(cudaEventSynchronize(H.done[b]));   // keeps the host at most two groups ahead
+    double* E = H.dE[b];
+    double* e_k = E;
+    double* f_k = E + g * n_o;
+    double* e_kq = E + 2 * g * n_o;
+    double* f_kq = E + 2 * g * n_o + g * n_u;
+    QSGW_H(cudaMemcpyAsync(H.dCk[b], static_cast<const double2*>(h_Ck) + (size_t)k * ck_1, sizeof(double2) * ck_1 * g, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(H.dCkq[b], static_cast<const double2*>(h_Ckq) + (size_t)k * ckq_1, sizeof(double2) * ckq_1 * g, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(e_k, h_eps_k + (size_t)k * n_o, sizeof(double) * n_o * g, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(f_k, h_f_k + (size_t)k * n_o, sizeof(double) * n_o * g, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(e_kq, h_eps_kq + (size_t)k * n_u, sizeof(double) * n_u * g, cudaMemcpyHostToDevice, st));
+    QSGW_H(cudaMemcpyAsync(f_kq, h_f_kq + (size_t)k * n_u, sizeof(double) * n_u * g, cudaMemcpyHostToDevice, st));
+    rc = qsgw_chi0_add_kpoints(c, H.dCk[b], nb, (long long)ck_1, H.dCkq[b], nb, (long long)ckq_1, e_k, f_k, e_kq, f_kq, n_o,
+                               n_u, (int)g);
     if (rc != QSGW_OK) return rc;
     QSGW_H(cudaEventRecord(H.done[b], st));
   }

@@ -23,6 +23,10 @@ constexpr int kZdMaxSeg = 16;     // a 16-column group touches at most 16 sites
 template <int kZdNB>
 __global__ void __launch_bounds__(kZdThreads, 2) zmel_dmma_kernel(ZmelArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  a.Ck += (long long)blockIdx.z * a.Ck_bs;               // k-point of this CTA
+  a.Ckq += (long long)blockIdx.z * a.Ckq_bs;
+  a.zws += (long long)blockIdx.z * a.z_bs * kCG;
+  if (a.zmax) a.zmax += blockIdx.z;
   const int bmax = a.st.b_max, kt = a.kt;
   double* cs_re = reinterpret_cast<double*>(smem_raw);    // [NB][bmax]
   double* cs_im = cs_re + kZdNB * bmax;
@@ -178,7 +182,7 @@ static cudaError_t launch_nb(const ZmelArgs& a, cudaStream_t s) {
     if (e != cudaSuccess) return e;
     configured[dev] = smem;
   }
-  dim3 grid(a.ncg, (a.n_o + NB - 1) / NB);
+  dim3 grid(a.ncg, (a.n_o + NB - 1) / NB, a.n_batch);
   zmel_dmma_kernel<NB><<<grid, kZdThreads, smem, s>>>(a);
   return cudaGetLastError();
 }
@@ -190,7 +194,7 @@ cudaError_t launch_zmel_dmma(const ZmelArgs& a, cudaStream_t s) {
   long long best = -1;
   for (int nb = 4; nb <= kZdNBMax; ++nb) {
     const int per_sm = smem_for(nb, a.st.b_max, a.kt) <= 110 * 1024 ? 2 : 1;
-    const long long ctas = (long long)a.ncg * ((a.n_o + nb - 1) / nb);
+    const long long ctas = (long long)a.ncg * ((a.n_o + nb - 1) / nb) * a.n_batch;
     const long long cost = ((ctas + (long long)n_sm * per_sm - 1) / ((long long)n_sm * per_sm)) * nb;
     if (best < 0 || cost < best) { best = cost; best_nb = nb; }
   }

@@ -20,6 +20,10 @@ constexpr int kZmelNB = 8;  // occupied-side bands per CTA (register accumulator
 template <typename T>
 __global__ void __launch_bounds__(kZmelThreads) zmel_kernel(ZmelArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  a.Ck += (long long)blockIdx.z * a.Ck_bs;               // k-point of this CTA
+  a.Ckq += (long long)blockIdx.z * a.Ckq_bs;
+  a.zws += (long long)blockIdx.z * a.z_bs * kCG;
+  if (a.zmax) a.zmax += blockIdx.z;
   const int bmax = a.st.b_max;
   T* cs_re = reinterpret_cast<T*>(smem_raw);              // [NB][bmax]
   T* cs_im = cs_re + kZmelNB * bmax;
@@ -165,8 +169,14 @@ __global__ void pair_weights_kernel(const double* __restrict__ eps_k, const doub
                                     double occ_tol, double* __restrict__ wtab, long long kpad,
                                     long long n_pairs_padded, const float* __restrict__ zmax) {
   const long long n_pairs = (long long)n_o * n_u;
+  const int kb = blockIdx.y;                                // k-point of this block
+  eps_k += (long long)kb * n_o;
+  f_k += (long long)kb * n_o;
+  eps_kq += (long long)kb * n_u;
+  f_kq += (long long)kb * n_u;
+  wtab += (long long)kb * n_pairs_padded;
   // FP16-split mixed mode: this batch's z is staged as z * 2^S, so its weights carry 2^(-2S) (exact)
-  const double zfac = zmax ? exp2(-2.0 * (double)f16_scale_exp(*zmax)) : 1.0;
+  const double zfac = zmax ? exp2(-2.0 * (double)f16_scale_exp(zmax[kb])) : 1.0;
   for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < n_pairs_padded;
        p += (long long)gridDim.x * blockDim.x) {
     double num = 0.0, d2 = 0.0;
@@ -195,9 +205,14 @@ __global__ void pair_weights_kernel(const double* __restrict__ eps_k, const doub
 __global__ void __launch_bounds__(256) z_to_hl16_kernel(const double* __restrict__ zws, long long kpad, int ncg,
                                                         int n_m, long long n_pairs, __half* __restrict__ out,
                                                         unsigned char* __restrict__ out8, int n_m_pad,
-                                                        const float* __restrict__ zmax, long long n_rows) {
+                                                        const float* __restrict__ zmax, long long n_rows,
+                                                        long long z_bs) {
   __shared__ float tx[kCG][129], ty[kCG][129];
   const int cg = blockIdx.y;
+  zws += (long long)blockIdx.z * z_bs * kCG;                // batch of this block: workspace slot at pair offset b*z_bs
+  out += (long long)blockIdx.z * (z_bs / kPairStage) * 64;
+  if (out8) out8 += (long long)blockIdx.z * (z_bs / kPairStage) * 128;
+  zmax += blockIdx.z;
   const long long p0 = (long long)blockIdx.x * 128;
   const long long plane = (long long)ncg * kpad * kCG;
   const double scale = exp2((double)f16_scale_exp(*zmax));
@@ -339,7 +354,7 @@ cudaError_t launch_zmel_f64(const ZmelArgs& a, cudaStream_t s) {
     if (e != cudaSuccess) return e;
     configured[dev] = smem;
   }
-  dim3 grid(a.ncg, (a.n_o + kZmelNB - 1) / kZmelNB);
+  dim3 grid(a.ncg, (a.n_o + kZmelNB - 1) / kZmelNB, a.n_batch);
   zmel_kernel<double><<<grid, kZmelThreads, smem, s>>>(a);
   return cudaGetLastError();
 }
@@ -366,18 +381,19 @@ cudaError_t launch_z_import(double* zws, long long kpad, int ncg, int n_m, long 
 cudaError_t launch_pair_weights(const double* eps_k, const double* f_k, const double* eps_kq,
                                 const double* f_kq, int n_o, int n_u, const double* d_omega, int n_freq,
                                 double occ_tol, double* wtab, long long kpad, long long n_pairs_padded,
-                                const float* zmax, cudaStream_t s) {
-  pair_weights_kernel<<<grid_for(n_pairs_padded, 128), 128, 0, s>>>(eps_k, f_k, eps_kq, f_kq, n_o, n_u, d_omega,
+                                const float* zmax, int n_batch, cudaStream_t s) {
+  pair_weights_kernel<<<dim3(grid_for(n_pairs_padded, 128), n_batch), 128, 0, s>>>(eps_k, f_k, eps_kq, f_kq, n_o, n_u, d_omega,
                                                                    n_freq, occ_tol, wtab, kpad, n_pairs_padded, zmax);
   return cudaGetLastError();
 }
 
 cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs, void* zhl,
-                             void* zhb8, int n_m_pad, const float* zmax, cudaStream_t s) {
+                             void* zhb8, int n_m_pad, const float* zmax, int n_batch, long long z_bs,
+                             cudaStream_t s) {
   const long long n_rows = (n_pairs + kPairStage - 1) / kPairStage * kPairStage;   // this batch's padded rows
-  dim3 grid((unsigned)((n_rows + 127) / 128), ncg);
+  dim3 grid((unsigned)((n_rows + 127) / 128), ncg, n_batch);
   z_to_hl16_kernel<<<grid, 256, 0, s>>>(zws, kpad, ncg, n_m, n_pairs, static_cast<__half*>(zhl),
-                                        static_cast<unsigned char*>(zhb8), n_m_pad, zmax, n_rows);
+                                        static_cast<unsigned char*>(zhb8), n_m_pad, zmax, n_rows, z_bs);
   return cudaGetLastError();
 }
 

@@ -7,7 +7,7 @@ def sites_of(prob):
 
 
 def run_cuda(prob, spin=0, precision=0, max_n_o=None, max_n_u=None, n_k_norm=None, return_ctx=False, options=None,
-             stats=None):
+             stats=None, multi_k=False):
     import torch
     import paper_2506_03477_b200 as q
     cfg = prob.cfg
@@ -24,9 +24,14 @@ def run_cuda(prob, spin=0, precision=0, max_n_o=None, max_n_u=None, n_k_norm=Non
     Ck = torch.from_numpy(sp.Ck).to(dev); Ckq = torch.from_numpy(sp.Ckq).to(dev)
     ek = torch.from_numpy(sp.eps_k).to(dev); fk = torch.from_numpy(sp.f_k).to(dev)
     ekq = torch.from_numpy(sp.eps_kq).to(dev); fkq = torch.from_numpy(sp.f_kq).to(dev)
-    for k in range(n_k):
-        ctx.chi0_add_kpoint(Ck[k], Ckq[k], ek[k], fk[k], ekq[k], fkq[k])
+    if multi_k:                       # all k-points through qsgw_chi0_add_kpoints (one stage (a) launch per group)
+        ctx.chi0_add_kpoints(Ck, Ckq, ek, fk, ekq, fkq)
+    else:
+        for k in range(n_k):
+            ctx.chi0_add_kpoint(Ck[k], Ckq[k], ek[k], fk[k], ekq[k], fkq[k])
     out = ctx.chi0_finalize()
+    if stats is not None:
+        stats["kernel_launches"] = ctx.kernel_launches
     ctx.sync()
     res = out.cpu().numpy()
     if stats is not None and precision == 1:

@@ -296,3 +296,34 @@ def test_random_small_shapes(seed):
         err = rel_fro_per_freq(got, ref).max()
         assert err <= tol, (cfg, mo, mu, precision, err)
         check_hermitian(got)
+
+
+@pytest.mark.parametrize("precision,tol", [(0, TOL_FP64), (1, TOL_MIXED)])
+@pytest.mark.parametrize("case", ["cfg0", "cfg1", "ragged", "cfg1_groups", "cfg1_band_batches"])
+def test_add_kpoints_multi_k_launches(case, precision, tol):
+    """qsgw_chi0_add_kpoints: the k-points that fit the z workspace are built by one stage (a) launch and one weight
+    launch (grid.z = k-point, one FP16 scale per k-point in mixed mode).  Whole cfg 0 / cfg 1 jobs in one group, the
+    ragged cell, cfg 1 forced into groups of 3 k-points (flushes between groups, a partial last group), and the
+    fallback through the band-batch loop when a k-point does not fit one band batch -- all against the oracle, and
+    with far fewer launches than the k-point-by-k-point path."""
+    opts, kw = {}, {}
+    if case == "cfg0":
+        prob = generate(get_config(0))
+    elif case == "ragged":
+        prob = generate(RAGGED)
+    else:
+        prob = generate(get_config(1), n_k=20)
+        if case == "cfg1_groups":
+            opts = {"stage_batches": 3}
+        if case == "cfg1_band_batches":
+            kw = {"max_n_o": 3, "max_n_u": 20}
+    n_k_norm = prob.cfg.n_k
+    st, st1 = {}, {}
+    got = run_cuda(prob, precision=precision, n_k_norm=n_k_norm, options=opts, stats=st, multi_k=True, **kw)
+    assert rel_fro_per_freq(got, oracle_chi(prob, n_k_norm=n_k_norm)).max() <= tol
+    check_hermitian(got)
+    one = run_cuda(prob, precision=precision, n_k_norm=n_k_norm, options=opts, stats=st1, **kw)
+    if precision == 0:
+        assert rel_fro_per_freq(got, one).max() <= 1e-14          # same kernels on the same slots
+    if case in ("cfg0", "cfg1", "ragged"):
+        assert st["kernel_launches"] <= 7 and st1["kernel_launches"] > 2 * prob.spins[0].Ck.shape[0]
