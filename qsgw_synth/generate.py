@@ -136,3 +136,47 @@ def synthetic_wc(n_m: int, omega: np.ndarray, seed: int = 0, hermitian: bool = T
         if not hermitian:
             out[i] += 0.2 * c(n_m, n_m) / (1.0 + w * w)
     return out
+
+
+def log_bin_edges(n_bins: int, w_first: float = 1e-3, w_max: float = 2.5) -> np.ndarray:
+    """Edges of the logarithmic histogram mesh on the real axis ("omega_j = 1e-5 x 1.03^j Ry ... ~100
+    mesh points"): n_bins + 1 geometric edges from w_first > 0 to w_max (Ha)."""
+    return np.geomspace(w_first, w_max, n_bins + 1)
+
+
+def binned_pair_weights(eps_k, f_k, eps_kq, f_kq, edges, rel_width: float = 0.05, occ_tol: float = 1e-12):
+    """Synthetic stand-in for the tetrahedron weights w(n', n, k, bin) of Eqs. (16)-(17), which
+    the paper computes on the CPU before the accumulation loop (Alg. 1 line 8) and which are INPUTS of the binned
+    accumulation: every kept pair (f_n (1 - f_n') > occ_tol, D = eps_kq[n'] - eps_k[n] > 0) spreads its occupation
+    factor f_n (1 - f_n') uniformly over the energy window [D (1 - rel_width), D (1 + rel_width)] -- the stand-in
+    for the band dispersion inside a tetrahedron -- and a bin receives the fraction of the window it overlaps.
+    Returns the CSR-by-bin triple (bin_ptr int32 [n_bins+1], pair int32 [nnz] = n * n_u + n', w float64 [nnz]);
+    the part of a window outside [edges[0], edges[-1]) is dropped."""
+    eps_k = np.asarray(eps_k); eps_kq = np.asarray(eps_kq)
+    edges = np.asarray(edges, dtype=np.float64)
+    n_o, n_u = len(eps_k), len(eps_kq)
+    D = eps_kq[None, :] - eps_k[:, None]
+    occ = np.asarray(f_k)[:, None] * (1.0 - np.asarray(f_kq)[None, :])
+    keep = (occ > occ_tol) & (D > 0)
+    n_idx, u_idx = np.nonzero(keep)
+    lo = D[keep] * (1.0 - rel_width)
+    hi = D[keep] * (1.0 + rel_width)
+    wgt = occ[keep]
+    pidx = (n_idx * n_u + u_idx).astype(np.int32)
+    j_lo = np.clip(np.searchsorted(edges, lo, side="right") - 1, 0, len(edges) - 2)
+    j_hi = np.clip(np.searchsorted(edges, hi, side="left") - 1, 0, len(edges) - 2)
+    bins, pairs, ws = [], [], []
+    for off in range(int((j_hi - j_lo).max()) + 1 if len(lo) else 0):
+        j = j_lo + off
+        sel = j <= j_hi
+        ov = np.minimum(hi[sel], edges[j[sel] + 1]) - np.maximum(lo[sel], edges[j[sel]])
+        ok = ov > 0
+        bins.append(j[sel][ok]); pairs.append(pidx[sel][ok]); ws.append(wgt[sel][ok] * ov[ok] / (hi[sel][ok] - lo[sel][ok]))
+    if bins:
+        bins = np.concatenate(bins); pairs = np.concatenate(pairs); ws = np.concatenate(ws)
+    else:
+        bins = np.zeros(0, dtype=np.int64); pairs = np.zeros(0, dtype=np.int32); ws = np.zeros(0)
+    order = np.lexsort((pairs, bins))
+    bin_ptr = np.zeros(len(edges), dtype=np.int32)
+    np.add.at(bin_ptr, bins + 1, 1)
+    return np.cumsum(bin_ptr).astype(np.int32), pairs[order].astype(np.int32), ws[order].astype(np.float64)
