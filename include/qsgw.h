@@ -189,6 +189,37 @@ int32_t qsgw_wc_from_chi0(int32_t n_m, int32_t n_freq, const void* d_chi0, const
 int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_chi0, const void* d_U, void* d_out,
                                    void* cuda_stream);
 
+/* The paper's own real-axis route (Eqs. 15-18; Alg. 1 lines 9-27), FP64 mode.
+ * A context whose n_freq "frequencies" are the histogram bins [edges[j], edges[j+1]) of the real axis (h_omega = any
+ * increasing labels, e.g. the lower edges; they are not used by this path) accumulates the bin-integrated spectral
+ * weight
+ *   A[j][I, J] = (1/N_k) sum_k sum_{pairs with w != 0} w(pair, j, k) conj(z[pair, I]) z[pair, J]        (Eq. 15 without pi/i)
+ * qsgw_imchi_add_batch = Alg. 1 lines 12-21 for one k-point and band batch: stage (a) (as qsgw_zmel_build) and
+ * the per-bin  Z_pair^dagger x W_Zpair  products.  The weights are inputs (the paper computes its tetrahedron weights,
+ * Eqs. 16-17, on the CPU before the loop, Alg. 1 line 8) in CSR-by-bin form:
+ *   d_bin_ptr : int32 [n_freq + 1], d_bin_ptr[0] = 0, non-decreasing, d_bin_ptr[n_freq] = nnz
+ *   d_pair    : int32 [nnz]  pair index n_local * n_u + n'_local of the batch (n_local < n_o, n'_local < n_u)
+ *   d_w       : float64 [nnz] weight of that pair in that bin (entries of one (pair, bin) add up)
+ * The gather of Alg. 1 line 17 is a permutation applied when z is written (pairs sorted by the first bin that carries
+ * them), so each bin multiplies one short contiguous row range; pairs without an entry cost nothing in stage (b).
+ * Accumulates into the context's accumulator (qsgw_reset zeroes it, qsgw_chi0_finalize returns A with the Hermitian
+ * mirror and 1/N_k); batches staged by qsgw_chi0_accumulate are flushed first.  QSGW_ERR_UNSUPPORTED in mixed mode.
+ * The summation order inside a bin is not fixed (atomic placement): results agree to rounding between runs. */
+int32_t qsgw_imchi_add_batch(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const void* d_Ckq, int64_t ld_kq,
+                             int32_t n_begin, int32_t n_o, int32_t np_begin, int32_t n_u, const int32_t* d_bin_ptr,
+                             const int32_t* d_pair, const double* d_w, int32_t nnz);
+
+/* Hilbert transform of the spectral part to the imaginary axis (Eq. 18; Alg. 1 line 27):
+ *   out[i] = sum_j K[i][j] A[j],   K[i][j] = -log((R_j^2 + omega_i^2) / (L_j^2 + omega_i^2)) / (R_j - L_j),
+ * the bracket of Eq. (14) at omega = i omega_i averaged over bin j = [L_j, R_j) = [d_edges[j], d_edges[j+1])
+ * ("taking into account the size of histogram bins"; reading R20).
+ *   d_edges : float64 [n_bins + 1], increasing, d_edges[0] > 0 when omega_out contains 0;  d_omega_out : float64 [n_out]
+ *   d_A : complex128 [n_bins][N_M][N_M];  d_out : complex128 [n_out][N_M][N_M]; may not alias.  n_bins <= 384.
+ * One streaming pass over A per 16 output frequencies (HBM-bound).  Stream-ordered; error text in
+ * qsgw_last_create_error(). */
+int32_t qsgw_hilbert_to_imag_axis(int32_t n_m, int32_t n_bins, const double* d_edges, int32_t n_out,
+                                  const double* d_omega_out, const void* d_A, void* d_out, void* cuda_stream);
+
 /* Imaginary-axis part of the correlation self-energy for one k-point and one batch of intermediate states
  * (the step after W^c; Eq. (22); Alg. 2 lines 11-25 and 44):
  *   ZW^c[n', n, nu] = sum_i w^I_i(eps_qn - eps_{q-k,n'}) sum_mu z[n', n, mu] W^c[i][mu, nu]

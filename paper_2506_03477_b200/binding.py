@@ -62,11 +62,14 @@ def lib() -> C.CDLL:
     L.qsgw_chi0_run_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp, C.POINTER(i64)]
     L.qsgw_set_option.argtypes = [vp, C.c_char_p, i64]
     L.qsgw_sigc_imag_accumulate.argtypes = [vp, vp, dp, dp, vp, i32, i32, vp]
+    L.qsgw_imchi_add_batch.argtypes = [vp, vp, i64, vp, i64, i32, i32, i32, i32, vp, vp, dp, i32]
+    L.qsgw_hilbert_to_imag_axis.argtypes = [i32, i32, dp, i32, dp, vp, vp, vp]
     L.qsgw_mixed_stats.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(C.c_double)]
     for name in ("qsgw_create", "qsgw_set_product_tensor", "qsgw_zmel_build", "qsgw_chi0_accumulate",
                  "qsgw_chi0_add_kpoint", "qsgw_chi0_finalize", "qsgw_reset", "qsgw_sync",
                  "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_set_option", "qsgw_mixed_stats", "qsgw_wc_from_chi0",
-                 "qsgw_sigc_imag_accumulate", "qsgw_chi0_add_kpoints",
+                 "qsgw_sigc_imag_accumulate", "qsgw_chi0_add_kpoints", "qsgw_imchi_add_batch",
+                 "qsgw_hilbert_to_imag_axis",
                  "qsgw_chi0_to_coulomb_basis"):
         getattr(L, name).restype = i32
     for name in ("qsgw_last_error", "qsgw_last_create_error", "qsgw_version"):
@@ -217,6 +220,15 @@ class Chi0Context:
                                                       _ptr(d_eps_qk, f64), _ptr(d_wc, torch.complex128), n_all, n_qp,
                                                       _ptr(d_sigc, torch.complex128)))
 
+    def imchi_add_batch(self, d_Ck, d_Ckq, n_begin: int, n_o: int, np_begin: int, n_u: int, d_bin_ptr, d_pair, d_w):
+        """Binned spectral part (Eq. 15, Alg. 1 lines 12-21) of one k-point / band batch; CSR-by-bin weights."""
+        import torch
+        nnz = int(d_pair.shape[0]) if d_pair is not None else 0
+        self._check(self._L.qsgw_imchi_add_batch(
+            self._h, _ptr(d_Ck, torch.complex128), d_Ck.shape[-1], _ptr(d_Ckq, torch.complex128), d_Ckq.shape[-1],
+            n_begin, n_o, np_begin, n_u, _ptr(d_bin_ptr, torch.int32), _ptr(d_pair, torch.int32) if nnz else None,
+            _ptr(d_w, torch.float64) if nnz else None, nnz))
+
     def reset(self):
         self._check(self._L.qsgw_reset(self._h))
 
@@ -311,6 +323,21 @@ def chi0_to_coulomb_basis(chi0, U, out=None):
                                       _ptr(out, torch.complex128), stream)
     if rc != 0:
         raise QsgwError(rc, L.qsgw_last_create_error().decode())
+    return out
+
+
+def hilbert_to_imag_axis(A, edges, omega_out, out=None):
+    """Eq. (18) on the imaginary axis: out[i] = sum_j K[i][j] A[j] (qsgw_hilbert_to_imag_axis)."""
+    import torch
+    n_bins, n_m = int(A.shape[0]), int(A.shape[1])
+    n_out = int(omega_out.shape[0])
+    if out is None:
+        out = torch.empty((n_out, n_m, n_m), dtype=torch.complex128, device=A.device)
+    st = torch.cuda.current_stream(A.device).cuda_stream
+    rc = lib().qsgw_hilbert_to_imag_axis(n_m, n_bins, _ptr(edges, torch.float64), n_out, _ptr(omega_out, torch.float64),
+                                         _ptr(A, torch.complex128), _ptr(out, torch.complex128), C.c_void_p(st))
+    if rc != 0:
+        raise QsgwError(rc, lib().qsgw_last_create_error().decode())
     return out
 
 

@@ -49,8 +49,14 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
   const int2 tt = a.d_tiles[tile];
   const bool diag = (tt.x == tt.y);
   const int n_all = (int)(a.n_pairs_padded / KP3);
-  const int it_base = (int)((long long)n_all * chunk / a.split);
-  const int n_iter = (int)((long long)n_all * (chunk + 1) / a.split) - it_base;
+  int it_base = (int)((long long)n_all * chunk / a.split);
+  int n_iter = (int)((long long)n_all * (chunk + 1) / a.split) - it_base;
+  if (a.d_ranges) {           // binned path: only the stages that cover the rows carrying weight in this bin
+    const int2 r = a.d_ranges[j];
+    it_base = r.x / KP3;
+    n_iter = r.y > r.x ? (r.y + KP3 - 1) / KP3 - it_base : 0;
+    if (n_iter <= 0) return;
+  }
   const double* wrow = a.wtab + (long long)j * a.kpad;
 
   if (tid == 0) {
@@ -226,7 +232,7 @@ cudaError_t launch_chi0_f64(const Chi0F64Args& a_in, cudaStream_t s) {
   if (a_in.n_pairs_padded <= 0 || a_in.n_tiles <= 0) return cudaSuccess;
   Chi0F64Args a = a_in;
   a.split = 1;
-  {   // few (tile, frequency) items (1 CTA/SM): split the staged pairs over 2..4 CTAs (see launch_chi0_f16)
+  if (!a.d_ranges) {   // few (tile, frequency) items (1 CTA/SM): split the staged pairs over 2..4 CTAs (see launch_chi0_f16)
     const int n_sm = a.n_sm;
     const long long items = (long long)a.n_tiles * a.n_freq, n_it = a.n_pairs_padded / KP3;
     double best = (double)((items + n_sm - 1) / n_sm);

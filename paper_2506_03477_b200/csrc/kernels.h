@@ -46,6 +46,7 @@ struct ZmelArgs {
   // writes the workspace slot at pair offset b*z_bs
   int n_batch = 1;
   long long Ck_bs = 0, Ckq_bs = 0, z_bs = 0;
+  const int* row_map = nullptr;  // optional [n_o*n_u]: workspace row of pair n*n_u + n' (binned real-axis path)
   int kt = 0;            // DMMA kernel: padded contraction length, max over column groups of sum_seg pad4(b_seg)
   int n_sm = 148;        // SMs of the context's device
 };
@@ -79,6 +80,8 @@ struct Chi0F64Args {
   long long n_pairs_padded;   // multiple of kPairAlign
   const int2* d_tiles;        // (tile_i, tile_j), tile_i <= tile_j
   int n_tiles;
+  const int2* d_ranges = nullptr;   // optional [n_freq]: pair rows [x, y) that carry weight at that frequency (bin);
+                                    // the CTA runs only the 32-pair stages that cover them (no split)
 };
 constexpr int kChi0F64KP3M = 32;  // pairs per pipeline stage (box rows of the tensor map)
 cudaError_t launch_chi0_f64(const Chi0F64Args& a, cudaStream_t s);
@@ -195,6 +198,19 @@ cudaError_t launch_sigc_weights(const double* eps_q, const double* eps_qk, int n
 // z: complex128 [n_all][n_qp][n_m]; wc: [n_freq][n_m][n_m]; zw: workspace of the size of z; sigc [n_qp][n_qp] += ...
 cudaError_t launch_sigc_imag(const double2* z, const double* w, long long ld_w, const double2* wc, int n_all, int n_qp,
                              int n_m, int n_freq, double inv_nk, double2* zw, double2* sigc, int n_sm, cudaStream_t s);
+
+// ---- real-axis route (realaxis_kernels.cu; Eqs. 15-18, Alg. 1 lines 13-27) ---------------------------------------
+// From the CSR-by-bin weights (bin_ptr[n_bins+1], pair[nnz], w[nnz]) of one band batch: row_map[n_pairs] = workspace row
+// of every pair after a counting sort by the first bin that carries it (pairs without weight last), the dense table
+// wtab[n_bins][kpad] (zero except the entries) and ranges[n_bins] = rows touched by each bin.
+// scratch: n_pairs + 2*(n_bins + 2) ints.
+cudaError_t launch_bin_setup(const int* bin_ptr, const int* pair, const double* w, int nnz, int n_bins, long long n_pairs,
+                             long long n_pad, int* row_map, int* scratch, double* wtab, long long kpad, int2* ranges,
+                             cudaStream_t s);
+// out[i][e] = sum_j K[i][j] A[j][e], K[i][j] = -log1p((R^2 - L^2) / (L^2 + omega_i^2)) / (R - L) over bin j = [L, R)
+// (Eq. 18 on the imaginary axis); A, out complex128 [.][n_m][n_m]
+cudaError_t launch_hilbert_imag(int n_m, int n_bins, const double* edges, int n_out, const double* omega_out,
+                                const double2* A, double2* out, cudaStream_t s);
 
 // issue-rate probes (probe_kernels.cu): measured MMA-pipe peaks for the roofline denominators
 cudaError_t probe_fp64_mma(cudaStream_t s, double* out_tflops, double* out_ms);

@@ -107,6 +107,11 @@ struct qsgw_ctx {
   int z_zi = 0;                 // ... and the index of its FP16 scale in d_zmax
   int zslot = 0;                // batches staged since the last flush (next free index of d_zmax)
   int e2e_groups = 4;           // frequency groups of the last flush of qsgw_chi0_run_host
+  // binned real-axis path (qsgw_imchi_add_batch; allocated by its first call)
+  int* d_rowmap = nullptr;      // [batch_pad] workspace row of every pair of the batch
+  int* d_binscratch = nullptr;  // [batch_pad + 2 (n_freq + 2)]
+  int2* d_ranges = nullptr;     // [n_freq] rows touched by each bin
+  const int* cur_row_map = nullptr;   // row map of the stage (a) launch being issued (NULL: natural pair order)
   // I^c workspace (qsgw_sigc_imag_accumulate; allocated by its first call)
   double2* d_sz = nullptr;      // z of the batch, complex128 [pairs][N_M]
   double2* d_szw = nullptr;     // ZW^c, same shape
@@ -190,6 +195,9 @@ void free_all(qsgw_ctx* c) {
   }
   for (int i = 0; i < 4; ++i) if (c->hr.ready[i]) cudaEventDestroy(c->hr.ready[i]);
   if (c->hr.cp) cudaStreamDestroy(c->hr.cp);
+  cudaFree(c->d_rowmap);
+  cudaFree(c->d_binscratch);
+  cudaFree(c->d_ranges);
   cudaFree(c->d_sz);
   cudaFree(c->d_szw);
   cudaFree(c->d_sw);
@@ -771,6 +779,7 @@ static int build_batches(qsgw_ctx* ctx, const double2* Ck, long long ld_k, long 
   a.kt = ctx->zmel_kt;
   a.n_sm = ctx->n_sm;
   a.n_batch = n_batch;
+  a.row_map = ctx->cur_row_map;
   a.Ck_bs = ck_bs;
   a.Ckq_bs = ckq_bs;
   a.z_bs = n_pad;
@@ -1070,6 +1079,84 @@ int32_t qsgw_chi0_finalize(qsgw_ctx* ctx, void* d_chi0_out) {
   if (e != cudaSuccess) return ctx->cuda_fail(e, "finalize kernel launch");
   ctx->launches += 1;
   ctx->err.clear();
+  return QSGW_OK;
+}
+
+int32_t qsgw_imchi_add_batch(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const void* d_Ckq, int64_t ld_kq,
+                             int32_t n_begin, int32_t n_o, int32_t np_begin, int32_t n_u, const int32_t* d_bin_ptr,
+                             const int32_t* d_pair, const double* d_w, int32_t nnz) {
+  if (!ctx) return QSGW_ERR_INVALID_ARG;
+  if (ctx->state == ST_CREATED) return ctx->fail(QSGW_ERR_STATE, "set_product_tensor must precede imchi_add_batch");
+  if (ctx->f16) return ctx->fail(QSGW_ERR_UNSUPPORTED, "the binned real-axis path is built for QSGW_PREC_FP64 only");
+  if (!d_Ck || !d_Ckq || !d_bin_ptr || (nnz > 0 && (!d_pair || !d_w))) return ctx->fail(QSGW_ERR_INVALID_ARG, "NULL argument");
+  if (ld_k < ctx->n_b || ld_kq < ctx->n_b)
+    return ctx->fail(QSGW_ERR_INVALID_ARG, "leading dimension smaller than N_b=%d", ctx->n_b);
+  if (n_begin < 0 || np_begin < 0 || nnz < 0) return ctx->fail(QSGW_ERR_SHAPE, "negative band offset or entry count");
+  int rc = check_batch(ctx, n_o, n_u);
+  if (rc != QSGW_OK) return rc;
+  rc = flush_pending(ctx);              // the batch uses the whole workspace on its own
+  if (rc != QSGW_OK) return rc;
+  cudaError_t e;
+  if (!ctx->d_ranges) {
+    e = dev_alloc(ctx, &ctx->d_rowmap, (size_t)ctx->batch_pad);
+    if (e == cudaSuccess) e = dev_alloc(ctx, &ctx->d_binscratch, (size_t)ctx->batch_pad + 2 * ((size_t)ctx->n_freq + 2));
+    if (e == cudaSuccess) e = dev_alloc(ctx, &ctx->d_ranges, (size_t)ctx->n_freq);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      cudaFree(ctx->d_rowmap); cudaFree(ctx->d_binscratch); cudaFree(ctx->d_ranges);
+      ctx->d_rowmap = ctx->d_binscratch = nullptr; ctx->d_ranges = nullptr;
+      return ctx->fail(QSGW_ERR_ALLOC, "workspace of the binned path: %s", cudaGetErrorString(e));
+    }
+  }
+  const long long n_pairs = (long long)n_o * n_u, n_pad = round_up(n_pairs, qsgw::kPairAlign);
+  {
+    StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
+    e = qsgw::launch_bin_setup(d_bin_ptr, d_pair, d_w, nnz, ctx->n_freq, n_pairs, n_pad, ctx->d_rowmap,
+                               ctx->d_binscratch, ctx->d_wtab, ctx->kpad, ctx->d_ranges, ctx->stream);
+  }
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "bin set-up kernels");
+  ctx->launches += nnz > 0 ? 6 : 4;
+  ctx->cur_row_map = ctx->d_rowmap;
+  rc = build_batches(ctx, static_cast<const double2*>(d_Ck), ld_k, 0, static_cast<const double2*>(d_Ckq), ld_kq, 0,
+                     n_begin, n_o, np_begin, n_u, 1, 0, n_pad, 0);
+  ctx->cur_row_map = nullptr;
+  if (rc != QSGW_OK) return rc;
+  qsgw::Chi0F64Args a;
+  a.tmap_z = ctx->tmap_z;
+  a.wtab = ctx->d_wtab;
+  a.kpad = ctx->kpad;
+  a.acc_re = ctx->d_acc_re;
+  a.acc_im = ctx->d_acc_im;
+  a.n_m_pad = ctx->n_m_pad;
+  a.n_freq = ctx->n_freq;
+  a.j0 = 0;
+  a.n_pairs_padded = n_pad;
+  a.n_sm = ctx->n_sm;
+  a.d_tiles = ctx->d_tiles;
+  a.n_tiles = ctx->n_tiles;
+  a.d_ranges = ctx->d_ranges;
+  {
+    StageScope ts(ctx, QSGW_STAGE_CHI0);
+    e = qsgw::launch_chi0_f64(a, ctx->stream);
+  }
+  if (e != cudaSuccess) return ctx->cuda_fail(e, "binned accumulation kernel launch");
+  ctx->launches += 1;
+  ctx->pairs += n_pairs;
+  ctx->state = ST_READY;               // the batch is consumed: nothing stays staged
+  ctx->err.clear();
+  return QSGW_OK;
+}
+
+int32_t qsgw_hilbert_to_imag_axis(int32_t n_m, int32_t n_bins, const double* d_edges, int32_t n_out,
+                                  const double* d_omega_out, const void* d_A, void* d_out, void* cuda_stream) {
+  g_create_error.clear();
+  if (!d_edges || !d_omega_out || !d_A || !d_out) { g_create_error = "NULL argument"; return QSGW_ERR_INVALID_ARG; }
+  if (d_A == d_out) { g_create_error = "d_out aliases d_A"; return QSGW_ERR_INVALID_ARG; }
+  if (n_m < 1 || n_bins < 1 || n_out < 1) { g_create_error = "n_m, n_bins and n_out must be positive"; return QSGW_ERR_SHAPE; }
+  if (n_bins > 384) { g_create_error = "at most 384 bins (the transform matrix is held in shared memory)"; return QSGW_ERR_SHAPE; }
+  cudaError_t e = qsgw::launch_hilbert_imag(n_m, n_bins, d_edges, n_out, d_omega_out, static_cast<const double2*>(d_A),
+                                            static_cast<double2*>(d_out), static_cast<cudaStream_t>(cuda_stream));
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("Hilbert transform kernel: ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
   return QSGW_OK;
 }
 

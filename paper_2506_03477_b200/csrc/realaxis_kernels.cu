@@ -1,0 +1,144 @@
+// The paper's real-axis route: set-up of the binned accumulation of the spectral part (Eqs. 15-17,
+// PAPER.md:165-173; Alg. 1 lines 13-21) and the Hilbert transform to the imaginary axis (Eq. 18,
+// PAPER.md:175-177; Alg. 1 line 27).
+//
+// Alg. 1 gathers, for every histogram bin, the band pairs whose weight is non-zero into Z_pair and multiplies
+// Z_pair^dagger x W_Zpair.  Here the gather is a PERMUTATION made before z is written: the pairs of a band batch are
+// sorted by the first bin that carries them, stage (a) writes each pair's row at its sorted position, and a bin
+// then touches one short contiguous range of rows (a pair's tetrahedron weight spreads over a few neighbouring
+// bins only), which stage (b) (chi0_f64_3m_kernel with Chi0F64Args::d_ranges) streams by TMA like any other batch;
+// the per-bin weights sit in the dense, mostly zero table the kernel already reads.
+#include "kernels.h"
+
+namespace qsgw {
+
+namespace {
+
+__device__ __forceinline__ int bin_of_entry(const int* __restrict__ bin_ptr, int n_bins, int e) {
+  int lo = 0, hi = n_bins;              // largest j with bin_ptr[j] <= e
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (bin_ptr[mid] <= e) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+__global__ void bin_init_kernel(int* __restrict__ first_bin, long long n_pairs, int n_bins, int* __restrict__ count,
+                                int2* __restrict__ ranges) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i < n_pairs) first_bin[i] = n_bins;                // n_bins = "carries no weight"
+  if (i < n_bins + 2) count[i] = 0;
+  if (i < n_bins) ranges[i] = make_int2(0x7fffffff, 0);
+}
+
+__global__ void bin_first_kernel(const int* __restrict__ bin_ptr, const int* __restrict__ pair, int nnz, int n_bins,
+                                 int* __restrict__ first_bin) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e < nnz) atomicMin(&first_bin[pair[e]], bin_of_entry(bin_ptr, n_bins, e));
+}
+
+__global__ void bin_count_kernel(const int* __restrict__ first_bin, long long n_pairs, int* __restrict__ count) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i < n_pairs) atomicAdd(&count[first_bin[i]], 1);
+}
+
+// exclusive scan of count[0 .. n_bins] (one block), result in offs; count is reused as the running cursor
+__global__ void bin_scan_kernel(int* __restrict__ count, int* __restrict__ offs, int n) {
+  if (threadIdx.x == 0) {
+    int run = 0;
+    for (int i = 0; i < n; ++i) {
+      const int c = count[i];
+      offs[i] = run;
+      count[i] = run;
+      run += c;
+    }
+  }
+}
+
+// Stable within a bucket would need a second pass; the order inside a bucket only changes the summation order.
+__global__ void bin_place_kernel(const int* __restrict__ first_bin, long long n_pairs, int* __restrict__ cursor,
+                                 int* __restrict__ row_map) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i < n_pairs) row_map[i] = atomicAdd(&cursor[first_bin[i]], 1);
+}
+
+__global__ void bin_scatter_kernel(const int* __restrict__ bin_ptr, const int* __restrict__ pair,
+                                   const double* __restrict__ w, int nnz, int n_bins, const int* __restrict__ row_map,
+                                   double* __restrict__ wtab, long long kpad, int2* __restrict__ ranges) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= nnz) return;
+  const int j = bin_of_entry(bin_ptr, n_bins, e);
+  const int row = row_map[pair[e]];
+  atomicAdd(&wtab[(long long)j * kpad + row], w[e]);      // duplicates of a (pair, bin) entry add up
+  atomicMin(&ranges[j].x, row);
+  atomicMax(&ranges[j].y, row + 1);
+}
+
+constexpr int kHilbertOut = 16;      // output frequencies per pass (register accumulators)
+
+// One thread = one real component of one matrix element; K in shared memory.
+__global__ void __launch_bounds__(256) hilbert_imag_kernel(long long n_elem, int n_bins, const double* __restrict__ edges,
+                                                           int n_out, int i0, const double* __restrict__ omega_out,
+                                                           const double* __restrict__ A, double* __restrict__ out) {
+  extern __shared__ double Ks[];       // [kHilbertOut][n_bins]
+  const int n_i = min(kHilbertOut, n_out - i0);
+  for (int idx = threadIdx.x; idx < n_i * n_bins; idx += blockDim.x) {
+    const int i = idx / n_bins, j = idx - i * n_bins;
+    const double L = edges[j], R = edges[j + 1], om = omega_out[i0 + i];
+    Ks[idx] = -log1p((R - L) * (R + L) / (L * L + om * om)) / (R - L);
+  }
+  __syncthreads();
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n_elem; e += (long long)gridDim.x * blockDim.x) {
+    double acc[kHilbertOut];
+#pragma unroll
+    for (int i = 0; i < kHilbertOut; ++i) acc[i] = 0.0;
+    for (int j = 0; j < n_bins; ++j) {
+      const double a = A[(long long)j * n_elem + e];
+#pragma unroll
+      for (int i = 0; i < kHilbertOut; ++i)
+        if (i < n_i) acc[i] += Ks[i * n_bins + j] * a;
+    }
+#pragma unroll
+    for (int i = 0; i < kHilbertOut; ++i)
+      if (i < n_i) out[(long long)(i0 + i) * n_elem + e] = acc[i];
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_bin_setup(const int* bin_ptr, const int* pair, const double* w, int nnz, int n_bins, long long n_pairs,
+                             long long n_pad, int* row_map, int* scratch, double* wtab, long long kpad, int2* ranges,
+                             cudaStream_t s) {
+  int* first_bin = scratch;
+  int* count = scratch + n_pairs;
+  int* offs = count + n_bins + 2;
+  const long long n_init = n_pairs > n_bins + 2 ? n_pairs : n_bins + 2;
+  const unsigned gp = (unsigned)((n_pairs + 255) / 256), ge = (unsigned)((nnz + 255) / 256);
+  bin_init_kernel<<<(unsigned)((n_init + 255) / 256), 256, 0, s>>>(first_bin, n_pairs, n_bins, count, ranges);
+  cudaError_t e = cudaMemset2DAsync(wtab, sizeof(double) * kpad, 0, sizeof(double) * n_pad, n_bins, s);
+  if (e != cudaSuccess) return e;
+  if (nnz > 0) bin_first_kernel<<<ge, 256, 0, s>>>(bin_ptr, pair, nnz, n_bins, first_bin);
+  bin_count_kernel<<<gp, 256, 0, s>>>(first_bin, n_pairs, count);
+  bin_scan_kernel<<<1, 32, 0, s>>>(count, offs, n_bins + 1);
+  bin_place_kernel<<<gp, 256, 0, s>>>(first_bin, n_pairs, count, row_map);
+  if (nnz > 0) bin_scatter_kernel<<<ge, 256, 0, s>>>(bin_ptr, pair, w, nnz, n_bins, row_map, wtab, kpad, ranges);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_hilbert_imag(int n_m, int n_bins, const double* edges, int n_out, const double* omega_out,
+                                const double2* A, double2* out, cudaStream_t s) {
+  const long long n_elem = 2LL * n_m * n_m;
+  const size_t smem = sizeof(double) * kHilbertOut * n_bins;
+  if (smem > 48 * 1024) return cudaErrorInvalidValue;
+  long long blocks = (n_elem + 255) / 256;
+  if (blocks > 148LL * 32) blocks = 148LL * 32;
+  for (int i0 = 0; i0 < n_out; i0 += kHilbertOut) {
+    hilbert_imag_kernel<<<(unsigned)blocks, 256, smem, s>>>(n_elem, n_bins, edges, n_out, i0, omega_out,
+                                                            reinterpret_cast<const double*>(A), reinterpret_cast<double*>(out));
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+}  // namespace qsgw

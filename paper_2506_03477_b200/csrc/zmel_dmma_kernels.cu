@@ -141,7 +141,8 @@ __global__ void __launch_bounds__(kZdThreads, 2) zmel_dmma_kernel(ZmelArgs a) {
 #pragma unroll
       for (int n = 0; n < kZdNB; ++n) {
         if (n < nb) {
-          const long long pair = (long long)(n0 + n) * a.n_u + np;
+          long long pair = (long long)(n0 + n) * a.n_u + np;
+          if (a.row_map) pair = a.row_map[pair];
 #pragma unroll
           for (int nt = 0; nt < 2; ++nt) {
             const long long off = ((long long)cg * a.kpad + pair) * kCG + 8 * nt + 2 * t;

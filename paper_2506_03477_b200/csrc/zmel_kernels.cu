@@ -107,7 +107,8 @@ __global__ void __launch_bounds__(kZmelThreads) zmel_kernel(ZmelArgs a) {
 #pragma unroll
         for (int n = 0; n < kZmelNB; ++n) {
           if (n < nb) {
-            const long long pair = (long long)(n0 + n) * a.n_u + np;
+            long long pair = (long long)(n0 + n) * a.n_u + np;
+            if (a.row_map) pair = a.row_map[pair];
             const long long off = ((long long)cg * a.kpad + pair) * kCG + col;
             zx[off] = ar[n];
             zy[off] = ai[n];
