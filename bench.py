@@ -331,6 +331,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
     # the chi0 just built (Eqs. 10, 19): blocked Cholesky inverse of N_omega matrices of order N_M on the GPU.
     wc = None
     sigc = None
+    realaxis = None
     if precision == q.PREC_FP64 and not args.no_wc and not light and rank == 0:
         from qsgw_synth import coulomb_eigenvalues, haar_unitary
         import numpy as _np
@@ -423,7 +424,73 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
                                                f"{nks} k-points, W^c from the GPU", "tolerance": 1e-10}
             sctx.destroy()
             del d_Cq, d_Cqk, sig
-        del w_out, d_v, d_U
+        # next row f3: the paper's own real-axis route (Eqs. 15-18, Alg. 1 lines 12-27): binned spectral part of two
+        # k-points with 100 logarithmic bins (seeded stand-in for the tetrahedron weights), then the Hilbert transform
+        # of the 100 bin matrices to the n_freq imaginary frequencies
+        if not args.no_realaxis:
+            from qsgw_synth import binned_pair_weights, log_bin_edges
+            del w_out
+            torch.cuda.empty_cache()
+            n_bins, nks = 100, min(2, n_k)
+            edges = log_bin_edges(n_bins, 1e-3, 2.5)
+            sp0 = prob.spins[0]
+            wts = [binned_pair_weights(sp0.eps_k[k], sp0.f_k[k], sp0.eps_kq[k], sp0.f_kq[k], edges, 0.05, cfg.occ_tol)
+                   for k in range(nks)]
+            d_w = [[torch.from_numpy(a).to(dev) for a in w] for w in wts]
+            rctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, edges[:-1], cfg.n_k, cfg.n_o, cfg.n_u, precision=q.PREC_FP64)
+            rctx.set_product_tensor(torch.from_numpy(prob.P).to(dev))
+            Ck, Ckq = d_in[0][0], d_in[0][1]
+            A = torch.empty((n_bins, cfg.n_m, cfg.n_m), dtype=torch.complex128, device=dev)
+            d_edges, d_om = torch.from_numpy(edges).to(dev), torch.from_numpy(prob.omega).to(dev)
+
+            def ra_pass():
+                rctx.reset()
+                for k in range(nks):
+                    rctx.imchi_add_batch(Ck[k], Ckq[k], 0, cfg.n_o, 0, cfg.n_u, *d_w[k])
+                rctx.chi0_finalize(A)
+
+            ra_ms = timed(ra_pass)
+            h_out = torch.empty_like(out)
+            hil_ms = timed(lambda: q.hilbert_to_imag_axis(A, d_edges, d_om, out=h_out))
+            nnz = sum(len(w[1]) for w in wts)
+            fl_ra = 8.0 * nnz * (cfg.n_m * (cfg.n_m + 1) // 2) + 8.0 * nks * cfg.stage_a_cmac()
+            hil_bytes = 16.0 * (n_bins + n_f) * float(cfg.n_m) ** 2
+            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f_:
+                hbm = float(json.load(f_).get("hbm_gbs", 0.0)) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else 0.0
+            realaxis = {"imchi_ms": ra_ms, "imchi_value": fl_ra / (ra_ms * 1e-3) / 1e12, "unit": UNIT, "k_points": nks,
+                        "n_bins": n_bins, "entries": nnz, "pairs": nks * cfg.n_o * cfg.n_u, "credited_flop": fl_ra,
+                        "what": "qsgw_imchi_add_batch per k-point (sort, stage (a), per-bin products) + finalize; credited "
+                                "8 x entries x N_M (N_M + 1) / 2 + stage (a)",
+                        "hilbert_ms": hil_ms, "hilbert_gbs": hil_bytes / (hil_ms * 1e-3) / 1e9,
+                        "hilbert_roofline": {"bound": "hbm", "achieved": hil_bytes / (hil_ms * 1e-3) / 1e9, "peak": hbm or None,
+                                             "unit": "GB/s", "frac": (hil_bytes / (hil_ms * 1e-3) / 1e9 / hbm) if hbm else None,
+                                             "algorithmic_bytes": hil_bytes,
+                                             "what": "qsgw_hilbert_to_imag_axis: (n_bins + n_freq) N_M^2 complex128 read + written once"}}
+            if not args.no_accuracy:
+                import oracle
+                got = h_out.cpu().numpy()
+                A_h = A.cpu().numpy()
+                ref = oracle.hilbert_imag_ref(A_h, edges, prob.omega)
+                realaxis["hilbert_accuracy"] = float((_np.linalg.norm((got - ref).reshape(n_f, -1), axis=1) /
+                                                      _np.linalg.norm(ref.reshape(n_f, -1), axis=1)).max())
+                # one bin of the timed A against the oracle's gather / scale / GEMM (the fullest bin of k-point 0 + 1)
+                sites = [prob.P_site(s_) for s_ in range(cfg.n_sites)]
+                jb = int(_np.argmax(_np.diff(wts[0][0])))
+                ref_b = _np.zeros((cfg.n_m, cfg.n_m), dtype=_np.complex128)
+                for k in range(nks):
+                    z = oracle.zmel_ref(sites, sp0.Ck[k], sp0.Ckq[k]).reshape(-1, cfg.n_m)
+                    bp, pr, ww = wts[k]
+                    Zp = z[pr[bp[jb]:bp[jb + 1]]]
+                    ref_b += Zp.conj().T @ (ww[bp[jb]:bp[jb + 1], None] * Zp)
+                ref_b = oracle.hermitian_finalize_ref((ref_b / cfg.n_k)[None])[0]
+                realaxis["imchi_accuracy"] = {"bin": jb, "rel_frobenius_err": float(_np.linalg.norm(A_h[jb] - ref_b) / _np.linalg.norm(ref_b)),
+                                              "tolerance": 1e-11}
+                del A_h, got
+            rctx.destroy()
+            del A, h_out
+        else:
+            del w_out
+        del d_v, d_U
     del d_in, out
     torch.cuda.empty_cache()
 
@@ -541,7 +608,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
 
     return {"mode": mode_name, "value": value, "ms_per_step": ms_total / args.steps, "launches": launches,
             "roofline": roofline, "e2e": e2e, "clocks": clocks, "flops_step": flops_step,
-            "flops_stage_a": fa, "flops_stage_b": fb, "pairs_kept": pairs, "wc": wc, "sigc": sigc, "mixed_selection": mixed_stats,
+            "flops_stage_a": fa, "flops_stage_b": fb, "pairs_kept": pairs, "wc": wc, "sigc": sigc, "realaxis": realaxis, "mixed_selection": mixed_stats,
             "_out": outs_host}
 
 
@@ -624,6 +691,8 @@ def main_cuda(args):
             line["wc"] = r["wc"]
         if r.get("sigc"):
             line["sigc"] = r["sigc"]
+        if r.get("realaxis"):
+            line["realaxis"] = r["realaxis"]
         if r is not main:
             line[r["mode"]] = r
     if main.get("mixed_selection"):
@@ -660,6 +729,7 @@ def parse_args(argv=None):
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-wc", action="store_true", help="skip the W^c(i omega) leg reported beside the FP64 step")
+    ap.add_argument("--no-realaxis", action="store_true", help="skip the real-axis (binned Im chi0 + Hilbert) leg")
     ap.add_argument("--no-sigc", action="store_true", help="skip the I^c (imaginary-axis self-energy) leg")
     ap.add_argument("--no-accuracy", action="store_true", help="skip the oracle check of the timed outputs")
     ap.add_argument("--no-configs", action="store_true", help="skip the side runs of the other configurations")

@@ -76,31 +76,43 @@ __global__ void bin_scatter_kernel(const int* __restrict__ bin_ptr, const int* _
 
 constexpr int kHilbertOut = 16;      // output frequencies per pass (register accumulators)
 
-// One thread = one real component of one matrix element; K in shared memory.
-__global__ void __launch_bounds__(256) hilbert_imag_kernel(long long n_elem, int n_bins, const double* __restrict__ edges,
-                                                           int n_out, int i0, const double* __restrict__ omega_out,
-                                                           const double* __restrict__ A, double* __restrict__ out) {
-  extern __shared__ double Ks[];       // [kHilbertOut][n_bins]
+// One thread = one complex element of every bin matrix, 16 output frequencies in registers; the transform
+// coefficients are broadcast reads from shared memory.  Two CTAs per SM and eight loads in flight per thread keep
+// enough bytes in flight for HBM.
+__global__ void __launch_bounds__(256, 2) hilbert_imag_kernel(long long n_cplx, int n_bins, const double* __restrict__ edges,
+                                                              int n_out, int i0, const double* __restrict__ omega_out,
+                                                              const double2* __restrict__ A, double2* __restrict__ out) {
+  extern __shared__ double Ks[];       // [n_bins][kHilbertOut]
   const int n_i = min(kHilbertOut, n_out - i0);
-  for (int idx = threadIdx.x; idx < n_i * n_bins; idx += blockDim.x) {
-    const int i = idx / n_bins, j = idx - i * n_bins;
-    const double L = edges[j], R = edges[j + 1], om = omega_out[i0 + i];
-    Ks[idx] = -log1p((R - L) * (R + L) / (L * L + om * om)) / (R - L);
+  for (int idx = threadIdx.x; idx < kHilbertOut * n_bins; idx += blockDim.x) {
+    const int j = idx / kHilbertOut, i = idx - j * kHilbertOut;
+    double v = 0.0;
+    if (i < n_i) {
+      const double L = edges[j], R = edges[j + 1], om = omega_out[i0 + i];
+      v = -log1p((R - L) * (R + L) / (L * L + om * om)) / (R - L);
+    }
+    Ks[idx] = v;
   }
   __syncthreads();
-  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n_elem; e += (long long)gridDim.x * blockDim.x) {
-    double acc[kHilbertOut];
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n_cplx; e += (long long)gridDim.x * blockDim.x) {
+    double ar[kHilbertOut], ai[kHilbertOut];
 #pragma unroll
-    for (int i = 0; i < kHilbertOut; ++i) acc[i] = 0.0;
+    for (int i = 0; i < kHilbertOut; ++i) ar[i] = ai[i] = 0.0;
+    const double2* ap = A + e;
+#pragma unroll 8
     for (int j = 0; j < n_bins; ++j) {
-      const double a = A[(long long)j * n_elem + e];
+      const double2 a = ap[(long long)j * n_cplx];
+      const double* kj = Ks + j * kHilbertOut;
 #pragma unroll
-      for (int i = 0; i < kHilbertOut; ++i)
-        if (i < n_i) acc[i] += Ks[i * n_bins + j] * a;
+      for (int i = 0; i < kHilbertOut; ++i) {
+        const double k = kj[i];
+        ar[i] += k * a.x;
+        ai[i] += k * a.y;
+      }
     }
 #pragma unroll
     for (int i = 0; i < kHilbertOut; ++i)
-      if (i < n_i) out[(long long)(i0 + i) * n_elem + e] = acc[i];
+      if (i < n_i) out[(long long)(i0 + i) * n_cplx + e] = make_double2(ar[i], ai[i]);
   }
 }
 
@@ -127,14 +139,13 @@ cudaError_t launch_bin_setup(const int* bin_ptr, const int* pair, const double* 
 
 cudaError_t launch_hilbert_imag(int n_m, int n_bins, const double* edges, int n_out, const double* omega_out,
                                 const double2* A, double2* out, cudaStream_t s) {
-  const long long n_elem = 2LL * n_m * n_m;
+  const long long n_cplx = (long long)n_m * n_m;
   const size_t smem = sizeof(double) * kHilbertOut * n_bins;
   if (smem > 48 * 1024) return cudaErrorInvalidValue;
-  long long blocks = (n_elem + 255) / 256;
-  if (blocks > 148LL * 32) blocks = 148LL * 32;
+  long long blocks = (n_cplx + 255) / 256;
+  if (blocks > 148LL * 8) blocks = 148LL * 8;
   for (int i0 = 0; i0 < n_out; i0 += kHilbertOut) {
-    hilbert_imag_kernel<<<(unsigned)blocks, 256, smem, s>>>(n_elem, n_bins, edges, n_out, i0, omega_out,
-                                                            reinterpret_cast<const double*>(A), reinterpret_cast<double*>(out));
+    hilbert_imag_kernel<<<(unsigned)blocks, 256, smem, s>>>(n_cplx, n_bins, edges, n_out, i0, omega_out, A, out);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }
