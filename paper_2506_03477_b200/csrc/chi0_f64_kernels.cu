@@ -27,7 +27,11 @@ constexpr int W_BYTES3 = KP3 * 8;
 constexpr int SMEM_OPERANDS3 = STAGES * 2 * OPER_BYTES3;
 constexpr int SMEM_BYTES3 = SMEM_OPERANDS3 + STAGES * W_BYTES3 + 2 * STAGES * 8 + 1024 /*align slack*/;
 
-__global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid_constant__ Chi0F64Args a) {
+// NARROW: the tile's last 32 columns are padding (N_M mod 64 in 1..32, last tile column): the 8 warps are laid out
+// 4 along I x 2 along J with 16x16 sub-tiles and cover 64 x 32 outputs -- half the DMMAs of a full tile.
+template <bool NARROW>
+__device__ __forceinline__ void chi0_f64_3m_body(const Chi0F64Args& a, const unsigned block) {
+  constexpr int MI = NARROW ? 2 : 4;
   extern __shared__ unsigned char smem_dyn[];
   const uint32_t raw = smem_u32(smem_dyn);
   const uint32_t base = (raw + 1023u) & ~1023u;
@@ -39,14 +43,14 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
   const int tid = threadIdx.x;
   const int lane = tid & 31, warp = tid >> 5;
   const int g = lane >> 2, t = lane & 3;
-  const int wm = warp >> 2, wn = warp & 3;
+  const int wm = NARROW ? warp >> 1 : warp >> 2, wn = NARROW ? warp & 1 : warp & 3;
 
   // blockIdx.x = ((tile * n_freq) + j) * split + chunk: `split` CTAs share the staged pairs of a (tile, j) when
   // the grid would not fill the SMs; their partial sums meet in the accumulator by atomic adds
-  const int chunk = blockIdx.x % a.split, bid = blockIdx.x / a.split;
+  const int chunk = block % a.split, bid = block / a.split;
   const int j = a.j0 + bid % a.n_freq;
   const int tile = bid / a.n_freq;
-  const int2 tt = a.d_tiles[tile];
+  const int2 tt = (NARROW ? a.d_tiles_narrow : a.d_tiles)[tile];
   const bool diag = (tt.x == tt.y);
   const int n_all = (int)(a.n_pairs_padded / KP3);
   int it_base = (int)((long long)n_all * chunk / a.split);
@@ -91,9 +95,9 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
     for (int par = 0; par < 2; ++par)
       thr_off[s][par] = (uint32_t)((2 * t + s) * 128 + ((((4 * par + (g >> 1)) ^ (2 * t + s)) << 4) | ((g & 1) << 3)));
 
-  double t1[4][2][2], t2[4][2][2], t3[4][2][2];
+  double t1[MI][2][2], t2[MI][2][2], t3[MI][2][2];
 #pragma unroll
-  for (int mi = 0; mi < 4; ++mi)
+  for (int mi = 0; mi < MI; ++mi)
 #pragma unroll
     for (int ni = 0; ni < 2; ++ni)
 #pragma unroll
@@ -112,7 +116,7 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
     __syncwarp();
     mbar_wait(&full[slot], (it / STAGES) & 1);
 
-    const uint32_t aBase = base + slot * (2 * OPER_BYTES3) + (2 * wm) * CGRP_BYTES3;
+    const uint32_t aBase = base + slot * (2 * OPER_BYTES3) + (NARROW ? wm : 2 * wm) * CGRP_BYTES3;
     const uint32_t bBase = base + slot * (2 * OPER_BYTES3) + (diag ? 0 : OPER_BYTES3) + wn * CGRP_BYTES3;
     const uint32_t wBase = base + SMEM_OPERANDS3 + slot * W_BYTES3;
 
@@ -120,9 +124,9 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
     for (int q = 0; q < KP3 / 4; ++q) {
       const uint32_t rq = (uint32_t)((q >> 1) * 1024);
       const double w = ld_shared_f64(wBase + (uint32_t)((8 * (q >> 1) + 2 * t + (q & 1)) * 8));
-      double ax[4], ay[4], as[4], bx[2], by[2], bd[2];
+      double ax[MI], ay[MI], as[MI], bx[2], by[2], bd[2];
 #pragma unroll
-      for (int mi = 0; mi < 4; ++mi) {
+      for (int mi = 0; mi < MI; ++mi) {
         const uint32_t ad = aBase + (mi >> 1) * CGRP_BYTES3 + rq + thr_off[q & 1][mi & 1];
         ax[mi] = ld_shared_f64(ad);
         ay[mi] = ld_shared_f64(ad + PLANE_BYTES3);
@@ -136,7 +140,7 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
         bd[ni] = by[ni] - bx[ni];
       }
 #pragma unroll
-      for (int mi = 0; mi < 4; ++mi)
+      for (int mi = 0; mi < MI; ++mi)
 #pragma unroll
         for (int ni = 0; ni < 2; ++ni) {
           dmma884(t1[mi][ni][0], t1[mi][ni][1], ax[mi], bx[ni]);
@@ -153,8 +157,8 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
   double* are = a.acc_re + (long long)j * plane;
   double* aim = a.acc_im + (long long)j * plane;
 #pragma unroll
-  for (int mi = 0; mi < 4; ++mi) {
-    const int row = tt.x * kTile + (4 * wm + mi) * 8 + g;
+  for (int mi = 0; mi < MI; ++mi) {
+    const int row = tt.x * kTile + (MI * wm + mi) * 8 + g;
 #pragma unroll
     for (int ni = 0; ni < 2; ++ni) {
       const int col = tt.y * kTile + (2 * wn + ni) * 8 + 2 * t;
@@ -179,6 +183,14 @@ __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid
       }
     }
   }
+}
+
+// One grid for both tile kinds: the full tiles first, the half-width tiles of the last tile column behind them
+// (short CTAs at the tail of the grid).
+__global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid_constant__ Chi0F64Args a) {
+  const unsigned n_full = (unsigned)(a.n_tiles * a.n_freq * a.split);
+  if (blockIdx.x < n_full) chi0_f64_3m_body<false>(a, blockIdx.x);
+  else chi0_f64_3m_body<true>(a, blockIdx.x - n_full);
 }
 
 // chi0[j][I][J] = acc/N_k, lower = conj(upper), Im(diag) = 0  (Hermiticity)
@@ -229,12 +241,12 @@ cudaError_t chi0_f64_configure() {
 }
 
 cudaError_t launch_chi0_f64(const Chi0F64Args& a_in, cudaStream_t s) {
-  if (a_in.n_pairs_padded <= 0 || a_in.n_tiles <= 0) return cudaSuccess;
+  if (a_in.n_pairs_padded <= 0 || a_in.n_tiles + a_in.n_tiles_narrow <= 0) return cudaSuccess;
   Chi0F64Args a = a_in;
   a.split = 1;
   if (!a.d_ranges) {   // few (tile, frequency) items (1 CTA/SM): split the staged pairs over 2..4 CTAs (see launch_chi0_f16)
     const int n_sm = a.n_sm;
-    const long long items = (long long)a.n_tiles * a.n_freq, n_it = a.n_pairs_padded / KP3;
+    const long long items = (long long)(a.n_tiles + a.n_tiles_narrow) * a.n_freq, n_it = a.n_pairs_padded / KP3;
     double best = (double)((items + n_sm - 1) / n_sm);
     for (int sp = 2; sp <= 4; ++sp) {
       if (n_it < 16 * sp || items * sp > 8LL * n_sm) break;
@@ -242,8 +254,7 @@ cudaError_t launch_chi0_f64(const Chi0F64Args& a_in, cudaStream_t s) {
       if (cost < 0.95 * best) { best = cost; a.split = sp; }
     }
   }
-  dim3 grid((unsigned)(a.n_tiles * a.n_freq * a.split));
-  chi0_f64_3m_kernel<<<grid, kThreads3M, SMEM_BYTES3, s>>>(a);
+  chi0_f64_3m_kernel<<<dim3((unsigned)((a.n_tiles + a.n_tiles_narrow) * a.n_freq * a.split)), kThreads3M, SMEM_BYTES3, s>>>(a);
   return cudaGetLastError();
 }
 

@@ -80,6 +80,8 @@ struct Chi0F64Args {
   long long n_pairs_padded;   // multiple of kPairAlign
   const int2* d_tiles;        // (tile_i, tile_j), tile_i <= tile_j
   int n_tiles;
+  const int2* d_tiles_narrow = nullptr;   // tiles of the last tile column when its last 32 columns are padding
+  int n_tiles_narrow = 0;                 // (N_M mod 64 in 1..32): computed 64 x 32 wide by a second launch
   const int2* d_ranges = nullptr;   // optional [n_freq]: pair rows [x, y) that carry weight at that frequency (bin);
                                     // the CTA runs only the 32-pair stages that cover them (no split)
 };

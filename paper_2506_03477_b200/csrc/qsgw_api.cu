@@ -72,7 +72,7 @@ struct qsgw_ctx {
   std::vector<double> omega;
   cudaStream_t stream = nullptr;
   // derived
-  int ncg = 0, n_m_pad = 0, n_tiles = 0;
+  int ncg = 0, n_m_pad = 0, n_tiles = 0, n_tiles_narrow = 0;
   long long kpad = 0;           // pair capacity of the z workspace (multiple of 32): several band batches are
   long long fill = 0;           // staged back to back ([0, fill) is pending) and accumulated by ONE stage (b) launch
   // device
@@ -527,10 +527,16 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     return create_fail(c, QSGW_ERR_ALLOC, buf);
   }
   const int nt = c->n_m_pad / tile_edge;
-  std::vector<int2> tiles;
+  // FP64 mode: when the last 32 columns of the last tile column are padding its tiles go to a second list that the
+  // half-width kernel variant computes (cfg 2: N_M = 600 = 9 x 64 + 24; cfg 4: 2400 = 37 x 64 + 32)
+  const int rem = c->n_m % tile_edge;
+  const bool narrow_last = !mixed && rem >= 1 && rem <= 32;
+  std::vector<int2> tiles, tiles_narrow;
   for (int tj = 0; tj < nt; ++tj)
-    for (int ti = 0; ti <= tj; ++ti) tiles.push_back(make_int2(ti, tj));
+    for (int ti = 0; ti <= tj; ++ti) (narrow_last && tj == nt - 1 ? tiles_narrow : tiles).push_back(make_int2(ti, tj));
   c->n_tiles = (int)tiles.size();
+  c->n_tiles_narrow = (int)tiles_narrow.size();
+  tiles.insert(tiles.end(), tiles_narrow.begin(), tiles_narrow.end());     // one device array: full tiles, then narrow
 
 #define QSGW_TRY_ALLOC(expr)                                                                     \
   do {                                                                                           \
@@ -896,6 +902,8 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
   a.n_sm = ctx->n_sm;
   a.d_tiles = ctx->d_tiles;
   a.n_tiles = ctx->n_tiles;
+  a.d_tiles_narrow = ctx->d_tiles + ctx->n_tiles;
+  a.n_tiles_narrow = ctx->n_tiles_narrow;
   {
     StageScope ts(ctx, QSGW_STAGE_CHI0);
     e = qsgw::launch_chi0_f64(a, ctx->stream);
@@ -1134,6 +1142,8 @@ int32_t qsgw_imchi_add_batch(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, cons
   a.n_sm = ctx->n_sm;
   a.d_tiles = ctx->d_tiles;
   a.n_tiles = ctx->n_tiles;
+  a.d_tiles_narrow = ctx->d_tiles + ctx->n_tiles;
+  a.n_tiles_narrow = ctx->n_tiles_narrow;
   a.d_ranges = ctx->d_ranges;
   {
     StageScope ts(ctx, QSGW_STAGE_CHI0);
