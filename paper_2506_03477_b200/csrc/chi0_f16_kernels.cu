@@ -48,8 +48,8 @@ constexpr int kBoxBytes = 64 * 128;      // one TMA box: 64 rows x 128 B
 // registers), so that the scaling warps' data runs ahead of the MMAs instead of waiting for a slot the tensor pipe
 // still reads (ncu, round 2: 25 % of the scaling warps' time was the wait for the common ring).
 struct HCfg {
-  static constexpr int STAGES = 3;                               // B ring
-  static constexpr int ASTAGES = 3;                              // A-source ring
+  static constexpr int STAGES = 4;                               // B ring
+  static constexpr int ASTAGES = 2;                              // A-source ring
   static constexpr int B_BYTES = 2 * kPlaneTileH;
   static constexpr int A_BYTES = 2 * kPlaneTileH;
   static constexpr int W_BYTES = kPairStage * 4;                 // w_h[32] | w_l[32] halves
