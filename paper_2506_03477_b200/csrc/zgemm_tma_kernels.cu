@@ -45,7 +45,15 @@ __device__ __forceinline__ double2 ld_shared_f64x2(uint32_t addr) {
 
 template <bool A_KC, bool B_KC>
 __global__ void __launch_bounds__(kZThreads, 1) zgemm_tma_kernel(const __grid_constant__ ZKernelArgs a) {
-  const int tj = blockIdx.x, ti = blockIdx.y;
+  // tile order: groups of 8 tile columns, tile rows fastest inside a group, so that the CTAs resident at one time share
+  // a narrow slab of B (and a few row panels of A) in L2 instead of streaming all of B per wave
+  int tj, ti;
+  {
+    const int nN = gridDim.x, nM = gridDim.y, pid = blockIdx.y * nN + blockIdx.x;
+    const int grp = pid / (8 * nM), first = grp * 8, width = min(8, nN - first), r = pid - grp * 8 * nM;
+    ti = r / width;
+    tj = first + r - ti * width;
+  }
   if ((a.tri == 1 || a.tri == 2) && tj > ti) return;
   extern __shared__ unsigned char smem_dyn[];
   const uint32_t raw = smem_u32(smem_dyn);
@@ -106,18 +114,22 @@ __global__ void __launch_bounds__(kZThreads, 1) zgemm_tma_kernel(const __grid_co
   // -------------------------------------------------------------------- compute warps
   const int g = lane >> 2, t = lane & 3;
   const int wm = warp >> 2, wn = warp & 3;
-  // per-thread fragment offsets inside an operand stage, for the four 4-deep steps q of a stage
+  // per-thread fragment offsets inside an operand stage, for the four 4-deep steps q of a stage.  Step q contracts the
+  // k rows 8 (q >> 1) + 2 t + (q & 1) (t = lane & 3; the order of the contraction is free): a 16-byte shared load is
+  // served per quarter-warp (lanes 8i..8i+7 = two values of g, all t), and with this mapping its 8 lanes hit the 8
+  // distinct 16-byte chunks of a 128-byte row set (k = 4 (q & 1) + t would make the two g collide: 2x the wavefronts).
   uint32_t offA[4][4], offB[4][2];
 #pragma unroll
   for (int q = 0; q < 4; ++q) {
-    const int kq = 4 * q + t;
+    const int kl = 2 * t + (q & 1);            // k inside the 8-deep half
+    const int kq = 8 * (q >> 1) + kl;          // k inside the stage
 #pragma unroll
     for (int mi = 0; mi < 4; ++mi)
-      offA[q][mi] = A_KC ? (uint32_t)((q >> 1) * 8192 + (32 * wm + 8 * mi + g) * 128 + (((4 * (q & 1) + t) ^ g) << 4))
+      offA[q][mi] = A_KC ? (uint32_t)((q >> 1) * 8192 + (32 * wm + 8 * mi + g) * 128 + ((kl ^ g) << 4))
                          : (uint32_t)((4 * wm + mi) * 2048 + kq * 128 + ((g ^ (kq & 7)) << 4));
 #pragma unroll
     for (int ni = 0; ni < 2; ++ni)
-      offB[q][ni] = B_KC ? (uint32_t)((q >> 1) * 8192 + (16 * wn + 8 * ni + g) * 128 + (((4 * (q & 1) + t) ^ g) << 4))
+      offB[q][ni] = B_KC ? (uint32_t)((q >> 1) * 8192 + (16 * wn + 8 * ni + g) * 128 + ((kl ^ g) << 4))
                          : (uint32_t)((2 * wn + ni) * 2048 + kq * 128 + ((g ^ (kq & 7)) << 4));
   }
 
