@@ -175,3 +175,38 @@ def test_fp8_corrected_products_medium_size(seed_offset):
     got = run_cuda(prob, precision=MIXED, stats=st)
     assert rel_fro_per_freq(got, ref).max() <= TOL_MIXED
     assert (st["launches_fp8"] > 0) == (st["min_eff_pairs"] >= 2.0 * cfg.n_m), st
+
+
+def test_e5m2_error_table_and_threshold(capsys):
+    """The measured basis of the selection rule (profiles/r02_fp8_error_vs_pairs.md): with the E5M2
+    correction products FORCED, the error against the oracle as a function of the effective pair count P_eff / N_M.
+    Asserted: every case with P_eff >= 4 N_M (what the device-side choice accepts) is within 2e-5 with a 25 % margin,
+    the three-FP16-product form stays below 5e-6 everywhere.  `pytest -s` prints the table."""
+    from qsgw_synth import scaled_config
+    rows = []
+    cases = [("cfg4 1k n_o=8", scaled_config(get_config(4), n_o=8), 1, [0, 9]),
+             ("cfg4 1k n_o=32", scaled_config(get_config(4), n_o=32), 1, [0, 9]),
+             ("cfg4 1k n_o=64", get_config(4), 1, [0, 9]),
+             ("cfg1 4k", get_config(1), 4, [0, 5, 15]), ("cfg1 16k", get_config(1), 16, [0, 5, 15]),
+             ("cfg1 64k", get_config(1), 64, [0, 5, 15]), ("cfg3 2k", get_config(3), 2, [0, 8, 15]),
+             ("cfg3 8k", get_config(3), 8, [0, 8, 15])]
+    for name, cfg, n_k, sel in cases:
+        prob = generate(cfg, n_k=n_k)
+        sp = prob.spins[0]
+        chi = oracle.chi0_ref(sites_of(prob), sp.Ck, sp.Ckq, sp.eps_k, sp.f_k, sp.eps_kq, sp.f_kq, prob.omega[sel],
+                              occ_tol=cfg.occ_tol, n_k_norm=cfg.n_k)
+        ref = oracle.hermitian_finalize_ref(chi)
+        errs = {}
+        for variant in (FP16X3, E5M2):
+            st = {}
+            got = run_cuda(prob, precision=MIXED, n_k_norm=cfg.n_k, options={"mixed_fp8": variant}, stats=st,
+                           multi_k=True)
+            errs[variant] = rel_fro_per_freq(got[sel], ref).max()
+        rows.append((name, cfg.n_m, st["min_eff_pairs"] / cfg.n_m, errs[FP16X3], errs[E5M2]))
+    print("\n| case | N_M | min P_eff / N_M per launch | err FP16x3 | err E5M2 forced |\n|---|---|---|---|---|")
+    for r in rows:
+        print("| %s | %d | %.2f | %.2e | %.2e |" % r)
+    for name, n_m, pe, e16, e8 in rows:
+        assert e16 <= 5e-6, (name, e16)
+        if pe >= 4.0:
+            assert e8 <= 1.5e-5, (name, pe, e8)
