@@ -43,9 +43,10 @@ UNIT = "TFLOP/s"
 # Nominal dense B200 tensor peaks (guide: B200_PROFILING.md / blackwell_cuda_programming.md) used
 # only as RATIOS to the measured bf16 peak of MEASURED_PEAKS.json.
 # dram__bytes_read.sum + dram__bytes_write.sum of the stage (b) kernel for ONE cfg-4 k-point (21504 pairs), from the
-# `ncu --set full` captures under profiles/ (r01_*_full.md); a launch covers the k-points staged in the workspace.
-NCU_DRAM_BYTES_PER_KPOINT_CFG4 = {"chi0_f64_3m_kernel": 19.889e9 + 0.777e9,
-                                  "chi0_f16_kernel<fp8>": 5.826e9 + 0.820e9, "chi0_f16_kernel": 5.537e9 + 0.802e9}
+# `ncu --set full` captures under profiles/ (r02_*_full.md; the FP16-only variant: r01); a launch covers the k-points staged
+# in the workspace.
+NCU_DRAM_BYTES_PER_KPOINT_CFG4 = {"chi0_f64_3m_kernel": (40.162e9 + 0.771e9) / 2,          # r02 captures: two k-points per launch
+                                  "chi0_f16_kernel<fp8>": (10.860e9 + 0.936e9) / 2, "chi0_f16_kernel": 5.537e9 + 0.802e9}
 
 NOMINAL_TF = {"bf16": 2250.0, "f16": 2250.0, "tf32": 1100.0, "f64": 40.0}
 
