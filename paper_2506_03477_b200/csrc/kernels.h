@@ -121,7 +121,6 @@ struct Chi0F16Args {
   CUtensorMap tmap_b;    // FP8 variant: 3-D UINT8 {4*kpad, n_m_pad, 2}, box {128, 64, 1}, SWIZZLE_128B
   const __half* wtab16;  // [n_freq][kpad/32][64]
   const double* wscale;  // [n_freq]
-  const float* zmax;     // batch maximum of |Re z|, |Im z|
   long long kpad;
   double* acc_re;
   double* acc_im;

@@ -869,7 +869,6 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
     m.wtab16 = reinterpret_cast<const __half*>(ctx->d_wtab32);   // same bytes per pair as an FP32 table
     m.wscale = ctx->d_wscale;
     m.win = ctx->win;
-    m.zmax = ctx->d_zmax;
     m.kpad = ctx->kpad;
     m.acc_re = ctx->d_acc_re;
     m.acc_im = ctx->d_acc_im;

@@ -3,9 +3,9 @@
 //   PAPER.md:179-182; the paper inverts with a library routine).
 // eps_j is Hermitian positive definite (chi0(i omega) is negative semidefinite), so the inverse goes
 // through a blocked Cholesky factorisation eps = L L^H, X = L^-1, eps^-1 = X^H X, all frequencies batched:
-//   - zgemm_dmma_kernel: complex FP64 GEMM on the FP64 tensor pipe (DMMA.8x8x4), 3M complex product, 64x64 tiles,
-//     operands staged through shared memory; it carries the panel solve, the trailing update (lower tiles only),
-//     the triangular inverse and X^H X (zero blocks of the triangular factor skipped);
+//   - zgemm_tma_kernel (zgemm_tma_kernels.cu): complex FP64 GEMM on the FP64 tensor pipe (DMMA.8x8x4), 3M complex product,
+//     64x64 tiles, TMA-staged operands; it carries the panel solve, the trailing update (lower tiles only), the
+//     triangular inverse and X^H X (zero blocks of the triangular factor skipped);
 //   - potrf_inv_kernel: Cholesky factor of one 64x64 diagonal block and its triangular inverse in shared memory;
 //   - element-wise kernels for eps and W^c.
 #include "kernels.h"
