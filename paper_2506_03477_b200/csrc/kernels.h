@@ -202,9 +202,9 @@ cudaError_t launch_sigc_imag(const double2* z, const double* w, long long ld_w, 
 
 // ---- real-axis route (realaxis_kernels.cu; Eqs. 15-18, Alg. 1 lines 13-27) ---------------------------------------
 // From the CSR-by-bin weights (bin_ptr[n_bins+1], pair[nnz], w[nnz]) of one band batch: row_map[n_pairs] = workspace row
-// of every pair after a counting sort by the first bin that carries it (pairs without weight last), the dense table
+// of every pair after a counting sort by first + last bin that carry it (pairs without weight last), the dense table
 // wtab[n_bins][kpad] (zero except the entries) and ranges[n_bins] = rows touched by each bin.
-// scratch: n_pairs + 2*(n_bins + 2) ints.
+// scratch: 2*n_pairs + 4*(n_bins + 1) ints.
 cudaError_t launch_bin_setup(const int* bin_ptr, const int* pair, const double* w, int nnz, int n_bins, long long n_pairs,
                              long long n_pad, int* row_map, int* scratch, double* wtab, long long kpad, int2* ranges,
                              cudaStream_t s);

@@ -109,7 +109,7 @@ struct qsgw_ctx {
   int e2e_groups = 4;           // frequency groups of the last flush of qsgw_chi0_run_host
   // binned real-axis path (qsgw_imchi_add_batch; allocated by its first call)
   int* d_rowmap = nullptr;      // [batch_pad] workspace row of every pair of the batch
-  int* d_binscratch = nullptr;  // [batch_pad + 2 (n_freq + 2)]
+  int* d_binscratch = nullptr;  // [2 batch_pad + 4 (n_freq + 1)]
   int2* d_ranges = nullptr;     // [n_freq] rows touched by each bin
   const int* cur_row_map = nullptr;   // row map of the stage (a) launch being issued (NULL: natural pair order)
   // I^c workspace (qsgw_sigc_imag_accumulate; allocated by its first call)
@@ -1106,7 +1106,7 @@ int32_t qsgw_imchi_add_batch(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, cons
   cudaError_t e;
   if (!ctx->d_ranges) {
     e = dev_alloc(ctx, &ctx->d_rowmap, (size_t)ctx->batch_pad);
-    if (e == cudaSuccess) e = dev_alloc(ctx, &ctx->d_binscratch, (size_t)ctx->batch_pad + 2 * ((size_t)ctx->n_freq + 2));
+    if (e == cudaSuccess) e = dev_alloc(ctx, &ctx->d_binscratch, 2 * (size_t)ctx->batch_pad + 4 * ((size_t)ctx->n_freq + 1));
     if (e == cudaSuccess) e = dev_alloc(ctx, &ctx->d_ranges, (size_t)ctx->n_freq);
     if (e != cudaSuccess) {
       cudaGetLastError();

@@ -4,10 +4,11 @@
 //
 // Alg. 1 gathers, for every histogram bin, the band pairs whose weight is non-zero into Z_pair and multiplies
 // Z_pair^dagger x W_Zpair.  Here the gather is a PERMUTATION made before z is written: the pairs of a band batch are
-// sorted by the first bin that carries them, stage (a) writes each pair's row at its sorted position, and a bin
-// then touches one short contiguous range of rows (a pair's tetrahedron weight spreads over a few neighbouring
-// bins only), which stage (b) (chi0_f64_3m_kernel with Chi0F64Args::d_ranges) streams by TMA like any other batch;
-// the per-bin weights sit in the dense, mostly zero table the kernel already reads.
+// sorted by first bin + last bin that carry them (twice the centre of their window: the order of their excitation
+// energies), stage (a) writes each pair's row at its sorted position, and a bin then touches one short contiguous
+// range of rows with few foreign pairs in it (a pair's tetrahedron weight spreads over a few neighbouring bins only),
+// which stage (b) (chi0_f64_3m_kernel with Chi0F64Args::d_ranges) streams by TMA like any other batch; the per-bin
+// weights sit in the dense, mostly zero table the kernel already reads.
 #include "kernels.h"
 
 namespace qsgw {
@@ -23,23 +24,36 @@ __device__ __forceinline__ int bin_of_entry(const int* __restrict__ bin_ptr, int
   return lo;
 }
 
-__global__ void bin_init_kernel(int* __restrict__ first_bin, long long n_pairs, int n_bins, int* __restrict__ count,
-                                int2* __restrict__ ranges) {
+// sort key of a pair = first bin + last bin with weight (0 .. 2 n_bins - 2); 2 n_bins = "carries no weight" (sorted last)
+__global__ void bin_init_kernel(int* __restrict__ first_bin, int* __restrict__ last_bin, long long n_pairs, int n_bins,
+                                int* __restrict__ count, int2* __restrict__ ranges) {
   const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (i < n_pairs) first_bin[i] = n_bins;                // n_bins = "carries no weight"
-  if (i < n_bins + 2) count[i] = 0;
+  if (i < n_pairs) {
+    first_bin[i] = n_bins;
+    last_bin[i] = -1;
+  }
+  if (i < 2 * n_bins + 2) count[i] = 0;
   if (i < n_bins) ranges[i] = make_int2(0x7fffffff, 0);
 }
 
 __global__ void bin_first_kernel(const int* __restrict__ bin_ptr, const int* __restrict__ pair, int nnz, int n_bins,
-                                 int* __restrict__ first_bin) {
+                                 int* __restrict__ first_bin, int* __restrict__ last_bin) {
   const int e = blockIdx.x * blockDim.x + threadIdx.x;
-  if (e < nnz) atomicMin(&first_bin[pair[e]], bin_of_entry(bin_ptr, n_bins, e));
+  if (e >= nnz) return;
+  const int j = bin_of_entry(bin_ptr, n_bins, e), p = pair[e];
+  atomicMin(&first_bin[p], j);
+  atomicMax(&last_bin[p], j);
 }
 
-__global__ void bin_count_kernel(const int* __restrict__ first_bin, long long n_pairs, int* __restrict__ count) {
+// key[i] replaces first_bin[i]
+__global__ void bin_count_kernel(int* __restrict__ first_bin, const int* __restrict__ last_bin, long long n_pairs,
+                                 int n_bins, int* __restrict__ count) {
   const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (i < n_pairs) atomicAdd(&count[first_bin[i]], 1);
+  if (i >= n_pairs) return;
+  const int f = first_bin[i];
+  const int key = f >= n_bins ? 2 * n_bins : f + last_bin[i];
+  first_bin[i] = key;
+  atomicAdd(&count[key], 1);
 }
 
 // exclusive scan of count[0 .. n_bins] (one block), result in offs; count is reused as the running cursor
@@ -122,16 +136,17 @@ cudaError_t launch_bin_setup(const int* bin_ptr, const int* pair, const double* 
                              long long n_pad, int* row_map, int* scratch, double* wtab, long long kpad, int2* ranges,
                              cudaStream_t s) {
   int* first_bin = scratch;
-  int* count = scratch + n_pairs;
-  int* offs = count + n_bins + 2;
-  const long long n_init = n_pairs > n_bins + 2 ? n_pairs : n_bins + 2;
+  int* last_bin = scratch + n_pairs;
+  int* count = last_bin + n_pairs;
+  int* offs = count + 2 * n_bins + 2;
+  const long long n_init = n_pairs > 2 * n_bins + 2 ? n_pairs : 2 * n_bins + 2;
   const unsigned gp = (unsigned)((n_pairs + 255) / 256), ge = (unsigned)((nnz + 255) / 256);
-  bin_init_kernel<<<(unsigned)((n_init + 255) / 256), 256, 0, s>>>(first_bin, n_pairs, n_bins, count, ranges);
+  bin_init_kernel<<<(unsigned)((n_init + 255) / 256), 256, 0, s>>>(first_bin, last_bin, n_pairs, n_bins, count, ranges);
   cudaError_t e = cudaMemset2DAsync(wtab, sizeof(double) * kpad, 0, sizeof(double) * n_pad, n_bins, s);
   if (e != cudaSuccess) return e;
-  if (nnz > 0) bin_first_kernel<<<ge, 256, 0, s>>>(bin_ptr, pair, nnz, n_bins, first_bin);
-  bin_count_kernel<<<gp, 256, 0, s>>>(first_bin, n_pairs, count);
-  bin_scan_kernel<<<1, 32, 0, s>>>(count, offs, n_bins + 1);
+  if (nnz > 0) bin_first_kernel<<<ge, 256, 0, s>>>(bin_ptr, pair, nnz, n_bins, first_bin, last_bin);
+  bin_count_kernel<<<gp, 256, 0, s>>>(first_bin, last_bin, n_pairs, n_bins, count);
+  bin_scan_kernel<<<1, 32, 0, s>>>(count, offs, 2 * n_bins + 1);
   bin_place_kernel<<<gp, 256, 0, s>>>(first_bin, n_pairs, count, row_map);
   if (nnz > 0) bin_scatter_kernel<<<ge, 256, 0, s>>>(bin_ptr, pair, w, nnz, n_bins, row_map, wtab, kpad, ranges);
   return cudaGetLastError();
