@@ -66,6 +66,24 @@ def hilbert_matrix_imag(edges, omega_out) -> np.ndarray:
     return -np.log1p(x) / (R - L)[None, :]
 
 
+def hilbert_matrix_real(edges, omega_out) -> np.ndarray:
+    """K[i, j] of Eq. (18) for targets omega_i on the REAL axis (the paper's own use): the Hermitian
+    part of Eq. (14), P[1/(omega - w') - 1/(omega + w')] = 2 w' / (omega^2 - w'^2), averaged over bin j (reading R20):
+      K[i, j] = log|(omega_i^2 - L_j^2) / (omega_i^2 - R_j^2)| / (R_j - L_j).
+    Logarithmically singular where omega_i sits on a bin edge: targets are taken inside bins (e.g. their centres)."""
+    edges = np.asarray(edges, dtype=np.float64)
+    om = np.asarray(omega_out, dtype=np.float64)
+    L, R = edges[:-1], edges[1:]
+    num = np.abs(om[:, None] ** 2 - L[None, :] ** 2)
+    den = np.abs(om[:, None] ** 2 - R[None, :] ** 2)
+    return (np.log(num) - np.log(den)) / (R - L)[None, :]
+
+
+def hilbert_real_ref(A: np.ndarray, edges, omega_out) -> np.ndarray:
+    """Re Pi(omega_i)[I, J] = sum_j K[i, j] A[j][I, J] on the real axis (Eq. 18)."""
+    return np.tensordot(hilbert_matrix_real(edges, omega_out), A, axes=(1, 0))
+
+
 def hilbert_imag_ref(A: np.ndarray, edges, omega_out) -> np.ndarray:
     """chi0(i omega_i)[I, J] = sum_j K[i, j] A[j][I, J]   (Eq. 18; Alg. 1 line 27)."""
     K = hilbert_matrix_imag(edges, omega_out)

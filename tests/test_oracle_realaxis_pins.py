@@ -16,8 +16,8 @@ import pytest
 from scipy import integrate
 
 import oracle
-from oracle.realaxis_oracle import (hilbert_imag_ref, hilbert_matrix_imag, imchi_accumulate_ref, imchi_naive,
-                                    imchi_ref)
+from oracle.realaxis_oracle import (hilbert_imag_ref, hilbert_matrix_imag, hilbert_matrix_real, hilbert_real_ref,
+                                    imchi_accumulate_ref, imchi_naive, imchi_ref)
 from qsgw_synth import binned_pair_weights, generate, get_config, log_bin_edges, scaled_config
 
 
@@ -129,3 +129,29 @@ def test_generator_weights_are_a_partition_of_each_pair():
     inside = (D * 0.95 >= edges[0]) & (D * 1.05 < edges[-1]) & (occ > 1e-12)
     assert np.allclose(tot[inside], occ[inside], rtol=1e-12)
     assert np.all(tot[(D <= 0) | (occ <= 1e-12)] == 0)
+
+
+def test_hilbert_matrix_real_axis_principal_value_and_limits():
+    """Real-axis targets (Eq. 18 as the paper uses it): K against the Cauchy principal value computed by scipy
+    (weight='cauchy') for targets inside bins, against plain quadrature for targets outside the bin, the narrow-bin
+    limit 2 D / (omega^2 - D^2) = Re of the bracket of Eq. (14), and the static limit omega -> 0 shared with the
+    imaginary-axis matrix."""
+    edges = log_bin_edges(9, 0.02, 3.0)
+    om = np.concatenate([[1e-9], 0.5 * (edges[:-1] + edges[1:])[::2], [7.0]])
+    K = hilbert_matrix_real(edges, om)
+    f = lambda x, w: 2.0 * x / (w * w - x * x)
+    for i, w in enumerate(om):
+        for j in range(9):
+            L, R = edges[j], edges[j + 1]
+            if L < w < R:      # 2x/(w^2 - x^2) = -[2x/(w + x)] / (x - w): Cauchy weight 1/(x - w)
+                val = integrate.quad(lambda x: -2.0 * x / (w + x), L, R, weight="cauchy", wvar=w)[0] / (R - L)
+            else:
+                val = integrate.quad(f, L, R, args=(w,), epsabs=1e-13, epsrel=1e-12)[0] / (R - L)
+            assert abs(K[i, j] - val) <= 1e-9 * max(1.0, abs(val)), (i, j, K[i, j], val)
+    D = 0.37
+    w = np.array([0.1, 0.3, 0.5, 2.0])
+    Kn = hilbert_matrix_real([D * (1 - 1e-7), D * (1 + 1e-7)], w)
+    assert np.allclose(Kn[:, 0], (1.0 / (w - D) - 1.0 / (w + D)), rtol=1e-6)
+    assert np.allclose(hilbert_matrix_real(edges, [1e-9]), hilbert_matrix_imag(edges, [0.0]), rtol=1e-9)
+    A = np.random.default_rng(0).standard_normal((9, 3, 3)) + 0j
+    assert np.allclose(hilbert_real_ref(A, edges, om), np.einsum("ij,jab->iab", K, A))
