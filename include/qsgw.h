@@ -220,6 +220,14 @@ int32_t qsgw_imchi_add_batch(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, cons
 int32_t qsgw_hilbert_to_imag_axis(int32_t n_m, int32_t n_bins, const double* d_edges, int32_t n_out,
                                   const double* d_omega_out, const void* d_A, void* d_out, void* cuda_stream);
 
+/* The same transform for targets omega_i ON THE REAL AXIS (Eq. 18 as printed: the Hermitian part of Pi from its spectral
+ * part): K[i][j] = log|(omega_i^2 - L_j^2) / (omega_i^2 - R_j^2)| / (R_j - L_j), the principal value of
+ * 1/(omega - w') - 1/(omega + w') averaged over bin j.  Logarithmically singular where omega_i sits on a bin edge: take the
+ * targets inside bins (e.g. their centres).  Pi(omega_i) = out[i] - i pi A(omega_i) (the anti-Hermitian part is the
+ * spectral part itself, reading R19).  Arguments as qsgw_hilbert_to_imag_axis. */
+int32_t qsgw_hilbert_to_real_axis(int32_t n_m, int32_t n_bins, const double* d_edges, int32_t n_out,
+                                  const double* d_omega_out, const void* d_A, void* d_out, void* cuda_stream);
+
 /* Imaginary-axis part of the correlation self-energy for one k-point and one batch of intermediate states
  * (the step after W^c; Eq. (22); Alg. 2 lines 11-25 and 44):
  *   ZW^c[n', n, nu] = sum_i w^I_i(eps_qn - eps_{q-k,n'}) sum_mu z[n', n, mu] W^c[i][mu, nu]

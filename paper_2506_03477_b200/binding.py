@@ -64,12 +64,13 @@ def lib() -> C.CDLL:
     L.qsgw_sigc_imag_accumulate.argtypes = [vp, vp, dp, dp, vp, i32, i32, vp]
     L.qsgw_imchi_add_batch.argtypes = [vp, vp, i64, vp, i64, i32, i32, i32, i32, vp, vp, dp, i32]
     L.qsgw_hilbert_to_imag_axis.argtypes = [i32, i32, dp, i32, dp, vp, vp, vp]
+    L.qsgw_hilbert_to_real_axis.argtypes = [i32, i32, dp, i32, dp, vp, vp, vp]
     L.qsgw_mixed_stats.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(C.c_double)]
     for name in ("qsgw_create", "qsgw_set_product_tensor", "qsgw_zmel_build", "qsgw_chi0_accumulate",
                  "qsgw_chi0_add_kpoint", "qsgw_chi0_finalize", "qsgw_reset", "qsgw_sync",
                  "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_set_option", "qsgw_mixed_stats", "qsgw_wc_from_chi0",
                  "qsgw_sigc_imag_accumulate", "qsgw_chi0_add_kpoints", "qsgw_imchi_add_batch",
-                 "qsgw_hilbert_to_imag_axis",
+                 "qsgw_hilbert_to_imag_axis", "qsgw_hilbert_to_real_axis",
                  "qsgw_chi0_to_coulomb_basis"):
         getattr(L, name).restype = i32
     for name in ("qsgw_last_error", "qsgw_last_create_error", "qsgw_version"):
@@ -326,7 +327,12 @@ def chi0_to_coulomb_basis(chi0, U, out=None):
     return out
 
 
-def hilbert_to_imag_axis(A, edges, omega_out, out=None):
+def hilbert_to_real_axis(A, edges, omega_out, out=None):
+    """Eq. (18) for real-axis targets (principal value): qsgw_hilbert_to_real_axis."""
+    return hilbert_to_imag_axis(A, edges, omega_out, out=out, _real=True)
+
+
+def hilbert_to_imag_axis(A, edges, omega_out, out=None, _real=False):
     """Eq. (18) on the imaginary axis: out[i] = sum_j K[i][j] A[j] (qsgw_hilbert_to_imag_axis)."""
     import torch
     n_bins, n_m = int(A.shape[0]), int(A.shape[1])
@@ -334,7 +340,8 @@ def hilbert_to_imag_axis(A, edges, omega_out, out=None):
     if out is None:
         out = torch.empty((n_out, n_m, n_m), dtype=torch.complex128, device=A.device)
     st = torch.cuda.current_stream(A.device).cuda_stream
-    rc = lib().qsgw_hilbert_to_imag_axis(n_m, n_bins, _ptr(edges, torch.float64), n_out, _ptr(omega_out, torch.float64),
+    fn = lib().qsgw_hilbert_to_real_axis if _real else lib().qsgw_hilbert_to_imag_axis
+    rc = fn(n_m, n_bins, _ptr(edges, torch.float64), n_out, _ptr(omega_out, torch.float64),
                                          _ptr(A, torch.complex128), _ptr(out, torch.complex128), C.c_void_p(st))
     if rc != 0:
         raise QsgwError(rc, lib().qsgw_last_create_error().decode())

@@ -209,9 +209,10 @@ cudaError_t launch_bin_setup(const int* bin_ptr, const int* pair, const double* 
                              long long n_pad, int* row_map, int* scratch, double* wtab, long long kpad, int2* ranges,
                              cudaStream_t s);
 // out[i][e] = sum_j K[i][j] A[j][e], K[i][j] = -log1p((R^2 - L^2) / (L^2 + omega_i^2)) / (R - L) over bin j = [L, R)
-// (Eq. 18 on the imaginary axis); A, out complex128 [.][n_m][n_m]
-cudaError_t launch_hilbert_imag(int n_m, int n_bins, const double* edges, int n_out, const double* omega_out,
-                                const double2* A, double2* out, cudaStream_t s);
+// (Eq. 18 on the imaginary axis), or for real_axis = 1 K[i][j] = log|(omega_i^2 - L^2) / (omega_i^2 - R^2)| / (R - L) (targets on
+// the real axis, principal value); A, out complex128 [.][n_m][n_m]
+cudaError_t launch_hilbert(int n_m, int n_bins, const double* edges, int n_out, const double* omega_out,
+                           const double2* A, double2* out, int real_axis, cudaStream_t s);
 
 // issue-rate probes (probe_kernels.cu): measured MMA-pipe peaks for the roofline denominators
 cudaError_t probe_fp64_mma(cudaStream_t s, double* out_tflops, double* out_ms);

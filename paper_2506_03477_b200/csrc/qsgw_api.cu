@@ -1156,17 +1156,27 @@ int32_t qsgw_imchi_add_batch(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, cons
   return QSGW_OK;
 }
 
-int32_t qsgw_hilbert_to_imag_axis(int32_t n_m, int32_t n_bins, const double* d_edges, int32_t n_out,
-                                  const double* d_omega_out, const void* d_A, void* d_out, void* cuda_stream) {
+static int32_t hilbert_common(int32_t n_m, int32_t n_bins, const double* d_edges, int32_t n_out, const double* d_omega_out,
+                              const void* d_A, void* d_out, void* cuda_stream, int real_axis) {
   g_create_error.clear();
   if (!d_edges || !d_omega_out || !d_A || !d_out) { g_create_error = "NULL argument"; return QSGW_ERR_INVALID_ARG; }
   if (d_A == d_out) { g_create_error = "d_out aliases d_A"; return QSGW_ERR_INVALID_ARG; }
   if (n_m < 1 || n_bins < 1 || n_out < 1) { g_create_error = "n_m, n_bins and n_out must be positive"; return QSGW_ERR_SHAPE; }
   if (n_bins > 384) { g_create_error = "at most 384 bins (the transform matrix is held in shared memory)"; return QSGW_ERR_SHAPE; }
-  cudaError_t e = qsgw::launch_hilbert_imag(n_m, n_bins, d_edges, n_out, d_omega_out, static_cast<const double2*>(d_A),
-                                            static_cast<double2*>(d_out), static_cast<cudaStream_t>(cuda_stream));
+  cudaError_t e = qsgw::launch_hilbert(n_m, n_bins, d_edges, n_out, d_omega_out, static_cast<const double2*>(d_A),
+                                       static_cast<double2*>(d_out), real_axis, static_cast<cudaStream_t>(cuda_stream));
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("Hilbert transform kernel: ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
   return QSGW_OK;
+}
+
+int32_t qsgw_hilbert_to_imag_axis(int32_t n_m, int32_t n_bins, const double* d_edges, int32_t n_out,
+                                  const double* d_omega_out, const void* d_A, void* d_out, void* cuda_stream) {
+  return hilbert_common(n_m, n_bins, d_edges, n_out, d_omega_out, d_A, d_out, cuda_stream, 0);
+}
+
+int32_t qsgw_hilbert_to_real_axis(int32_t n_m, int32_t n_bins, const double* d_edges, int32_t n_out,
+                                  const double* d_omega_out, const void* d_A, void* d_out, void* cuda_stream) {
+  return hilbert_common(n_m, n_bins, d_edges, n_out, d_omega_out, d_A, d_out, cuda_stream, 1);
 }
 
 int32_t qsgw_sigc_imag_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps_q, const double* d_eps_qk,

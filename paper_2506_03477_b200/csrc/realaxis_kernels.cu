@@ -93,9 +93,12 @@ constexpr int kHilbertOut = 16;      // output frequencies per pass (register ac
 // One thread = one complex element of every bin matrix, 16 output frequencies in registers; the transform
 // coefficients are broadcast reads from shared memory.  Two CTAs per SM and eight loads in flight per thread keep
 // enough bytes in flight for HBM.
-__global__ void __launch_bounds__(256, 2) hilbert_imag_kernel(long long n_cplx, int n_bins, const double* __restrict__ edges,
-                                                              int n_out, int i0, const double* __restrict__ omega_out,
-                                                              const double2* __restrict__ A, double2* __restrict__ out) {
+// real_axis = 0: K = -log1p((R^2 - L^2) / (L^2 + omega^2)) / (R - L)   (targets i omega, Eq. 14 at omega = i omega_i)
+// real_axis = 1: K = log|(omega^2 - L^2) / (omega^2 - R^2)| / (R - L)       (targets omega on the real axis: principal value)
+__global__ void __launch_bounds__(256, 2) hilbert_kernel(long long n_cplx, int n_bins, const double* __restrict__ edges,
+                                                         int n_out, int i0, const double* __restrict__ omega_out,
+                                                         const double2* __restrict__ A, double2* __restrict__ out,
+                                                         int real_axis) {
   extern __shared__ double Ks[];       // [n_bins][kHilbertOut]
   const int n_i = min(kHilbertOut, n_out - i0);
   for (int idx = threadIdx.x; idx < kHilbertOut * n_bins; idx += blockDim.x) {
@@ -103,7 +106,8 @@ __global__ void __launch_bounds__(256, 2) hilbert_imag_kernel(long long n_cplx, 
     double v = 0.0;
     if (i < n_i) {
       const double L = edges[j], R = edges[j + 1], om = omega_out[i0 + i];
-      v = -log1p((R - L) * (R + L) / (L * L + om * om)) / (R - L);
+      v = real_axis ? (log(fabs(om * om - L * L)) - log(fabs(om * om - R * R))) / (R - L)
+                    : -log1p((R - L) * (R + L) / (L * L + om * om)) / (R - L);
     }
     Ks[idx] = v;
   }
@@ -152,15 +156,15 @@ cudaError_t launch_bin_setup(const int* bin_ptr, const int* pair, const double* 
   return cudaGetLastError();
 }
 
-cudaError_t launch_hilbert_imag(int n_m, int n_bins, const double* edges, int n_out, const double* omega_out,
-                                const double2* A, double2* out, cudaStream_t s) {
+cudaError_t launch_hilbert(int n_m, int n_bins, const double* edges, int n_out, const double* omega_out,
+                           const double2* A, double2* out, int real_axis, cudaStream_t s) {
   const long long n_cplx = (long long)n_m * n_m;
   const size_t smem = sizeof(double) * kHilbertOut * n_bins;
   if (smem > 48 * 1024) return cudaErrorInvalidValue;
   long long blocks = (n_cplx + 255) / 256;
   if (blocks > 148LL * 8) blocks = 148LL * 8;
   for (int i0 = 0; i0 < n_out; i0 += kHilbertOut) {
-    hilbert_imag_kernel<<<(unsigned)blocks, 256, smem, s>>>(n_cplx, n_bins, edges, n_out, i0, omega_out, A, out);
+    hilbert_kernel<<<(unsigned)blocks, 256, smem, s>>>(n_cplx, n_bins, edges, n_out, i0, omega_out, A, out, real_axis);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }

@@ -157,6 +157,13 @@ def test_hilbert_transform_and_chain_to_imaginary_axis():
     chain = oracle.hilbert_imag_ref(A_ref, edges, om)
     err = np.linalg.norm((got - chain).reshape(len(om), -1), axis=1) / np.linalg.norm(chain.reshape(len(om), -1), axis=1)
     assert err.max() <= 1e-11, err
+    # real-axis targets (bin centres and a point beyond the mesh): principal-value form of the same transform
+    om_r = np.concatenate([0.5 * (edges[:-1] + edges[1:])[::9], [3.7]])
+    got_r = q.hilbert_to_real_axis(torch.from_numpy(A).cuda(), torch.from_numpy(edges).cuda(),
+                                   torch.from_numpy(om_r).cuda()).cpu().numpy()
+    ref_r = oracle.hilbert_real_ref(A, edges, om_r)
+    err = np.linalg.norm((got_r - ref_r).reshape(len(om_r), -1), axis=1) / np.linalg.norm(ref_r.reshape(len(om_r), -1), axis=1)
+    assert err.max() <= 1e-12, err
     exact = oracle.hermitian_finalize_ref(oracle.chi0_ref(sites_of(prob), sp.Ck, sp.Ckq, sp.eps_k, sp.f_k, sp.eps_kq,
                                                           sp.f_kq, prob.omega))
     dev = np.linalg.norm((got[:16] - exact).reshape(16, -1), axis=1) / np.linalg.norm(exact.reshape(16, -1), axis=1)
