@@ -87,7 +87,8 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   // (few-tile problems: fills the SMs; their partial sums meet in the FP64 accumulator by atomic adds)
   const int chunk = blockIdx.x % a.split, bid = blockIdx.x / a.split;
   const int j = a.j0 + bid % a.n_freq;
-  const int2 tt = a.d_tiles[bid / a.n_freq];
+  const int4 tq = a.d_tiles[bid / a.n_freq];
+  const int2 tt = make_int2(tq.x, tq.y);
   const int s_base = (int)((long long)a.n_stages * chunk / a.split);          // first global stage of this CTA
   const int n_stages = (int)((long long)a.n_stages * (chunk + 1) / a.split) - s_base, win = a.win;
 

@@ -27,11 +27,17 @@ constexpr int W_BYTES3 = KP3 * 8;
 constexpr int SMEM_OPERANDS3 = STAGES * 2 * OPER_BYTES3;
 constexpr int SMEM_BYTES3 = SMEM_OPERANDS3 + STAGES * W_BYTES3 + 2 * STAGES * 8 + 1024 /*align slack*/;
 
-// NARROW: the tile's last 32 columns are padding (N_M mod 64 in 1..32, last tile column): the 8 warps are laid out
-// 4 along I x 2 along J with 16x16 sub-tiles and cover 64 x 32 outputs -- half the DMMAs of a full tile.
-template <bool NARROW>
+// Three CTA shapes over the same 64-column TMA boxes (KIND):
+//   0 full     64 x 64: 8 warps 2 (I) x 4 (J), 32 x 16 sub-tiles                      -- off-diagonal tiles
+//   1 half     64 x 32 at column offset 0 or 32: warps 4 x 2, 16 x 16 sub-tiles       -- last tile column when its last 32
+//              columns are padding (N_M mod 64 in 1..32); right half of a diagonal tile
+//   2 quarter  32 x 32 (rows and columns 0..31): warps 2 x 4, 16 x 8 sub-tiles        -- upper-left block of a diagonal tile
+// A diagonal tile is computed as half (columns 32..63) + quarter: 3/4 of the DMMAs of a full tile (its lower-left
+// 32 x 32 block is never needed: finalize mirrors the upper triangle).
+template <int KIND>
 __device__ __forceinline__ void chi0_f64_3m_body(const Chi0F64Args& a, const unsigned block) {
-  constexpr int MI = NARROW ? 2 : 4;
+  constexpr int MI = KIND == 0 ? 4 : 2;
+  constexpr int NI = KIND == 2 ? 1 : 2;
   extern __shared__ unsigned char smem_dyn[];
   const uint32_t raw = smem_u32(smem_dyn);
   const uint32_t base = (raw + 1023u) & ~1023u;
@@ -43,14 +49,16 @@ __device__ __forceinline__ void chi0_f64_3m_body(const Chi0F64Args& a, const uns
   const int tid = threadIdx.x;
   const int lane = tid & 31, warp = tid >> 5;
   const int g = lane >> 2, t = lane & 3;
-  const int wm = NARROW ? warp >> 1 : warp >> 2, wn = NARROW ? warp & 1 : warp & 3;
+  const int wm = KIND == 1 ? warp >> 1 : warp >> 2, wn = KIND == 1 ? warp & 1 : warp & 3;
 
   // blockIdx.x = ((tile * n_freq) + j) * split + chunk: `split` CTAs share the staged pairs of a (tile, j) when
   // the grid would not fill the SMs; their partial sums meet in the accumulator by atomic adds
   const int chunk = block % a.split, bid = block / a.split;
   const int j = a.j0 + bid % a.n_freq;
   const int tile = bid / a.n_freq;
-  const int2 tt = (NARROW ? a.d_tiles_narrow : a.d_tiles)[tile];
+  const int4 tq = a.d_tiles[(KIND == 0 ? 0 : KIND == 1 ? a.n_tiles : a.n_tiles + a.n_tiles_half) + tile];
+  const int2 tt = make_int2(tq.x, tq.y);
+  const int col_cg = tq.z;                 // first 16-column group of the CTA's columns inside the tile (half: 0 or 2)
   const bool diag = (tt.x == tt.y);
   const int n_all = (int)(a.n_pairs_padded / KP3);
   int it_base = (int)((long long)n_all * chunk / a.split);
@@ -95,11 +103,11 @@ __device__ __forceinline__ void chi0_f64_3m_body(const Chi0F64Args& a, const uns
     for (int par = 0; par < 2; ++par)
       thr_off[s][par] = (uint32_t)((2 * t + s) * 128 + ((((4 * par + (g >> 1)) ^ (2 * t + s)) << 4) | ((g & 1) << 3)));
 
-  double t1[MI][2][2], t2[MI][2][2], t3[MI][2][2];
+  double t1[MI][NI][2], t2[MI][NI][2], t3[MI][NI][2];
 #pragma unroll
   for (int mi = 0; mi < MI; ++mi)
 #pragma unroll
-    for (int ni = 0; ni < 2; ++ni)
+    for (int ni = 0; ni < NI; ++ni)
 #pragma unroll
       for (int e = 0; e < 2; ++e) t1[mi][ni][e] = t2[mi][ni][e] = t3[mi][ni][e] = 0.0;
 
@@ -116,15 +124,16 @@ __device__ __forceinline__ void chi0_f64_3m_body(const Chi0F64Args& a, const uns
     __syncwarp();
     mbar_wait(&full[slot], (it / STAGES) & 1);
 
-    const uint32_t aBase = base + slot * (2 * OPER_BYTES3) + (NARROW ? wm : 2 * wm) * CGRP_BYTES3;
-    const uint32_t bBase = base + slot * (2 * OPER_BYTES3) + (diag ? 0 : OPER_BYTES3) + wn * CGRP_BYTES3;
+    const uint32_t aBase = base + slot * (2 * OPER_BYTES3) + (KIND == 0 ? 2 * wm : wm) * CGRP_BYTES3;
+    const uint32_t bBase = base + slot * (2 * OPER_BYTES3) + (diag ? 0 : OPER_BYTES3) +
+                           (col_cg + (KIND == 2 ? wn >> 1 : wn)) * CGRP_BYTES3;
     const uint32_t wBase = base + SMEM_OPERANDS3 + slot * W_BYTES3;
 
 #pragma unroll
     for (int q = 0; q < KP3 / 4; ++q) {
       const uint32_t rq = (uint32_t)((q >> 1) * 1024);
       const double w = ld_shared_f64(wBase + (uint32_t)((8 * (q >> 1) + 2 * t + (q & 1)) * 8));
-      double ax[MI], ay[MI], as[MI], bx[2], by[2], bd[2];
+      double ax[MI], ay[MI], as[MI], bx[NI], by[NI], bd[NI];
 #pragma unroll
       for (int mi = 0; mi < MI; ++mi) {
         const uint32_t ad = aBase + (mi >> 1) * CGRP_BYTES3 + rq + thr_off[q & 1][mi & 1];
@@ -133,8 +142,8 @@ __device__ __forceinline__ void chi0_f64_3m_body(const Chi0F64Args& a, const uns
         as[mi] = ax[mi] + ay[mi];
       }
 #pragma unroll
-      for (int ni = 0; ni < 2; ++ni) {
-        const uint32_t ad = bBase + rq + thr_off[q & 1][ni];
+      for (int ni = 0; ni < NI; ++ni) {
+        const uint32_t ad = bBase + rq + thr_off[q & 1][KIND == 2 ? (wn & 1) : ni];
         bx[ni] = w * ld_shared_f64(ad);
         by[ni] = w * ld_shared_f64(ad + PLANE_BYTES3);
         bd[ni] = by[ni] - bx[ni];
@@ -142,7 +151,7 @@ __device__ __forceinline__ void chi0_f64_3m_body(const Chi0F64Args& a, const uns
 #pragma unroll
       for (int mi = 0; mi < MI; ++mi)
 #pragma unroll
-        for (int ni = 0; ni < 2; ++ni) {
+        for (int ni = 0; ni < NI; ++ni) {
           dmma884(t1[mi][ni][0], t1[mi][ni][1], ax[mi], bx[ni]);
           dmma884(t2[mi][ni][0], t2[mi][ni][1], ay[mi], by[ni]);
           dmma884(t3[mi][ni][0], t3[mi][ni][1], as[mi], bd[ni]);
@@ -160,8 +169,8 @@ __device__ __forceinline__ void chi0_f64_3m_body(const Chi0F64Args& a, const uns
   for (int mi = 0; mi < MI; ++mi) {
     const int row = tt.x * kTile + (MI * wm + mi) * 8 + g;
 #pragma unroll
-    for (int ni = 0; ni < 2; ++ni) {
-      const int col = tt.y * kTile + (2 * wn + ni) * 8 + 2 * t;
+    for (int ni = 0; ni < NI; ++ni) {
+      const int col = tt.y * kTile + 16 * col_cg + (KIND == 2 ? wn : 2 * wn + ni) * 8 + 2 * t;
       const long long off = (long long)row * a.n_m_pad + col;
       const double r0 = t1[mi][ni][0] + t2[mi][ni][0], r1 = t1[mi][ni][1] + t2[mi][ni][1];
       const double m0 = t3[mi][ni][0] + (t1[mi][ni][0] - t2[mi][ni][0]);
@@ -185,12 +194,13 @@ __device__ __forceinline__ void chi0_f64_3m_body(const Chi0F64Args& a, const uns
   }
 }
 
-// One grid for both tile kinds: the full tiles first, the half-width tiles of the last tile column behind them
-// (short CTAs at the tail of the grid).
+// One grid for the three CTA shapes: the full tiles first, then the half and quarter tiles (short CTAs at the tail).
 __global__ void __launch_bounds__(kThreads3M, 1) chi0_f64_3m_kernel(const __grid_constant__ Chi0F64Args a) {
-  const unsigned n_full = (unsigned)(a.n_tiles * a.n_freq * a.split);
-  if (blockIdx.x < n_full) chi0_f64_3m_body<false>(a, blockIdx.x);
-  else chi0_f64_3m_body<true>(a, blockIdx.x - n_full);
+  const unsigned per = (unsigned)(a.n_freq * a.split);
+  const unsigned n_full = (unsigned)a.n_tiles * per, n_half = (unsigned)a.n_tiles_half * per;
+  if (blockIdx.x < n_full) chi0_f64_3m_body<0>(a, blockIdx.x);
+  else if (blockIdx.x < n_full + n_half) chi0_f64_3m_body<1>(a, blockIdx.x - n_full);
+  else chi0_f64_3m_body<2>(a, blockIdx.x - n_full - n_half);
 }
 
 // chi0[j][I][J] = acc/N_k, lower = conj(upper), Im(diag) = 0  (Hermiticity)
@@ -241,20 +251,28 @@ cudaError_t chi0_f64_configure() {
 }
 
 cudaError_t launch_chi0_f64(const Chi0F64Args& a_in, cudaStream_t s) {
-  if (a_in.n_pairs_padded <= 0 || a_in.n_tiles + a_in.n_tiles_narrow <= 0) return cudaSuccess;
+  if (a_in.n_pairs_padded <= 0 || a_in.n_tiles + a_in.n_tiles_half + a_in.n_tiles_quarter <= 0) return cudaSuccess;
   Chi0F64Args a = a_in;
   a.split = 1;
-  if (!a.d_ranges) {   // few (tile, frequency) items (1 CTA/SM): split the staged pairs over 2..4 CTAs (see launch_chi0_f16)
+  if (!a.d_ranges) {
+    // Few work items (1 CTA/SM): split the staged pairs over 2..4 CTAs per item when that shortens the schedule.
+    // Estimate in units of one full tile (half tiles 0.5, quarter tiles 0.3), CTAs dispatched longest first:
+    //   length(sp) = max(units / SMs, largest item / sp) + (half the smallest item) / sp + 0.01 (sp - 1)
+    // (the last term: the atomic epilogues of split items).
     const int n_sm = a.n_sm;
-    const long long items = (long long)(a.n_tiles + a.n_tiles_narrow) * a.n_freq, n_it = a.n_pairs_padded / KP3;
-    double best = (double)((items + n_sm - 1) / n_sm);
-    for (int sp = 2; sp <= 4; ++sp) {
-      if (n_it < 16 * sp || items * sp > 8LL * n_sm) break;
-      const double cost = (double)((items * sp + n_sm - 1) / n_sm) / sp;
-      if (cost < 0.95 * best) { best = cost; a.split = sp; }
+    const long long items = (long long)(a.n_tiles + a.n_tiles_half + a.n_tiles_quarter) * a.n_freq, n_it = a.n_pairs_padded / KP3;
+    const double units = ((double)a.n_tiles + 0.5 * a.n_tiles_half + 0.3 * a.n_tiles_quarter) * a.n_freq;
+    const double largest = a.n_tiles ? 1.0 : (a.n_tiles_half ? 0.5 : 0.3);
+    const double tail = 0.5 * (a.n_tiles_quarter ? 0.3 : (a.n_tiles_half ? 0.5 : 1.0));
+    double best = 1e300;
+    for (int sp = 1; sp <= 4; ++sp) {
+      if (sp > 1 && (n_it < 16 * sp || items * sp > 16LL * n_sm)) break;
+      const double len = fmax(units / n_sm, largest / sp) + tail / sp + 0.01 * (sp - 1);
+      if (len < best) { best = len; a.split = sp; }
     }
   }
-  chi0_f64_3m_kernel<<<dim3((unsigned)((a.n_tiles + a.n_tiles_narrow) * a.n_freq * a.split)), kThreads3M, SMEM_BYTES3, s>>>(a);
+  chi0_f64_3m_kernel<<<dim3((unsigned)((a.n_tiles + a.n_tiles_half + a.n_tiles_quarter) * a.n_freq * a.split)), kThreads3M,
+                       SMEM_BYTES3, s>>>(a);
   return cudaGetLastError();
 }
 

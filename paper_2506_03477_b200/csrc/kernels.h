@@ -78,10 +78,13 @@ struct Chi0F64Args {
   int split = 1;              // CTAs sharing the staged pairs of one (tile, frequency); set by launch_chi0_f64
   int n_sm = 148;             // SMs of the context's device
   long long n_pairs_padded;   // multiple of kPairAlign
-  const int2* d_tiles;        // (tile_i, tile_j), tile_i <= tile_j
+  // CTA work list (tile_i, tile_j, first 16-column group, 0), tile_i <= tile_j: n_tiles full 64 x 64 tiles, then
+  // n_tiles_half 64 x 32 pieces (last tile column when N_M mod 64 is in 1..32; right half of a diagonal tile), then
+  // n_tiles_quarter 32 x 32 pieces (upper-left block of a diagonal tile)
+  const int4* d_tiles;
   int n_tiles;
-  const int2* d_tiles_narrow = nullptr;   // tiles of the last tile column when its last 32 columns are padding
-  int n_tiles_narrow = 0;                 // (N_M mod 64 in 1..32): computed 64 x 32 wide by a second launch
+  int n_tiles_half = 0;
+  int n_tiles_quarter = 0;
   const int2* d_ranges = nullptr;   // optional [n_freq]: pair rows [x, y) that carry weight at that frequency (bin);
                                     // the CTA runs only the 32-pair stages that cover them (no split)
 };
@@ -132,7 +135,7 @@ struct Chi0F16Args {
   int split = 1;         // CTAs sharing the staged pairs of one (tile, frequency); set by launch_chi0_f16
   int n_sm = 148;        // SMs of the context's device
   const MixedCtl* ctl;   // device: use_fp8 selects the variant that runs (the other one exits at once)
-  const int2* d_tiles;   // 128x128 tiles, tile_i <= tile_j
+  const int4* d_tiles;   // 128x128 tiles (tile_i, tile_j, 0, 0), tile_i <= tile_j
   int n_tiles;
 };
 cudaError_t chi0_f16_configure();

@@ -72,7 +72,7 @@ struct qsgw_ctx {
   std::vector<double> omega;
   cudaStream_t stream = nullptr;
   // derived
-  int ncg = 0, n_m_pad = 0, n_tiles = 0, n_tiles_narrow = 0;
+  int ncg = 0, n_m_pad = 0, n_tiles = 0, n_tiles_half = 0, n_tiles_quarter = 0;
   long long kpad = 0;           // pair capacity of the z workspace (multiple of 32): several band batches are
   long long fill = 0;           // staged back to back ([0, fill) is pending) and accumulated by ONE stage (b) launch
   // device
@@ -80,7 +80,7 @@ struct qsgw_ctx {
   int* d_pb_off = nullptr;
   int* d_orb_off = nullptr;
   long long* d_p_off = nullptr;
-  int2* d_tiles = nullptr;
+  int4* d_tiles = nullptr;
   double* d_omega = nullptr;
   double2* d_P = nullptr;
   long long p_elems = 0;
@@ -527,16 +527,30 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     return create_fail(c, QSGW_ERR_ALLOC, buf);
   }
   const int nt = c->n_m_pad / tile_edge;
-  // FP64 mode: when the last 32 columns of the last tile column are padding its tiles go to a second list that the
-  // half-width kernel variant computes (cfg 2: N_M = 600 = 9 x 64 + 24; cfg 4: 2400 = 37 x 64 + 32)
+  // Work list of the stage (b) kernels.  Mixed mode: the upper 128 x 128 tiles.  FP64 mode (chi0_f64_kernels.cu): full
+  // 64 x 64 tiles off the diagonal; 64 x 32 pieces for the last tile column when its last 32 columns are padding (cfg 2:
+  // N_M = 600 = 9 x 64 + 24; cfg 4: 2400 = 37 x 64 + 32) and for the right half of every diagonal tile; 32 x 32 pieces for
+  // the upper-left block of every diagonal tile (a diagonal tile costs 3/4 of a full one).
   const int rem = c->n_m % tile_edge;
   const bool narrow_last = !mixed && rem >= 1 && rem <= 32;
-  std::vector<int2> tiles, tiles_narrow;
+  std::vector<int4> tiles, tiles_half, tiles_quarter;
   for (int tj = 0; tj < nt; ++tj)
-    for (int ti = 0; ti <= tj; ++ti) (narrow_last && tj == nt - 1 ? tiles_narrow : tiles).push_back(make_int2(ti, tj));
+    for (int ti = 0; ti <= tj; ++ti) {
+      const bool last_narrow = narrow_last && tj == nt - 1;
+      if (mixed) {
+        tiles.push_back(make_int4(ti, tj, 0, 0));
+      } else if (ti == tj) {
+        tiles_quarter.push_back(make_int4(ti, tj, 0, 0));
+        if (!last_narrow) tiles_half.push_back(make_int4(ti, tj, 2, 0));
+      } else {
+        (last_narrow ? tiles_half : tiles).push_back(make_int4(ti, tj, 0, 0));
+      }
+    }
   c->n_tiles = (int)tiles.size();
-  c->n_tiles_narrow = (int)tiles_narrow.size();
-  tiles.insert(tiles.end(), tiles_narrow.begin(), tiles_narrow.end());     // one device array: full tiles, then narrow
+  c->n_tiles_half = (int)tiles_half.size();
+  c->n_tiles_quarter = (int)tiles_quarter.size();
+  tiles.insert(tiles.end(), tiles_half.begin(), tiles_half.end());         // one device array: full, half, quarter
+  tiles.insert(tiles.end(), tiles_quarter.begin(), tiles_quarter.end());
 
 #define QSGW_TRY_ALLOC(expr)                                                                     \
   do {                                                                                           \
@@ -579,7 +593,7 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_pb_off, pb_off.data(), sizeof(int) * (c->n_sites + 1), cudaMemcpyHostToDevice, st));
   QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_orb_off, orb_off.data(), sizeof(int) * (c->n_sites + 1), cudaMemcpyHostToDevice, st));
   QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_p_off, p_off.data(), sizeof(long long) * c->n_sites, cudaMemcpyHostToDevice, st));
-  QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_tiles, tiles.data(), sizeof(int2) * tiles.size(), cudaMemcpyHostToDevice, st));
+  QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_tiles, tiles.data(), sizeof(int4) * tiles.size(), cudaMemcpyHostToDevice, st));
   QSGW_TRY_CUDA(cudaMemcpyAsync(c->d_omega, c->omega.data(), sizeof(double) * c->n_freq, cudaMemcpyHostToDevice, st));
   QSGW_TRY_CUDA(cudaMemsetAsync(c->d_zws, 0, z64_bytes, st));
   if (c->f16) {
@@ -901,8 +915,8 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
   a.n_sm = ctx->n_sm;
   a.d_tiles = ctx->d_tiles;
   a.n_tiles = ctx->n_tiles;
-  a.d_tiles_narrow = ctx->d_tiles + ctx->n_tiles;
-  a.n_tiles_narrow = ctx->n_tiles_narrow;
+  a.n_tiles_half = ctx->n_tiles_half;
+  a.n_tiles_quarter = ctx->n_tiles_quarter;
   {
     StageScope ts(ctx, QSGW_STAGE_CHI0);
     e = qsgw::launch_chi0_f64(a, ctx->stream);
@@ -1141,8 +1155,8 @@ int32_t qsgw_imchi_add_batch(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, cons
   a.n_sm = ctx->n_sm;
   a.d_tiles = ctx->d_tiles;
   a.n_tiles = ctx->n_tiles;
-  a.d_tiles_narrow = ctx->d_tiles + ctx->n_tiles;
-  a.n_tiles_narrow = ctx->n_tiles_narrow;
+  a.n_tiles_half = ctx->n_tiles_half;
+  a.n_tiles_quarter = ctx->n_tiles_quarter;
   a.d_ranges = ctx->d_ranges;
   {
     StageScope ts(ctx, QSGW_STAGE_CHI0);
