@@ -423,6 +423,35 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
                 sigc["accuracy"] = {"rel_frobenius_err": float(_np.linalg.norm(got - ref) / _np.linalg.norm(ref)),
                                     "against": f"oracle.sigc_imag_ref on the first {n_sub} intermediate states of "
                                                f"{nks} k-points, W^c from the GPU", "tolerance": 1e-10}
+            sig64 = None
+            if not args.no_accuracy:
+                sigc_pass()
+                torch.cuda.synchronize(dev)
+                sig64 = sig.clone()
+            sctx.destroy()
+            # the same pass on a QSGW_PREC_MIXED context: ZW^c on tcgen05 with FP16-split operands (sigc_f16_kernel)
+            sctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, cfg.n_k, n_all, n_qp, precision=q.PREC_MIXED)
+            sctx.set_product_tensor(torch.from_numpy(prob.P).to(dev))
+            sigc_pass()
+            torch.cuda.synchronize(dev)
+            ts = []
+            for _ in range(3):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                sigc_pass()
+                e1.record()
+                torch.cuda.synchronize(dev)
+                ts.append(e0.elapsed_time(e1))
+            m_ms = statistics.median(ts)
+            tf32_peak, psrc = tensor_peak("tf32", True)
+            sigc["mixed"] = {"ms": m_ms, "ms_runs": [round(t, 2) for t in ts], "value": (fl_a + fl_zw + fl_c) / (m_ms * 1e-3) / 1e12,
+                             "unit": UNIT, "peak": tf32_peak, "frac": (fl_a + fl_zw + fl_c) / (m_ms * 1e-3) / 1e12 / tf32_peak,
+                             "peak_source": f"{psrc} bf16 cuBLAS sustained x nominal tf32/bf16 ratio (1100/2250)",
+                             "what": "same pass on a QSGW_PREC_MIXED context: three FP16 products per term on tcgen05 "
+                                     "(sigc_f16_kernel), FP32 sums, closing contraction in FP64; same credited flop"}
+            if sig64 is not None:
+                sigc["mixed"]["rel_frobenius_dev_from_fp64"] = float((sig - sig64).norm() / sig64.norm())
+                sigc["mixed"]["tolerance"] = 1e-5
             sctx.destroy()
             del d_Cq, d_Cqk, sig
         # next row f3: the paper's own real-axis route (Eqs. 15-18, Alg. 1 lines 12-27): binned spectral part of two

@@ -217,6 +217,19 @@ cudaError_t launch_bin_setup(const int* bin_ptr, const int* pair, const double* 
 cudaError_t launch_hilbert(int n_m, int n_bins, const double* edges, int n_out, const double* omega_out,
                            const double2* A, double2* out, int real_axis, cudaStream_t s);
 
+// mixed mode (sigc_f16_kernels.cu): ZW^c on tcgen05 with FP16-split operands.  zk16 / w16: workspaces of sigc_f16_z_halves /
+// sigc_f16_w_halves halves; amax: 1 + n_freq floats.  z: complex128 [pairs][n_m], wc: [n_freq][n_m][n_m], zw: out [pairs][n_m].
+size_t sigc_f16_z_halves(long long pairs_cap, int n_m);
+size_t sigc_f16_w_halves(int n_m, int n_freq);
+cudaError_t sigc_f16_configure();
+cudaError_t launch_sigc_zw_f16(const double2* z, const double2* wc, const double* w, long long ld_w, int pairs, int n_m,
+                               int n_freq, __half* zk16, __half* w16, float* amax, double2* zw, cudaStream_t s);
+// 3-D FLOAT16 tensor map over hl16 rows: dims {row_halves, rows, 2 planes}, box {64, 64, 1}, 128-byte swizzle (qsgw_api.cu)
+cudaError_t make_hl16_map(CUtensorMap* out, const void* base, long long row_halves, long long rows, long long plane_halves);
+// closing contraction of I^c alone (sigc_kernels.cu): sigc[n, m] += -(1/N_k) sum_{n', nu} zw[(n', n), nu] conj(z[(n', m), nu])
+cudaError_t launch_sigc_close(const double2* z, const double2* zw, int n_all, int n_qp, int n_m, double inv_nk, double2* sigc,
+                              int n_sm, cudaStream_t s);
+
 // issue-rate probes (probe_kernels.cu): measured MMA-pipe peaks for the roofline denominators
 cudaError_t probe_fp64_mma(cudaStream_t s, double* out_tflops, double* out_ms);
 cudaError_t probe_tf32_mma(cudaStream_t s, double* out_tflops, double* out_ms);

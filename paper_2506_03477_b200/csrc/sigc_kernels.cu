@@ -67,6 +67,11 @@ cudaError_t launch_sigc_imag(const double2* z, const double* w, long long ld_w, 
   g.row_scale = w; g.ld_scale = ld_w;
   cudaError_t e = launch_zgemm(true, false, g, s);
   if (e != cudaSuccess) return e;
+  return launch_sigc_close(z, zw, n_all, n_qp, n_m, inv_nk, sigc, n_sm, s);
+}
+
+cudaError_t launch_sigc_close(const double2* z, const double2* zw, int n_all, int n_qp, int n_m, double inv_nk, double2* sigc,
+                              int n_sm, cudaStream_t s) {
   ZgemmArgs c;
   c.A = zw; c.lda = n_m; c.rA = (long long)n_qp * n_m;
   c.B = z; c.ldb = n_m; c.rB = (long long)n_qp * n_m;

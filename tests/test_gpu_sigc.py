@@ -29,7 +29,7 @@ def oracle_sigc(prob, wcs, n_k_norm=None, spin=0):
     return oracle.sigc_imag_ref(z, sp.eps_k[0], [sp.eps_kq[k] for k in range(n_k)], wcs, prob.omega, n_k_norm=n_k_norm)
 
 
-def cuda_sigc(prob, wcs, precision=0, n_k_norm=None, batch_all=None, pass_z=False, spin=0):
+def cuda_sigc(prob, wcs, precision=0, n_k_norm=None, batch_all=None, pass_z=False, spin=0, options=None):
     """I^c through the C ABI; batch_all splits the intermediate states into band batches (Alg. 2 line 10)."""
     import torch
     import paper_2506_03477_b200 as q
@@ -39,6 +39,8 @@ def cuda_sigc(prob, wcs, precision=0, n_k_norm=None, batch_all=None, pass_z=Fals
     b_all = batch_all or n_all
     ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, n_k if n_k_norm is None else n_k_norm,
                         b_all, n_qp, precision=precision)
+    for key, val in (options or {}).items():
+        ctx.set_option(key, val)
     ctx.set_product_tensor(torch.from_numpy(prob.P).cuda())
     Cq = torch.from_numpy(sp.Ck[0]).cuda()
     eq = torch.from_numpy(sp.eps_k[0]).cuda()
@@ -128,13 +130,29 @@ def test_degenerate_weights_zero_dE_and_empty_tail():
     assert rel_fro(got, ref) <= TOL
 
 
-def test_mixed_context_fp32_grade_z():
-    """A QSGW_PREC_MIXED context: z comes from the FP16-split planes (FP32-grade values), the I^c GEMMs stay FP64."""
-    prob = generate(RAGGED)
-    wcs = [synthetic_wc(prob.cfg.n_m, prob.omega, seed=k) for k in range(prob.cfg.n_k)]
-    ref = oracle_sigc(prob, wcs)
-    got = cuda_sigc(prob, wcs, precision=1)
-    assert 1e-12 < rel_fro(got, ref) <= 1e-6
+@pytest.mark.parametrize("case", ["ragged", "cfg1", "cfg2"])
+def test_mixed_context_tcgen05_zw(case):
+    """A QSGW_PREC_MIXED context runs the frequency loop ZW^c on tcgen05 with FP16-split operands (FP32-grade products,
+    FP32 sums over mu and i, the closing contraction in FP64): tolerance 1e-5 relative Frobenius on I^c (the north_star
+    mixed bar is 2e-5); option "sigc_f64" keeps the FP64 GEMM on the FP32-grade z (<= 1e-6)."""
+    if case == "ragged":
+        prob = generate(RAGGED)
+        n_k_norm = None
+        wcs = [synthetic_wc(prob.cfg.n_m, prob.omega, seed=k, hermitian=False) for k in range(prob.cfg.n_k)]
+    else:
+        cfg = get_config(1 if case == "cfg1" else 2)
+        prob = generate(cfg, n_k=3)
+        n_k_norm = cfg.n_k
+        wcs = [synthetic_wc(cfg.n_m, prob.omega, seed=k) for k in range(3)]
+    ref = oracle_sigc(prob, wcs, n_k_norm=n_k_norm)
+    got = cuda_sigc(prob, wcs, precision=1, n_k_norm=n_k_norm)
+    err = rel_fro(got, ref)
+    assert 1e-12 < err <= 1e-5, err
+    if case == "ragged":
+        got64 = cuda_sigc(prob, wcs, precision=1, n_k_norm=n_k_norm, options={"sigc_f64": 1})
+        assert 1e-12 < rel_fro(got64, ref) <= 1e-6
+        got_b = cuda_sigc(prob, wcs, precision=1, n_k_norm=n_k_norm, batch_all=8, pass_z=True)
+        assert rel_fro(got_b, ref) <= 1e-5
 
 
 def test_state_and_shape_errors():
