@@ -246,8 +246,12 @@ int32_t qsgw_hilbert_to_real_axis(int32_t n_m, int32_t n_bins, const double* d_e
  *   d_sigc   : complex128 [n_qp][n_qp] row-major, ACCUMULATED (the caller zeroes it before the first call);
  *              1/N_k is the context's n_k.  Not Hermitian: the weight carries eps_qn of the row index (Eq. 3
  *              symmetrises later).
- * FP64 arithmetic on the FP64 tensor pipe in both precision modes.  n_all <= max_n_o, n_qp <= max_n_u.  The
- * context allocates its I^c workspace (two z-sized buffers and the weight table) at the first call.
+ * QSGW_PREC_FP64: FP64 arithmetic on the FP64 tensor pipe (parity <= 1e-10).  QSGW_PREC_MIXED: the frequency loop ZW^c
+ * runs on the tcgen05 tensor cores with z and W^c carried as FP16 pieces (FP32-grade products, three FP16 MMAs per
+ * term; the paper runs this GEMM in TF32), FP32 sums over mu and the frequencies, the closing
+ * contraction in FP64: relative Frobenius error of I^c <= 1e-5; option "sigc_f64" = 1 keeps the FP64 GEMM on the
+ * context's FP32-grade z.  n_all <= max_n_o, n_qp <= max_n_u.  The context allocates its I^c workspace (two z-sized
+ * buffers, the weight table and, in mixed mode, the FP16-split copies of z and W^c) at the first call.
  * Stream-ordered, does not synchronise; does not touch the chi0 accumulator or the staged batches. */
 int32_t qsgw_sigc_imag_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps_q, const double* d_eps_qk,
                                   const void* d_wc, int32_t n_all, int32_t n_qp, void* d_sigc);
@@ -293,6 +297,7 @@ int32_t qsgw_mixed_stats(qsgw_ctx* ctx, int64_t* out_launches, int64_t* out_laun
  *   "mixed_fp8"       0 | 1 | 2  E5M2 correction products never | always | chosen on the device (default 2)
  *   "mixed_fp8_threshold_x100"  T*100: automatic choice takes E5M2 when P_eff >= T * N_M (default T = 4)
  *   "mixed_window"    1..64    pipeline stages per TMEM drain window (default 8)
+ *   "sigc_f64"        0 | 1    mixed context: qsgw_sigc_imag_accumulate on tcgen05 (default) | with the FP64 GEMM
  *   "e2e_groups"      1..4     frequency groups of the last launch of qsgw_chi0_run_host (default 4)
  * ctx == NULL, process-wide:
  *   "wc_graph"        0 | 1 | 2  qsgw_wc_from_chi0: plain launches | CUDA graph with fallback (default) | graph or fail

@@ -152,11 +152,10 @@ def test_wc_full_size_cfg4(cfg4_case):
     assert rel_fro_per_freq(got, ref).max() <= 1e-10
 
 
-def test_sigc_full_size_cfg4():
-    """I^c (Eq. 22) at cfg-4 size as bench.py times it: N_M = 2400, 336 intermediate states x 64 q states, 16
-    frequencies, one k-point; the whole 64 x 64 matrix against the oracle (1.6e13 flop of NumPy, ~40 s)."""
-    import torch
-    import paper_2506_03477_b200 as q
+@pytest.fixture(scope="module")
+def sigc_cfg4_case():
+    """I^c at cfg-4 size: one k-point, 336 intermediate states x 64 q states, 16 frequencies; the oracle's 64 x 64 matrix
+    (1.6e13 flop of NumPy, ~40 s), computed once for both precision modes."""
     from qsgw_synth import synthetic_wc
     cfg = get_config(4)
     prob = generate(cfg, n_k=1)
@@ -165,7 +164,18 @@ def test_sigc_full_size_cfg4():
     sites = [prob.P_site(s) for s in range(cfg.n_sites)]
     z = oracle.zmel_ref(sites, sp.Ckq[0], sp.Ck[0])
     ref = oracle.sigc_imag_ref([z], sp.eps_k[0], [sp.eps_kq[0]], [wc], prob.omega, n_k_norm=cfg.n_k)
-    ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, cfg.n_k, cfg.n_u, cfg.n_o)
+    return prob, wc, ref
+
+
+@pytest.mark.parametrize("precision,tol", [(0, 1e-10), (1, 1e-5)])
+def test_sigc_full_size_cfg4(sigc_cfg4_case, precision, tol):
+    """I^c (Eq. 22) at cfg-4 size as bench.py times it (N_M = 2400): the whole 64 x 64 matrix against the oracle, in FP64
+    (zgemm_tma_kernel) and on a mixed context (sigc_f16_kernel: FP16-split operands on tcgen05)."""
+    import torch
+    import paper_2506_03477_b200 as q
+    prob, wc, ref = sigc_cfg4_case
+    cfg, sp = prob.cfg, prob.spins[0]
+    ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, cfg.n_k, cfg.n_u, cfg.n_o, precision=precision)
     ctx.set_product_tensor(torch.from_numpy(prob.P).cuda())
     sig = torch.zeros((cfg.n_o, cfg.n_o), dtype=torch.complex128, device="cuda")
     ctx.zmel_build(torch.from_numpy(sp.Ckq[0]).cuda(), torch.from_numpy(sp.Ck[0]).cuda(), 0, cfg.n_u, 0, cfg.n_o)
@@ -174,4 +184,7 @@ def test_sigc_full_size_cfg4():
     ctx.sync()
     got = sig.cpu().numpy()
     ctx.destroy()
-    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 1e-10
+    err = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    assert err <= tol, err
+    if precision == 1:
+        assert err > 1e-12
