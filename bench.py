@@ -517,6 +517,20 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
                                               "tolerance": 1e-11}
                 del A_h, got
             rctx.destroy()
+            # the same binned accumulation on a QSGW_PREC_MIXED context (per-bin products on tcgen05, FP16-split rows)
+            A64 = A.clone() if not args.no_accuracy else None
+            rctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, edges[:-1], cfg.n_k, cfg.n_o, cfg.n_u, precision=q.PREC_MIXED)
+            rctx.set_product_tensor(torch.from_numpy(prob.P).to(dev))
+            ram_ms = timed(ra_pass)
+            realaxis["mixed"] = {"imchi_ms": ram_ms, "imchi_value": fl_ra / (ram_ms * 1e-3) / 1e12, "unit": UNIT,
+                                 "what": "same pass on a QSGW_PREC_MIXED context: chi0_f16_kernel over the per-bin row ranges"}
+            if A64 is not None:
+                num = (A - A64).flatten(1).norm(dim=1)
+                den = A64.flatten(1).norm(dim=1)
+                realaxis["mixed"]["max_rel_frobenius_dev_from_fp64_per_bin"] = float((num / den.clamp_min(1e-300))[den > 0].max())
+                realaxis["mixed"]["tolerance"] = 2e-5
+                del A64
+            rctx.destroy()
             del A, h_out
         else:
             del w_out

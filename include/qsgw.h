@@ -189,7 +189,7 @@ int32_t qsgw_wc_from_chi0(int32_t n_m, int32_t n_freq, const void* d_chi0, const
 int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_chi0, const void* d_U, void* d_out,
                                    void* cuda_stream);
 
-/* The paper's own real-axis route (Eqs. 15-18; Alg. 1 lines 9-27), FP64 mode.
+/* The paper's own real-axis route (Eqs. 15-18; Alg. 1 lines 9-27).
  * A context whose n_freq "frequencies" are the histogram bins [edges[j], edges[j+1]) of the real axis (h_omega = any
  * increasing labels, e.g. the lower edges; they are not used by this path) accumulates the bin-integrated spectral
  * weight
@@ -203,7 +203,8 @@ int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_ch
  * The gather of Alg. 1 line 17 is a permutation applied when z is written (pairs sorted by the first bin that carries
  * them), so each bin multiplies one short contiguous row range; pairs without an entry cost nothing in stage (b).
  * Accumulates into the context's accumulator (qsgw_reset zeroes it, qsgw_chi0_finalize returns A with the Hermitian
- * mirror and 1/N_k); batches staged by qsgw_chi0_accumulate are flushed first.  QSGW_ERR_UNSUPPORTED in mixed mode.
+ * mirror and 1/N_k); batches staged by qsgw_chi0_accumulate are flushed first.  QSGW_PREC_MIXED runs the per-bin products on
+ * tcgen05 with FP16-split operands (three FP16 products unless "mixed_fp8" forces E5M2; <= 2e-5 per bin).
  * The summation order inside a bin is not fixed (atomic placement): results agree to rounding between runs. */
 int32_t qsgw_imchi_add_batch(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const void* d_Ckq, int64_t ld_kq,
                              int32_t n_begin, int32_t n_o, int32_t np_begin, int32_t n_u, const int32_t* d_bin_ptr,

@@ -89,8 +89,15 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   const int j = a.j0 + bid % a.n_freq;
   const int4 tq = a.d_tiles[bid / a.n_freq];
   const int2 tt = make_int2(tq.x, tq.y);
-  const int s_base = (int)((long long)a.n_stages * chunk / a.split);          // first global stage of this CTA
-  const int n_stages = (int)((long long)a.n_stages * (chunk + 1) / a.split) - s_base, win = a.win;
+  int s_base = (int)((long long)a.n_stages * chunk / a.split);          // first global stage of this CTA
+  int n_stages = (int)((long long)a.n_stages * (chunk + 1) / a.split) - s_base;
+  const int win = a.win;
+  if (a.d_ranges) {           // binned real-axis path: only the stages that cover the rows carrying weight in this bin
+    const int2 r = a.d_ranges[j];
+    s_base = r.x / kPairStage;
+    n_stages = r.y > r.x ? (r.y + kPairStage - 1) / kPairStage - s_base : 0;
+    if (n_stages <= 0) return;
+  }
 
   if (tid == 0) {
     tma_prefetch_desc(&a.tmap);
@@ -346,7 +353,7 @@ cudaError_t launch_chi0_f16(const Chi0F16Args& a_in, cudaStream_t s) {
   // Few (tile, frequency) work items: split the staged pairs over 2..4 CTAs each, choosing the split that
   // minimises rounds(CTAs / SMs) / split; every CTA keeps >= 32 stages.
   a.split = 1;
-  {
+  if (!a.d_ranges) {
     const int n_sm = a.n_sm;
     const long long items = (long long)a.n_tiles * a.n_freq;
     double best = (double)((items + n_sm - 1) / n_sm);

@@ -135,6 +135,7 @@ struct Chi0F16Args {
   int split = 1;         // CTAs sharing the staged pairs of one (tile, frequency); set by launch_chi0_f16
   int n_sm = 148;        // SMs of the context's device
   const MixedCtl* ctl;   // device: use_fp8 selects the variant that runs (the other one exits at once)
+  const int2* d_ranges = nullptr;   // optional [n_freq]: pair rows [x, y) that carry weight at that frequency (bin); no split
   const int4* d_tiles;   // 128x128 tiles (tile_i, tile_j, 0, 0), tile_i <= tile_j
   int n_tiles;
 };
@@ -149,8 +150,10 @@ cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m
                              long long z_bs, cudaStream_t s);
 cudaError_t launch_z_export_hl16(const void* zhl, long long kpad, int n_m_pad, int n_m, long long n_pairs,
                                  const float* zmax, double2* out, cudaStream_t s);
+// zfold (optional): the weights are multiplied by 2^(-2S), S = f16_scale_exp(*zfold) (binned path: one batch per flush, its
+// weights come from the caller and do not carry the batch's FP16 scale yet)
 cudaError_t launch_weights_scale_hl16(const double* wtab, void* wtab16, double* wscale, long long kpad, long long n_pad,
-                                      int n_freq, MixedCtl* ctl, cudaStream_t s);
+                                      int n_freq, MixedCtl* ctl, const float* zfold, cudaStream_t s);
 
 // ---- batched complex FP64 GEMM on the FP64 tensor pipe, operands staged by TMA (zgemm_tma_kernels.cu) ----------
 // C (+)= alpha * sum_{r < reps} diag(row_scale[r]) opA(A_r) opB(B_r)   on 64x64 tiles, complex128 interleaved, row-major.

@@ -125,6 +125,8 @@ struct qsgw_ctx {
   int* d_binscratch = nullptr;  // [2 batch_pad + 4 (n_freq + 1)]
   int2* d_ranges = nullptr;     // [n_freq] rows touched by each bin
   const int* cur_row_map = nullptr;   // row map of the stage (a) launch being issued (NULL: natural pair order)
+  const int2* flush_ranges = nullptr; // binned path, mixed mode: per-bin row ranges of the flush being issued
+  const float* flush_zfold = nullptr; // ... and the batch maximum whose FP16 scale its caller-made weights still lack
   // I^c workspace (qsgw_sigc_imag_accumulate; allocated by its first call)
   double2* d_sz = nullptr;      // z of the batch, complex128 [pairs][N_M]
   double2* d_szw = nullptr;     // ZW^c, same shape
@@ -895,7 +897,7 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
     if (first) {
       StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
       e = qsgw::launch_weights_scale_hl16(ctx->d_wtab, ctx->d_wtab32, ctx->d_wscale, ctx->kpad, n_pad, ctx->n_freq,
-                                          ctx->d_ctl, ctx->stream);
+                                          ctx->d_ctl, ctx->flush_zfold, ctx->stream);
       if (e != cudaSuccess) return ctx->cuda_fail(e, "weight scaling kernel launch");
       ctx->launches += 1;
     }
@@ -914,6 +916,7 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
     m.n_stages = (int)(n_pad / qsgw::kPairStage);
     m.n_sm = ctx->n_sm;
     m.ctl = ctx->d_ctl;
+    m.d_ranges = ctx->flush_ranges;
     m.d_tiles = ctx->d_tiles;
     m.n_tiles = ctx->n_tiles;
     {
@@ -1130,7 +1133,6 @@ int32_t qsgw_imchi_add_batch(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, cons
                              const int32_t* d_pair, const double* d_w, int32_t nnz) {
   if (!ctx) return QSGW_ERR_INVALID_ARG;
   if (ctx->state == ST_CREATED) return ctx->fail(QSGW_ERR_STATE, "set_product_tensor must precede imchi_add_batch");
-  if (ctx->f16) return ctx->fail(QSGW_ERR_UNSUPPORTED, "the binned real-axis path is built for QSGW_PREC_FP64 only");
   if (!d_Ck || !d_Ckq || !d_bin_ptr || (nnz > 0 && (!d_pair || !d_w))) return ctx->fail(QSGW_ERR_INVALID_ARG, "NULL argument");
   if (ld_k < ctx->n_b || ld_kq < ctx->n_b)
     return ctx->fail(QSGW_ERR_INVALID_ARG, "leading dimension smaller than N_b=%d", ctx->n_b);
@@ -1164,6 +1166,21 @@ int32_t qsgw_imchi_add_batch(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, cons
                      n_begin, n_o, np_begin, n_u, 1, 0, n_pad, 0);
   ctx->cur_row_map = nullptr;
   if (rc != QSGW_OK) return rc;
+  if (ctx->f16) {
+    // mixed mode: the batch (FP16-split rows, scale from its measured maximum) is accumulated at once by the tcgen05
+    // kernel over the per-bin row ranges; the caller's weights get the batch's 2^(-2S) when they are split into FP16 pieces
+    ctx->fill = n_pad;
+    ctx->flush_ranges = ctx->d_ranges;
+    ctx->flush_zfold = ctx->d_zmax;
+    rc = flush_pending(ctx);
+    ctx->flush_ranges = nullptr;
+    ctx->flush_zfold = nullptr;
+    if (rc != QSGW_OK) return rc;
+    ctx->pairs += n_pairs;
+    ctx->state = ST_READY;
+    ctx->err.clear();
+    return QSGW_OK;
+  }
   qsgw::Chi0F64Args a;
   a.tmap_z = ctx->tmap_z;
   a.wtab = ctx->d_wtab;

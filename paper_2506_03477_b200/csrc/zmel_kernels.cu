@@ -281,13 +281,15 @@ __global__ void z_export_hl16_kernel(const __half* __restrict__ zhl, long long k
 // finish takes the minimum over j and sets ctl->use_fp8.
 __global__ void __launch_bounds__(1024) weights_scale_hl16_kernel(const double* __restrict__ wtab,
                                                                   __half* __restrict__ w16, double* __restrict__ wscale,
-                                                                  long long kpad, long long n_pad, MixedCtl* ctl) {
+                                                                  long long kpad, long long n_pad, MixedCtl* ctl,
+                                                                  const float* __restrict__ zfold) {
   __shared__ double red[3][32];
   const int j = blockIdx.x;
   const double* wr = wtab + (long long)j * kpad;
+  const double fold = zfold ? exp2(-2.0 * (double)f16_scale_exp(*zfold)) : 1.0;
   double m = 0.0, s1 = 0.0, s2 = 0.0;
   for (long long p = threadIdx.x; p < n_pad; p += blockDim.x) {
-    const double w = wr[p];
+    const double w = wr[p] * fold;
     m = fmax(m, fabs(w));
     s1 += w;
     s2 += w * w;
@@ -318,7 +320,7 @@ __global__ void __launch_bounds__(1024) weights_scale_hl16_kernel(const double* 
   if (threadIdx.x == 0) wscale[j] = exp2((double)e);
   __half* o = w16 + (long long)j * kpad * 2;
   for (long long p = threadIdx.x; p < n_pad; p += blockDim.x) {
-    const float v = (float)(wr[p] * sigma);
+    const float v = (float)(wr[p] * fold * sigma);
     const __half h = __float2half_rn(v);
     o[(p >> 5) * 64 + (p & 31)] = h;
     o[(p >> 5) * 64 + 32 + (p & 31)] = __float2half_rn(v - __half2float(h));
@@ -406,8 +408,8 @@ cudaError_t launch_z_export_hl16(const void* zhl, long long kpad, int n_m_pad, i
 }
 
 cudaError_t launch_weights_scale_hl16(const double* wtab, void* wtab16, double* wscale, long long kpad, long long n_pad,
-                                      int n_freq, MixedCtl* ctl, cudaStream_t s) {
-  weights_scale_hl16_kernel<<<n_freq, 1024, 0, s>>>(wtab, static_cast<__half*>(wtab16), wscale, kpad, n_pad, ctl);
+                                      int n_freq, MixedCtl* ctl, const float* zfold, cudaStream_t s) {
+  weights_scale_hl16_kernel<<<n_freq, 1024, 0, s>>>(wtab, static_cast<__half*>(wtab16), wscale, kpad, n_pad, ctl, zfold);
   return cudaGetLastError();
 }
 

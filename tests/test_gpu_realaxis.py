@@ -29,13 +29,14 @@ def batch_csr(w, n_u, n0, no, u0, nu, n_bins):
     return np.cumsum(ptr).astype(np.int32), ((n[sel] - n0) * nu + (u[sel] - u0)).astype(np.int32), ww[sel]
 
 
-def cuda_imchi(prob, edges, wts, n_k_norm=None, max_n_o=None, max_n_u=None, spin=0, stats=None):
+def cuda_imchi(prob, edges, wts, n_k_norm=None, max_n_o=None, max_n_u=None, spin=0, stats=None, precision=0):
     import torch
     import paper_2506_03477_b200 as q
     cfg, sp = prob.cfg, prob.spins[spin]
     n_k, n_bins = sp.Ck.shape[0], len(edges) - 1
     mo, mu = max_n_o or cfg.n_o, max_n_u or cfg.n_u
-    ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, edges[:-1], n_k if n_k_norm is None else n_k_norm, mo, mu)
+    ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, edges[:-1], n_k if n_k_norm is None else n_k_norm, mo, mu,
+                        precision=precision)
     ctx.set_product_tensor(torch.from_numpy(prob.P).cuda())
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     for k in range(n_k):
@@ -178,12 +179,6 @@ def test_realaxis_errors():
     edges = log_bin_edges(7, 1e-2, 2.0)
     bp, pr, ww = weights_of(prob, edges, 0.1)[0]
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-    ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, edges[:-1], 1, cfg.n_o, cfg.n_u, precision=q.PREC_MIXED)
-    ctx.set_product_tensor(t(prob.P))
-    with pytest.raises(q.QsgwError) as e:
-        ctx.imchi_add_batch(t(sp.Ck[0]), t(sp.Ckq[0]), 0, cfg.n_o, 0, cfg.n_u, t(bp), t(pr), t(ww))
-    assert e.value.code == 6                                          # FP64 only
-    ctx.destroy()
     ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, edges[:-1], 1, cfg.n_o, cfg.n_u)
     with pytest.raises(q.QsgwError) as e:
         ctx.imchi_add_batch(t(sp.Ck[0]), t(sp.Ckq[0]), 0, cfg.n_o, 0, cfg.n_u, t(bp), t(pr), t(ww))
@@ -200,3 +195,28 @@ def test_realaxis_errors():
         q.hilbert_to_imag_axis(torch.zeros((400, 4, 4), dtype=torch.complex128, device="cuda"),
                                torch.linspace(1, 2, 401, dtype=torch.float64, device="cuda"),
                                torch.zeros(1, dtype=torch.float64, device="cuda"))
+
+
+@pytest.mark.parametrize("case", ["ragged", "ragged_batches", "cfg1", "cfg2"])
+def test_imchi_mixed_mode(case):
+    """The binned spectral part on a QSGW_PREC_MIXED context: FP16-split rows, the per-bin products on tcgen05 over the
+    per-bin row ranges (three FP16 products: a bin holds too few pairs for the E5M2 corrections), the caller's weights
+    scaled by the batch's 2^(-2S).  Tolerance: the north_star mixed bar, 2e-5 relative Frobenius per bin."""
+    kw = {}
+    if case.startswith("ragged"):
+        prob, n_bins, n_k_norm = generate(RAGGED), 30, None
+        edges = log_bin_edges(n_bins, 1e-2, 2.0)
+        wts = weights_of(prob, edges, 0.3)
+        if case == "ragged_batches":
+            kw = {"max_n_o": 2, "max_n_u": 7}
+    else:
+        cfg = get_config(1 if case == "cfg1" else 2)
+        prob, n_bins, n_k_norm = generate(cfg, n_k=5), 100, cfg.n_k
+        edges = log_bin_edges(n_bins, 1e-3, 2.0)
+        wts = weights_of(prob, edges, 0.06)
+    sp = prob.spins[0]
+    ref = oracle.hermitian_finalize_ref(oracle.imchi_ref(sites_of(prob), sp.Ck, sp.Ckq, wts, n_bins, n_k_norm=n_k_norm))
+    got = cuda_imchi(prob, edges, wts, n_k_norm=n_k_norm, precision=1, **kw)
+    check_bins(got, ref, tol=2e-5)
+    worst = max(np.linalg.norm(got[j] - ref[j]) / np.linalg.norm(ref[j]) for j in range(n_bins) if np.linalg.norm(ref[j]) > 0)
+    assert worst > 1e-12          # really the FP32-grade path
