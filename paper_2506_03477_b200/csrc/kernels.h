@@ -134,6 +134,7 @@ struct Chi0F16Args {
   int j0 = 0;            // first frequency of this launch (n_freq = count)
   int split = 1;         // CTAs sharing the staged pairs of one (tile, frequency); set by launch_chi0_f16
   int n_sm = 148;        // SMs of the context's device
+  int pair = 1;          // CTA pairs (cta_group::2) sharing the B tiles of two frequencies; 0 = one CTA per (tile, frequency)
   const MixedCtl* ctl;   // device: use_fp8 selects the variant that runs (the other one exits at once)
   const int2* d_ranges = nullptr;   // optional [n_freq]: pair rows [x, y) that carry weight at that frequency (bin); no split
   const int4* d_tiles;   // 128x128 tiles (tile_i, tile_j, 0, 0), tile_i <= tile_j

@@ -111,6 +111,7 @@ struct qsgw_ctx {
   double fp8_thr = 4.0;         // automatic choice: E5M2 when P_eff >= fp8_thr * N_M (measured, DESIGN.md 4b:
                                 // 1.2e-5 at P_eff = 4.8 N_M, 1.6e-5 at 2.4 N_M, 2.2e-5 at 0.7 N_M)
   int win = 8;                  // stages per TMEM drain window
+  int mixed_pair = 1;           // stage (b) on CTA pairs (cta_group::2) (option "mixed_pair")
   int zmel_kt = 0;              // stage (a) DMMA kernel: padded contraction length (0 = CUDA-core kernel)
   int zmel_kt_avail = 0;        // ... as computed at creation (option "zmel_dmma" switches zmel_kt between 0 and this)
   int device = 0, n_sm = 148;   // device the context lives on
@@ -718,6 +719,8 @@ int32_t qsgw_set_option(qsgw_ctx* ctx, const char* key, int64_t value) {
     if (upload_ctl(ctx) != cudaSuccess) return ctx->fail(QSGW_ERR_CUDA, "upload of the mixed-mode control block failed");
   } else if (k == "mixed_window" && value >= 1 && value <= 64 && ctx->f16) {
     ctx->win = (int)value;
+  } else if (k == "mixed_pair" && (value == 0 || value == 1) && ctx->f16) {
+    ctx->mixed_pair = (int)value;
   } else if (k == "sigc_f64" && (value == 0 || value == 1) && ctx->f16) {
     ctx->sigc_f64 = value != 0;
   } else if (k == "e2e_groups" && value >= 1 && value <= 4) {
@@ -907,6 +910,7 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
     m.wtab16 = reinterpret_cast<const __half*>(ctx->d_wtab32);   // same bytes per pair as an FP32 table
     m.wscale = ctx->d_wscale;
     m.win = ctx->win;
+    m.pair = ctx->mixed_pair;
     m.kpad = ctx->kpad;
     m.acc_re = ctx->d_acc_re;
     m.acc_im = ctx->d_acc_im;

@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(kThreadsS, 1) sigc_f16_kernel(const __grid_con
   uint64_t* d_empty = d_full + 1;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(d_empty + 1);
 
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tid = threadIdx.x, warp = uniform_warp_idx(), lane = tid & 31;
   const int tn = blockIdx.x % a.n_tiles_n, tp = blockIdx.x / a.n_tiles_n;     // tile column (nu), tile row (pairs)
   const int kst = a.kst, n_stages = a.n_freq * kst;
 
@@ -96,38 +96,45 @@ __global__ void __launch_bounds__(kThreadsS, 1) sigc_f16_kernel(const __grid_con
 
   if (warp < 4) {
     setmaxnreg_dec<56>();
-    if (warp == 0 && lane == 0) {
+    // warps 0-2: the whole warp runs its loop (uniform control flow and operands), one elected lane issues
+    if (warp == 0) {
       // ------------------------------------------------------------------ B tiles: (W_i)^T rows of this tile column
       int st = 0, u = 0;
       for (int s = 0; s < n_stages; ++s) {
         const int i = s / kst, ks = s - i * kst;
         if (u > 0) mbar_wait(&empty[st], (u - 1) & 1);
         unsigned char* sb = sm + st * C::B_BYTES;
-        mbar_arrive_expect_tx(&full[st], C::B_BYTES);
+        if (elect_one()) {
+          mbar_arrive_expect_tx(&full[st], C::B_BYTES);
 #pragma unroll
-        for (int b = 0; b < 4; ++b) {
-          const int plane = b >> 1, rh = b & 1;
-          tma_load_3d(sb + plane * kTileS + rh * kBoxS, &a.tmap_w, &full[st], ks * 64,
-                      i * a.n_m_pad + tn * 128 + rh * 64, plane);
+          for (int b = 0; b < 4; ++b) {
+            const int plane = b >> 1, rh = b & 1;
+            tma_load_3d(sb + plane * kTileS + rh * kBoxS, &a.tmap_w, &full[st], ks * 64,
+                        i * a.n_m_pad + tn * 128 + rh * 64, plane);
+          }
         }
+        __syncwarp();
         if (++st == C::STAGES) { st = 0; ++u; }
       }
-    } else if (warp == 2 && lane == 0) {
+    } else if (warp == 2) {
       // ------------------------------------------------------------------ A-source tiles: z rows of this tile row
       int st = 0, u = 0;
       for (int s = 0; s < n_stages; ++s) {
         const int ks = s % kst;
         if (u > 0) mbar_wait(&s_empty[st], (u - 1) & 1);
         unsigned char* sa = sm + C::A_RING_OFF + st * C::A_BYTES;
-        mbar_arrive_expect_tx(&s_full[st], C::A_BYTES);
+        if (elect_one()) {
+          mbar_arrive_expect_tx(&s_full[st], C::A_BYTES);
 #pragma unroll
-        for (int b = 0; b < 4; ++b) {
-          const int plane = b >> 1, rh = b & 1;
-          tma_load_3d(sa + plane * kTileS + rh * kBoxS, &a.tmap_z, &s_full[st], ks * 64, tp * 128 + rh * 64, plane);
+          for (int b = 0; b < 4; ++b) {
+            const int plane = b >> 1, rh = b & 1;
+            tma_load_3d(sa + plane * kTileS + rh * kBoxS, &a.tmap_z, &s_full[st], ks * 64, tp * 128 + rh * 64, plane);
+          }
         }
+        __syncwarp();
         if (++st == C::ASTAGES) { st = 0; ++u; }
       }
-    } else if (warp == 1 && lane == 0) {
+    } else if (warp == 1) {
       // ------------------------------------------------------------------ MMA issuer
       const uint32_t idesc = umma_idesc_f16(128, 128, 0), idesc_neg = umma_idesc_f16(128, 128, 1);
       int st = 0, u = 0, ts = 0, tu = 0, kpos = 0, wpos = 0, widx = 0;
@@ -140,6 +147,10 @@ __global__ void __launch_bounds__(kThreadsS, 1) sigc_f16_kernel(const __grid_con
         const uint32_t sb = base + st * C::B_BYTES;
         const uint64_t bu = umma_desc_k_sw128(sb), bv = umma_desc_k_sw128(sb + kTileS);
         const uint32_t ab = a_ring + ts * C::TSLOT_COLS;
+        ++wpos;
+        if (++kpos == kst) kpos = 0;
+        const bool win_last = wpos == kSigcWin || kpos == 0;    // a window ends with its frequency
+        if (elect_one()) {
 #pragma unroll
         for (int g = 0; g < 2; ++g) {                       // 16 mu = one K step
           const uint32_t acc0 = (first && g == 0) ? 0u : 1u;
@@ -160,9 +171,10 @@ __global__ void __launch_bounds__(kThreadsS, 1) sigc_f16_kernel(const __grid_con
         }
         umma_commit(&empty[st]);
         umma_commit(&a_empty[ts]);
-        ++wpos;
-        if (++kpos == kst) kpos = 0;
-        if (wpos == kSigcWin || kpos == 0) { wpos = 0; ++widx; umma_commit(d_full); }   // a window ends with its frequency
+        if (win_last) umma_commit(d_full);
+        }
+        __syncwarp();
+        if (win_last) { wpos = 0; ++widx; }
         if (++st == C::STAGES) { st = 0; ++u; }
         if (++ts == C::TSLOTS) { ts = 0; ++tu; }
       }
