@@ -43,10 +43,10 @@ UNIT = "TFLOP/s"
 # Nominal dense B200 tensor peaks (guide: B200_PROFILING.md / blackwell_cuda_programming.md) used
 # only as RATIOS to the measured bf16 peak of MEASURED_PEAKS.json.
 # dram__bytes_read.sum + dram__bytes_write.sum of the stage (b) kernel for ONE cfg-4 k-point (21504 pairs), from the
-# `ncu --set full` captures under profiles/ (r02_*_full.md; the FP16-only variant: r01); a launch covers the k-points staged
+# `ncu --set full` captures under profiles/ (r02_*_full.md; the FP16-only variant was not captured: traffic null); a launch covers the k-points staged
 # in the workspace.
 NCU_DRAM_BYTES_PER_KPOINT_CFG4 = {"chi0_f64_3m_kernel": (40.162e9 + 0.771e9) / 2,          # r02 captures: two k-points per launch
-                                  "chi0_f16_kernel<fp8>": (10.860e9 + 0.936e9) / 2, "chi0_f16_kernel": 5.537e9 + 0.802e9}
+                                  "chi0_f16_pair_kernel<fp8>": (12.035e9 + 0.981e9) / 2, "chi0_f16_pair_kernel": None}
 
 NOMINAL_TF = {"bf16": 2250.0, "f16": 2250.0, "tf32": 1100.0, "f64": 40.0}
 
@@ -568,7 +568,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
     # tensor-pipe flops the kernel executes per credited flop (full tiles, no padding counted): the FP64 kernel's
     # 3M product executes 3 real products per complex one (0.75 of the credited 4); the FP16 split 3 per term
     passes = {q.PREC_FP64: 0.75, q.PREC_MIXED: 3}[precision]
-    kname = {"f64": "chi0_f64_3m_kernel", "f16": "chi0_f16_kernel"}[dkey]
+    kname = {"f64": "chi0_f64_3m_kernel", "f16": "chi0_f16_pair_kernel"}[dkey]
     pipe_txt = dkey
     extra = {}
     if precision == q.PREC_MIXED:
@@ -584,7 +584,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
         peak = tf32_peak
         peak_src = f"{src} bf16 cuBLAS sustained (MEASURED_PEAKS.json) x nominal tf32/bf16 ratio (1100/2250)"
         if mixed_fp8:
-            kname, pipe_txt = "chi0_f16_kernel<fp8>", "f16 + e5m2"
+            kname, pipe_txt = "chi0_f16_pair_kernel<fp8>", "f16 + e5m2"
         roof_exec_frac = extra["frac_pipe_mix"]
     else:
         roof_exec_frac = (ach * passes / peak) if ach else None
@@ -594,7 +594,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
                 "frac_executed": roof_exec_frac,
                 "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": (ach / peak) if ach else None,
                 "traffic": (NCU_DRAM_BYTES_PER_KPOINT_CFG4[kname] * n_k * n_spin * args.steps / max(chi_n, 1)
-                            if (cfg.index == 4 and kname in NCU_DRAM_BYTES_PER_KPOINT_CFG4 and chi_n) else None),
+                            if (cfg.index == 4 and NCU_DRAM_BYTES_PER_KPOINT_CFG4.get(kname) and chi_n) else None),
                 "note": ("credited flops count 4 real products per complex multiply-add; the 3M kernel executes 3, so "
                          "`frac` (credited / peak) can exceed 1 while `frac_executed` stays below it"
                          if dkey == "f64" else "frac = credited / TF32 peak (north_star denominator); frac_executed = "

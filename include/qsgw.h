@@ -298,6 +298,8 @@ int32_t qsgw_mixed_stats(qsgw_ctx* ctx, int64_t* out_launches, int64_t* out_laun
  *   "mixed_fp8"       0 | 1 | 2  E5M2 correction products never | always | chosen on the device (default 2)
  *   "mixed_fp8_threshold_x100"  T*100: automatic choice takes E5M2 when P_eff >= T * N_M (default T = 4)
  *   "mixed_window"    1..64    pipeline stages per TMEM drain window (default 8)
+ *   "mixed_pair"      0 | 1    mixed stage (b): one CTA per (tile, frequency) | CTA pairs (tcgen05 cta_group::2) that share
+ *                              the B tiles of two consecutive frequencies (default 1; the binned real-axis path always uses 0)
  *   "sigc_f64"        0 | 1    mixed context: qsgw_sigc_imag_accumulate on tcgen05 (default) | with the FP64 GEMM
  *   "e2e_groups"      1..4     frequency groups of the last launch of qsgw_chi0_run_host (default 4)
  * ctx == NULL, process-wide:
