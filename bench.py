@@ -333,6 +333,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
     wc = None
     sigc = None
     realaxis = None
+    ipw = None
     if precision == q.PREC_FP64 and not args.no_wc and not light and rank == 0:
         from qsgw_synth import coulomb_eigenvalues, haar_unitary
         import numpy as _np
@@ -535,6 +536,30 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
         else:
             del w_out
         del d_v, d_U
+        # next row f4: the interstitial-plane-wave block of the matrix elements (Eqs. 4, 5, 8) for the band counts of this
+        # configuration and a cell with ~290 plane waves per eigenfunction and ~370 IPWs (3 Ry / 3.5 Ry cutoffs)
+        if not args.no_ipw:
+            from qsgw_synth import synthetic_ipw
+            torch.cuda.empty_cache()
+            ip = synthetic_ipw(n_o=cfg.n_o, n_u=cfg.n_u, a0=16.0, cut_pw=3.0, cut_ipw=3.5, n_spheres=4, seed=1)
+            t_ = lambda a: torch.from_numpy(_np.ascontiguousarray(a)).to(dev)
+            di = [t_(ip.theta), t_(ip.g_kq), t_(ip.g_k), t_(ip.g_ipw), t_(ip.Bk), t_(ip.Bkq)]
+            zi = torch.empty((cfg.n_o, cfg.n_u, len(ip.g_ipw)), dtype=torch.complex128, device=dev)
+            ipw_ms = timed(lambda: q.zmel_ipw_build(ip.L, *di, out=zi))
+            n_kq_, n_k_, n_i_ = len(ip.g_kq), len(ip.g_k), len(ip.g_ipw)
+            fl_ipw = 8.0 * n_i_ * n_kq_ * cfg.n_o * (n_k_ + cfg.n_u)
+            ipw = {"ms": ipw_ms, "value": fl_ipw / (ipw_ms * 1e-3) / 1e12, "unit": UNIT, "n_pw": [n_kq_, n_k_], "n_ipw": n_i_,
+                   "n_o": cfg.n_o, "n_u": cfg.n_u, "credited_flop": fl_ipw,
+                   "what": "qsgw_zmel_ipw_build: gather of theta differences + two FP64 tensor-pipe GEMMs; credited "
+                           "n_ipw N_kq n_o (N_k + n_u) complex multiply-adds, 8 real flop each"}
+            if not args.no_accuracy:
+                import oracle
+                sel = _np.linspace(0, n_i_ - 1, 6).astype(int)
+                ref = oracle.zmel_ipw_ref(ip.theta, ip.L, ip.g_kq, ip.g_k, ip.g_ipw[sel], ip.Bk, ip.Bkq)
+                got = zi[:, :, torch.from_numpy(sel).to(dev)].cpu().numpy()
+                ipw["accuracy"] = {"max_abs_err_over_max": float(_np.abs(got - ref).max() / _np.abs(ref).max()),
+                                   "against": "oracle.zmel_ipw_ref on 6 of the IPW columns, all band pairs", "tolerance": 1e-12}
+            del di, zi
     del d_in, out
     torch.cuda.empty_cache()
 
@@ -652,7 +677,7 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
 
     return {"mode": mode_name, "value": value, "ms_per_step": ms_total / args.steps, "launches": launches,
             "roofline": roofline, "e2e": e2e, "clocks": clocks, "flops_step": flops_step,
-            "flops_stage_a": fa, "flops_stage_b": fb, "pairs_kept": pairs, "wc": wc, "sigc": sigc, "realaxis": realaxis, "mixed_selection": mixed_stats,
+            "flops_stage_a": fa, "flops_stage_b": fb, "pairs_kept": pairs, "wc": wc, "sigc": sigc, "realaxis": realaxis, "ipw": ipw, "mixed_selection": mixed_stats,
             "_out": outs_host}
 
 
@@ -737,6 +762,8 @@ def main_cuda(args):
             line["sigc"] = r["sigc"]
         if r.get("realaxis"):
             line["realaxis"] = r["realaxis"]
+        if r.get("ipw"):
+            line["ipw"] = r["ipw"]
         if r is not main:
             line[r["mode"]] = r
     if main.get("mixed_selection"):
@@ -774,6 +801,7 @@ def parse_args(argv=None):
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-wc", action="store_true", help="skip the W^c(i omega) leg reported beside the FP64 step")
     ap.add_argument("--no-realaxis", action="store_true", help="skip the real-axis (binned Im chi0 + Hilbert) leg")
+    ap.add_argument("--no-ipw", action="store_true", help="skip the IPW block (row f4) leg")
     ap.add_argument("--no-sigc", action="store_true", help="skip the I^c (imaginary-axis self-energy) leg")
     ap.add_argument("--no-accuracy", action="store_true", help="skip the oracle check of the timed outputs")
     ap.add_argument("--no-configs", action="store_true", help="skip the side runs of the other configurations")

@@ -286,6 +286,28 @@ int32_t qsgw_n_m(const qsgw_ctx* ctx);                  /* N_M                  
 int32_t qsgw_n_b(const qsgw_ctx* ctx);                  /* N_b                                 */
 const char* qsgw_version(void);
 
+/* Interstitial-plane-wave (IPW) block of the matrix elements (row f4; Eqs. 4, 5 and 8; DESIGN.md
+ * reading R21).  For the product functions of the mixed product basis that are IPWs, M_I = P_{G_I} of Eq. (5), the matrix
+ * element is an integral over the interstitial region of three plane-wave expansions:
+ *   z[n, n', I] = sum_{alpha, beta} conj(Bkq[n', alpha]) theta(g_k[beta] - g_kq[alpha] - g_ipw[I]) Bk[n, beta]
+ * per unit cell volume, the same bilinear form and band-index convention as the muffin-tin block of qsgw_zmel_build
+ * (bands n' = the conjugated eigenfunction that the IPW multiplies; crystal momenta k_kq + k_ipw = k_k, any umklapp is
+ * the caller's shift of an integer list).  theta(g) = (1/Omega) int_cell Theta_I(r) exp(i G.r) d^3r are the Fourier
+ * coefficients of the interstitial indicator function, an INPUT table on the integer box |g_i| <= L_i.
+ *   h_L      : HOST int32[3], box half extents;  d_theta : device complex128 [2 L0 + 1][2 L1 + 1][2 L2 + 1], theta[g + L];
+ *              a difference outside the box counts as theta = 0
+ *   d_g_kq   : device int32 [n_pw_kq][3], d_g_k : [n_pw_k][3], d_g_ipw : [n_ipw][3]   integer reciprocal vectors
+ *   d_Bk     : device complex128, beta^n_G at d_Bk[n * ld_k + beta] (n_o bands);  d_Bkq : d_Bkq[n' * ld_kq + alpha] (n_u bands)
+ *   d_z_out  : device complex128, z[n, n', I] at d_z_out[(n * n_u + n') * ld_z + I]: with ld_z = N_MT + n_ipw and the pointer
+ *              advanced by N_MT the block lands beside the muffin-tin columns of a z array for qsgw_chi0_accumulate(d_z).
+ * Stream-ordered on `cuda_stream` (gather of the structured product tensor + two FP64 tensor-pipe GEMMs, workspace from
+ * the stream-ordered allocator, at most 1 GiB + the output-sized buffer); no synchronisation.  Error text in
+ * qsgw_last_create_error(). */
+int32_t qsgw_zmel_ipw_build(const int32_t* h_L, const void* d_theta, int32_t n_pw_kq, const int32_t* d_g_kq, int32_t n_pw_k,
+                            const int32_t* d_g_k, int32_t n_ipw, const int32_t* d_g_ipw, const void* d_Bk, int64_t ld_k,
+                            int32_t n_o, const void* d_Bkq, int64_t ld_kq, int32_t n_u, void* d_z_out, int64_t ld_z,
+                            void* cuda_stream);
+
 /* Mixed mode: what the device-side selection did since the last qsgw_reset (synchronises the stream):
  * stage (b) launches in all, those that ran the E5M2 correction products, and the smallest effective pair
  * count P_eff any launch saw (qsgw.h, QSGW_PREC_MIXED).  QSGW_ERR_STATE in FP64 mode. */

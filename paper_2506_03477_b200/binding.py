@@ -66,11 +66,12 @@ def lib() -> C.CDLL:
     L.qsgw_hilbert_to_imag_axis.argtypes = [i32, i32, dp, i32, dp, vp, vp, vp]
     L.qsgw_hilbert_to_real_axis.argtypes = [i32, i32, dp, i32, dp, vp, vp, vp]
     L.qsgw_mixed_stats.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(C.c_double)]
+    L.qsgw_zmel_ipw_build.argtypes = [C.POINTER(i32), vp, i32, vp, i32, vp, i32, vp, vp, i64, i32, vp, i64, i32, vp, i64, vp]
     for name in ("qsgw_create", "qsgw_set_product_tensor", "qsgw_zmel_build", "qsgw_chi0_accumulate",
                  "qsgw_chi0_add_kpoint", "qsgw_chi0_finalize", "qsgw_reset", "qsgw_sync",
                  "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_set_option", "qsgw_mixed_stats", "qsgw_wc_from_chi0",
                  "qsgw_sigc_imag_accumulate", "qsgw_chi0_add_kpoints", "qsgw_imchi_add_batch",
-                 "qsgw_hilbert_to_imag_axis", "qsgw_hilbert_to_real_axis",
+                 "qsgw_hilbert_to_imag_axis", "qsgw_hilbert_to_real_axis", "qsgw_zmel_ipw_build",
                  "qsgw_chi0_to_coulomb_basis"):
         getattr(L, name).restype = i32
     for name in ("qsgw_last_error", "qsgw_last_create_error", "qsgw_version"):
@@ -343,6 +344,31 @@ def hilbert_to_imag_axis(A, edges, omega_out, out=None, _real=False):
     fn = lib().qsgw_hilbert_to_real_axis if _real else lib().qsgw_hilbert_to_imag_axis
     rc = fn(n_m, n_bins, _ptr(edges, torch.float64), n_out, _ptr(omega_out, torch.float64),
                                          _ptr(A, torch.complex128), _ptr(out, torch.complex128), C.c_void_p(st))
+    if rc != 0:
+        raise QsgwError(rc, lib().qsgw_last_create_error().decode())
+    return out
+
+
+def zmel_ipw_build(L, theta, g_kq, g_k, g_ipw, Bk, Bkq, out=None, col_offset=0):
+    """IPW block of the matrix elements (qsgw_zmel_ipw_build): z[n, n', I] into out[:, :, col_offset:col_offset + n_ipw].
+
+    L: three ints (host); theta complex128 (2 L0 + 1, 2 L1 + 1, 2 L2 + 1); g_*: int32 (N, 3); Bk (n_o, N_k), Bkq (n_u, N_kq).
+    out: complex128 (n_o, n_u, ld_z) or None (allocated with ld_z = n_ipw)."""
+    import torch
+    n_o, n_u, n_ipw = int(Bk.shape[0]), int(Bkq.shape[0]), int(g_ipw.shape[0])
+    if out is None:
+        out = torch.empty((n_o, n_u, n_ipw), dtype=torch.complex128, device=Bk.device)
+    if out.shape[0] != n_o or out.shape[1] != n_u or col_offset < 0 or col_offset + n_ipw > out.shape[2] or not out.is_contiguous():
+        raise QsgwError(2, "out must be a contiguous (n_o, n_u, >= col_offset + n_ipw) tensor")
+    hl = (C.c_int32 * 3)(int(L[0]), int(L[1]), int(L[2]))
+    if tuple(theta.shape) != tuple(2 * int(l) + 1 for l in L):
+        raise QsgwError(2, "theta must have shape (2 L0 + 1, 2 L1 + 1, 2 L2 + 1)")
+    st = torch.cuda.current_stream(Bk.device).cuda_stream
+    zp = C.c_void_p(_ptr(out, torch.complex128).value + 16 * int(col_offset))
+    rc = lib().qsgw_zmel_ipw_build(hl, _ptr(theta, torch.complex128), int(g_kq.shape[0]), _ptr(g_kq, torch.int32),
+                                   int(g_k.shape[0]), _ptr(g_k, torch.int32), n_ipw, _ptr(g_ipw, torch.int32),
+                                   _ptr(Bk, torch.complex128), int(Bk.shape[1]), n_o, _ptr(Bkq, torch.complex128),
+                                   int(Bkq.shape[1]), n_u, zp, int(out.shape[2]), C.c_void_p(st))
     if rc != 0:
         raise QsgwError(rc, lib().qsgw_last_create_error().decode())
     return out

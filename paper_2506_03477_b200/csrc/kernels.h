@@ -186,6 +186,16 @@ cudaError_t zgemm_configure();       // kernel attributes (per device)
 cudaError_t make_zmap(CUtensorMap* out, const double2* base, long long inner, long long outer, long long ld,
                       long long d2, long long s2, long long d3, long long s3, int box_rows);
 
+// ---- interstitial-plane-wave block of the matrix elements (ipw_kernels.cu) ---------------------------------
+// z_out[(n n_u + n') ld_z + I] = sum_{alpha, beta} conj(Bkq[n', alpha]) theta(g_k[beta] - g_kq[alpha] - g_ipw[I]) Bk[n, beta];
+// L = HOST array of the theta box half extents; work: ipw_work_elems complex elements; a_chunk from ipw_alpha_chunk.
+int ipw_alpha_chunk(int n_pw_kq, int n_pw_k, int n_ipw, int n_o, size_t cap_bytes);
+size_t ipw_work_elems(int a_chunk, int n_pw_k, int n_ipw, int n_o, int n_u);
+cudaError_t launch_zmel_ipw(const int L[3], const double2* theta, int n_pw_kq, const int* g_kq, int n_pw_k, const int* g_k,
+                            int n_ipw, const int* g_ipw, const double2* Bk, long long ld_k, int n_o, const double2* Bkq,
+                            long long ld_kq, int n_u, double2* z_out, long long ld_z, int a_chunk, double2* work,
+                            cudaStream_t s);
+
 // ---- screened Coulomb interaction W^c (wc_kernels.cu) ---------------------------------------------------
 // W^c[j] = sqrt(v) ((1 - sqrt(v) chi0[j] sqrt(v))^-1 - 1) sqrt(v) for all frequencies, stream-ordered.
 // work: n_freq * (2 * n_pad^2 + 64 * n_pad + nb * 64 * 64) complex elements, n_pad = ceil64(n_m), nb = n_pad / 64.

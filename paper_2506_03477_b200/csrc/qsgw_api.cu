@@ -1408,6 +1408,38 @@ int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_ch
   return QSGW_OK;
 }
 
+int32_t qsgw_zmel_ipw_build(const int32_t* h_L, const void* d_theta, int32_t n_pw_kq, const int32_t* d_g_kq, int32_t n_pw_k,
+                            const int32_t* d_g_k, int32_t n_ipw, const int32_t* d_g_ipw, const void* d_Bk, int64_t ld_k,
+                            int32_t n_o, const void* d_Bkq, int64_t ld_kq, int32_t n_u, void* d_z_out, int64_t ld_z,
+                            void* cuda_stream) {
+  g_create_error.clear();
+  if (!h_L || !d_theta || !d_g_kq || !d_g_k || !d_g_ipw || !d_Bk || !d_Bkq || !d_z_out) {
+    g_create_error = "NULL argument";
+    return QSGW_ERR_INVALID_ARG;
+  }
+  if (n_pw_kq < 1 || n_pw_k < 1 || n_ipw < 1 || n_o < 1 || n_u < 1) { g_create_error = "counts must be positive"; return QSGW_ERR_SHAPE; }
+  if (h_L[0] < 0 || h_L[1] < 0 || h_L[2] < 0) { g_create_error = "negative box half extent"; return QSGW_ERR_SHAPE; }
+  if (ld_k < n_pw_k || ld_kq < n_pw_kq || ld_z < n_ipw) { g_create_error = "leading dimension smaller than the row length"; return QSGW_ERR_INVALID_ARG; }
+  if ((long long)n_ipw * n_o > 2000000000ll || (long long)n_pw_kq * n_ipw > 2000000000ll) { g_create_error = "block too large for 32-bit GEMM extents"; return QSGW_ERR_SHAPE; }
+  DevInfo di;
+  int rc = wc_prologue(&di);
+  if (rc != QSGW_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int a_chunk = qsgw::ipw_alpha_chunk(n_pw_kq, n_pw_k, n_ipw, n_o, (size_t)1 << 30);
+  if ((long long)a_chunk * n_ipw > 2000000000ll) { g_create_error = "block too large for 32-bit GEMM extents"; return QSGW_ERR_SHAPE; }
+  double2* work = nullptr;
+  cudaError_t e = work_alloc(di.dev, reinterpret_cast<void**>(&work),
+                             sizeof(double2) * qsgw::ipw_work_elems(a_chunk, n_pw_k, n_ipw, n_o, n_u), st);
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("workspace allocation failed: ") + cudaGetErrorString(e); return QSGW_ERR_ALLOC; }
+  const int L[3] = {h_L[0], h_L[1], h_L[2]};
+  e = qsgw::launch_zmel_ipw(L, static_cast<const double2*>(d_theta), n_pw_kq, d_g_kq, n_pw_k, d_g_k, n_ipw, d_g_ipw,
+                            static_cast<const double2*>(d_Bk), ld_k, n_o, static_cast<const double2*>(d_Bkq), ld_kq, n_u,
+                            static_cast<double2*>(d_z_out), ld_z, a_chunk, work, st);
+  cudaFreeAsync(work, st);
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("IPW block kernels: ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
+  return QSGW_OK;
+}
+
 int32_t qsgw_chi0_run_host(qsgw_ctx* c, const void* h_P, const void* h_Ck, const void* h_Ckq, const double* h_eps_k,
                            const double* h_f_k, const double* h_eps_kq, const double* h_f_kq, int32_t n_k_points,
                            int32_t n_o, int32_t n_u, void* h_chi0_out, int64_t* out_kernel_launches) {
