@@ -180,3 +180,22 @@ def binned_pair_weights(eps_k, f_k, eps_kq, f_kq, edges, rel_width: float = 0.05
     bin_ptr = np.zeros(len(edges), dtype=np.int32)
     np.add.at(bin_ptr, bins + 1, 1)
     return np.cumsum(bin_ptr).astype(np.int32), pairs[order].astype(np.int32), ws[order].astype(np.float64)
+
+
+def synthetic_mpb_matrices(n_m: int, seed: int = 0, cond_o: float = 50.0, kappa: float = 0.05):
+    """Overlap and Coulomb matrices of a non-orthogonal mixed product basis (inputs of the generalized eigenproblem,
+    PAPER.md:116-118): M = E S with a seeded non-unitary S (condition number ~ cond_o: IPWs are not orthogonal), so
+    O = S^H S and v = S^H diag(lambda) S, lambda_mu = 4 pi / (|q_mu|^2 + kappa^2) on seeded |q_mu| (the plane-wave form
+    of the Coulomb interaction with the paper's exp(-kappa r) regularisation).  Returns (v, O, lambda sorted
+    descending): the generalized eigenvalues of (v, O) are lambda by construction."""
+    rng = np.random.default_rng(BASE_SEED + 9000 + seed)
+    Q1, Q2 = haar_unitary(rng, n_m), haar_unitary(rng, n_m)
+    sv = np.exp(np.linspace(0.0, np.log(cond_o), n_m))
+    S = (Q1 * sv[None, :]) @ Q2
+    qn = np.concatenate([[0.02], np.sort(rng.uniform(0.3, 6.0, n_m - 1))]) if n_m > 1 else np.array([0.02])
+    lam = 4.0 * np.pi / (qn ** 2 + kappa ** 2)
+    O = S.conj().T @ S
+    v = S.conj().T @ (lam[:, None] * S)
+    O = 0.5 * (O + O.conj().T)
+    v = 0.5 * (v + v.conj().T)
+    return v, O, np.sort(lam)[::-1]
