@@ -560,6 +560,37 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
                 ipw["accuracy"] = {"max_abs_err_over_max": float(_np.abs(got - ref).max() / _np.abs(ref).max()),
                                    "against": "oracle.zmel_ipw_ref on 6 of the IPW columns, all band pairs", "tolerance": 1e-12}
             del di, zi
+            # row f4: the generalized eigenproblem (v - v_mu O) z = 0 that yields the orthonormal basis E_mu and v_mu
+            # (PAPER.md:116-118), on a seeded pencil of order N_M with a known spectrum
+            from qsgw_synth import synthetic_mpb_matrices
+            v_m, O_m, lam_m = synthetic_mpb_matrices(cfg.n_m, seed=1)
+            d_vm, d_Om = torch.from_numpy(v_m).to(dev), torch.from_numpy(O_m).to(dev)
+            q.coulomb_eigenbasis(d_vm, d_Om)                                  # warm-up (workspace pool)
+            torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            w_g, U_g, sweeps = q.coulomb_eigenbasis(d_vm, d_Om)
+            torch.cuda.synchronize(dev)
+            eig_s = time.perf_counter() - t0
+            Nn = (cfg.n_m + 63) // 64 * 64
+            ipw["eigenbasis"] = {"seconds": eig_s, "n_m": cfg.n_m, "sweeps": sweeps,
+                                 "jacobi_bytes": 64.0 * Nn * Nn * (Nn - 1) * sweeps,
+                                 "jacobi_gbs": 64.0 * Nn * Nn * (Nn - 1) * sweeps / eig_s / 1e9,
+                                 "what": "qsgw_coulomb_eigenbasis (host-synchronised once per sweep; wall clock of the call): "
+                                         "Cholesky reduction + two-sided parallel Jacobi + back transformation; jacobi_bytes = "
+                                         "C and Q read and written once per round"}
+            if not args.no_accuracy:
+                import oracle
+                t0 = time.perf_counter()
+                w_r, U_r = oracle.coulomb_eigenbasis_ref(v_m, O_m)
+                ipw["eigenbasis"]["oracle_seconds"] = time.perf_counter() - t0
+                Un = U_g.cpu().numpy()
+                wn = w_g.cpu().numpy()
+                ipw["eigenbasis"]["accuracy"] = {
+                    "eigenvalues_max_err_over_max": float(_np.abs(wn - w_r).max() / w_r.max()),
+                    "residual_rel": float(_np.linalg.norm(v_m @ Un - (O_m @ Un) * wn[None, :]) / _np.linalg.norm(v_m)),
+                    "orthonormality_max_dev": float(_np.abs(Un.conj().T @ O_m @ Un - _np.eye(cfg.n_m)).max()),
+                    "against": "oracle.coulomb_eigenbasis_ref (LAPACK zhegvd on the host cores)", "tolerance": 1e-11}
+            del d_vm, d_Om
     del d_in, out
     torch.cuda.empty_cache()
 

@@ -286,6 +286,24 @@ int32_t qsgw_n_m(const qsgw_ctx* ctx);                  /* N_M                  
 int32_t qsgw_n_b(const qsgw_ctx* ctx);                  /* N_b                                 */
 const char* qsgw_version(void);
 
+/* Orthonormal mixed product basis that diagonalises the Coulomb matrix (row f4; Eq. 7):
+ *   |E_mu> = sum_I z_{mu I} |M_I>,   sum_J (v_IJ - v_mu O_IJ) z_{mu J} = 0,   z^H O z = 1,
+ * O_IJ = <M_I|M_J> the overlap matrix (Hermitian positive definite), v_IJ = <M_I|v|M_J> the Coulomb matrix (Hermitian) of
+ * the non-orthogonal basis {M_I}.  Eigenvalues in DESCENDING order ("mu = 1 corresponds to the largest eigenvalue",
+ * PAPER.md:128).
+ *   d_v, d_O   : device complex128 [N_M][N_M] row-major; the upper triangle (and the real part of the diagonal) is read
+ *   d_vmu_out  : device double [N_M]
+ *   d_U_out    : device complex128 [N_M][N_M] row-major, U[I][mu] = z_{mu I} (the layout qsgw_chi0_to_coulomb_basis takes;
+ *                a column is fixed up to a phase, and up to a unitary mixing inside a degenerate eigenvalue)
+ *   h_info     : HOST int32 (optional): 0 | 1 + index of the first non-positive Cholesky pivot of O (not positive
+ *                definite; QSGW_ERR_INVALID_ARG) | -1 the Jacobi iteration did not converge (QSGW_ERR_CUDA)
+ *   h_sweeps   : HOST int32 (optional): Jacobi sweeps taken
+ * Method: blocked Cholesky O = L L^H and X = L^-1 on the FP64 tensor pipe, C = X v X^H, two-sided Jacobi with the
+ * round-robin parallel ordering (N_M / 2 rotations per round, every 2 x 2 block updated by one thread), U = X^H Q.
+ * SYNCHRONISES `cuda_stream` once per sweep (convergence is decided on the host).  Error text in qsgw_last_create_error(). */
+int32_t qsgw_coulomb_eigenbasis(int32_t n_m, const void* d_v, const void* d_O, double* d_vmu_out, void* d_U_out,
+                                int32_t* h_info, int32_t* h_sweeps, void* cuda_stream);
+
 /* Interstitial-plane-wave (IPW) block of the matrix elements (row f4; Eqs. 4, 5 and 8; DESIGN.md
  * reading R21).  For the product functions of the mixed product basis that are IPWs, M_I = P_{G_I} of Eq. (5), the matrix
  * element is an integral over the interstitial region of three plane-wave expansions:

@@ -66,12 +66,13 @@ def lib() -> C.CDLL:
     L.qsgw_hilbert_to_imag_axis.argtypes = [i32, i32, dp, i32, dp, vp, vp, vp]
     L.qsgw_hilbert_to_real_axis.argtypes = [i32, i32, dp, i32, dp, vp, vp, vp]
     L.qsgw_mixed_stats.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(C.c_double)]
+    L.qsgw_coulomb_eigenbasis.argtypes = [i32, vp, vp, vp, vp, C.POINTER(i32), C.POINTER(i32), vp]
     L.qsgw_zmel_ipw_build.argtypes = [C.POINTER(i32), vp, i32, vp, i32, vp, i32, vp, vp, i64, i32, vp, i64, i32, vp, i64, vp]
     for name in ("qsgw_create", "qsgw_set_product_tensor", "qsgw_zmel_build", "qsgw_chi0_accumulate",
                  "qsgw_chi0_add_kpoint", "qsgw_chi0_finalize", "qsgw_reset", "qsgw_sync",
                  "qsgw_chi0_run_host", "qsgw_n_m", "qsgw_n_b", "qsgw_set_option", "qsgw_mixed_stats", "qsgw_wc_from_chi0",
                  "qsgw_sigc_imag_accumulate", "qsgw_chi0_add_kpoints", "qsgw_imchi_add_batch",
-                 "qsgw_hilbert_to_imag_axis", "qsgw_hilbert_to_real_axis", "qsgw_zmel_ipw_build",
+                 "qsgw_hilbert_to_imag_axis", "qsgw_hilbert_to_real_axis", "qsgw_zmel_ipw_build", "qsgw_coulomb_eigenbasis",
                  "qsgw_chi0_to_coulomb_basis"):
         getattr(L, name).restype = i32
     for name in ("qsgw_last_error", "qsgw_last_create_error", "qsgw_version"):
@@ -372,6 +373,22 @@ def zmel_ipw_build(L, theta, g_kq, g_k, g_ipw, Bk, Bkq, out=None, col_offset=0):
     if rc != 0:
         raise QsgwError(rc, lib().qsgw_last_create_error().decode())
     return out
+
+
+def coulomb_eigenbasis(v, O):
+    """Generalized eigenproblem (v - v_mu O) z = 0 of the mixed product basis (qsgw_coulomb_eigenbasis):
+    returns (v_mu [N_M] float64 descending, U [N_M, N_M] complex128 with U[I, mu] = z_{mu I}, sweeps)."""
+    import torch
+    n = int(v.shape[0])
+    vmu = torch.empty((n,), dtype=torch.float64, device=v.device)
+    U = torch.empty((n, n), dtype=torch.complex128, device=v.device)
+    info, sweeps = C.c_int32(0), C.c_int32(0)
+    st = torch.cuda.current_stream(v.device).cuda_stream
+    rc = lib().qsgw_coulomb_eigenbasis(n, _ptr(v, torch.complex128), _ptr(O, torch.complex128), _ptr(vmu, torch.float64),
+                                       _ptr(U, torch.complex128), C.byref(info), C.byref(sweeps), C.c_void_p(st))
+    if rc != 0:
+        raise QsgwError(rc, lib().qsgw_last_create_error().decode() + f" (info = {info.value})")
+    return vmu, U, int(sweeps.value)
 
 
 def set_global_option(key: str, value: int):

@@ -196,11 +196,26 @@ cudaError_t launch_zmel_ipw(const int L[3], const double2* theta, int n_pw_kq, c
                             long long ld_kq, int n_u, double2* z_out, long long ld_z, int a_chunk, double2* work,
                             cudaStream_t s);
 
+// ---- generalized eigenproblem of the Coulomb matrix in the mixed product basis (eig_kernels.cu) ---------------
+// (v - v_mu O) z = 0, z^H O z = 1: Cholesky reduction to a standard Hermitian problem + two-sided parallel Jacobi.
+// work: eig_work_elems complex elements.  Call order: launch_eig_reduce, launch_eig_sweep until converged
+// (d_norms[0] = |off-diagonal|^2, d_norms[1] = |diagonal|^2 after each sweep), launch_eig_diag (eigenvalues, unsorted),
+// launch_eig_finish with the column permutation (descending eigenvalues).
+size_t eig_work_elems(int n_m);
+cudaError_t launch_eig_reduce(int n_m, const double2* v, const double2* O, double2* work, int* d_info, cudaStream_t s);
+cudaError_t launch_eig_sweep(int n_m, double2* work, double* d_norms, cudaStream_t s);
+cudaError_t launch_eig_diag(int n_m, const double2* work, double* d_diag, cudaStream_t s);
+cudaError_t launch_eig_finish(int n_m, double2* work, const int* d_perm, double2* U_out, cudaStream_t s);
+
 // ---- screened Coulomb interaction W^c (wc_kernels.cu) ---------------------------------------------------
 // W^c[j] = sqrt(v) ((1 - sqrt(v) chi0[j] sqrt(v))^-1 - 1) sqrt(v) for all frequencies, stream-ordered.
 // work: n_freq * (2 * n_pad^2 + 64 * n_pad + nb * 64 * 64) complex elements, n_pad = ceil64(n_m), nb = n_pad / 64.
 // d_info: 0, or 1 + index of the first non-positive Cholesky pivot (eps not positive definite).
 size_t wc_work_elems(int n_m, int n_freq);
+// Blocked Cholesky A = L L^H of `batch` HPD matrices of order N (multiple of 64; lower triangle overwritten by L) and X = L^-1;
+// Tbuf: batch * 64 * N, Linv: batch * (N / 64) * 4096 complex elements; d_info as below.
+cudaError_t launch_chol_inverse(int N, int batch, double2* Abuf, double2* Xbuf, double2* Tbuf, double2* Linv, int* d_info,
+                                cudaStream_t s);
 cudaError_t wc_configure();          // kernel attributes (per device)
 // chi0 -> U^H chi0 U for all frequencies (work: rotate_work_elems complex elements)
 size_t rotate_work_elems(int n_m, int n_freq);

@@ -9,6 +9,7 @@
 #include <cstring>
 #include <mutex>
 #include <new>
+#include <algorithm>
 #include <string>
 #include <vector>
 
@@ -1437,6 +1438,91 @@ int32_t qsgw_zmel_ipw_build(const int32_t* h_L, const void* d_theta, int32_t n_p
                             static_cast<double2*>(d_z_out), ld_z, a_chunk, work, st);
   cudaFreeAsync(work, st);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("IPW block kernels: ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
+  return QSGW_OK;
+}
+
+int32_t qsgw_coulomb_eigenbasis(int32_t n_m, const void* d_v, const void* d_O, double* d_vmu_out, void* d_U_out,
+                                int32_t* h_info, int32_t* h_sweeps, void* cuda_stream) {
+  g_create_error.clear();
+  if (h_info) *h_info = 0;
+  if (h_sweeps) *h_sweeps = 0;
+  if (!d_v || !d_O || !d_vmu_out || !d_U_out) { g_create_error = "NULL argument"; return QSGW_ERR_INVALID_ARG; }
+  if (n_m < 1) { g_create_error = "n_m must be positive"; return QSGW_ERR_SHAPE; }
+  DevInfo di;
+  int rc = wc_prologue(&di);
+  if (rc != QSGW_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int N = (n_m + 63) / 64 * 64;
+  const size_t small_bytes = 256 + sizeof(double) * (size_t)n_m + sizeof(int) * (size_t)n_m + 64;
+  double2* work = nullptr;
+  cudaError_t e = work_alloc(di.dev, reinterpret_cast<void**>(&work),
+                             sizeof(double2) * qsgw::eig_work_elems(n_m) + small_bytes, st);
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("workspace allocation failed: ") + cudaGetErrorString(e); return QSGW_ERR_ALLOC; }
+  unsigned char* sm = reinterpret_cast<unsigned char*>(work + qsgw::eig_work_elems(n_m));
+  int* d_info = reinterpret_cast<int*>(sm);
+  double* d_norms = reinterpret_cast<double*>(sm + 64);
+  double* d_diag = reinterpret_cast<double*>(sm + 256);
+  int* d_perm = reinterpret_cast<int*>(sm + 256 + sizeof(double) * (size_t)n_m);
+#define QSGW_E(expr, what)                                                                              \
+  do {                                                                                                  \
+    e = (expr);                                                                                         \
+    if (e != cudaSuccess) {                                                                             \
+      cudaGetLastError(); cudaFreeAsync(work, st);                                                      \
+      g_create_error = std::string(what) + ": " + cudaGetErrorString(e);                                \
+      return QSGW_ERR_CUDA;                                                                             \
+    }                                                                                                   \
+  } while (0)
+  QSGW_E(qsgw::launch_eig_reduce(n_m, static_cast<const double2*>(d_v), static_cast<const double2*>(d_O), work, d_info, st),
+         "reduction to the standard problem");
+  int info = 0;
+  QSGW_E(cudaMemcpyAsync(&info, d_info, sizeof(int), cudaMemcpyDeviceToHost, st), "copy of info");
+  QSGW_E(cudaStreamSynchronize(st), "stream synchronisation");
+  if (info != 0) {                                     // O is not positive definite
+    cudaFreeAsync(work, st);
+    if (h_info) *h_info = info;
+    g_create_error = "the overlap matrix is not positive definite";
+    return QSGW_ERR_INVALID_ARG;
+  }
+  // Jacobi sweeps until the off-diagonal part reaches its rounding floor: quadratic convergence, so once the ratio
+  // |off|^2 / |C|^2 is below 1e-18 the next sweep lands on the floor and the one after that no longer improves
+  const double floor_ratio = 4e-32 * (double)N * (double)N;
+  double prev = 1.0;
+  int sweeps = 0;
+  bool converged = false;
+  for (; sweeps < 60 && !converged;) {
+    QSGW_E(qsgw::launch_eig_sweep(n_m, work, d_norms, st), "Jacobi sweep");
+    double nr[2] = {0.0, 0.0};
+    QSGW_E(cudaMemcpyAsync(nr, d_norms, 2 * sizeof(double), cudaMemcpyDeviceToHost, st), "copy of the norms");
+    QSGW_E(cudaStreamSynchronize(st), "stream synchronisation");
+    ++sweeps;
+    const double tot = nr[0] + nr[1];
+    const double ratio = tot > 0.0 ? nr[0] / tot : 0.0;
+    if (ratio <= floor_ratio || (prev <= 1e-18 && ratio >= 0.25 * prev)) converged = true;
+    prev = ratio;
+  }
+  if (h_sweeps) *h_sweeps = sweeps;
+  if (!converged) {
+    cudaFreeAsync(work, st);
+    if (h_info) *h_info = -1;
+    g_create_error = "Jacobi iteration did not converge in 60 sweeps";
+    return QSGW_ERR_CUDA;
+  }
+  // eigenvalues to the host, descending order ("mu = 1 corresponds to the largest eigenvalue")
+  std::vector<double> lam((size_t)n_m);
+  QSGW_E(qsgw::launch_eig_diag(n_m, work, d_diag, st), "eigenvalue extraction");
+  QSGW_E(cudaMemcpyAsync(lam.data(), d_diag, sizeof(double) * (size_t)n_m, cudaMemcpyDeviceToHost, st), "copy of the eigenvalues");
+  QSGW_E(cudaStreamSynchronize(st), "stream synchronisation");
+  std::vector<int> perm((size_t)n_m);
+  for (int i = 0; i < n_m; ++i) perm[(size_t)i] = i;
+  std::stable_sort(perm.begin(), perm.end(), [&](int a, int b) { return lam[(size_t)a] > lam[(size_t)b]; });
+  std::vector<double> sorted((size_t)n_m);
+  for (int i = 0; i < n_m; ++i) sorted[(size_t)i] = lam[(size_t)perm[(size_t)i]];
+  QSGW_E(cudaMemcpyAsync(d_perm, perm.data(), sizeof(int) * (size_t)n_m, cudaMemcpyHostToDevice, st), "upload of the order");
+  QSGW_E(cudaMemcpyAsync(d_vmu_out, sorted.data(), sizeof(double) * (size_t)n_m, cudaMemcpyHostToDevice, st), "upload of v_mu");
+  QSGW_E(qsgw::launch_eig_finish(n_m, work, d_perm, static_cast<double2*>(d_U_out), st), "back transformation");
+  QSGW_E(cudaStreamSynchronize(st), "stream synchronisation");     // perm / sorted are host temporaries
+#undef QSGW_E
+  cudaFreeAsync(work, st);
   return QSGW_OK;
 }
 

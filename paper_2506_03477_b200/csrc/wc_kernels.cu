@@ -154,14 +154,13 @@ size_t wc_work_elems(int n_m, int n_freq) {
   return (size_t)n_freq * (2 * n * n + 64 * n + nb * 64 * 64);
 }
 
-cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const double* v, double2* wc_out,
-                                double2* work, int* d_info, cudaStream_t s) {
-  const int N = (n_m + 63) / 64 * 64, nb = N / 64;
+// Blocked Cholesky A = L L^H of `batch` Hermitian positive definite matrices of order N (multiple of 64; lower triangle
+// of A is read and overwritten by L) and X = L^-1 (lower triangular; X is zeroed here).  Tbuf: batch * 64 * N elements,
+// Linv: batch * (N / 64) * 4096 elements.  d_info: 0, or 1 + index of the first non-positive pivot (zeroed here).
+cudaError_t launch_chol_inverse(int N, int batch, double2* Abuf, double2* Xbuf, double2* Tbuf, double2* Linv, int* d_info,
+                                cudaStream_t s) {
+  const int nb = N / 64, n_freq = batch;
   const long long sM = (long long)N * N, sT = 64LL * N, sL = (long long)nb * 4096;
-  double2* Abuf = work;
-  double2* Xbuf = Abuf + (long long)n_freq * sM;
-  double2* Tbuf = Xbuf + (long long)n_freq * sM;
-  double2* Linv = Tbuf + (long long)n_freq * sT;
   constexpr int kPotrfSmem = 4 * kPB * kPLD * 8;
   cudaError_t e;   // function attributes: wc_configure(), called by the C-ABI layer
 #define WC_TRY(expr) do { e = (expr); if (e != cudaSuccess) return e; } while (0)
@@ -175,10 +174,8 @@ cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const 
   };
   WC_TRY(cudaMemsetAsync(d_info, 0, sizeof(int), s));
   WC_TRY(cudaMemsetAsync(Xbuf, 0, sizeof(double2) * n_freq * sM, s));
-  wc_form_eps_kernel<<<dim3(592, n_freq), 256, 0, s>>>(chi0, v, n_m, N, Abuf);
-  WC_TRY(cudaGetLastError());
 
-  // blocked Cholesky eps = L L^H (right-looking), L in the lower triangle of Abuf.  Two 64-column blocks j0, j1 are
+  // blocked Cholesky A = L L^H (right-looking), L in the lower triangle of Abuf.  Two 64-column blocks j0, j1 are
   // factored per step (j1 after a narrow K = 64 update of its own block column), so that the trailing update runs
   // with K = 128 and touches every C tile half as often.
   auto block = [&](int r, int c) { return Abuf + (long long)r * 64 * N + (long long)c * 64; };
@@ -210,12 +207,31 @@ cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const 
     WC_TRY(gemm(true, false, Linv + (long long)i * 4096, Tbuf, Xbuf + (long long)i * 64 * N, 64, N, N, sL, sT, sM,
                 64, 64 * i, 64, -1.0, 0, 0));
   }
-  // eps^-1 = X^H X (lower tiles into Abuf), then W^c
-  WC_TRY(gemm(false, false, Xbuf, Xbuf, Abuf, N, N, N, sM, sM, sM, N, N, N, 1.0, 0, 2));
-  wc_finish_kernel<<<dim3(592, n_freq), 256, 0, s>>>(Abuf, v, n_m, N, wc_out);
-  WC_TRY(cudaGetLastError());
 #undef WC_TRY
   return cudaSuccess;
+}
+
+cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const double* v, double2* wc_out,
+                                double2* work, int* d_info, cudaStream_t s) {
+  const int N = (n_m + 63) / 64 * 64, nb = N / 64;
+  const long long sM = (long long)N * N, sT = 64LL * N;
+  double2* Abuf = work;
+  double2* Xbuf = Abuf + (long long)n_freq * sM;
+  double2* Tbuf = Xbuf + (long long)n_freq * sM;
+  double2* Linv = Tbuf + (long long)n_freq * sT;
+  (void)nb;
+  wc_form_eps_kernel<<<dim3(592, n_freq), 256, 0, s>>>(chi0, v, n_m, N, Abuf);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  // eps = L L^H, X = L^-1
+  if ((e = launch_chol_inverse(N, n_freq, Abuf, Xbuf, Tbuf, Linv, d_info, s)) != cudaSuccess) return e;
+  // eps^-1 = X^H X (lower tiles into Abuf), then W^c
+  ZgemmArgs g;
+  g.A = Xbuf; g.B = Xbuf; g.C = Abuf; g.lda = g.ldb = g.ldc = N; g.sA = g.sB = g.sC = sM;
+  g.m = g.n = g.k = N; g.batch = n_freq; g.tri = 2;
+  if ((e = launch_zgemm(false, false, g, s)) != cudaSuccess) return e;
+  wc_finish_kernel<<<dim3(592, n_freq), 256, 0, s>>>(Abuf, v, n_m, N, wc_out);
+  return cudaGetLastError();
 }
 
 }  // namespace qsgw
