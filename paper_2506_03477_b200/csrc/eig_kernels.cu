@@ -53,6 +53,15 @@ __device__ __forceinline__ double2 cmulc(double2 a, double2 b) {   // a * conj(b
   return make_double2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
 }
 
+__device__ __forceinline__ double2 ldcs2(const double2* p) {
+  double2 v;
+  asm volatile("ld.global.cs.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ void stcs2(double2* p, double2 v) {
+  asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+
 // grid.y in [0, N/2): rows (p_i, q_i) of A with the row rotation J_i^H; grid.y in [N/2, N): rows (2k, 2k+1) of V, no row
 // rotation.  Thread <-> column pair j: B <- J_i^H B J_j on the 2 x 2 block.
 __global__ void __launch_bounds__(256) jacobi_apply_kernel(double2* __restrict__ A, double2* __restrict__ V, int N, int r,
@@ -82,7 +91,14 @@ __global__ void __launch_bounds__(256) jacobi_apply_kernel(double2* __restrict__
   }
   double2* rp = M + (long long)p * N;
   double2* rq = M + (long long)q * N;
-  const double2 bpp = rp[pj], bpq = rp[qj], bqp = rq[pj], bqq = rq[qj];
+  // Q is streamed (evict-first) so that C, which every round reads twice (parameters + update), stays in the 126 MB L2
+  const bool stream = M == V;
+  double2 bpp, bpq, bqp, bqq;
+  if (stream) {
+    bpp = ldcs2(rp + pj); bpq = ldcs2(rp + qj); bqp = ldcs2(rq + pj); bqq = ldcs2(rq + qj);
+  } else {
+    bpp = rp[pj]; bpq = rp[qj]; bqp = rq[pj]; bqq = rq[qj];
+  }
   // rows: x_p = c b_p - sigma b_q,  x_q = conj(sigma) b_p + c b_q
   double2 t;
   t = cmul(si, bqp);  const double2 xpp = make_double2(ci * bpp.x - t.x, ci * bpp.y - t.y);
@@ -90,10 +106,15 @@ __global__ void __launch_bounds__(256) jacobi_apply_kernel(double2* __restrict__
   t = cmulc(bpp, si); const double2 xqp = make_double2(t.x + ci * bqp.x, t.y + ci * bqp.y);      // conj(sigma) b_pp = b_pp conj(sigma)
   t = cmulc(bpq, si); const double2 xqq = make_double2(t.x + ci * bqq.x, t.y + ci * bqq.y);
   // columns: y_p = c x_p - conj(sigma_j) x_q,  y_q = sigma_j x_p + c x_q
-  t = cmulc(xpq, sj); rp[pj] = make_double2(cj * xpp.x - t.x, cj * xpp.y - t.y);
-  t = cmul(xpp, sj);  rp[qj] = make_double2(t.x + cj * xpq.x, t.y + cj * xpq.y);
-  t = cmulc(xqq, sj); rq[pj] = make_double2(cj * xqp.x - t.x, cj * xqp.y - t.y);
-  t = cmul(xqp, sj);  rq[qj] = make_double2(t.x + cj * xqq.x, t.y + cj * xqq.y);
+  t = cmulc(xpq, sj); const double2 ypp = make_double2(cj * xpp.x - t.x, cj * xpp.y - t.y);
+  t = cmul(xpp, sj);  const double2 ypq = make_double2(t.x + cj * xpq.x, t.y + cj * xpq.y);
+  t = cmulc(xqq, sj); const double2 yqp = make_double2(cj * xqp.x - t.x, cj * xqp.y - t.y);
+  t = cmul(xqp, sj);  const double2 yqq = make_double2(t.x + cj * xqq.x, t.y + cj * xqq.y);
+  if (stream) {
+    stcs2(rp + pj, ypp); stcs2(rp + qj, ypq); stcs2(rq + pj, yqp); stcs2(rq + qj, yqq);
+  } else {
+    rp[pj] = ypp; rp[qj] = ypq; rq[pj] = yqp; rq[qj] = yqq;
+  }
 }
 
 // out[0] += sum of |off-diagonal|^2, out[1] += sum of |diagonal|^2
