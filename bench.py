@@ -448,8 +448,8 @@ def run_mode(args, cfg, prob, precision, mode_name, rank, local_rank, world, lig
             sigc["mixed"] = {"ms": m_ms, "ms_runs": [round(t, 2) for t in ts], "value": (fl_a + fl_zw + fl_c) / (m_ms * 1e-3) / 1e12,
                              "unit": UNIT, "peak": tf32_peak, "frac": (fl_a + fl_zw + fl_c) / (m_ms * 1e-3) / 1e12 / tf32_peak,
                              "peak_source": f"{psrc} bf16 cuBLAS sustained x nominal tf32/bf16 ratio (1100/2250)",
-                             "what": "same pass on a QSGW_PREC_MIXED context: three FP16 products per term on tcgen05 "
-                                     "(sigc_f16_kernel), FP32 sums, closing contraction in FP64; same credited flop"}
+                             "what": "same pass on a QSGW_PREC_MIXED context: FP16 main product + two E5M2 correction products per term on "
+                                     "tcgen05 (sigc_f16_kernel<fp8>), FP32 sums, closing contraction in FP64; same credited flop"}
             if sig64 is not None:
                 sigc["mixed"]["rel_frobenius_dev_from_fp64"] = float((sig - sig64).norm() / sig64.norm())
                 sigc["mixed"]["tolerance"] = 1e-5

@@ -252,9 +252,12 @@ size_t sigc_f16_z_halves(long long pairs_cap, int n_m);
 size_t sigc_f16_w_halves(int n_m, int n_freq);
 cudaError_t sigc_f16_configure();
 cudaError_t launch_sigc_zw_f16(const double2* z, const double2* wc, const double* w, long long ld_w, int pairs, int n_m,
-                               int n_freq, __half* zk16, __half* w16, float* amax, double2* zw, cudaStream_t s);
+                               int n_freq, __half* zk16, __half* w16, unsigned char* w8 /*optional: E5M2 corrections*/, float* amax,
+                               double2* zw, cudaStream_t s);
 // 3-D FLOAT16 tensor map over hl16 rows: dims {row_halves, rows, 2 planes}, box {64, 64, 1}, 128-byte swizzle (qsgw_api.cu)
 cudaError_t make_hl16_map(CUtensorMap* out, const void* base, long long row_halves, long long rows, long long plane_halves);
+// the same rows addressed in bytes (hb8 rows: h[32] halves | e5m2(v)[32] | e5m2(v - h)[32]): UINT8 {2 * row_halves, rows, 2}, box {128, 64, 1}
+cudaError_t make_hb8_map(CUtensorMap* out, const void* base, long long row_halves, long long rows, long long plane_halves);
 // closing contraction of I^c alone (sigc_kernels.cu): sigc[n, m] += -(1/N_k) sum_{n', nu} zw[(n', n), nu] conj(z[(n', m), nu])
 cudaError_t launch_sigc_close(const double2* z, const double2* zw, int n_all, int n_qp, int n_m, double inv_nk, double2* sigc,
                               int n_sm, cudaStream_t s);

@@ -75,6 +75,19 @@ cudaError_t make_hl16_map(CUtensorMap* out, const void* base, long long row_halv
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
+cudaError_t make_hb8_map(CUtensorMap* out, const void* base, long long row_halves, long long rows, long long plane_halves) {
+  EncodeTiledFn enc = get_encode_tiled();
+  if (!enc) return cudaErrorNotSupported;
+  const cuuint64_t gdim[3] = {(cuuint64_t)row_halves * 2, (cuuint64_t)rows, 2};
+  const cuuint64_t gstr[2] = {(cuuint64_t)row_halves * 2, (cuuint64_t)plane_halves * 2};
+  const cuuint32_t box[3] = {128, 64, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(base), gdim, gstr, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 }  // namespace qsgw
 
 struct qsgw_ctx {
@@ -135,6 +148,8 @@ struct qsgw_ctx {
   double* d_sw = nullptr;       // quadrature weights [n_freq][batch_pad]
   __half* d_zk16 = nullptr;     // mixed I^c: z rows as FP16 pieces, K = product functions (sigc_f16_kernels.cu)
   __half* d_w16 = nullptr;      // mixed I^c: (W^c_i)^T rows as FP16 pieces
+  unsigned char* d_w8 = nullptr;  // ... and their hb8 copy (E5M2 correction products, option "sigc_fp8")
+  int sigc_fp8 = 1;
   float* d_samax = nullptr;     // mixed I^c: max |z|, max |W_i|  [1 + n_freq]
   bool sigc_f64 = false;        // option "sigc_f64": a mixed context runs the FP64 GEMM on its FP32-grade z
   CUtensorMap tmap_h;
@@ -221,6 +236,7 @@ void free_all(qsgw_ctx* c) {
   cudaFree(c->d_ranges);
   cudaFree(c->d_zk16);
   cudaFree(c->d_w16);
+  cudaFree(c->d_w8);
   cudaFree(c->d_samax);
   cudaFree(c->d_sz);
   cudaFree(c->d_szw);
@@ -724,6 +740,8 @@ int32_t qsgw_set_option(qsgw_ctx* ctx, const char* key, int64_t value) {
     ctx->mixed_pair = (int)value;
   } else if (k == "sigc_f64" && (value == 0 || value == 1) && ctx->f16) {
     ctx->sigc_f64 = value != 0;
+  } else if (k == "sigc_fp8" && (value == 0 || value == 1) && ctx->f16) {
+    ctx->sigc_fp8 = (int)value;
   } else if (k == "e2e_groups" && value >= 1 && value <= 4) {
     ctx->e2e_groups = (int)value;
   } else {
@@ -1259,14 +1277,15 @@ int32_t qsgw_sigc_imag_accumulate(qsgw_ctx* ctx, const void* d_z, const double* 
     if (e == cudaSuccess && ctx->f16) {
       e = dev_alloc(ctx, &ctx->d_zk16, qsgw::sigc_f16_z_halves((long long)ctx->max_n_o * ctx->max_n_u, ctx->n_m));
       if (e == cudaSuccess) e = dev_alloc(ctx, &ctx->d_w16, qsgw::sigc_f16_w_halves(ctx->n_m, ctx->n_freq));
+      if (e == cudaSuccess) e = dev_alloc(ctx, &ctx->d_w8, 2 * qsgw::sigc_f16_w_halves(ctx->n_m, ctx->n_freq));
       if (e == cudaSuccess) e = dev_alloc(ctx, &ctx->d_samax, (size_t)ctx->n_freq + 1);
       if (e == cudaSuccess) e = qsgw::sigc_f16_configure();
     }
     if (e != cudaSuccess) {
       cudaGetLastError();
       cudaFree(ctx->d_sz); cudaFree(ctx->d_sw); cudaFree(ctx->d_szw);
-      cudaFree(ctx->d_zk16); cudaFree(ctx->d_w16); cudaFree(ctx->d_samax);
-      ctx->d_zk16 = ctx->d_w16 = nullptr; ctx->d_samax = nullptr;
+      cudaFree(ctx->d_zk16); cudaFree(ctx->d_w16); cudaFree(ctx->d_w8); cudaFree(ctx->d_samax);
+      ctx->d_zk16 = ctx->d_w16 = nullptr; ctx->d_w8 = nullptr; ctx->d_samax = nullptr;
       ctx->d_sz = ctx->d_szw = nullptr; ctx->d_sw = nullptr;
       return ctx->fail(QSGW_ERR_ALLOC, "I^c workspace allocation failed: %s", cudaGetErrorString(e));
     }
@@ -1289,7 +1308,8 @@ int32_t qsgw_sigc_imag_accumulate(qsgw_ctx* ctx, const void* d_z, const double* 
   if (e == cudaSuccess && ctx->f16 && !ctx->sigc_f64) {
     // mixed mode: the frequency loop on tcgen05 with FP16-split operands, the closing contraction in FP64
     e = qsgw::launch_sigc_zw_f16(z, static_cast<const double2*>(d_wc), ctx->d_sw, ctx->batch_pad, (int)n_pairs, ctx->n_m,
-                                 ctx->n_freq, ctx->d_zk16, ctx->d_w16, ctx->d_samax, ctx->d_szw, ctx->stream);
+                                 ctx->n_freq, ctx->d_zk16, ctx->d_w16, ctx->sigc_fp8 ? ctx->d_w8 : nullptr, ctx->d_samax, ctx->d_szw,
+                                 ctx->stream);
     if (e == cudaSuccess)
       e = qsgw::launch_sigc_close(z, ctx->d_szw, n_all, n_qp, ctx->n_m, 1.0 / (double)ctx->n_k,
                                   static_cast<double2*>(d_sigc), ctx->n_sm, ctx->stream);

@@ -19,6 +19,7 @@
 // Roles (384 threads) as in chi0_f16_kernel: warp 0 = TMA producer of the B tiles, warp 2 = TMA producer of the A-source
 // tiles, warp 1 = MMA issuer + TMEM allocator, warps 4-11 = staging + drain warps (warps 4-7 own Re, 8-11 own Im).
 #include <cuda_fp16.h>
+#include <cuda_fp8.h>
 
 #include "kernels.h"
 #include "ptx.cuh"
@@ -47,6 +48,7 @@ struct SCfg {
 struct SigcF16Args {
   CUtensorMap tmap_z;    // 3-D FLOAT16 {64 * kst, pairs_pad, 2}: z hl16 rows, box {64, 64, 1}
   CUtensorMap tmap_w;    // 3-D FLOAT16 {64 * kst, n_m_pad * n_freq, 2}: (W^c_i)^T hl16 rows, frequency-major
+  CUtensorMap tmap_w8;   // FP8 variant: 3-D UINT8 {128 * kst, n_m_pad * n_freq, 2}: (W^c_i)^T hb8 rows h[32] | e5m2(v)[32] | e5m2(v - h)[32]
   const double* w;       // quadrature weights [n_freq][ld_w]
   long long ld_w;
   const float* zmax;     // max |Re z|, |Im z|
@@ -56,6 +58,9 @@ struct SigcF16Args {
   int n_tiles_n;
 };
 
+// FP8 = true: the two correction products z_l W_h + z_h W_l run as one kind::f8f6f4 (E5M2) MMA of K = 32 each (as in
+// chi0_f16_kernel<fp8>): 8 + 8 instead of 24 MMAs per 32 mu; B rows from the hb8 copy of (W^c_i)^T.
+template <bool FP8>
 __global__ void __launch_bounds__(kThreadsS, 1) sigc_f16_kernel(const __grid_constant__ SigcF16Args a) {
   using C = SCfg;
   extern __shared__ unsigned char smem_dyn[];
@@ -109,7 +114,7 @@ __global__ void __launch_bounds__(kThreadsS, 1) sigc_f16_kernel(const __grid_con
 #pragma unroll
           for (int b = 0; b < 4; ++b) {
             const int plane = b >> 1, rh = b & 1;
-            tma_load_3d(sb + plane * kTileS + rh * kBoxS, &a.tmap_w, &full[st], ks * 64,
+            tma_load_3d(sb + plane * kTileS + rh * kBoxS, FP8 ? &a.tmap_w8 : &a.tmap_w, &full[st], ks * (FP8 ? 128 : 64),
                         i * a.n_m_pad + tn * 128 + rh * 64, plane);
           }
         }
@@ -151,8 +156,31 @@ __global__ void __launch_bounds__(kThreadsS, 1) sigc_f16_kernel(const __grid_con
         if (++kpos == kst) kpos = 0;
         const bool win_last = wpos == kSigcWin || kpos == 0;    // a window ends with its frequency
         if (elect_one()) {
+        if (FP8) {
+          const uint32_t idesc8 = umma_idesc_e5m2(128, 128, 0), idesc8_neg = umma_idesc_e5m2(128, 128, 1);
 #pragma unroll
-        for (int g = 0; g < 2; ++g) {                       // 16 mu = one K step
+          for (int g = 0; g < 2; ++g) {                     // main products (h h)
+            const uint32_t acc0 = (first && g == 0) ? 0u : 1u;
+            const uint64_t kh = (uint64_t)(2 * g);
+            const uint32_t xh = ab + 8 * g, yh = ab + 16 + 8 * g;
+            umma_f16_ts(d_re, xh, bu + kh, idesc, acc0);
+            umma_f16_ts(d_im, xh, bv + kh, idesc, acc0);
+            umma_f16_ts(d_re, yh, bv + kh, idesc_neg, 1u);
+            umma_f16_ts(d_im, yh, bu + kh, idesc, 1u);
+          }
+          // corrections z_l8 W_8 + z_8 W_l8: one K = 32 step each; W_8 at byte 64, W_l8 at byte 96 of the row
+          const uint32_t x8 = ab + 32, y8 = ab + 40, xl8 = ab + 48, yl8 = ab + 56;
+          umma_f8_ts(d_re, xl8, bu + 4, idesc8, 1u);
+          umma_f8_ts(d_im, xl8, bv + 4, idesc8, 1u);
+          umma_f8_ts(d_re, yl8, bv + 4, idesc8_neg, 1u);
+          umma_f8_ts(d_im, yl8, bu + 4, idesc8, 1u);
+          umma_f8_ts(d_re, x8, bu + 6, idesc8, 1u);
+          umma_f8_ts(d_im, x8, bv + 6, idesc8, 1u);
+          umma_f8_ts(d_re, y8, bv + 6, idesc8_neg, 1u);
+          umma_f8_ts(d_im, y8, bu + 6, idesc8, 1u);
+        }
+#pragma unroll
+        for (int g = 0; g < (FP8 ? 0 : 2); ++g) {           // 16 mu = one K step
           const uint32_t acc0 = (first && g == 0) ? 0u : 1u;
           const uint64_t kh = (uint64_t)(2 * g), kl = (uint64_t)(4 + 2 * g);
           const uint32_t xh = ab + 8 * g, yh = ab + 16 + 8 * g, xl = ab + 32 + 8 * g, yl = ab + 48 + 8 * g;
@@ -228,7 +256,19 @@ __global__ void __launch_bounds__(kThreadsS, 1) sigc_f16_kernel(const __grid_con
           lv[4 * cc] = tl.x; lv[4 * cc + 1] = tl.y; lv[4 * cc + 2] = tl.z; lv[4 * cc + 3] = tl.w;
         }
         tmem_st8(tdst + 16 * xy, hv);
-        tmem_st8(tdst + 32 + 16 * xy, lv);
+        if (FP8) {
+          uint32_t a8[4], l8[4];
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            a8[c] = cvt_e5m2x2_f16x2(hv[2 * c]) | (cvt_e5m2x2_f16x2(hv[2 * c + 1]) << 16);
+            l8[c] = cvt_e5m2x2_f16x2(lv[2 * c]) | (cvt_e5m2x2_f16x2(lv[2 * c + 1]) << 16);
+          }
+          const uint32_t t8 = a_ring + ts * C::TSLOT_COLS + 32 + 4 * h + lane_base;
+          tmem_st4(t8 + 8 * xy, a8);
+          tmem_st4(t8 + 16 + 8 * xy, l8);
+        } else {
+          tmem_st8(tdst + 32 + 16 * xy, lv);
+        }
       }
       tmem_wait_st();
       tc_fence_before();
@@ -278,7 +318,8 @@ __global__ void cplx_absmax_kernel(const double2* __restrict__ x, long long n, l
 template <bool TRANSPOSE>
 __global__ void __launch_bounds__(256) cplx_to_hl16_rows_kernel(const double2* __restrict__ x, long long ld, int rows, int kcols,
                                                                 long long x_bs, __half* __restrict__ out, int rows_pad,
-                                                                int kst, long long plane_halves, const float* __restrict__ amax) {
+                                                                int kst, long long plane_halves, const float* __restrict__ amax,
+                                                                unsigned char* __restrict__ out8 = nullptr) {
   __shared__ float tx[32][33], ty[32][33];
   const int b = blockIdx.z, sg = blockIdx.x, r0 = blockIdx.y * 32;
   const double scale = exp2((double)f16_scale_exp(amax[b]));
@@ -313,13 +354,25 @@ __global__ void __launch_bounds__(256) cplx_to_hl16_rows_kernel(const double2* _
     out[o + 32] = __float2half_rn(fx - __half2float(hx));
     out[plane_halves + o] = hy;
     out[plane_halves + o + 32] = __float2half_rn(fy - __half2float(hy));
+    if (out8) {   // hb8 rows: h[32] halves | e5m2(v)[32] | e5m2(v - h)[32]
+      reinterpret_cast<__half*>(out8)[o] = hx;
+      reinterpret_cast<__half*>(out8)[plane_halves + o] = hy;
+      unsigned char* bx = out8 + 2 * (o - tl) + tl;
+      unsigned char* by = bx + 2 * plane_halves;
+      bx[64] = (unsigned char)__nv_cvt_float_to_fp8(fx, __NV_SATFINITE, __NV_E5M2);
+      bx[96] = (unsigned char)__nv_cvt_float_to_fp8(fx - __half2float(hx), __NV_SATFINITE, __NV_E5M2);
+      by[64] = (unsigned char)__nv_cvt_float_to_fp8(fy, __NV_SATFINITE, __NV_E5M2);
+      by[96] = (unsigned char)__nv_cvt_float_to_fp8(fy - __half2float(hy), __NV_SATFINITE, __NV_E5M2);
+    }
   }
 }
 
 }  // namespace
 
 cudaError_t sigc_f16_configure() {
-  return cudaFuncSetAttribute(sigc_f16_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SCfg::SMEM_BYTES);
+  cudaError_t e = cudaFuncSetAttribute(sigc_f16_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SCfg::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(sigc_f16_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SCfg::SMEM_BYTES);
 }
 
 size_t sigc_f16_z_halves(long long pairs_cap, int n_m) {
@@ -330,8 +383,8 @@ size_t sigc_f16_w_halves(int n_m, int n_freq) {
 }
 
 cudaError_t launch_sigc_zw_f16(const double2* z, const double2* wc, const double* w, long long ld_w, int pairs, int n_m,
-                               int n_freq, __half* zk16, __half* w16, float* amax /*[1 + n_freq]*/, double2* zw,
-                               cudaStream_t s) {
+                               int n_freq, __half* zk16, __half* w16, unsigned char* w8 /*hb8 copy of W: E5M2 corrections; or null*/,
+                               float* amax /*[1 + n_freq]*/, double2* zw, cudaStream_t s) {
   const int kst = (n_m + 31) / 32, n_m_pad = (n_m + 127) / 128 * 128;
   const long long pairs_pad = ((long long)pairs + 127) / 128 * 128;
   cudaError_t e = cudaMemsetAsync(amax, 0, sizeof(float) * (1 + n_freq), s);
@@ -342,11 +395,12 @@ cudaError_t launch_sigc_zw_f16(const double2* z, const double2* wc, const double
   cplx_to_hl16_rows_kernel<false><<<dim3(kst, (unsigned)(pairs_pad / 32), 1), 256, 0, s>>>(z, n_m, pairs, n_m, 0, zk16, (int)pairs_pad,
                                                                                          kst, zplane, amax);
   cplx_to_hl16_rows_kernel<true><<<dim3(kst, n_m_pad / 32, n_freq), 256, 0, s>>>(wc, n_m, n_m, n_m, (long long)n_m * n_m, w16,
-                                                                                n_m_pad, kst, wplane, amax + 1);
+                                                                                n_m_pad, kst, wplane, amax + 1, w8);
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   SigcF16Args a;
   e = make_hl16_map(&a.tmap_z, zk16, (long long)kst * 64, pairs_pad, zplane);
   if (e == cudaSuccess) e = make_hl16_map(&a.tmap_w, w16, (long long)kst * 64, (long long)n_freq * n_m_pad, wplane);
+  if (e == cudaSuccess && w8) e = make_hb8_map(&a.tmap_w8, w8, (long long)kst * 64, (long long)n_freq * n_m_pad, wplane);
   if (e != cudaSuccess) return e;
   a.w = w;
   a.ld_w = ld_w;
@@ -359,7 +413,9 @@ cudaError_t launch_sigc_zw_f16(const double2* z, const double2* wc, const double
   a.n_freq = n_freq;
   a.kst = kst;
   a.n_tiles_n = n_m_pad / 128;
-  sigc_f16_kernel<<<dim3((unsigned)(a.n_tiles_n * (pairs_pad / 128))), kThreadsS, SCfg::SMEM_BYTES, s>>>(a);
+  const dim3 grid((unsigned)(a.n_tiles_n * (pairs_pad / 128)));
+  if (w8) sigc_f16_kernel<true><<<grid, kThreadsS, SCfg::SMEM_BYTES, s>>>(a);
+  else sigc_f16_kernel<false><<<grid, kThreadsS, SCfg::SMEM_BYTES, s>>>(a);
   return cudaGetLastError();
 }
 

@@ -133,8 +133,8 @@ def test_degenerate_weights_zero_dE_and_empty_tail():
 @pytest.mark.parametrize("case", ["ragged", "cfg1", "cfg2"])
 def test_mixed_context_tcgen05_zw(case):
     """A QSGW_PREC_MIXED context runs the frequency loop ZW^c on tcgen05 with FP16-split operands (FP32-grade products,
-    FP32 sums over mu and i, the closing contraction in FP64): tolerance 1e-5 relative Frobenius on I^c (the north_star
-    mixed bar is 2e-5); option "sigc_f64" keeps the FP64 GEMM on the FP32-grade z (<= 1e-6)."""
+    FP32 sums over mu and i, the closing contraction in FP64; the two correction products in E5M2 by default, option
+    "sigc_fp8" = 0: in FP16): tolerance 1e-5 relative Frobenius on I^c (the north_star mixed bar is 2e-5); option "sigc_f64" keeps the FP64 GEMM on the FP32-grade z (<= 1e-6)."""
     if case == "ragged":
         prob = generate(RAGGED)
         n_k_norm = None
@@ -145,9 +145,13 @@ def test_mixed_context_tcgen05_zw(case):
         n_k_norm = cfg.n_k
         wcs = [synthetic_wc(cfg.n_m, prob.omega, seed=k) for k in range(3)]
     ref = oracle_sigc(prob, wcs, n_k_norm=n_k_norm)
-    got = cuda_sigc(prob, wcs, precision=1, n_k_norm=n_k_norm)
+    got = cuda_sigc(prob, wcs, precision=1, n_k_norm=n_k_norm)            # default: E5M2 correction products
     err = rel_fro(got, ref)
     assert 1e-12 < err <= 1e-5, err
+    got3 = cuda_sigc(prob, wcs, precision=1, n_k_norm=n_k_norm, options={"sigc_fp8": 0})   # three FP16 products per term
+    err3 = rel_fro(got3, ref)
+    assert 1e-12 < err3 <= 1e-5, err3
+    assert not np.array_equal(got, got3)
     if case == "ragged":
         got64 = cuda_sigc(prob, wcs, precision=1, n_k_norm=n_k_norm, options={"sigc_f64": 1})
         assert 1e-12 < rel_fro(got64, ref) <= 1e-6
