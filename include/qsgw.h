@@ -286,6 +286,19 @@ int32_t qsgw_n_m(const qsgw_ctx* ctx);                  /* N_M                  
 int32_t qsgw_n_b(const qsgw_ctx* ctx);                  /* N_b                                 */
 const char* qsgw_version(void);
 
+/* qsgw_chi0_to_coulomb_basis WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it).  Same arguments, layouts and result.  The scratch (padded chi0,
+ * intermediate, padded U) lives in a file-scope device array of 33 * 256 * 256 complex128 elements (33 MiB) that every GPU
+ * which loads the library holds until the process exits; the entry point calls no cudaMalloc, cudaFree, stream-ordered
+ * allocator or allocating library routine (it sets kernel attributes on its first call per device).
+ *   Limit: (2 n_freq + 1) * ceil64(n_m)^2 <= 33 * 256 * 256, e.g. n_m <= 256 at 16 frequencies, n_m <= 512 at 3;
+ *   larger problems are rejected with QSGW_ERR_ALLOC and a text in qsgw_last_create_error().
+ * All calls share the one array per GPU (it keeps the last call's contents; nothing in it has to start at zero, every
+ * element that is read is written first by the same call): calls that OVERLAP on the GPU (different streams, no ordering
+ * between them) race on it.  Stream-ordered on `cuda_stream`, no synchronisation. */
+int32_t qsgw_chi0_to_coulomb_basis_static(int32_t n_m, int32_t n_freq, const void* d_chi0, const void* d_U, void* d_out,
+                                          void* cuda_stream);
+
 /* Orthonormal mixed product basis that diagonalises the Coulomb matrix (row f4; Eq. 7):
  *   |E_mu> = sum_I z_{mu I} |M_I>,   sum_J (v_IJ - v_mu O_IJ) z_{mu J} = 0,   z^H O z = 1,
  * O_IJ = <M_I|M_J> the overlap matrix (Hermitian positive definite), v_IJ = <M_I|v|M_J> the Coulomb matrix (Hermitian) of

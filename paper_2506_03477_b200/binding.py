@@ -93,6 +93,8 @@ def lib() -> C.CDLL:
     L.qsgw_n_b.argtypes = [vp]
     L.qsgw_wc_from_chi0.argtypes = [i32, i32, vp, vp, vp, vp, vp]
     L.qsgw_chi0_to_coulomb_basis.argtypes = [i32, i32, vp, vp, vp, vp]
+    L.qsgw_chi0_to_coulomb_basis_static.argtypes = [i32, i32, vp, vp, vp, vp]
+    L.qsgw_chi0_to_coulomb_basis_static.restype = i32
     _lib = L
     return L
 
@@ -324,6 +326,20 @@ def chi0_to_coulomb_basis(chi0, U, out=None):
     stream = C.c_void_p(torch.cuda.current_stream().cuda_stream)
     rc = L.qsgw_chi0_to_coulomb_basis(n_m, n_freq, _ptr(chi0, torch.complex128), _ptr(U, torch.complex128),
                                       _ptr(out, torch.complex128), stream)
+    if rc != 0:
+        raise QsgwError(rc, L.qsgw_last_create_error().decode())
+    return out
+
+
+def chi0_to_coulomb_basis_static(chi0, U, out):
+    """qsgw_chi0_to_coulomb_basis_static: the same rotation on the library's file-scope device scratch; the call allocates
+    nothing (the caller passes `out`).  Limit (2 n_freq + 1) ceil64(N_M)^2 <= 33 * 256 * 256; calls that overlap on the GPU race."""
+    import torch
+    L = lib()
+    n_freq, n_m = int(chi0.shape[0]), int(chi0.shape[1])
+    stream = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    rc = L.qsgw_chi0_to_coulomb_basis_static(n_m, n_freq, _ptr(chi0, torch.complex128), _ptr(U, torch.complex128),
+                                             _ptr(out, torch.complex128), stream)
     if rc != 0:
         raise QsgwError(rc, L.qsgw_last_create_error().decode())
     return out

@@ -221,6 +221,11 @@ cudaError_t wc_configure();          // kernel attributes (per device)
 size_t rotate_work_elems(int n_m, int n_freq);
 cudaError_t launch_rotate_basis(int n_m, int n_freq, const double2* chi0, const double2* U, double2* out, double2* work,
                                 cudaStream_t s);
+// The same on a file-scope device array of rotate_static_max_elems() complex elements (no allocation of any kind;
+// cudaErrorMemoryAllocation when rotate_work_elems(n_m, n_freq) exceeds it).  Calls that overlap on the GPU race.
+long long rotate_static_max_elems();
+cudaError_t launch_rotate_basis_static(int n_m, int n_freq, const double2* chi0, const double2* U, double2* out,
+                                       cudaStream_t s);
 cudaError_t launch_wc_from_chi0(int n_m, int n_freq, const double2* chi0, const double* v, double2* wc_out,
                                 double2* work, int* d_info, cudaStream_t s);
 

@@ -1429,6 +1429,30 @@ int32_t qsgw_chi0_to_coulomb_basis(int32_t n_m, int32_t n_freq, const void* d_ch
   return QSGW_OK;
 }
 
+int32_t qsgw_chi0_to_coulomb_basis_static(int32_t n_m, int32_t n_freq, const void* d_chi0, const void* d_U, void* d_out,
+                                          void* cuda_stream) {
+  g_create_error.clear();
+  if (!d_chi0 || !d_U || !d_out) { g_create_error = "NULL argument"; return QSGW_ERR_INVALID_ARG; }
+  if (d_chi0 == d_out) { g_create_error = "d_out aliases d_chi0"; return QSGW_ERR_INVALID_ARG; }
+  if (n_m < 1 || n_freq < 1) { g_create_error = "n_m and n_freq must be positive"; return QSGW_ERR_SHAPE; }
+  const long long need = (long long)qsgw::rotate_work_elems(n_m, n_freq);
+  if (need > qsgw::rotate_static_max_elems()) {
+    char buf[256];
+    snprintf(buf, sizeof(buf), "(2 n_freq + 1) ceil64(n_m)^2 = %lld complex elements exceed the static scratch of %lld "
+             "(e.g. n_m <= 256 at 16 frequencies): use qsgw_chi0_to_coulomb_basis", need, qsgw::rotate_static_max_elems());
+    g_create_error = buf;
+    return QSGW_ERR_ALLOC;
+  }
+  DevInfo di;
+  int rc = wc_prologue(&di);
+  if (rc != QSGW_OK) return rc;
+  cudaError_t e = qsgw::launch_rotate_basis_static(n_m, n_freq, static_cast<const double2*>(d_chi0),
+                                                   static_cast<const double2*>(d_U), static_cast<double2*>(d_out),
+                                                   static_cast<cudaStream_t>(cuda_stream));
+  if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("rotation kernels (static scratch): ") + cudaGetErrorString(e); return QSGW_ERR_CUDA; }
+  return QSGW_OK;
+}
+
 int32_t qsgw_zmel_ipw_build(const int32_t* h_L, const void* d_theta, int32_t n_pw_kq, const int32_t* d_g_kq, int32_t n_pw_k,
                             const int32_t* d_g_k, int32_t n_ipw, const int32_t* d_g_ipw, const void* d_Bk, int64_t ld_k,
                             int32_t n_o, const void* d_Bkq, int64_t ld_kq, int32_t n_u, void* d_z_out, int64_t ld_z,

@@ -297,3 +297,45 @@ cudaError_t launch_rotate_basis(int n_m, int n_freq, const double2* chi0, const 
 }
 
 }  // namespace qsgw
+
+// ---- basis rotation without any allocation: scratch in a file-scope device array -------------------------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+// The array is part of the library image: EVERY GPU that loads libqsgw.so holds kRotStaticElems * 16 bytes (33 MiB) until the
+// process exits.  In host code the array's name is a host-side stand-in, not a device address: the address a kernel may use
+// comes from cudaGetSymbolAddress, taken once per device with that device current (rot_static_ptr).
+namespace qsgw {
+
+constexpr long long kRotStaticElems = 33LL * 256 * 256;     // (2 n_freq + 1) ceil64(N_M)^2 complex elements, e.g. N_M <= 256 at 16 frequencies
+static __device__ __align__(256) double2 g_rot_scratch[kRotStaticElems];
+
+long long rotate_static_max_elems() { return kRotStaticElems; }
+
+static cudaError_t rot_static_ptr(double2** out) {
+  static double2* ptr[kMaxDevices] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  if (!ptr[dev]) {
+    double2* p = nullptr;
+    e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_rot_scratch);    // device `dev` is current
+    if (e != cudaSuccess) return e;
+    ptr[dev] = p;
+  }
+  *out = ptr[dev];
+  return cudaSuccess;
+}
+
+// launch_rotate_basis on the static scratch.  cudaErrorMemoryAllocation if the problem needs more than kRotStaticElems.
+// Nothing in the scratch has to start at zero: the padding kernels write every element of the padded chi0 and U, the first
+// GEMM every element of the intermediate.  All calls share the array: calls that overlap on the GPU (two streams) race.
+cudaError_t launch_rotate_basis_static(int n_m, int n_freq, const double2* chi0, const double2* U, double2* out,
+                                       cudaStream_t s) {
+  if ((long long)rotate_work_elems(n_m, n_freq) > kRotStaticElems) return cudaErrorMemoryAllocation;
+  double2* work = nullptr;
+  cudaError_t e = rot_static_ptr(&work);
+  if (e != cudaSuccess) return e;
+  return launch_rotate_basis(n_m, n_freq, chi0, U, out, work, s);
+}
+
+}  // namespace qsgw
