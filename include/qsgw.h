@@ -354,6 +354,8 @@ int32_t qsgw_mixed_stats(qsgw_ctx* ctx, int64_t* out_launches, int64_t* out_laun
  *   "mixed_pair"      0 | 1    mixed stage (b): one CTA per (tile, frequency) | CTA pairs (tcgen05 cta_group::2) that share
  *                              the B tiles of two consecutive frequencies (default 1; the binned real-axis path always uses 0)
  *   "sigc_f64"        0 | 1    mixed context: qsgw_sigc_imag_accumulate on tcgen05 (default) | with the FP64 GEMM
+ *   "sigc_fp8"        0 | 1    mixed context, tcgen05 path of qsgw_sigc_imag_accumulate: three FP16 products per term | FP16 main
+ *                              product + two E5M2 correction products (default 1)
  *   "e2e_groups"      1..4     frequency groups of the last launch of qsgw_chi0_run_host (default 4)
  * ctx == NULL, process-wide:
  *   "wc_graph"        0 | 1 | 2  qsgw_wc_from_chi0: plain launches | CUDA graph with fallback (default) | graph or fail
