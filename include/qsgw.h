@@ -311,8 +311,9 @@ int32_t qsgw_chi0_to_coulomb_basis_static(int32_t n_m, int32_t n_freq, const voi
  *   h_info     : HOST int32 (optional): 0 | 1 + index of the first non-positive Cholesky pivot of O (not positive
  *                definite; QSGW_ERR_INVALID_ARG) | -1 the Jacobi iteration did not converge (QSGW_ERR_CUDA)
  *   h_sweeps   : HOST int32 (optional): Jacobi sweeps taken
- * Method: blocked Cholesky O = L L^H and X = L^-1 on the FP64 tensor pipe, C = X v X^H, two-sided Jacobi with the
- * round-robin parallel ordering (N_M / 2 rotations per round, every 2 x 2 block updated by one thread), U = X^H Q.
+ * Method: blocked Cholesky O = L L^H and X = L^-1 on the FP64 tensor pipe, C = X v X^H, two-sided block Jacobi with the
+ * round-robin parallel ordering (64 x 64 subproblems in shared memory, their unitaries applied to C and Q by 64^3 complex
+ * GEMMs on the FP64 tensor pipe; process-wide option "eig_blocked" = 0: element-wise rounds), U = X^H Q.
  * SYNCHRONISES `cuda_stream` once per sweep (convergence is decided on the host).  Error text in qsgw_last_create_error(). */
 int32_t qsgw_coulomb_eigenbasis(int32_t n_m, const void* d_v, const void* d_O, double* d_vmu_out, void* d_U_out,
                                 int32_t* h_info, int32_t* h_sweeps, void* cuda_stream);
@@ -359,6 +360,7 @@ int32_t qsgw_mixed_stats(qsgw_ctx* ctx, int64_t* out_launches, int64_t* out_laun
  *   "e2e_groups"      1..4     frequency groups of the last launch of qsgw_chi0_run_host (default 4)
  * ctx == NULL, process-wide:
  *   "wc_graph"        0 | 1 | 2  qsgw_wc_from_chi0: plain launches | CUDA graph with fallback (default) | graph or fail
+ *   "eig_blocked"     0 | 1    qsgw_coulomb_eigenbasis: element-wise Jacobi rounds | block rounds on the tensor pipe (default 1)
  *   "trim_workspace"  bytes    qsgw_wc_from_chi0 / qsgw_chi0_to_coulomb_basis keep their stream-ordered workspace in a
  *                              private memory pool between calls; this returns all but `bytes` of it to the driver
  * Unknown key or value out of range: QSGW_ERR_INVALID_ARG. */

@@ -362,6 +362,7 @@ cudaError_t wc_configure_device(int dev) {
   std::lock_guard<std::mutex> lock(mu);
   if (dev >= 0 && dev < qsgw::kMaxDevices && done[dev]) return cudaSuccess;
   cudaError_t e = qsgw::wc_configure();
+  if (e == cudaSuccess) e = qsgw::eig_configure();
   if (e == cudaSuccess && dev >= 0 && dev < qsgw::kMaxDevices) done[dev] = true;
   return e;
 }
@@ -397,6 +398,7 @@ cudaError_t work_alloc(int dev, void** p, size_t bytes, cudaStream_t st) {
   return pool ? cudaMallocFromPoolAsync(p, bytes, pool, st) : cudaMallocAsync(p, bytes, st);
 }
 
+int g_eig_blocked = 1;  // option "eig_blocked": qsgw_coulomb_eigenbasis with block rounds (1) | element-wise rounds (0)
 int g_wc_graph = 1;     // option "wc_graph": 0 plain launches | 1 graph with fallback | 2 graph or fail
 
 // Internal streams (one per device) and in-flight executable graphs of qsgw_wc_from_chi0 (destroyed once their
@@ -711,6 +713,7 @@ int32_t qsgw_set_option(qsgw_ctx* ctx, const char* key, int64_t value) {
   if (!ctx) {
     g_create_error.clear();
     if (k == "wc_graph" && value >= 0 && value <= 2) { g_wc_graph = (int)value; return QSGW_OK; }
+    if (k == "eig_blocked" && (value == 0 || value == 1)) { g_eig_blocked = (int)value; return QSGW_OK; }
     if (k == "trim_workspace") {     // hand the cached W^c / rotation workspace of every device back to the driver
       std::lock_guard<std::mutex> lock(g_work_pool_mu);
       for (int d = 0; d < qsgw::kMaxDevices; ++d)
@@ -1534,7 +1537,7 @@ int32_t qsgw_coulomb_eigenbasis(int32_t n_m, const void* d_v, const void* d_O, d
   int sweeps = 0;
   bool converged = false;
   for (; sweeps < 60 && !converged;) {
-    QSGW_E(qsgw::launch_eig_sweep(n_m, work, d_norms, st), "Jacobi sweep");
+    QSGW_E(qsgw::launch_eig_sweep(n_m, work, d_norms, g_eig_blocked != 0, st), "Jacobi sweep");
     double nr[2] = {0.0, 0.0};
     QSGW_E(cudaMemcpyAsync(nr, d_norms, 2 * sizeof(double), cudaMemcpyDeviceToHost, st), "copy of the norms");
     QSGW_E(cudaStreamSynchronize(st), "stream synchronisation");

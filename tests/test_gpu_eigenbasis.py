@@ -86,3 +86,20 @@ def test_cfg4_size():
     w_ref, U_ref = oracle.coulomb_eigenbasis_ref(v, O)
     assert np.abs(w - lam).max() <= 1e-9 * lam.max()
     check(v, O, w, U, w_ref, U_ref)
+
+
+@pytest.mark.parametrize("n", [99, 240])
+def test_elementwise_rounds_option(n):
+    """Process-wide option "eig_blocked" = 0: the element-wise parallel Jacobi rounds (the first round-2 version, kept for
+    comparison) give the same eigenvalues and a valid basis."""
+    import paper_2506_03477_b200 as q
+    v, O, lam = synthetic_mpb_matrices(n, seed=n + 1)
+    w_ref, U_ref = oracle.coulomb_eigenbasis_ref(v, O)
+    q.set_global_option("eig_blocked", 0)
+    try:
+        w0, U0, _ = run(v, O)
+    finally:
+        q.set_global_option("eig_blocked", 1)
+    w1, U1, _ = run(v, O)
+    check(v, O, w0, U0, w_ref, U_ref)
+    check(v, O, w1, U1, w_ref, U_ref)
