@@ -10,6 +10,8 @@
 //   jacobi_apply_kernel: N / 2 rotations per round, every 2 x 2 block updated by one thread, N - 1 passes per sweep) is kept
 //   for comparison: 2.13 s against 0.50 s at N = 2400.
 //   U = X^H Q with the columns ordered by descending eigenvalue (one more GEMM).
+#include <vector>
+
 #include "kernels.h"
 
 namespace qsgw {
@@ -243,8 +245,11 @@ __device__ __forceinline__ void dmma884e(double& c0, double& c1, double a, doubl
 // blockIdx.y < npairs: tile (rows of pair i = blockIdx.y) x (columns of pair j = blockIdx.x) of C <- W_i^H B W_j;
 // blockIdx.y >= npairs: rows 64 (blockIdx.y - npairs) .. + 63 of Q x (columns of pair j) <- B W_j.
 // 8 warps, warp tile 16 rows x 32 columns, complex product as four real DMMA products on separate Re / Im planes.
+// phase 0: every tile; phase 1: only the tiles of C flagged in `flags` (those the subproblems of the NEXT block round read);
+// phase 2: every other tile of C and all tiles of Q (runs while the next round's subproblems are being solved).
 __global__ void __launch_bounds__(256, 1) bj_update_kernel(double2* __restrict__ A, double2* __restrict__ V, int N, int r,
-                                                           const double2* __restrict__ Wall) {
+                                                           const double2* __restrict__ Wall,
+                                                           const unsigned char* __restrict__ flags, int phase) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* Bre = reinterpret_cast<double*>(smem_raw);      // [64][68] each
   double* Bim = Bre + kBJ2 * kBJLd;
@@ -256,6 +261,10 @@ __global__ void __launch_bounds__(256, 1) bj_update_kernel(double2* __restrict__
   const int npairs = N / kBJ2, nblk = N / kBJ;
   const bool is_a = (int)blockIdx.y < npairs;
   if (is_a && blockIdx.y > blockIdx.x) return;           // lower tiles of C are written by their mirror images
+  if (phase != 0) {
+    const bool flagged = is_a && flags[blockIdx.y * npairs + blockIdx.x] != 0;
+    if ((phase == 1) != flagged) return;
+  }
   int Pj, Qj, Pi = 0, Qi = 0;
   rr_pair(blockIdx.x, r, nblk, Pj, Qj);
   double2* M = V;
@@ -518,12 +527,80 @@ cudaError_t launch_eig_sweep(int n_m, double2* work, double* d_norms, bool block
   double2* Abuf = work;
   double2* Vbuf = work + 2 * sM;
   if (blocked) {
-    double2* Wall = work + 4 * sM;                       // Tbuf of the reduction: (N / 64) matrices of 64 x 64
-    const int npairs = N / kBJ2;
-    for (int r = 0; r < N / kBJ - 1; ++r) {
-      bj_solve_kernel<<<npairs, 1024, kBJSolveSmem, s>>>(Abuf, N, r, Wall, kBJInnerSweeps);
-      bj_update_kernel<<<dim3(npairs, 2 * npairs), 256, kBJUpdateSmem, s>>>(Abuf, Vbuf, N, r, Wall);
+    // Look-ahead: the subproblems of round r + 1 read only a few tiles of C (two diagonal tiles and one off-diagonal tile
+    // per pair).  Those are updated first (phase 1); the subproblems are then solved on a second stream while the first
+    // stream updates everything else (phase 2).  Two W buffers (Tbuf of the reduction, and the Q scratch of the back
+    // transformation); the per-round tile flags sit in the Linv region of the reduction (free during the sweeps).
+    double2* Wbuf[2] = {work + 4 * sM, work + 3 * sM};
+    unsigned char* flags = reinterpret_cast<unsigned char*>(work + 4 * sM + 64LL * N);
+    const int npairs = N / kBJ2, nblk = N / kBJ, rounds = nblk - 1;
+    const size_t flag_bytes = (size_t)rounds * npairs * npairs;
+    const bool ahead = rounds > 1 && flag_bytes <= (size_t)(N / 64) * 4096 * sizeof(double2);
+    cudaStream_t s2 = nullptr;
+    cudaEvent_t e1 = nullptr, e2 = nullptr;
+    cudaError_t e = cudaSuccess;
+    if (ahead) {
+      std::vector<unsigned char> h(flag_bytes, 0);
+      std::vector<int> pair_of((size_t)nblk);
+      auto host_pair = [&](int i, int r, int& p, int& q) {
+        const int m = nblk - 1;
+        if (i == 0) { p = r; q = nblk - 1; return; }
+        p = (r + i) % m;
+        q = ((r - i) % m + m) % m;
+      };
+      for (int r = 0; r + 1 < rounds; ++r) {
+        for (int i = 0; i < npairs; ++i) {
+          int p, q;
+          host_pair(i, r, p, q);
+          pair_of[(size_t)p] = i;
+          pair_of[(size_t)q] = i;
+        }
+        unsigned char* f = h.data() + (size_t)r * npairs * npairs;
+        for (int i = 0; i < npairs; ++i) {
+          int p, q;
+          host_pair(i, r + 1, p, q);
+          const int a = pair_of[(size_t)p], b = pair_of[(size_t)q];
+          f[a * npairs + a] = 1;
+          f[b * npairs + b] = 1;
+          f[(a < b ? a : b) * npairs + (a < b ? b : a)] = 1;
+        }
+      }
+      e = cudaMemcpyAsync(flags, h.data(), flag_bytes, cudaMemcpyHostToDevice, s);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(s);               // h is a host temporary
+      if (e == cudaSuccess) {       // highest priority: the 38 subproblem CTAs must get their SMs before the update's 2000+ CTAs
+        int lo = 0, hi = 0;
+        e = cudaDeviceGetStreamPriorityRange(&lo, &hi);
+        if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&s2, cudaStreamNonBlocking, hi);
+      }
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&e1, cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&e2, cudaEventDisableTiming);
     }
+    if (e == cudaSuccess) {
+      bj_solve_kernel<<<npairs, 1024, kBJSolveSmem, s>>>(Abuf, N, 0, Wbuf[0], kBJInnerSweeps);
+      for (int r = 0; r < rounds && e == cudaSuccess; ++r) {
+        const double2* W = Wbuf[r & 1];
+        const bool la = ahead && r + 1 < rounds;
+        if (!la) {
+          bj_update_kernel<<<dim3(npairs, 2 * npairs), 256, kBJUpdateSmem, s>>>(Abuf, Vbuf, N, r, W, nullptr, 0);
+          if (r + 1 < rounds) bj_solve_kernel<<<npairs, 1024, kBJSolveSmem, s>>>(Abuf, N, r + 1, Wbuf[(r + 1) & 1], kBJInnerSweeps);
+          continue;
+        }
+        const unsigned char* f = flags + (size_t)r * npairs * npairs;
+        bj_update_kernel<<<dim3(npairs, npairs), 256, kBJUpdateSmem, s>>>(Abuf, Vbuf, N, r, W, f, 1);
+        e = cudaEventRecord(e1, s);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s2, e1, 0);
+        if (e != cudaSuccess) break;
+        bj_solve_kernel<<<npairs, 1024, kBJSolveSmem, s2>>>(Abuf, N, r + 1, Wbuf[(r + 1) & 1], kBJInnerSweeps);
+        e = cudaEventRecord(e2, s2);
+        bj_update_kernel<<<dim3(npairs, 2 * npairs), 256, kBJUpdateSmem, s>>>(Abuf, Vbuf, N, r, W, f, 2);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s, e2, 0);
+      }
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e1) cudaEventDestroy(e1);
+    if (e2) cudaEventDestroy(e2);
+    if (s2) cudaStreamDestroy(s2);
+    if (e != cudaSuccess) return e;
   } else {
     double4* params = reinterpret_cast<double4*>(work + 4 * sM + 64LL * N + (long long)(N / 64) * 4096);
     const int half = N / 2;
