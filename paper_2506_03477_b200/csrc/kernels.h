@@ -54,6 +54,16 @@ struct ZmelArgs {
 cudaError_t launch_zmel_f64(const ZmelArgs& a, cudaStream_t s);    // CUDA-core fallback
 cudaError_t launch_zmel_dmma(const ZmelArgs& a, cudaStream_t s);   // step 2 on the FP64 tensor pipe (default)
 size_t zmel_dmma_smem_bytes(int b_max, int kt);
+// Mixed mode: stage (a) on tcgen05 that writes the hl16 / hb8 operand rows of stage (b) itself (zmel_umma_kernels.cu).
+// a.zmax[b] receives an upper BOUND of max |z| of batch b (the FP16 scale has to be known before the rows are written);
+// pmax[s] = max_{I in s} ||P_I||_F (launch_zmel_pnorm, once per product tensor); cnorm: scratch of (2 n_sites + 2) n_batch floats;
+// aop: scratch of zmel_umma_aop_halves halves; zhl / zhb8 = the slot of batch 0; n_rows = padded pair rows of a batch.
+bool zmel_umma_supported(int b_max);
+size_t zmel_umma_aop_halves(int n_sites, int n_u, int n_batch);
+cudaError_t zmel_umma_configure();
+cudaError_t launch_zmel_pnorm(const SiteTables& st, const double2* P, float* pmax, cudaStream_t s);
+cudaError_t launch_zmel_umma(const ZmelArgs& a, const float* pmax, float* cnorm, __half* aop, void* zhl, void* zhb8, int n_m_pad,
+                             long long n_rows, cudaStream_t s);
 cudaError_t launch_z_export(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs,
                             double2* out, cudaStream_t s);
 cudaError_t launch_z_import(double* zws, long long kpad, int ncg, int n_m, long long n_pairs,

@@ -120,6 +120,13 @@ struct qsgw_ctx {
   CUtensorMap tmap_hb8;
   double* d_wscale = nullptr;
   float* d_zmax = nullptr;
+  // mixed, direct stage (a) on tcgen05 (option "zmel_direct"): max_I ||P_I||_F per site, per-batch norm scratch, A operand
+  float* d_pmax = nullptr;
+  float* d_cnorm = nullptr;
+  size_t cnorm_cap = 0;
+  __half* d_aop = nullptr;
+  size_t aop_cap = 0;
+  int zmel_direct = 0;          // 0 never | 1 for launches of >= 8 M matrix elements (default where supported) | 2 always
   qsgw::MixedCtl* d_ctl = nullptr;   // device-side choice of the product variant per flush
   int fp8_mode = 2;             // 0 never | 1 always | 2 chosen on the device (option "mixed_fp8")
   double fp8_thr = 4.0;         // automatic choice: E5M2 when P_eff >= fp8_thr * N_M (measured, DESIGN.md 4b:
@@ -245,6 +252,9 @@ void free_all(qsgw_ctx* c) {
   cudaFree(c->d_zhb8);
   cudaFree(c->d_wscale);
   cudaFree(c->d_zmax);
+  cudaFree(c->d_pmax);
+  cudaFree(c->d_cnorm);
+  cudaFree(c->d_aop);
   cudaFree(c->d_acc_re);
   cudaFree(c->d_acc_im);
 }
@@ -618,6 +628,8 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wscale, (size_t)c->n_freq));
     QSGW_TRY_ALLOC(dev_alloc(c, &c->d_zmax, (size_t)(c->kpad / qsgw::kPairAlign + 1)));   // one scale per staged batch
     QSGW_TRY_ALLOC(dev_alloc(c, &c->d_ctl, (size_t)1));
+    QSGW_TRY_ALLOC(dev_alloc(c, &c->d_pmax, (size_t)c->n_sites));
+    c->zmel_direct = qsgw::zmel_umma_supported(c->b_max) ? 1 : 0;
   }
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab, (size_t)c->n_freq * c->kpad));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_acc_re, acc_elems));
@@ -739,6 +751,10 @@ int32_t qsgw_set_option(qsgw_ctx* ctx, const char* key, int64_t value) {
     if (upload_ctl(ctx) != cudaSuccess) return ctx->fail(QSGW_ERR_CUDA, "upload of the mixed-mode control block failed");
   } else if (k == "mixed_window" && value >= 1 && value <= 64 && ctx->f16) {
     ctx->win = (int)value;
+  } else if (k == "zmel_direct" && value >= 0 && value <= 2 && ctx->f16) {
+    if (value != 0 && !qsgw::zmel_umma_supported(ctx->b_max))
+      return ctx->fail(QSGW_ERR_UNSUPPORTED, "the tcgen05 stage (a) kernel holds at most 32 orbitals per site");
+    ctx->zmel_direct = (int)value;
   } else if (k == "mixed_pair" && (value == 0 || value == 1) && ctx->f16) {
     ctx->mixed_pair = (int)value;
   } else if (k == "sigc_f64" && (value == 0 || value == 1) && ctx->f16) {
@@ -777,10 +793,13 @@ int32_t qsgw_sync(qsgw_ctx* ctx) {
   return QSGW_OK;
 }
 
+static qsgw::SiteTables site_tables(const qsgw_ctx* ctx);
+
 int32_t qsgw_set_product_tensor(qsgw_ctx* ctx, const void* d_P) {
   if (!ctx) return QSGW_ERR_INVALID_ARG;
   if (!d_P) return ctx->fail(QSGW_ERR_INVALID_ARG, "d_P is NULL");
   cudaError_t e = cudaMemcpyAsync(ctx->d_P, d_P, sizeof(double2) * ctx->p_elems, cudaMemcpyDeviceToDevice, ctx->stream);
+  if (e == cudaSuccess && ctx->d_pmax) e = qsgw::launch_zmel_pnorm(site_tables(ctx), ctx->d_P, ctx->d_pmax, ctx->stream);
   if (e != cudaSuccess) return ctx->cuda_fail(e, "copy of P");
   if (ctx->state == ST_CREATED) ctx->state = ST_READY;
   ctx->err.clear();
@@ -818,6 +837,19 @@ static int check_batch(qsgw_ctx* ctx, int n_o, int n_u) {
   return QSGW_OK;
 }
 
+static qsgw::SiteTables site_tables(const qsgw_ctx* ctx) {
+  qsgw::SiteTables st;
+  st.n_sites = ctx->n_sites;
+  st.n_b = ctx->n_b;
+  st.n_m = ctx->n_m;
+  st.b_max = ctx->b_max;
+  st.d_pb_site = ctx->d_pb_site;
+  st.d_pb_off = ctx->d_pb_off;
+  st.d_orb_off = ctx->d_orb_off;
+  st.d_p_off = ctx->d_p_off;
+  return st;
+}
+
 // Stage (a) for `n_batch` k-points of equal band batch in ONE launch (grid.z = k-point): k-point b reads
 // Ck + b*ck_bs, Ckq + b*ckq_bs and fills the workspace slot at pair offset off + b*n_pad with batch-scale index
 // zi + b.  The caller has made room ([off, off + n_batch*n_pad) <= kpad).
@@ -825,14 +857,7 @@ static int build_batches(qsgw_ctx* ctx, const double2* Ck, long long ld_k, long 
                          long long ld_kq, long long ckq_bs, int n_begin, int n_o, int np_begin, int n_u, int n_batch,
                          long long off, long long n_pad, int zi) {
   qsgw::ZmelArgs a;
-  a.st.n_sites = ctx->n_sites;
-  a.st.n_b = ctx->n_b;
-  a.st.n_m = ctx->n_m;
-  a.st.b_max = ctx->b_max;
-  a.st.d_pb_site = ctx->d_pb_site;
-  a.st.d_pb_off = ctx->d_pb_off;
-  a.st.d_orb_off = ctx->d_orb_off;
-  a.st.d_p_off = ctx->d_p_off;
+  a.st = site_tables(ctx);
   a.P = ctx->d_P;
   a.Ck = Ck;
   a.ld_k = ld_k;
@@ -853,6 +878,39 @@ static int build_batches(qsgw_ctx* ctx, const double2* Ck, long long ld_k, long 
   a.Ckq_bs = ckq_bs;
   a.z_bs = n_pad;
   cudaError_t e;
+  // small launches keep the two-kernel FP64 path: the tcgen05 path has four launches and a tensor-map encode per call
+  const bool direct = ctx->f16 && (ctx->zmel_direct == 2 ||
+                                   (ctx->zmel_direct == 1 && (double)n_batch * n_o * n_u * ctx->n_m >= 8.0e6));
+  if (direct) {   // stage (a) on tcgen05, straight into the FP16-split rows (no FP64 z, no conversion pass)
+    a.zmax = ctx->d_zmax + zi;
+    const size_t need_c = ((size_t)2 * ctx->n_sites + 2) * n_batch, need_a = qsgw::zmel_umma_aop_halves(ctx->n_sites, n_u, n_batch);
+    e = qsgw::zmel_umma_configure();
+    if (e == cudaSuccess && need_c > ctx->cnorm_cap) {
+      cudaStreamSynchronize(ctx->stream);
+      cudaFree(ctx->d_cnorm);
+      ctx->d_cnorm = nullptr;
+      ctx->cnorm_cap = 0;
+      e = dev_alloc(ctx, &ctx->d_cnorm, need_c);
+      if (e == cudaSuccess) ctx->cnorm_cap = need_c;
+    }
+    if (e == cudaSuccess && need_a > ctx->aop_cap) {
+      cudaStreamSynchronize(ctx->stream);
+      cudaFree(ctx->d_aop);
+      ctx->d_aop = nullptr;
+      ctx->aop_cap = 0;
+      e = dev_alloc(ctx, &ctx->d_aop, need_a);
+      if (e == cudaSuccess) ctx->aop_cap = need_a;
+    }
+    if (e != cudaSuccess) { cudaGetLastError(); return ctx->fail(QSGW_ERR_ALLOC, "stage (a) scratch allocation failed: %s", cudaGetErrorString(e)); }
+    {
+      StageScope ts(ctx, QSGW_STAGE_ZMEL);
+      e = qsgw::launch_zmel_umma(a, ctx->d_pmax, ctx->d_cnorm, ctx->d_aop, hl_slot(ctx->d_zhl, off), hl_slot(ctx->d_zhb8, off),
+                                 ctx->n_m_pad, round_up((long long)n_o * n_u, qsgw::kPairAlign), ctx->stream);
+    }
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "zmel (tcgen05, FP16-split rows) kernel launch");
+    ctx->launches += 4;
+    return QSGW_OK;
+  }
   if (ctx->f16) {
     a.zmax = ctx->d_zmax + zi;
     e = cudaMemsetAsync(a.zmax, 0, sizeof(float) * n_batch, ctx->stream);

@@ -210,3 +210,39 @@ def test_e5m2_error_table_and_threshold(capsys):
         assert e16 <= 5e-6, (name, e16)
         if pe >= 4.0:
             assert e8 <= 1.5e-5, (name, pe, e8)
+
+
+@pytest.mark.parametrize("case", ["ragged", "cfg1", "cfg2"])
+def test_tcgen05_stage_a_forced(case):
+    """Option "zmel_direct" = 2: stage (a) on tcgen05 writing the FP16-split operand rows itself (default only for large
+    launches).  ragged: column groups that straddle sites (several segments), 19 bands n' (one ragged tile), 5..12 orbitals
+    (one K step); cfg 2: 70 bands n', sites of more than 16 orbitals (two K steps); cfg 1: multi-k launch.  z (exported
+    from the rows): <= 8e-7 of max |z| (FP32-grade products, FP32 sums over <= 32 orbitals); chi0: the mixed bar."""
+    import torch
+    import paper_2506_03477_b200 as q
+    if case == "ragged":
+        prob, n_k_norm = generate(RAGGED), None
+    else:
+        cfg = get_config(1 if case == "cfg1" else 2)
+        prob, n_k_norm = generate(cfg, n_k=3), cfg.n_k
+    cfg, sp = prob.cfg, prob.spins[0]
+    ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, prob.omega, cfg.n_k, cfg.n_o, cfg.n_u, precision=MIXED)
+    ctx.set_option("zmel_direct", 2)
+    ctx.set_product_tensor(torch.from_numpy(prob.P).cuda())
+    z = torch.empty((cfg.n_o, cfg.n_u, cfg.n_m), dtype=torch.complex128, device="cuda")
+    ctx.zmel_build(torch.from_numpy(sp.Ck[0]).cuda(), torch.from_numpy(sp.Ckq[0]).cuda(), 0, cfg.n_o, 0, cfg.n_u, d_z_out=z)
+    ctx.sync()
+    zref = oracle.zmel_ref(sites_of(prob), sp.Ck[0], sp.Ckq[0])
+    err = np.abs(z.cpu().numpy() - zref).max() / np.abs(zref).max()
+    assert 1e-9 < err <= 8e-7, err
+    # sub-batch with band offsets
+    z2 = torch.empty((2, 3, cfg.n_m), dtype=torch.complex128, device="cuda")
+    ctx.zmel_build(torch.from_numpy(sp.Ck[0]).cuda(), torch.from_numpy(sp.Ckq[0]).cuda(), 1, 2, 2, 3, d_z_out=z2)
+    ctx.sync()
+    assert np.abs(z2.cpu().numpy() - zref[1:3, 2:5]).max() <= 8e-7 * np.abs(zref).max()
+    ctx.destroy()
+    ref = oracle_chi(prob, n_k_norm=n_k_norm)
+    for multi_k in (False, True):
+        got = run_cuda(prob, precision=MIXED, n_k_norm=n_k_norm, options={"zmel_direct": 2}, multi_k=multi_k)
+        assert rel_fro_per_freq(got, ref).max() <= TOL_MIXED
+        check_hermitian(got)

@@ -29,7 +29,7 @@ def batch_csr(w, n_u, n0, no, u0, nu, n_bins):
     return np.cumsum(ptr).astype(np.int32), ((n[sel] - n0) * nu + (u[sel] - u0)).astype(np.int32), ww[sel]
 
 
-def cuda_imchi(prob, edges, wts, n_k_norm=None, max_n_o=None, max_n_u=None, spin=0, stats=None, precision=0):
+def cuda_imchi(prob, edges, wts, n_k_norm=None, max_n_o=None, max_n_u=None, spin=0, stats=None, precision=0, options=None):
     import torch
     import paper_2506_03477_b200 as q
     cfg, sp = prob.cfg, prob.spins[spin]
@@ -37,6 +37,8 @@ def cuda_imchi(prob, edges, wts, n_k_norm=None, max_n_o=None, max_n_u=None, spin
     mo, mu = max_n_o or cfg.n_o, max_n_u or cfg.n_u
     ctx = q.Chi0Context(cfg.orb_per_site, cfg.pb_per_site, edges[:-1], n_k if n_k_norm is None else n_k_norm, mo, mu,
                         precision=precision)
+    for key, val in (options or {}).items():
+        ctx.set_option(key, val)
     ctx.set_product_tensor(torch.from_numpy(prob.P).cuda())
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     for k in range(n_k):
@@ -220,3 +222,7 @@ def test_imchi_mixed_mode(case):
     check_bins(got, ref, tol=2e-5)
     worst = max(np.linalg.norm(got[j] - ref[j]) / np.linalg.norm(ref[j]) for j in range(n_bins) if np.linalg.norm(ref[j]) > 0)
     assert worst > 1e-12          # really the FP32-grade path
+    # the same with stage (a) on tcgen05 (writes the rows through the bin sort's row map)
+    got_d = cuda_imchi(prob, edges, wts, n_k_norm=n_k_norm, precision=1, options={"zmel_direct": 2}, **kw)
+    check_bins(got_d, ref, tol=2e-5)
+    assert not np.array_equal(got_d, got)
