@@ -257,10 +257,10 @@ __global__ void __launch_bounds__(kZuThreads, 2)
     {
       uint4* bz = reinterpret_cast<uint4*>(sm + C::B_OFF);
       for (int i = tid; i < C::B_BYTES / 16; i += kZuThreads) bz[i] = make_uint4(0u, 0u, 0u, 0u);
-      for (int idx = tid; idx < kZuNB * b; idx += kZuThreads) {
-        const int n = idx / b, beta = idx - n * b;
+      for (int idx = tid; idx < kZuNB * kZuK; idx += kZuThreads) {
+        const int n = idx / kZuK, beta = idx - n * kZuK;
         double2 v = make_double2(0.0, 0.0);
-        if (n < nb) v = a.Ck[(long long)(a.n_begin + n0 + n) * a.ld_k + o0 + beta];
+        if (n < nb && beta < b) v = a.Ck[(long long)(a.n_begin + n0 + n) * a.ld_k + o0 + beta];
         cs[n * kZuK + beta] = v;
       }
       __syncthreads();
@@ -274,13 +274,18 @@ __global__ void __launch_bounds__(kZuThreads, 2)
         double ar[kZuNB], ai[kZuNB];
 #pragma unroll
         for (int n = 0; n < kZuNB; ++n) ar[n] = ai[n] = 0.0;
-        for (int beta = 0; beta < b; ++beta) {
-          const double2 pd = prow[beta];
+        for (int beta0 = 0; beta0 < b; beta0 += 8) {       // eight independent loads of P in flight per thread
+          double2 pd[8];
 #pragma unroll
-          for (int n = 0; n < kZuNB; ++n) {
-            const double2 c = cs[n * kZuK + beta];
-            ar[n] += pd.x * c.x - pd.y * c.y;
-            ai[n] += pd.x * c.y + pd.y * c.x;
+          for (int j = 0; j < 8; ++j) pd[j] = beta0 + j < b ? prow[beta0 + j] : make_double2(0.0, 0.0);
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+#pragma unroll
+            for (int n = 0; n < kZuNB; ++n) {
+              const double2 c = cs[n * kZuK + beta0 + j];
+              ar[n] += pd[j].x * c.x - pd[j].y * c.y;
+              ai[n] += pd[j].x * c.y + pd[j].y * c.x;
+            }
           }
         }
         const uint32_t ch = (uint32_t)(alpha >> 3), within = (uint32_t)(alpha & 7) * 2u;
