@@ -350,8 +350,8 @@ int32_t qsgw_mixed_stats(qsgw_ctx* ctx, int64_t* out_launches, int64_t* out_laun
  *   "stage_batches"   n >= 1   band batches staged per stage (b) launch (capped by the workspace)
  *   "zmel_dmma"       0 | 1    stage (a) step 2 on CUDA cores | on the FP64 tensor pipe (default 1)
  *   "zmel_direct"     0 | 1 | 2  mixed context, stage (a): FP64 tensor-pipe kernel + conversion to the FP16-split rows | the tcgen05
- *                              kernel that writes those rows itself for launches of >= 8 M matrix elements (default; sites of
- *                              at most 32 orbitals) | always.  The tcgen05 kernel forms z with FP32-grade products and FP32 sums
+ *                              kernel that writes those rows itself for launches of >= 8 M matrix elements outside the binned
+ *                              real-axis path (default; sites of at most 32 orbitals) | always.  The tcgen05 kernel forms z with FP32-grade products and FP32 sums
  *                              (error <= 8e-7 of max |z| instead of 2.5e-7) and scales by a bound of max |z|
  *   "mixed_fp8"       0 | 1 | 2  E5M2 correction products never | always | chosen on the device (default 2)
  *   "mixed_fp8_threshold_x100"  T*100: automatic choice takes E5M2 when P_eff >= T * N_M (default T = 4)

@@ -878,9 +878,10 @@ static int build_batches(qsgw_ctx* ctx, const double2* Ck, long long ld_k, long 
   a.Ckq_bs = ckq_bs;
   a.z_bs = n_pad;
   cudaError_t e;
-  // small launches keep the two-kernel FP64 path: the tcgen05 path has four launches and a tensor-map encode per call
+  // small launches keep the two-kernel FP64 path: the tcgen05 path has four launches and a tensor-map encode per call;
+  // so does the binned real-axis path, whose row map scatters the 64-byte runs of the epilogue (measured: 16.0 -> 19.7 ms)
   const bool direct = ctx->f16 && (ctx->zmel_direct == 2 ||
-                                   (ctx->zmel_direct == 1 && (double)n_batch * n_o * n_u * ctx->n_m >= 8.0e6));
+                                   (ctx->zmel_direct == 1 && !ctx->cur_row_map && (double)n_batch * n_o * n_u * ctx->n_m >= 8.0e6));
   if (direct) {   // stage (a) on tcgen05, straight into the FP16-split rows (no FP64 z, no conversion pass)
     a.zmax = ctx->d_zmax + zi;
     const size_t need_c = ((size_t)2 * ctx->n_sites + 2) * n_batch, need_a = qsgw::zmel_umma_aop_halves(ctx->n_sites, n_u, n_batch);
