@@ -378,18 +378,58 @@ __global__ void __launch_bounds__(kZuThreads, 2)
         const int np = mt * 128 + 32 * q + lane;
         const bool np_ok = np < a.n_u;
         const uint32_t d_re = tbase + lane_base, d_im = d_re + 128;
+        // positions of this thread's eight pair rows inside an operand row (the same for every product function):
+        // off = halves from the start of the row, lo = pair index inside its 32-pair stage
+        uint32_t off[kZuNB], lo[kZuNB];
+#pragma unroll
+        for (int n = 0; n < kZuNB; ++n) {
+          long long pair = (long long)(n0 + n) * a.n_u + np;
+          if (a.row_map && np_ok && n < nb) pair = a.row_map[pair];
+          lo[n] = (uint32_t)(pair & 31);
+          off[n] = (uint32_t)(pair >> 5) * 64u + lo[n];
+        }
+        uint32_t nr[8], ni[8];                     // the next product function's columns are in flight while this one is stored
+        if (il0 < il1) {
+          tmem_ld8(d_re + il0 * kZuNB, nr);
+          tmem_ld8(d_im + il0 * kZuNB, ni);
+        }
         for (int il = il0; il < il1; ++il) {
           uint32_t vr[8], vi[8];
-          tmem_ld8(d_re + il * kZuNB, vr);
-          tmem_ld8(d_im + il * kZuNB, vi);
           tmem_wait_ld();
+#pragma unroll
+          for (int n = 0; n < kZuNB; ++n) { vr[n] = nr[n]; vi[n] = ni[n]; }
+          if (il + 1 < il1) {
+            tmem_ld8(d_re + (il + 1) * kZuNB, nr);
+            tmem_ld8(d_im + (il + 1) * kZuNB, ni);
+          }
           if (np_ok) {
+            const long long rowh = (long long)(I0 + il) * out.kpad * 2;              // halves
+            __half* h0 = out.hl + rowh;
+            __half* h1 = h0 + out.oplane;
+            __half* g0 = reinterpret_cast<__half*>(out.hb8) + rowh;
+            __half* g1 = g0 + out.oplane;
+            unsigned char* b0 = out.hb8 + 2 * rowh;
+            unsigned char* b1 = b0 + 2 * out.oplane;
 #pragma unroll
             for (int n = 0; n < kZuNB; ++n) {
               if (n < nb) {
-                long long pair = (long long)(n0 + n) * a.n_u + np;
-                if (a.row_map) pair = a.row_map[pair];
-                store_hl(out, I0 + il, pair, __uint_as_float(vr[n]), __uint_as_float(vi[n]));
+                const float x = __uint_as_float(vr[n]), y = __uint_as_float(vi[n]);
+                const __half hx = __float2half_rn(x), hy = __float2half_rn(y);
+                const float rx = x - __half2float(hx), ry = y - __half2float(hy);
+                const uint32_t o = off[n];
+                h0[o] = hx;
+                h0[o + 32] = __float2half_rn(rx);
+                h1[o] = hy;
+                h1[o + 32] = __float2half_rn(ry);
+                if (out.hb8) {
+                  g0[o] = hx;
+                  g1[o] = hy;
+                  const uint32_t ob = 2u * o - lo[n];                                // bytes: 2 (stage start) + lo
+                  b0[ob + 64] = (unsigned char)__nv_cvt_float_to_fp8(x, __NV_SATFINITE, __NV_E5M2);
+                  b0[ob + 96] = (unsigned char)__nv_cvt_float_to_fp8(rx, __NV_SATFINITE, __NV_E5M2);
+                  b1[ob + 64] = (unsigned char)__nv_cvt_float_to_fp8(y, __NV_SATFINITE, __NV_E5M2);
+                  b1[ob + 96] = (unsigned char)__nv_cvt_float_to_fp8(ry, __NV_SATFINITE, __NV_E5M2);
+                }
               }
             }
           }
