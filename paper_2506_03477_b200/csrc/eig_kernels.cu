@@ -521,7 +521,7 @@ cudaError_t eig_configure() {
 
 // One Jacobi sweep over C (work[0..)) and Q (work[2 N^2 ..)); then norms[0] = |off|^2, norms[1] = |diag|^2.
 // blocked: block rounds of 64 x 64 subproblems + tensor-pipe updates (default); else the element-wise rounds.
-cudaError_t launch_eig_sweep(int n_m, double2* work, double* d_norms, bool blocked, cudaStream_t s) {
+cudaError_t launch_eig_sweep(int n_m, double2* work, double* d_norms, bool blocked, bool first_sweep, cudaStream_t s) {
   const int N = (n_m + 63) / 64 * 64;
   const long long sM = (long long)N * N;
   double2* Abuf = work;
@@ -539,7 +539,7 @@ cudaError_t launch_eig_sweep(int n_m, double2* work, double* d_norms, bool block
     cudaStream_t s2 = nullptr;
     cudaEvent_t e1 = nullptr, e2 = nullptr;
     cudaError_t e = cudaSuccess;
-    if (ahead) {
+    if (ahead && first_sweep) {       // the flag table is the same for every sweep: uploaded once per call
       std::vector<unsigned char> h(flag_bytes, 0);
       std::vector<int> pair_of((size_t)nblk);
       auto host_pair = [&](int i, int r, int& p, int& q) {
@@ -567,6 +567,8 @@ cudaError_t launch_eig_sweep(int n_m, double2* work, double* d_norms, bool block
       }
       e = cudaMemcpyAsync(flags, h.data(), flag_bytes, cudaMemcpyHostToDevice, s);
       if (e == cudaSuccess) e = cudaStreamSynchronize(s);               // h is a host temporary
+    }
+    if (ahead) {
       if (e == cudaSuccess) {       // highest priority: the 38 subproblem CTAs must get their SMs before the update's 2000+ CTAs
         int lo = 0, hi = 0;
         e = cudaDeviceGetStreamPriorityRange(&lo, &hi);

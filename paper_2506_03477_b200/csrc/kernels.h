@@ -214,7 +214,7 @@ cudaError_t launch_zmel_ipw(const int L[3], const double2* theta, int n_pw_kq, c
 size_t eig_work_elems(int n_m);
 cudaError_t launch_eig_reduce(int n_m, const double2* v, const double2* O, double2* work, int* d_info, cudaStream_t s);
 cudaError_t eig_configure();        // kernel attributes (per device)
-cudaError_t launch_eig_sweep(int n_m, double2* work, double* d_norms, bool blocked, cudaStream_t s);
+cudaError_t launch_eig_sweep(int n_m, double2* work, double* d_norms, bool blocked, bool first_sweep, cudaStream_t s);
 cudaError_t launch_eig_diag(int n_m, const double2* work, double* d_diag, cudaStream_t s);
 cudaError_t launch_eig_finish(int n_m, double2* work, const int* d_perm, double2* U_out, cudaStream_t s);
 

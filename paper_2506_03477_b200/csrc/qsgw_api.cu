@@ -1596,7 +1596,7 @@ int32_t qsgw_coulomb_eigenbasis(int32_t n_m, const void* d_v, const void* d_O, d
   int sweeps = 0;
   bool converged = false;
   for (; sweeps < 60 && !converged;) {
-    QSGW_E(qsgw::launch_eig_sweep(n_m, work, d_norms, g_eig_blocked != 0, st), "Jacobi sweep");
+    QSGW_E(qsgw::launch_eig_sweep(n_m, work, d_norms, g_eig_blocked != 0, sweeps == 0, st), "Jacobi sweep");
     double nr[2] = {0.0, 0.0};
     QSGW_E(cudaMemcpyAsync(nr, d_norms, 2 * sizeof(double), cudaMemcpyDeviceToHost, st), "copy of the norms");
     QSGW_E(cudaStreamSynchronize(st), "stream synchronisation");
