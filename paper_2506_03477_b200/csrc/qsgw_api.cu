@@ -559,10 +559,18 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
   const int tile_edge = mixed ? qsgw::kTileMx : qsgw::kTile;
   c->n_m_pad = (int)round_up(c->n_m, tile_edge);
   const long long max_pairs = (long long)c->max_n_o * c->max_n_u;
-  // Workspace = room for `mult` padded band batches (about 32 Ki pairs): small batches (few bands, many k-points)
+  // Workspace = room for `mult` padded band batches (32 Ki .. 256 Ki pairs): small batches (few bands, many k-points)
   // are staged back to back and stage (b) runs once per full workspace instead of once per batch.
   c->batch_pad = round_up(max_pairs, qsgw::kPairAlign);
-  long long mult = (32768 + c->batch_pad - 1) / c->batch_pad;
+  // at least 32 Ki pairs; for small N_M as many as 1.5 GB of FP64 workspace hold (up to 256 Ki): fewer, longer launches
+  long long target = (long long)(1.5e9 / ((double)2 * c->ncg * qsgw::kCG * sizeof(double)));
+  target = target < 32768 ? 32768 : (target > 262144 ? 262144 : target);
+  long long mult = (target + c->batch_pad - 1) / c->batch_pad;
+  {   // ... but beyond 32 Ki pairs never more than the declared k-points need
+    const long long mult32k = (32768 + c->batch_pad - 1) / c->batch_pad;
+    const long long cap = mult32k > c->n_k ? mult32k : c->n_k;
+    if (mult > cap) mult = cap;
+  }
   size_t z64_bytes = 0, zhl_bytes = 0, z_bytes = 0;
   for (;; --mult) {
     c->kpad = c->batch_pad * mult;
