@@ -116,7 +116,7 @@ int32_t qsgw_zmel_build(qsgw_ctx* ctx, const void* d_Ck, int64_t ld_k, const voi
  *   With d_z == NULL, n_o and n_u must equal the last zmel_build's.
  * Adds into the accumulator (upper-triangle tiles only).  The library may stage the batch (its z and its
  * weights are computed now, stream-ordered; the caller's arrays are not read later) and run the accumulation
- * kernel once several band batches fill the z workspace (about 32 Ki pairs); qsgw_chi0_finalize and qsgw_sync
+ * kernel once several band batches fill the z workspace (32 Ki pairs; for small N_M up to 256 Ki pairs within 1.5 GB); qsgw_chi0_finalize and qsgw_sync
  * accumulate whatever is staged, qsgw_reset drops it. */
 int32_t qsgw_chi0_accumulate(qsgw_ctx* ctx, const void* d_z, const double* d_eps_k,
                              const double* d_f_k, const double* d_eps_kq, const double* d_f_kq,
