@@ -348,6 +348,9 @@ int32_t qsgw_mixed_stats(qsgw_ctx* ctx, int64_t* out_launches, int64_t* out_laun
 
 /* Tuning and test knobs (never read from the environment).  ctx != NULL, allowed while nothing is staged:
  *   "stage_batches"   n >= 1   band batches staged per stage (b) launch (capped by the workspace)
+ *   "skip_dead_stages" 0 | 1 | 2  stage (b) runs every staged 32-pair stage | skips the stages without weight at any frequency
+ *                              (metals: whole bands fail the occupation filter) for flushes of >= 4 M staged matrix elements
+ *                              (default; two small extra launches per flush) | always
  *   "zmel_dmma"       0 | 1    stage (a) step 2 on CUDA cores | on the FP64 tensor pipe (default 1)
  *   "zmel_direct"     0 | 1 | 2  mixed context, stage (a): FP64 tensor-pipe kernel + conversion to the FP16-split rows | the tcgen05
  *                              kernel that writes those rows itself for launches of >= 8 M matrix elements outside the binned

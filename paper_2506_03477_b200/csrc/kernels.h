@@ -97,6 +97,9 @@ struct Chi0F64Args {
   int n_tiles_quarter = 0;
   const int2* d_ranges = nullptr;   // optional [n_freq]: pair rows [x, y) that carry weight at that frequency (bin);
                                     // the CTA runs only the 32-pair stages that cover them (no split)
+  // optional: only the 32-pair stages listed in d_live[0 .. *d_n_live) are run (the others carry no weight at any frequency)
+  const int* d_live = nullptr;
+  const int* d_n_live = nullptr;
 };
 constexpr int kChi0F64KP3M = 32;  // pairs per pipeline stage (box rows of the tensor map)
 cudaError_t launch_chi0_f64(const Chi0F64Args& a, cudaStream_t s);
@@ -147,6 +150,8 @@ struct Chi0F16Args {
   int pair = 1;          // CTA pairs (cta_group::2) sharing the B tiles of two frequencies; 0 = one CTA per (tile, frequency)
   const MixedCtl* ctl;   // device: use_fp8 selects the variant that runs (the other one exits at once)
   const int2* d_ranges = nullptr;   // optional [n_freq]: pair rows [x, y) that carry weight at that frequency (bin); no split
+  const int* d_live = nullptr;      // optional: only the stages d_live[0 .. *d_n_live) are run (the others carry no weight)
+  const int* d_n_live = nullptr;
   const int4* d_tiles;   // 128x128 tiles (tile_i, tile_j, 0, 0), tile_i <= tile_j
   int n_tiles;
 };
@@ -156,6 +161,10 @@ cudaError_t chi0_f16_configure();
 // device from the weights of the staged pairs, see weights_scale_hl16_kernel: no host synchronisation).
 cudaError_t launch_chi0_f16(const Chi0F16Args& a, cudaStream_t s);
 // n_batch batches of n_pairs pairs at pair offsets b*z_bs (a multiple of 32), scales zmax[b]
+// live[0 .. *n_live) = the 32-pair stages of the first n_pad staged rows that carry a nonzero weight at some frequency, in
+// ascending order (metals: whole bands fail the occupation filter); flags: scratch of n_pad / 32 bytes
+cudaError_t launch_stage_compaction(const double* wtab, long long kpad, long long n_pad, int n_freq, unsigned char* flags,
+                                    int* live, int* n_live, cudaStream_t s);
 cudaError_t launch_z_to_hl16(const double* zws, long long kpad, int ncg, int n_m, long long n_pairs, void* zhl,
                              void* zhb8 /*optional FP8-variant B rows*/, int n_m_pad, const float* zmax, int n_batch,
                              long long z_bs, cudaStream_t s);

@@ -120,6 +120,11 @@ struct qsgw_ctx {
   CUtensorMap tmap_hb8;
   double* d_wscale = nullptr;
   float* d_zmax = nullptr;
+  // stage (b) runs only the 32-pair stages that carry weight (option "skip_dead_stages"): list, count, flag scratch
+  int* d_live = nullptr;
+  int* d_n_live = nullptr;
+  unsigned char* d_stage_flags = nullptr;
+  int skip_dead = 1;            // 0 never | 1 for flushes of >= 4 M staged matrix elements (default) | 2 always
   // mixed, direct stage (a) on tcgen05 (option "zmel_direct"): max_I ||P_I||_F per site, per-batch norm scratch, A operand
   float* d_pmax = nullptr;
   float* d_cnorm = nullptr;
@@ -252,6 +257,9 @@ void free_all(qsgw_ctx* c) {
   cudaFree(c->d_zhb8);
   cudaFree(c->d_wscale);
   cudaFree(c->d_zmax);
+  cudaFree(c->d_live);
+  cudaFree(c->d_n_live);
+  cudaFree(c->d_stage_flags);
   cudaFree(c->d_pmax);
   cudaFree(c->d_cnorm);
   cudaFree(c->d_aop);
@@ -640,6 +648,9 @@ int32_t qsgw_create(const qsgw_desc* desc, void* cuda_stream, qsgw_ctx** out) {
     c->zmel_direct = qsgw::zmel_umma_supported(c->b_max) ? 1 : 0;
   }
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_wtab, (size_t)c->n_freq * c->kpad));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_live, (size_t)(c->kpad / qsgw::kPairStage + 1)));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_n_live, (size_t)1));
+  QSGW_TRY_ALLOC(dev_alloc(c, &c->d_stage_flags, (size_t)(c->kpad / qsgw::kPairStage + 1)));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_acc_re, acc_elems));
   QSGW_TRY_ALLOC(dev_alloc(c, &c->d_acc_im, acc_elems));
 #undef QSGW_TRY_ALLOC
@@ -747,6 +758,8 @@ int32_t qsgw_set_option(qsgw_ctx* ctx, const char* key, int64_t value) {
   if (k == "stage_batches" && value >= 1) {
     const long long cap = ctx->batch_pad * (value > (1LL << 30) ? (1LL << 30) : value);
     ctx->stage_cap = cap < ctx->kpad ? cap : ctx->kpad;
+  } else if (k == "skip_dead_stages" && value >= 0 && value <= 2) {
+    ctx->skip_dead = (int)value;
   } else if (k == "zmel_dmma" && (value == 0 || value == 1)) {
     if (value == 1 && ctx->zmel_kt_avail == 0)
       return ctx->fail(QSGW_ERR_UNSUPPORTED, "the tensor-pipe stage (a) kernel does not fit this site structure");
@@ -985,6 +998,16 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
   const long long n_pad = ctx->fill;
   if (last) { ctx->fill = 0; ctx->zslot = 0; }
   cudaError_t e;
+  // metals: whole bands fail the occupation filter, their stages carry no weight at any frequency and are skipped
+  const bool skip = !ctx->flush_ranges &&
+                    (ctx->skip_dead == 2 || (ctx->skip_dead == 1 && (double)n_pad * ctx->n_m >= 4.0e6));
+  if (skip && first) {
+    StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
+    e = qsgw::launch_stage_compaction(ctx->d_wtab, ctx->kpad, n_pad, ctx->n_freq, ctx->d_stage_flags, ctx->d_live,
+                                      ctx->d_n_live, ctx->stream);
+    if (e != cudaSuccess) return ctx->cuda_fail(e, "stage compaction kernel launch");
+    ctx->launches += 2;
+  }
   if (ctx->f16) {
     if (first) {
       StageScope ts(ctx, QSGW_STAGE_WEIGHTS);
@@ -1010,6 +1033,7 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
     m.n_sm = ctx->n_sm;
     m.ctl = ctx->d_ctl;
     m.d_ranges = ctx->flush_ranges;
+    if (skip) { m.d_live = ctx->d_live; m.d_n_live = ctx->d_n_live; }
     m.d_tiles = ctx->d_tiles;
     m.n_tiles = ctx->n_tiles;
     {
@@ -1035,6 +1059,7 @@ static int flush_range(qsgw_ctx* ctx, int j0, int nj, bool first, bool last) {
   a.n_tiles = ctx->n_tiles;
   a.n_tiles_half = ctx->n_tiles_half;
   a.n_tiles_quarter = ctx->n_tiles_quarter;
+  if (skip) { a.d_live = ctx->d_live; a.d_n_live = ctx->d_n_live; }
   {
     StageScope ts(ctx, QSGW_STAGE_CHI0);
     e = qsgw::launch_chi0_f64(a, ctx->stream);

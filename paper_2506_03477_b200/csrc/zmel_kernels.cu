@@ -343,6 +343,45 @@ __global__ void __launch_bounds__(1024) weights_scale_hl16_kernel(const double* 
   }
 }
 
+// one warp per 32-pair stage: does any pair of the stage carry a nonzero weight at any frequency?
+__global__ void stage_flags_kernel(const double* __restrict__ wtab, long long kpad, int n_stages, int n_freq,
+                                   unsigned char* __restrict__ flags) {
+  const int st = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (st >= n_stages) return;
+  bool live = false;
+  for (int j = 0; j < n_freq; ++j) live = live || wtab[(long long)j * kpad + (long long)st * 32 + lane] != 0.0;
+  const unsigned any = __ballot_sync(0xffffffffu, live);
+  if (lane == 0) flags[st] = any ? 1 : 0;
+}
+
+// one block: ascending list of the live stages and their number
+__global__ void __launch_bounds__(1024) stage_compact_kernel(const unsigned char* __restrict__ flags, int n_stages,
+                                                             int* __restrict__ live, int* __restrict__ n_live) {
+  __shared__ int wsum[32];
+  __shared__ int base_s;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) base_s = 0;
+  __syncthreads();
+  for (int s0 = 0; s0 < n_stages; s0 += 1024) {
+    const int st = s0 + tid;
+    const int f = st < n_stages ? flags[st] : 0;
+    const unsigned m = __ballot_sync(0xffffffffu, f != 0);
+    if (lane == 0) wsum[warp] = __popc(m);
+    __syncthreads();
+    int before = base_s;
+    for (int w = 0; w < warp; ++w) before += wsum[w];
+    if (f) live[before + __popc(m & ((1u << lane) - 1u))] = st;
+    __syncthreads();
+    if (tid == 0) {
+      int tot = 0;
+      for (int w = 0; w < 32; ++w) tot += wsum[w];
+      base_s += tot;
+    }
+    __syncthreads();
+  }
+  if (tid == 0) *n_live = base_s;
+}
+
 }  // namespace
 
 cudaError_t launch_zmel_f64(const ZmelArgs& a, cudaStream_t s) {
@@ -387,6 +426,14 @@ cudaError_t launch_pair_weights(const double* eps_k, const double* f_k, const do
                                 const float* zmax, int n_batch, cudaStream_t s) {
   pair_weights_kernel<<<dim3(grid_for(n_pairs_padded, 128), n_batch), 128, 0, s>>>(eps_k, f_k, eps_kq, f_kq, n_o, n_u, d_omega,
                                                                    n_freq, occ_tol, wtab, kpad, n_pairs_padded, zmax);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_stage_compaction(const double* wtab, long long kpad, long long n_pad, int n_freq, unsigned char* flags,
+                                    int* live, int* n_live, cudaStream_t s) {
+  const int n_stages = (int)(n_pad / kPairStage);
+  stage_flags_kernel<<<(n_stages + 7) / 8, 256, 0, s>>>(wtab, kpad, n_stages, n_freq, flags);
+  stage_compact_kernel<<<1, 1024, 0, s>>>(flags, n_stages, live, n_live);
   return cudaGetLastError();
 }
 

@@ -327,3 +327,29 @@ def test_add_kpoints_multi_k_launches(case, precision, tol):
         assert rel_fro_per_freq(got, one).max() <= 1e-14          # same kernels on the same slots
     if case in ("cfg0", "cfg1", "ragged"):
         assert st["kernel_launches"] <= 7 and st1["kernel_launches"] > 2 * prob.spins[0].Ck.shape[0]
+
+
+@pytest.mark.parametrize("precision,tol", [(0, TOL_FP64), (1, 2e-5)])
+def test_dead_stage_skipping_forced(precision, tol):
+    """Option "skip_dead_stages" = 2 (default: only large flushes): stage (b) runs only the 32-pair stages that carry weight.
+    Metal-like occupations (cfg 2 shape, 3 k-points): whole bands n fail the occupation filter, so runs of stages are dead;
+    then every pair dropped (no live stage at all: exact zeros); both through the multi-k launch."""
+    cfg = get_config(2)
+    prob = generate(cfg, n_k=3)
+    sp = prob.spins[0]
+    f_k = sp.f_k.copy()
+    f_k[:, -4:] = 0.0                                    # the four highest O bands empty at every k: 280 consecutive dead pairs
+    sp = dataclasses.replace(sp, f_k=f_k)
+    prob = dataclasses.replace(prob, spins=[sp])
+    keep = sp.f_k[:, :, None] * (1.0 - sp.f_kq[:, None, :]) > cfg.occ_tol
+    dead = [int((~keep[k].reshape(-1)[:keep[k].size // 32 * 32].reshape(-1, 32).any(1)).sum()) for k in range(3)]
+    assert min(dead) >= 7                                # the case really has dead stages
+    ref = oracle_chi(prob, n_k_norm=cfg.n_k)
+    for multi_k in (False, True):
+        got = run_cuda(prob, precision=precision, n_k_norm=cfg.n_k, options={"skip_dead_stages": 2}, multi_k=multi_k)
+        assert rel_fro_per_freq(got, ref).max() <= tol
+        off = run_cuda(prob, precision=precision, n_k_norm=cfg.n_k, options={"skip_dead_stages": 0}, multi_k=multi_k)
+        assert rel_fro_per_freq(off, ref).max() <= tol
+    empty = dataclasses.replace(prob, spins=[dataclasses.replace(sp, f_k=np.zeros_like(sp.f_k))])
+    got = run_cuda(empty, precision=precision, n_k_norm=cfg.n_k, options={"skip_dead_stages": 2}, multi_k=True)
+    assert np.all(got == 0)
