@@ -62,7 +62,7 @@ struct HCfg {
 };
 
 // global stage index of the i-th stage a launch runs (the list of live stages, or all of them)
-__device__ __forceinline__ int stage_of(const Chi0F16Args& a, int i) { return a.d_live ? a.d_live[i] : i; }
+__device__ __forceinline__ int stage_of(const Chi0F16Args& a, bool mapped, int i) { return mapped ? a.d_live[i] : i; }
 
 // One 32-pair stage of the frequency-scaled operand: thread <-> tile row `row`, pair half h (16 pairs); reads the hl16 row of
 // both planes and the weight row from the A-source stage at shared address sb, writes the TMEM slot (address incl. lane base).
@@ -166,6 +166,7 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
   const int4 tq = a.d_tiles[bid / a.n_freq];
   const int2 tt = make_int2(tq.x, tq.y);
   const int n_all = a.d_live ? *a.d_n_live : a.n_stages;                // stages to run (dead stages are skipped)
+  const bool mapped = a.d_live && n_all != a.n_stages;                  // every stage live: no look-up
   int s_base = (int)((long long)n_all * chunk / a.split);               // first stage of this CTA
   int n_stages = (int)((long long)n_all * (chunk + 1) / a.split) - s_base;
   if (n_stages <= 0 && !a.d_ranges) return;
@@ -216,7 +217,7 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
           for (int i = 0; i < 4; ++i) {                  // box i: plane (x | y), row half
             const int plane = i >> 1, rh = i & 1;
             const CUtensorMap* tm = FP8 ? &a.tmap_b : &a.tmap;                 // hb8 rows are addressed in bytes
-            tma_load_3d(sb + plane * kPlaneTileH + rh * kBoxBytes, tm, &full[st], stage_of(a, s_base + s) * (FP8 ? 128 : 64),
+            tma_load_3d(sb + plane * kPlaneTileH + rh * kBoxBytes, tm, &full[st], stage_of(a, mapped, s_base + s) * (FP8 ? 128 : 64),
                         tt.y * kTileMx + rh * 64, plane);
           }
         }
@@ -235,10 +236,10 @@ __global__ void __launch_bounds__(kThreadsH, 1) chi0_f16_kernel(const __grid_con
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             const int plane = i >> 1, rh = i & 1;
-            tma_load_3d(sa + plane * kPlaneTileH + rh * kBoxBytes, &a.tmap, &s_full[st], stage_of(a, s_base + s) * 64,
+            tma_load_3d(sa + plane * kPlaneTileH + rh * kBoxBytes, &a.tmap, &s_full[st], stage_of(a, mapped, s_base + s) * 64,
                         tt.x * kTileMx + rh * 64, plane);
           }
-          bulk_load_1d(sa + C::A_BYTES, wrow + (long long)stage_of(a, s_base + s) * 64, C::W_BYTES, &s_full[st]);
+          bulk_load_1d(sa + C::A_BYTES, wrow + (long long)stage_of(a, mapped, s_base + s) * 64, C::W_BYTES, &s_full[st]);
         }
         __syncwarp();
         if (++st == C::ASTAGES) { st = 0; ++u; }
@@ -424,6 +425,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsH, 1)
   const int4 tq = a.d_tiles[bid / nf2];
   const int2 tt = make_int2(tq.x, tq.y);
   const int n_all = a.d_live ? *a.d_n_live : a.n_stages;                      // stages to run (dead stages are skipped)
+  const bool mapped = a.d_live && n_all != a.n_stages;                        // every stage live: no look-up
   const int s_base = (int)((long long)n_all * chunk / a.split);               // first stage of this pair
   const int n_stages = (int)((long long)n_all * (chunk + 1) / a.split) - s_base;
   if (n_stages <= 0) return;                                                  // both CTAs of the pair
@@ -468,7 +470,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsH, 1)
           if (rank == 0) mbar_arrive_expect_tx(&full[st], 2 * C::B_BYTES);   // both halves
 #pragma unroll
           for (int plane = 0; plane < 2; ++plane)
-            tma_load_3d_pair(sb + plane * kBoxBytes, tm, bar, stage_of(a, s_base + s) * (FP8 ? 128 : 64),
+            tma_load_3d_pair(sb + plane * kBoxBytes, tm, bar, stage_of(a, mapped, s_base + s) * (FP8 ? 128 : 64),
                              tt.y * kTileMx + (int)rank * 64, plane);
         }
         __syncwarp();
@@ -486,10 +488,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsH, 1)
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             const int plane = i >> 1, rh = i & 1;
-            tma_load_3d(sa + plane * kPlaneTileH + rh * kBoxBytes, &a.tmap, &s_full[st], stage_of(a, s_base + s) * 64,
+            tma_load_3d(sa + plane * kPlaneTileH + rh * kBoxBytes, &a.tmap, &s_full[st], stage_of(a, mapped, s_base + s) * 64,
                         tt.x * kTileMx + rh * 64, plane);
           }
-          bulk_load_1d(sa + C::A_BYTES, wrow + (long long)stage_of(a, s_base + s) * 64, C::W_BYTES, &s_full[st]);
+          bulk_load_1d(sa + C::A_BYTES, wrow + (long long)stage_of(a, mapped, s_base + s) * 64, C::W_BYTES, &s_full[st]);
         }
         __syncwarp();
         if (++st == C::ASTAGES) { st = 0; ++u; }

@@ -61,6 +61,7 @@ __device__ __forceinline__ void chi0_f64_3m_body(const Chi0F64Args& a, const uns
   const int col_cg = tq.z;                 // first 16-column group of the CTA's columns inside the tile (half: 0 or 2)
   const bool diag = (tt.x == tt.y);
   const int n_all = a.d_live ? *a.d_n_live : (int)(a.n_pairs_padded / KP3);     // stages to run (dead stages are skipped)
+  const bool mapped = a.d_live && n_all != (int)(a.n_pairs_padded / KP3);          // every stage live: no look-up
   int it_base = (int)((long long)n_all * chunk / a.split);
   int n_iter = (int)((long long)n_all * (chunk + 1) / a.split) - it_base;
   if (a.d_ranges) {           // binned path: only the stages that cover the rows carrying weight in this bin
@@ -85,7 +86,7 @@ __device__ __forceinline__ void chi0_f64_3m_body(const Chi0F64Args& a, const uns
   auto issue = [&](int slot, int it) {
     unsigned char* dstA = sm + slot * (2 * OPER_BYTES3);
     mbar_arrive_expect_tx(&full[slot], stage_bytes);
-    const int gi = a.d_live ? a.d_live[it_base + it] : it_base + it;
+    const int gi = mapped ? a.d_live[it_base + it] : it_base + it;
     tma_load_4d(dstA, &a.tmap_z, &full[slot], 0, gi * KP3, tt.x * 4, 0);
     if (!diag) tma_load_4d(dstA + OPER_BYTES3, &a.tmap_z, &full[slot], 0, gi * KP3, tt.y * 4, 0);
     bulk_load_1d(wsm + slot * KP3, wrow + (long long)gi * KP3, W_BYTES3, &full[slot]);
